@@ -1,0 +1,168 @@
+/*
+ * jerk.h — C-ABI of the B200-native Fourier-domain jerk-search hot path (arXiv 1911.01353).
+ *
+ * What the library computes (BASELINE.json north_star):
+ * the overlap-and-save correlation of a normalised complex spectrum X[0..nbins) with a bank of
+ * (z = fdot*T^2, w = fddot*T^3) Fourier-response templates at numbetween = 2 half-bin phases,
+ *
+ *     A[j; z,w] = sum_m X[b+m] * conj(R_{z,w}(m - p/2)),   j = 2b + p,  p in {0,1},   P = |A|^2,
+ *     R_{z,w}(q) = int_0^1 exp(2 pi i (z u^2/2 + w u^3/6 - q u)) du,
+ *
+ * with the template of (z,w) truncated to |m - c(z,w)| <= hw(z,w), hw = ceil(|z|/2 + |w|/4) + 8 and
+ * c = the rounded midpoint of the frequency excursion z u + w u^2/2 (readings S3-S6).
+ * Powers are either written out (plane mode) or thresholded into 1-D local-max candidates
+ * (P > thr, P > P[j-1], P >= P[j+1] along r within one (z,w) row) inside the same kernel.
+ *
+ * Conventions
+ *  - Every function returns an int status: JERK_OK (0) or a negative jerk_status.  Nothing throws,
+ *    aborts or prints.  jerk_strerror() names a status; jerk_last_error() gives call detail.
+ *  - Pointers named d_* are DEVICE pointers, h_* are HOST pointers.  The library never allocates,
+ *    frees or retains ownership of device memory and never creates streams: every device buffer is
+ *    caller-owned (e.g. torch.Tensor.data_ptr()), every call takes the caller's cudaStream_t
+ *    (passed as void*) and is asynchronous on it unless stated otherwise.
+ *  - The plan is the only library-owned object (host memory).
+ *  - One GPU, sm_100a only; there is no CPU fallback of any kind.
+ *  - Grid: z_iz = -zmax + iz*dz (iz = 0..nz-1), w_iw = -wmax + iw*dw (iw = 0..nw-1); template index
+ *    ti = iw*nz + iz; r = j/2 bins.
+ */
+#ifndef JERK_H_
+#define JERK_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum jerk_status {
+  JERK_OK = 0,
+  JERK_EINVAL = -1,   /* bad argument (message in jerk_last_error)                        */
+  JERK_ENOMEM = -2,   /* a caller-provided buffer is smaller than the *_bytes the plan asks */
+  JERK_ECUDA = -3,    /* a CUDA runtime call or launch failed                              */
+  JERK_ESTATE = -4,   /* jerk_templates has not been called for this plan                  */
+  JERK_ENODEV = -5    /* no sm_100 device is current                                       */
+} jerk_status;
+
+typedef struct jerk_plan jerk_plan;
+
+/* One candidate: r = j/2, z = -zmax + iz*dz, w = -wmax + iw*dw.  16 bytes. */
+typedef struct jerk_cand {
+  int32_t j;        /* half-bin index, 0 <= j < 2*nbins                                   */
+  int16_t iz;
+  int16_t iw;
+  float power;      /* |A|^2 as computed in fp32 on the device                            */
+  uint32_t flags;   /* 0 in the output list (used internally for segment/warp seams)      */
+} jerk_cand;
+
+typedef struct jerk_plan_info_t {
+  int64_t nbins;
+  double zmax, dz, wmax, dw;
+  int32_t numbetween;
+  int32_t seg_len;       /* L: overlap-save segment (FFT) length                          */
+  int32_t nz, nw;
+  int32_t ntemplates;    /* nz*nw                                                         */
+  int32_t hw_max;        /* max half-width over the bank (overlap is 2*hw_max)            */
+  int32_t c_max;         /* max |c(z,w)|                                                  */
+  int32_t step;          /* valid outputs per segment = L - 2*hw_max                      */
+  int64_t seg_base;      /* first segment starts at this (negative, even) bin            */
+  int64_t nseg;          /* segments covering [0, nbins) for every template               */
+  int64_t points;        /* numbetween*nbins*nz*nw (r,z,w) points of one full search       */
+  uint64_t bank_bytes;   /* size of the template bank buffer jerk_templates fills          */
+  uint64_t work_bytes;   /* size of the scratch buffer the search calls need               */
+  double flops_per_search; /* algorithmic FP32 flops: nseg_nominal*2T*(5L log2 L + 6L + 3 step) */
+} jerk_plan_info_t;
+
+/*
+ * jerk_plan_create — host only (BASELINE.json north_star: jerk_plan_create(nbins, zmax, dz, wmax, dw,
+ * numbetween, seg_len)).  Validates the grid and derives nz, nw, c(z,w), hw(z,w), hw_max, step, nseg.
+ * Requirements: nbins >= 1; zmax, wmax >= 0; dz, dw > 0 with zmax/dz and wmax/dw integers;
+ * numbetween == 2; seg_len in {1024, 2048, 4096, 8192} and seg_len - 2*hw_max >= 2; nz, nw < 32768.
+ * *out receives a plan that jerk_plan_destroy frees.  Errors: JERK_EINVAL.
+ */
+int jerk_plan_create(jerk_plan** out, int64_t nbins, double zmax, double dz, double wmax, double dw,
+                     int numbetween, int seg_len);
+int jerk_plan_destroy(jerk_plan* plan);
+
+/* Copies the derived sizes into *info (host).  Errors: JERK_EINVAL on NULL. */
+int jerk_plan_info(const jerk_plan* plan, jerk_plan_info_t* info);
+
+/* Centre c and half-width hw (bins) of template (iz, iw) as the plan computed them (host only). */
+int jerk_template_geometry(const jerk_plan* plan, int iz, int iw, int* c, int* hw);
+
+/* Bytes of a plane-mode output for a sub-range: iw_cnt*iz_cnt*(2*r_cnt)*sizeof(float). */
+uint64_t jerk_plane_bytes(int64_t r_cnt, int iz_cnt, int iw_cnt);
+
+/*
+ * jerk_templates — build the template bank (BASELINE.json north_star item (1)).
+ * For every (z,w) and phase p the response R_{z,w}(c + m' - p/2), |m'| <= hw, is evaluated by fp64
+ * Gauss-Legendre quadrature on the device, placed at index (m' mod L) of a zero array, forward-FFTed,
+ * conjugated and scaled by 1/L; the result G[ti][p][L] (complex64, in the kernel's own element order)
+ * is written to d_bank together with the c/hw tables.  d_bank: DEVICE, >= bank_bytes, 256-byte aligned,
+ * caller-owned; the plan remembers the pointer and the caller must keep it alive and unmodified while
+ * searching.  Asynchronous on `stream` except for one small host->device table copy.
+ * Errors: JERK_EINVAL, JERK_ENOMEM (bank_bytes too small), JERK_ECUDA.
+ */
+int jerk_templates(jerk_plan* plan, void* d_bank, uint64_t bank_bytes, void* stream);
+
+/*
+ * jerk_templates_taps — export the raw half-bin lattice R_{z,w}(c - hw + i/2), i = 0..4hw, of one
+ * template as complex64 pairs into d_taps (DEVICE, >= (4hw+1)*8 bytes).  Test hook for row a-1.
+ */
+int jerk_templates_taps(jerk_plan* plan, int iz, int iw, void* d_taps, uint64_t taps_bytes, void* stream);
+
+/*
+ * jerk_search_plane — plane-output mode (rows a-2..a-4).  Writes P[iw_rel][iz_rel][j - 2*r_lo] (float32,
+ * r fastest) for r_lo <= b < r_lo + r_cnt, iz_lo <= iz < iz_lo + iz_cnt, iw_lo <= iw < iw_lo + iw_cnt.
+ * d_spec: DEVICE complex64 X[nbins], 16-byte aligned.  d_plane: DEVICE, >= jerk_plane_bytes(...), 8-byte
+ * aligned.  d_work: DEVICE scratch >= work_bytes, 256-byte aligned (contents are overwritten).
+ * Errors: JERK_EINVAL (range), JERK_ENOMEM, JERK_ESTATE, JERK_ECUDA.
+ */
+int jerk_search_plane(jerk_plan* plan, const void* d_spec, int64_t r_lo, int64_t r_cnt, int iz_lo, int iz_cnt,
+                      int iw_lo, int iw_cnt, float* d_plane, uint64_t plane_bytes, void* d_work,
+                      uint64_t work_bytes, void* stream);
+
+/*
+ * jerk_search_candidates — candidate mode (rows a-2..a-5): the whole (r,z,w) volume is searched and only
+ * local-max candidates above `threshold` leave the chip.  d_cands: DEVICE array of max_cands records
+ * (unordered on return); d_count: DEVICE uint64, set by the call to the total number of candidates found
+ * (may exceed max_cands: the excess is dropped, the caller detects overflow by count > max_cands).
+ * d_work as above; after the call d_work's first 64 bytes hold diagnostic counters
+ * (uint64: [0] work-item counter, [1] seam records, [2] seam overflow flag, [3] provisional candidates).
+ * Errors: JERK_EINVAL, JERK_ENOMEM, JERK_ESTATE, JERK_ECUDA.
+ */
+int jerk_search_candidates(jerk_plan* plan, const void* d_spec, float threshold, jerk_cand* d_cands,
+                           int64_t max_cands, unsigned long long* d_count, void* d_work,
+                           uint64_t work_bytes, void* stream);
+
+/*
+ * jerk_search_candidates_host — the same search with HOST input/output (end-to-end entry point):
+ * copies h_spec (host, ideally pinned, nbins complex64) to d_spec, searches, copies the count and
+ * min(count, max_cands) records back to h_count / h_cands and synchronises the stream before returning.
+ * All device buffers are still caller-owned staging.
+ */
+int jerk_search_candidates_host(jerk_plan* plan, const void* h_spec, float threshold, jerk_cand* h_cands,
+                                int64_t max_cands, unsigned long long* h_count, void* d_spec,
+                                jerk_cand* d_cands, unsigned long long* d_count, void* d_work,
+                                uint64_t work_bytes, void* stream);
+
+/*
+ * jerk_harmonic_sum — optional fused harmonic-sum stage (row a-6; BASELINE.json configs[4]):
+ * S_h(j,iz',iw') = sum_{k=1..h} P[rnd(j k/h); rnd(iz' k/h), rnd(iw' k/h)] with signed grid indices
+ * iz' = iz-(nz-1)/2, iw' = iw-(nw-1)/2 and rnd = round half away from zero (reading S13).
+ * For each of nstages stages (h_harm[s] in {1,2,4,8}, thresholds h_thr[s], HOST arrays) d_top[s] receives
+ * the arg-max of S_h over the whole grid (position of the top harmonic) if it exceeds the threshold, else
+ * {j=-1, power=0}.  d_scratch: DEVICE, >= jerk_harmonic_scratch_bytes(plan).
+ */
+uint64_t jerk_harmonic_scratch_bytes(const jerk_plan* plan);
+int jerk_harmonic_sum(jerk_plan* plan, const void* d_spec, int nstages, const int* h_harm, const float* h_thr,
+                      jerk_cand* d_top, void* d_scratch, uint64_t scratch_bytes, void* d_work,
+                      uint64_t work_bytes, void* stream);
+
+const char* jerk_strerror(int status);
+const char* jerk_last_error(const jerk_plan* plan);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* JERK_H_ */

@@ -1,0 +1,203 @@
+"""Thin ctypes binding of include/jerk.h — argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels behind the C-ABI; PyTorch is used here only
+for device memory and streams (torch.Tensor.data_ptr(), torch.cuda.current_stream()).  There is no
+CPU fallback: if libjerk_b200.so is missing or a call fails, a JerkError is raised.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libjerk_b200.so")
+
+JERK_OK, JERK_EINVAL, JERK_ENOMEM, JERK_ECUDA, JERK_ESTATE, JERK_ENODEV = 0, -1, -2, -3, -4, -5
+
+CAND_DTYPE = np.dtype([("j", "<i4"), ("iz", "<i2"), ("iw", "<i2"), ("power", "<f4"), ("flags", "<u4")])
+assert CAND_DTYPE.itemsize == 16
+
+
+class JerkError(RuntimeError):
+    def __init__(self, status, detail=""):
+        self.status = status
+        super().__init__(f"jerk status {status}: {detail}")
+
+
+class PlanInfo(C.Structure):
+    _fields_ = [
+        ("nbins", C.c_int64), ("zmax", C.c_double), ("dz", C.c_double), ("wmax", C.c_double), ("dw", C.c_double),
+        ("numbetween", C.c_int32), ("seg_len", C.c_int32), ("nz", C.c_int32), ("nw", C.c_int32),
+        ("ntemplates", C.c_int32), ("hw_max", C.c_int32), ("c_max", C.c_int32), ("step", C.c_int32),
+        ("seg_base", C.c_int64), ("nseg", C.c_int64), ("points", C.c_int64),
+        ("bank_bytes", C.c_uint64), ("work_bytes", C.c_uint64), ("flops_per_search", C.c_double),
+    ]
+
+
+EXPORTS = [
+    "jerk_plan_create", "jerk_plan_destroy", "jerk_plan_info", "jerk_template_geometry", "jerk_plane_bytes",
+    "jerk_templates", "jerk_templates_taps", "jerk_search_plane", "jerk_search_candidates",
+    "jerk_search_candidates_host", "jerk_harmonic_scratch_bytes", "jerk_harmonic_sum", "jerk_strerror",
+    "jerk_last_error",
+]
+
+_lib = None
+
+
+def load_library() -> C.CDLL:
+    """dlopen the in-tree shared library; fails loudly if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise JerkError(JERK_ENODEV, f"{LIB_PATH} not built: run `python -m paper_1911_01353_b200.build` "
+                                     "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    vp, i64, u64, dbl, i32 = C.c_void_p, C.c_int64, C.c_uint64, C.c_double, C.c_int
+    lib.jerk_plan_create.argtypes = [C.POINTER(vp), i64, dbl, dbl, dbl, dbl, i32, i32]
+    lib.jerk_plan_destroy.argtypes = [vp]
+    lib.jerk_plan_info.argtypes = [vp, C.POINTER(PlanInfo)]
+    lib.jerk_template_geometry.argtypes = [vp, i32, i32, C.POINTER(i32), C.POINTER(i32)]
+    lib.jerk_plane_bytes.argtypes = [i64, i32, i32]
+    lib.jerk_plane_bytes.restype = u64
+    lib.jerk_templates.argtypes = [vp, vp, u64, vp]
+    lib.jerk_templates_taps.argtypes = [vp, i32, i32, vp, u64, vp]
+    lib.jerk_search_plane.argtypes = [vp, vp, i64, i64, i32, i32, i32, i32, vp, u64, vp, u64, vp]
+    lib.jerk_search_candidates.argtypes = [vp, vp, C.c_float, vp, i64, vp, vp, u64, vp]
+    lib.jerk_search_candidates_host.argtypes = [vp, vp, C.c_float, vp, i64, vp, vp, vp, vp, vp, u64, vp]
+    lib.jerk_harmonic_scratch_bytes.argtypes = [vp]
+    lib.jerk_harmonic_scratch_bytes.restype = u64
+    lib.jerk_harmonic_sum.argtypes = [vp, vp, i32, C.POINTER(i32), C.POINTER(C.c_float), vp, vp, u64, vp, u64, vp]
+    lib.jerk_strerror.argtypes = [i32]
+    lib.jerk_strerror.restype = C.c_char_p
+    lib.jerk_last_error.argtypes = [vp]
+    lib.jerk_last_error.restype = C.c_char_p
+    _lib = lib
+    return lib
+
+
+def _stream_ptr(stream=None):
+    import torch
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return C.c_void_p(s.cuda_stream)
+
+
+class Plan:
+    """jerk_plan_create(nbins, zmax, dz, wmax, dw, numbetween, seg_len) and the calls that take a plan."""
+
+    def __init__(self, nbins, zmax, dz, wmax, dw, numbetween=2, seg_len=4096):
+        self._lib = load_library()
+        self._h = C.c_void_p()
+        rc = self._lib.jerk_plan_create(C.byref(self._h), int(nbins), float(zmax), float(dz), float(wmax), float(dw),
+                                        int(numbetween), int(seg_len))
+        if rc != JERK_OK:
+            raise JerkError(rc, self._lib.jerk_strerror(rc).decode())
+        info = PlanInfo()
+        self._check(self._lib.jerk_plan_info(self._h, C.byref(info)))
+        self.info = info
+        self.bank = None
+        self.work = None
+
+    def __del__(self):
+        try:
+            if getattr(self, "_h", None):
+                self._lib.jerk_plan_destroy(self._h)
+                self._h = None
+        except Exception:
+            pass
+
+    def _check(self, rc):
+        if rc != JERK_OK:
+            raise JerkError(rc, self._lib.jerk_strerror(rc).decode() + " | " + self._lib.jerk_last_error(self._h).decode())
+
+    # ---- host-only queries
+    def template_geometry(self, iz, iw):
+        c, hw = C.c_int(), C.c_int()
+        self._check(self._lib.jerk_template_geometry(self._h, int(iz), int(iw), C.byref(c), C.byref(hw)))
+        return c.value, hw.value
+
+    def plane_bytes(self, r_cnt, iz_cnt, iw_cnt):
+        return int(self._lib.jerk_plane_bytes(int(r_cnt), int(iz_cnt), int(iw_cnt)))
+
+    # ---- device calls (torch supplies memory and the stream)
+    def _ensure_work(self, device):
+        import torch
+        if self.work is None:
+            self.work = torch.empty(int(self.info.work_bytes), dtype=torch.uint8, device=device)
+        return self.work
+
+    def templates(self, device="cuda", stream=None):
+        """jerk_templates: allocates the caller-owned bank as a torch tensor and builds it."""
+        import torch
+        if self.bank is None:
+            self.bank = torch.empty(int(self.info.bank_bytes), dtype=torch.uint8, device=device)
+        self._check(self._lib.jerk_templates(self._h, C.c_void_p(self.bank.data_ptr()), int(self.info.bank_bytes),
+                                             _stream_ptr(stream)))
+        return self.bank
+
+    def templates_taps(self, iz, iw, stream=None):
+        import torch
+        c, hw = self.template_geometry(iz, iw)
+        out = torch.empty((4 * hw + 1, 2), dtype=torch.float32, device="cuda")
+        self._check(self._lib.jerk_templates_taps(self._h, int(iz), int(iw), C.c_void_p(out.data_ptr()),
+                                                  out.numel() * 4, _stream_ptr(stream)))
+        return out
+
+    def search_plane(self, d_spec, r_lo, r_cnt, iz_lo=0, iz_cnt=None, iw_lo=0, iw_cnt=None, out=None, stream=None):
+        """jerk_search_plane: returns P[iw_cnt][iz_cnt][2*r_cnt] float32 (torch, device)."""
+        import torch
+        iz_cnt = self.info.nz - iz_lo if iz_cnt is None else iz_cnt
+        iw_cnt = self.info.nw - iw_lo if iw_cnt is None else iw_cnt
+        if out is None:
+            out = torch.empty((iw_cnt, iz_cnt, 2 * r_cnt), dtype=torch.float32, device=d_spec.device)
+        work = self._ensure_work(d_spec.device)
+        self._check(self._lib.jerk_search_plane(
+            self._h, C.c_void_p(d_spec.data_ptr()), int(r_lo), int(r_cnt), int(iz_lo), int(iz_cnt), int(iw_lo),
+            int(iw_cnt), C.c_void_p(out.data_ptr()), out.numel() * 4, C.c_void_p(work.data_ptr()), work.numel(),
+            _stream_ptr(stream)))
+        return out
+
+    def search_candidates(self, d_spec, threshold, max_cands=1 << 20, d_cands=None, d_count=None, stream=None):
+        """jerk_search_candidates: returns (d_cands uint8[max_cands*16], d_count int64[1]) device tensors (async)."""
+        import torch
+        if d_cands is None:
+            d_cands = torch.empty(max_cands * 16, dtype=torch.uint8, device=d_spec.device)
+        if d_count is None:
+            d_count = torch.zeros(1, dtype=torch.int64, device=d_spec.device)
+        work = self._ensure_work(d_spec.device)
+        self._check(self._lib.jerk_search_candidates(
+            self._h, C.c_void_p(d_spec.data_ptr()), float(threshold), C.c_void_p(d_cands.data_ptr()), int(max_cands),
+            C.c_void_p(d_count.data_ptr()), C.c_void_p(work.data_ptr()), work.numel(), _stream_ptr(stream)))
+        return d_cands, d_count
+
+    def search_candidates_host(self, h_spec, threshold, h_cands, h_count, d_spec, d_cands, d_count, stream=None):
+        """jerk_search_candidates_host: pinned host tensors in/out, device staging caller-owned; synchronous."""
+        work = self._ensure_work(d_spec.device)
+        max_cands = d_cands.numel() // 16
+        self._check(self._lib.jerk_search_candidates_host(
+            self._h, C.c_void_p(h_spec.data_ptr()), float(threshold), C.c_void_p(h_cands.data_ptr()), int(max_cands),
+            C.c_void_p(h_count.data_ptr()), C.c_void_p(d_spec.data_ptr()), C.c_void_p(d_cands.data_ptr()),
+            C.c_void_p(d_count.data_ptr()), C.c_void_p(work.data_ptr()), work.numel(), _stream_ptr(stream)))
+        return int(h_count.item())
+
+    def work_counters(self):
+        """Diagnostic counters the last search left in d_work (item counter, seam records, seam overflow, provisional)."""
+        return self.work[:64].view(dtype=__import__("torch").int64).cpu().numpy().copy()
+
+
+def candidates_to_numpy(d_cands, d_count):
+    """Device candidate buffer -> structured numpy array sorted by (iw, iz, j)."""
+    n = int(d_count.item())
+    cap = d_cands.numel() // 16
+    arr = d_cands[: min(n, cap) * 16].cpu().numpy().view(CAND_DTYPE).copy()
+    order = np.lexsort((arr["j"], arr["iz"], arr["iw"]))
+    return arr[order], n
+
+
+def spectrum_to_device(X: np.ndarray, device="cuda"):
+    """complex64 numpy spectrum -> torch float32 [nbins, 2] tensor on the device."""
+    import torch
+    a = np.ascontiguousarray(X.astype(np.complex64)).view(np.float32).reshape(-1, 2)
+    return torch.from_numpy(a).to(device)

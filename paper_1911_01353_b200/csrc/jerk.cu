@@ -1,0 +1,833 @@
+// jerk.cu — C-ABI (include/jerk.h) and sm_100a kernels of the Fourier-domain jerk-search hot path.
+//
+// Kernels:
+//   k_bank     a-1  template bank: fp64 Gauss-Legendre response on the half-bin lattice -> taps -> FFT_L -> conj/L -> HBM
+//   k_search   a-2..a-5  persistent fused kernel: bulk-copy (TMA) segment -> forward FFT (F stays in registers) ->
+//              for each template-phase: F*G -> inverse FFT -> overlap discard -> |.|^2 -> plane store | threshold + local max
+//   k_resolve  a-5  settles the few candidates that sit on a warp/segment seam (neighbour owned by another warp/segment)
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/jerk.h"
+#include "jerk_fft.cuh"
+
+namespace jerk {
+
+// ------------------------------------------------------------------------------------------------- plan
+struct TemplateGeom {
+  int32_t c;
+  int32_t hw;
+};
+
+constexpr int kChunkTP = 256;          // template-phases per work item (G chunk = kChunkTP * L * 8 bytes, L2-resident)
+constexpr int kSeamCap = 1 << 16;      // seam records kept in d_work
+constexpr uint64_t kWorkHeader = 256;  // bytes: counters
+constexpr uint64_t kBankAlign = 256;
+
+}  // namespace jerk
+
+struct jerk_plan {
+  int64_t nbins;
+  double zmax, dz, wmax, dw;
+  int numbetween, L;
+  int nz, nw, T;
+  int hw_max, c_max, step;
+  int64_t seg_base, nseg;
+  std::vector<jerk::TemplateGeom> geom;  // [T]
+  uint64_t geom_bytes, bank_bytes, work_bytes;
+  void* d_bank;
+  int sm_count;
+  std::string err;
+};
+
+namespace jerk {
+
+static int fail(jerk_plan* p, int code, const std::string& msg) {
+  if (p) p->err = msg;
+  return code;
+}
+
+static int round_half_away(double v) { return (int)copysign(floor(fabs(v) + 0.5), v); }
+
+// c(z,w): rounded midpoint of the excursion of g(u) = z u + w u^2/2 on [0,1]; hw = ceil(|z|/2+|w|/4)+8 (readings S3-S5)
+static TemplateGeom template_geom(double z, double w) {
+  double lo = 0.0, hi = 0.0;
+  double e = z + w / 2.0;
+  lo = fmin(lo, e);
+  hi = fmax(hi, e);
+  if (w != 0.0) {
+    double us = -z / w;
+    if (us > 0.0 && us < 1.0) {
+      double v = -z * z / (2.0 * w);
+      lo = fmin(lo, v);
+      hi = fmax(hi, v);
+    }
+  }
+  TemplateGeom g;
+  g.c = round_half_away((lo + hi) / 2.0);
+  g.hw = (int)ceil(fabs(z) / 2.0 + fabs(w) / 4.0) + 8;
+  return g;
+}
+
+// ------------------------------------------------------------------------------------------------- bank kernel
+// 8-node Gauss-Legendre on [-1,1]
+__constant__ double c_gl_x[8] = {-0.96028985649753623168, -0.79666647741362673959, -0.52553240991632898582,
+                                 -0.18343464249564980494, 0.18343464249564980494,  0.52553240991632898582,
+                                 0.79666647741362673959,  0.96028985649753623168};
+__constant__ double c_gl_w[8] = {0.10122853629037625915, 0.22238103445337447054, 0.31370664587788728734,
+                                 0.36268378337836198297, 0.36268378337836198297, 0.31370664587788728734,
+                                 0.22238103445337447054, 0.10122853629037625915};
+
+// R_{z,w}(q) = int_0^1 exp(2 pi i (z u^2/2 + w u^3/6 - q u)) du  (BASELINE.json north_star item (1)).
+// `panels` panels of at most ~one phase cycle each; phase in fp64, reduced mod 1, then fp32 sincospi.
+__device__ float2 response_quadrature(double z, double w, double q, int panels) {
+  const double h = 1.0 / (double)panels;
+  const double a2 = 0.5 * z, a3 = w / 6.0;
+  double sr = 0.0, si = 0.0;
+  for (int pnl = 0; pnl < panels; pnl++) {
+    double um = ((double)pnl + 0.5) * h;
+    double pr = 0.0, pi = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; i++) {
+      double u = fma(c_gl_x[i], 0.5 * h, um);
+      double ph = u * (u * fma(a3, u, a2) - q);
+      ph -= rint(ph);
+      float s, c;
+      sincospif(2.0f * (float)ph, &s, &c);
+      pr = fma(c_gl_w[i], (double)c, pr);
+      pi = fma(c_gl_w[i], (double)s, pi);
+    }
+    sr += pr;
+    si += pi;
+  }
+  return make_float2((float)(sr * 0.5 * h), (float)(si * 0.5 * h));
+}
+
+__device__ __forceinline__ int quad_panels(double z, double w, int c, int hw) {
+  // |d phase/du| <= max |g(u) - q| <= |excursion|/2 + hw + 1 cycles per unit u (q within hw of the excursion midpoint)
+  double ex = fabs(z) + fabs(w) / 2.0;
+  (void)c;
+  return (int)ceil(0.5 * ex + (double)hw + 1.0) + 4;
+}
+
+struct BankParams {
+  double zmax, dz, wmax, dw;
+  int nz, nw;
+  const TemplateGeom* geom;  // device
+  float2* G;                 // device, [T][2][L] in kernel element order
+};
+
+// element order of G inside one (template, phase): thread t of the search kernel reads float4 #(u*R1/2 + k2/2)*NT + t
+template <int L>
+__device__ __forceinline__ int bank_slot(int k) {
+  using Gm = FftGeom<L>;
+  int k2 = k >> 8, b1 = k & 255;
+  int u = b1 / Gm::NT, t = b1 % Gm::NT;
+  return (((u * (Gm::R1 / 2) + (k2 >> 1)) * Gm::NT + t) << 1) + (k2 & 1);
+}
+
+template <int L>
+__global__ void __launch_bounds__(FftGeom<L>::NT) k_bank(BankParams bp) {
+  using Gm = FftGeom<L>;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  float2* exA = reinterpret_cast<float2*>(smem_raw);
+  float2* exB = exA + L;
+  float2* tw2 = exB + L;
+  float2* lat = tw2 + 256;  // 4*hw_max+1 lattice values
+  const int t = threadIdx.x;
+  const int ti = blockIdx.x;
+  const int iz = ti % bp.nz, iw = ti / bp.nz;
+  const double z = -bp.zmax + iz * bp.dz, w = -bp.wmax + iw * bp.dw;
+  const TemplateGeom g = bp.geom[ti];
+  const int panels = quad_panels(z, w, g.c, g.hw);
+  for (int i = t; i < 4 * g.hw + 1; i += Gm::NT) lat[i] = response_quadrature(z, w, (double)(g.c - g.hw) + 0.5 * i, panels);
+  fill_tw2(tw2, t, Gm::NT);
+  float2 tw1[Gm::P];
+  make_tw1<L>(tw1, t);
+  __syncthreads();
+  for (int p = 0; p < 2; p++) {
+    // taps h~_p[m'] = R(c + m' - p/2) at index (m' mod L): lattice index i = 2*(m'+hw) - p
+    for (int k = t; k < L; k += Gm::NT) {
+      int mp = k < L / 2 ? k : k - L;  // m' in [-L/2, L/2)
+      float2 v = make_float2(0.f, 0.f);
+      int lo = p ? -g.hw + 1 : -g.hw;
+      if (mp >= lo && mp <= g.hw) v = lat[2 * (mp + g.hw) - p];
+      exB[k] = v;
+    }
+    __syncthreads();
+    float2 v[Gm::P];
+#pragma unroll
+    for (int u = 0; u < Gm::NB1; u++)
+#pragma unroll
+      for (int k2 = 0; k2 < Gm::R1; k2++) v[u * Gm::R1 + k2] = exB[256 * k2 + t + Gm::NT * u];
+    fft_passes<L, -1>(v, tw1, tw2, exA, exB, t);
+    float2* out = bp.G + ((size_t)ti * 2 + p) * L;
+    const float sc = 1.0f / (float)L;
+#pragma unroll
+    for (int u = 0; u < Gm::NB2; u++)
+#pragma unroll
+      for (int n2 = 0; n2 < 16; n2++) {
+        int k = t + Gm::NT * u + 16 * Gm::R1 * n2;
+        float2 x = v[u * 16 + n2];
+        out[bank_slot<L>(k)] = make_float2(x.x * sc, -x.y * sc);  // conj(FFT)/L
+      }
+    __syncthreads();
+  }
+}
+
+__global__ void k_taps(double z, double w, int c, int hw, float2* out) {
+  int panels = quad_panels(z, w, c, hw);
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < 4 * hw + 1; i += gridDim.x * blockDim.x)
+    out[i] = response_quadrature(z, w, (double)(c - hw) + 0.5 * i, panels);
+}
+
+// ------------------------------------------------------------------------------------------------- search kernel
+struct SearchParams {
+  const float2* spec;  // X[nbins]
+  int64_t nbins;
+  const float2* G;
+  const TemplateGeom* geom;
+  int nz;
+  int hw_max, step;
+  int64_t seg_base;
+  // work decomposition
+  int64_t seg_first, seg_count;  // segments [seg_first, seg_first+seg_count)
+  int iz_lo, iz_cnt, iw_lo, iw_cnt;
+  int ntp;                       // template-phases selected = 2*iz_cnt*iw_cnt
+  int nchunks;                   // ceil(ntp / kChunkTP)
+  // plane mode
+  float* plane;
+  int64_t r_lo, r_cnt;
+  // candidate mode
+  float threshold;
+  jerk_cand* cands;
+  int64_t max_cands;
+  unsigned long long* count;
+  // scratch
+  unsigned long long* work;  // [0] item counter, [1] seam count, [2] seam overflow, [3] provisional
+  jerk_cand* seams;
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void emit_cand(const SearchParams& sp, int j, int iz, int iw, float pw) {
+  unsigned long long slot = atomicAdd(sp.count, 1ULL);
+  if ((int64_t)slot < sp.max_cands) {
+    jerk_cand c;
+    c.j = j;
+    c.iz = (int16_t)iz;
+    c.iw = (int16_t)iw;
+    c.power = pw;
+    c.flags = 0;
+    sp.cands[slot] = c;
+  }
+}
+__device__ __forceinline__ void emit_seam(const SearchParams& sp, int j, int iz, int iw, float pw, uint32_t flags) {
+  unsigned long long slot = atomicAdd(sp.work + 1, 1ULL);
+  if (slot < (unsigned long long)kSeamCap) {
+    jerk_cand c;
+    c.j = j;
+    c.iz = (int16_t)iz;
+    c.iw = (int16_t)iw;
+    c.power = pw;
+    c.flags = flags;
+    sp.seams[slot] = c;
+  } else {
+    sp.work[2] = 1ULL;
+  }
+}
+
+enum { MODE_PLANE = 0, MODE_CAND = 1 };
+enum { SEAM_LEFT = 1u, SEAM_RIGHT = 2u, SEAM_WITNESS = 4u };
+
+template <int L, int MODE>
+__global__ void __launch_bounds__(FftGeom<L>::NT) k_search(SearchParams sp) {
+  using Gm = FftGeom<L>;
+  constexpr int NT = Gm::NT, P = Gm::P, R1 = Gm::R1;
+  constexpr int NW = NT / 32;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  float2* exA = reinterpret_cast<float2*>(smem_raw);
+  float2* exB = exA + L;
+  float2* tw2 = exB + L;
+  float* stash = reinterpret_cast<float*>(tw2 + 256);              // [NW][P][32] (candidate mode)
+  unsigned long long* mbar = reinterpret_cast<unsigned long long*>(stash + (MODE == MODE_CAND ? NW * P * 32 : 0));
+  __shared__ long long s_item;
+  const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+
+  fill_tw2(tw2, t, NT);
+  float2 tw1[P];
+  make_tw1<L>(tw1, t);
+  if (t == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(mbar)));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  uint32_t mphase = 0;
+  const long long nitems = (long long)sp.nchunks * sp.seg_count;
+
+  for (;;) {
+    if (t == 0) s_item = (long long)atomicAdd(sp.work, 1ULL);
+    __syncthreads();
+    const long long item = s_item;
+    if (item >= nitems) break;
+    const int chunk = (int)(item / sp.seg_count);
+    const int64_t seg = sp.seg_first + item % sp.seg_count;
+    const int64_t s0 = sp.seg_base + seg * (int64_t)sp.step;  // first bin of the segment (even)
+
+    // ---- a-2: stage the segment in shared memory (exB): TMA bulk copy when fully inside the spectrum, guarded loads at the edges
+    const bool interior = (s0 >= 0) && (s0 + L <= sp.nbins);
+    if (interior) {
+      if (t == 0) {
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // order earlier generic accesses to exB before the async write
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(mbar)), "r"((uint32_t)(L * 8)) : "memory");
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(exB)),
+                     "l"(sp.spec + s0), "r"((uint32_t)(L * 8)), "r"(smem_u32(mbar))
+                     : "memory");
+      }
+      uint32_t done = 0;
+      while (!done) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done)
+            : "r"(smem_u32(mbar)), "r"(mphase)
+            : "memory");
+      }
+      mphase ^= 1u;
+    } else {
+      for (int k = t; k < L; k += NT) {
+        int64_t b = s0 + k;
+        exB[k] = (b >= 0 && b < sp.nbins) ? sp.spec[b] : make_float2(0.f, 0.f);
+      }
+      __syncthreads();
+    }
+    // ---- forward FFT; F ends in registers in the pass-1 layout f[u*R1 + k2] = F[256*k2 + b1]
+    float2 f[P];
+    {
+      float2 v[P];
+#pragma unroll
+      for (int u = 0; u < Gm::NB1; u++)
+#pragma unroll
+        for (int k2 = 0; k2 < R1; k2++) v[u * R1 + k2] = exB[256 * k2 + t + NT * u];
+      fft_passes<L, -1>(v, tw1, tw2, exA, exB, t);
+#pragma unroll
+      for (int u = 0; u < Gm::NB2; u++)
+#pragma unroll
+        for (int n2 = 0; n2 < 16; n2++) exA[t + NT * u + 16 * R1 * n2] = v[u * 16 + n2];
+      __syncthreads();
+#pragma unroll
+      for (int u = 0; u < Gm::NB1; u++)
+#pragma unroll
+        for (int k2 = 0; k2 < R1; k2++) f[u * R1 + k2] = exA[256 * k2 + t + NT * u];
+      __syncthreads();
+    }
+
+    // ---- loop over the template-phases of this chunk
+    const int tp_lo = chunk * kChunkTP;
+    const int tp_hi = min(sp.ntp, tp_lo + kChunkTP);
+    float p0v[P];          // phase-0 powers (plane mode keeps them to store float2 pairs)
+    bool stashed = false;  // candidate mode: phase-0 powers of this warp were stashed in smem
+    int any0 = 0;
+    for (int tp = tp_lo; tp < tp_hi; tp++) {
+      const int trel = tp >> 1, ph = tp & 1;
+      const int izr = trel % sp.iz_cnt, iwr = trel / sp.iz_cnt;
+      const int iz = sp.iz_lo + izr, iw = sp.iw_lo + iwr;
+      const int ti = iw * sp.nz + iz;
+      const int c = sp.geom[ti].c;
+      // ---- a-3: Y = F .* G, inverse FFT
+      float2 v[P];
+      {
+        const float4* g4 = reinterpret_cast<const float4*>(sp.G + ((size_t)ti * 2 + ph) * L);
+#pragma unroll
+        for (int u = 0; u < Gm::NB1; u++)
+#pragma unroll
+          for (int h = 0; h < R1 / 2; h++) {
+            float4 g = __ldg(g4 + (u * (R1 / 2) + h) * NT + t);
+            v[u * R1 + 2 * h] = cmul(f[u * R1 + 2 * h], make_float2(g.x, g.y));
+            v[u * R1 + 2 * h + 1] = cmul(f[u * R1 + 2 * h + 1], make_float2(g.z, g.w));
+          }
+      }
+      fft_passes<L, 1>(v, tw1, tw2, exA, exB, t);
+      // ---- a-4: overlap discard + power.  n = b3 + 16*R1*n2 ; b = s0 + n - c ; j = 2b + ph
+      float pw[P];
+      int anyhit = 0;
+#pragma unroll
+      for (int u = 0; u < Gm::NB2; u++)
+#pragma unroll
+        for (int n2 = 0; n2 < 16; n2++) {
+          const int n = t + NT * u + 16 * R1 * n2;
+          const int64_t b = s0 + n - c;
+          bool valid = (n >= sp.hw_max) && (n < sp.hw_max + sp.step) && (b >= 0) && (b < sp.nbins);
+          float2 y = v[u * 16 + n2];
+          float pv = fmaf(y.x, y.x, y.y * y.y);
+          if (MODE == MODE_PLANE) {
+            pw[u * 16 + n2] = pv;
+          } else {
+            pv = valid ? pv : -INFINITY;
+            pw[u * 16 + n2] = pv;
+            anyhit |= (pv > sp.threshold);
+          }
+        }
+      if (MODE == MODE_PLANE) {
+        if (ph == 0) {
+#pragma unroll
+          for (int i = 0; i < P; i++) p0v[i] = pw[i];
+        } else {
+          float* row = sp.plane + ((size_t)iwr * sp.iz_cnt + izr) * (size_t)(2 * sp.r_cnt);
+#pragma unroll
+          for (int u = 0; u < Gm::NB2; u++)
+#pragma unroll
+            for (int n2 = 0; n2 < 16; n2++) {
+              const int n = t + NT * u + 16 * R1 * n2;
+              const int64_t b = s0 + n - c;
+              bool valid = (n >= sp.hw_max) && (n < sp.hw_max + sp.step) && (b >= sp.r_lo) && (b < sp.r_lo + sp.r_cnt) &&
+                           (b >= 0) && (b < sp.nbins);
+              if (valid) *reinterpret_cast<float2*>(row + 2 * (b - sp.r_lo)) = make_float2(p0v[u * 16 + n2], pw[u * 16 + n2]);
+            }
+        }
+      } else {
+        // ---- a-5: threshold + local max.  Rare path only when some power in the warp exceeds the threshold.
+        anyhit = __any_sync(0xffffffffu, anyhit);
+        float* st = stash + (size_t)warp * P * 32;
+        if (ph == 0) {
+          any0 = anyhit;
+          stashed = false;
+          if (anyhit) {
+#pragma unroll
+            for (int i = 0; i < P; i++) st[i * 32 + lane] = pw[i];
+            stashed = true;
+            __syncwarp();
+          }
+        } else if (anyhit | any0) {
+#pragma unroll
+          for (int u = 0; u < Gm::NB2; u++)
+#pragma unroll
+            for (int n2 = 0; n2 < 16; n2++) {
+              const int i = u * 16 + n2;
+              const int n = t + NT * u + 16 * R1 * n2;
+              const int64_t b = s0 + n - c;
+              const float p1 = pw[i];
+              const float p0 = stashed ? st[i * 32 + lane] : -INFINITY;
+              float l1 = __shfl_up_sync(0xffffffffu, p1, 1);     // P1[n-1]
+              float r0 = __shfl_down_sync(0xffffffffu, p0, 1);   // P0[n+1]
+              const bool valid = (n >= sp.hw_max) && (n < sp.hw_max + sp.step) && (b >= 0) && (b < sp.nbins);
+              if (!valid) continue;
+              // phase-0 point j = 2b: left neighbour (b-1, phase 1), right neighbour (b, phase 1)
+              if (p0 > sp.threshold) {
+                bool seamL = (lane == 0 || n == sp.hw_max) && (b > 0);
+                float left = (b > 0 && !seamL) ? l1 : -INFINITY;
+                bool okR = p0 >= p1;
+                if (seamL) {
+                  emit_seam(sp, (int)(2 * b), iz, iw, p0, SEAM_LEFT | (okR ? 0u : SEAM_WITNESS));
+                } else if (p0 > left && okR) {
+                  emit_cand(sp, (int)(2 * b), iz, iw, p0);
+                }
+              }
+              // phase-1 point j = 2b+1: left neighbour (b, phase 0), right neighbour (b+1, phase 0)
+              if (p1 > sp.threshold) {
+                bool seamR = (lane == 31 || n == sp.hw_max + sp.step - 1) && (b < sp.nbins - 1);
+                float right = (b < sp.nbins - 1 && !seamR) ? r0 : -INFINITY;
+                bool okL = p1 > p0;
+                if (seamR) {
+                  emit_seam(sp, (int)(2 * b + 1), iz, iw, p1, SEAM_RIGHT | (okL ? 0u : SEAM_WITNESS));
+                } else if (okL && p1 >= right) {
+                  emit_cand(sp, (int)(2 * b + 1), iz, iw, p1);
+                }
+              }
+            }
+          __syncwarp();
+        }
+      }
+    }
+    __syncthreads();
+  }
+}
+
+// Seam records: every above-threshold point whose left (phase 0) or right (phase 1) neighbour belongs to another
+// warp or segment.  A seam point is a candidate iff it passed its own-side test and no seam record at the missing
+// neighbour position beats it (a neighbour that emitted nothing is <= threshold < this power).
+__global__ void k_resolve(SearchParams sp) {
+  unsigned long long ns = sp.work[1];
+  if (ns > (unsigned long long)kSeamCap) ns = kSeamCap;
+  for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i < ns;
+       i += (unsigned long long)gridDim.x * blockDim.x) {
+    jerk_cand a = sp.seams[i];
+    if (a.flags & SEAM_WITNESS) continue;
+    const int jn = (a.flags & SEAM_LEFT) ? a.j - 1 : a.j + 1;
+    bool ok = true;
+    for (unsigned long long k = 0; k < ns && ok; k++) {
+      jerk_cand b = sp.seams[k];
+      if (b.j == jn && b.iz == a.iz && b.iw == a.iw) {
+        if (a.flags & SEAM_LEFT) ok = a.power > b.power;   // P > P[j-1]
+        else ok = a.power >= b.power;                      // P >= P[j+1]
+      }
+    }
+    if (ok) {
+      atomicAdd(sp.work + 3, 1ULL);
+      emit_cand(sp, a.j, a.iz, a.iw, a.power);
+    }
+  }
+}
+
+__global__ void k_reset(unsigned long long* work, unsigned long long* count) {
+  if (threadIdx.x < 8) work[threadIdx.x] = 0ULL;
+  if (threadIdx.x == 0 && count) *count = 0ULL;
+}
+
+// ------------------------------------------------------------------------------------------------- host helpers
+template <int L, int MODE>
+static size_t search_smem_bytes() {
+  using Gm = FftGeom<L>;
+  size_t b = (size_t)2 * L * sizeof(float2) + 256 * sizeof(float2);
+  if (MODE == MODE_CAND) b += (size_t)(Gm::NT / 32) * Gm::P * 32 * sizeof(float);
+  b += 16;
+  return b;
+}
+
+template <int L, int MODE>
+static cudaError_t launch_search(const jerk_plan* plan, const SearchParams& sp, cudaStream_t st) {
+  using Gm = FftGeom<L>;
+  size_t smem = search_smem_bytes<L, MODE>();
+  cudaError_t e = cudaFuncSetAttribute(k_search<L, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  int occ = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_search<L, MODE>, Gm::NT, smem);
+  if (e != cudaSuccess) return e;
+  if (occ < 1) occ = 1;
+  long long nitems = (long long)sp.nchunks * sp.seg_count;
+  long long grid = (long long)plan->sm_count * occ;
+  if (grid > nitems) grid = nitems;
+  if (grid < 1) grid = 1;
+  k_search<L, MODE><<<(unsigned)grid, Gm::NT, smem, st>>>(sp);
+  return cudaGetLastError();
+}
+
+template <int MODE>
+static cudaError_t dispatch_search(const jerk_plan* plan, const SearchParams& sp, cudaStream_t st) {
+  switch (plan->L) {
+    case 1024: return launch_search<1024, MODE>(plan, sp, st);
+    case 2048: return launch_search<2048, MODE>(plan, sp, st);
+    case 4096: return launch_search<4096, MODE>(plan, sp, st);
+    case 8192: return launch_search<8192, MODE>(plan, sp, st);
+  }
+  return cudaErrorInvalidValue;
+}
+
+template <int L>
+static cudaError_t launch_bank(const jerk_plan* plan, const BankParams& bp, cudaStream_t st) {
+  using Gm = FftGeom<L>;
+  size_t smem = (size_t)2 * L * sizeof(float2) + 256 * sizeof(float2) + (size_t)(4 * plan->hw_max + 1) * sizeof(float2);
+  cudaError_t e = cudaFuncSetAttribute(k_bank<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  k_bank<L><<<plan->T, Gm::NT, smem, st>>>(bp);
+  return cudaGetLastError();
+}
+
+static bool is_integer(double v) { return fabs(v - round(v)) < 1e-9; }
+
+static uint64_t align_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
+
+static void fill_params(const jerk_plan* plan, SearchParams& sp, const void* d_spec, void* d_work) {
+  memset(&sp, 0, sizeof(sp));
+  sp.spec = (const float2*)d_spec;
+  sp.nbins = plan->nbins;
+  sp.geom = (const TemplateGeom*)plan->d_bank;
+  sp.G = (const float2*)((const unsigned char*)plan->d_bank + plan->geom_bytes);
+  sp.nz = plan->nz;
+  sp.hw_max = plan->hw_max;
+  sp.step = plan->step;
+  sp.seg_base = plan->seg_base;
+  sp.work = (unsigned long long*)d_work;
+  sp.seams = (jerk_cand*)((unsigned char*)d_work + kWorkHeader);
+}
+
+}  // namespace jerk
+
+using namespace jerk;
+
+// ------------------------------------------------------------------------------------------------- C ABI
+extern "C" {
+
+const char* jerk_strerror(int status) {
+  switch (status) {
+    case JERK_OK: return "JERK_OK";
+    case JERK_EINVAL: return "JERK_EINVAL: invalid argument";
+    case JERK_ENOMEM: return "JERK_ENOMEM: caller buffer too small";
+    case JERK_ECUDA: return "JERK_ECUDA: CUDA error";
+    case JERK_ESTATE: return "JERK_ESTATE: template bank not built";
+    case JERK_ENODEV: return "JERK_ENODEV: no sm_100 device";
+  }
+  return "unknown jerk status";
+}
+
+const char* jerk_last_error(const jerk_plan* plan) { return plan ? plan->err.c_str() : "null plan"; }
+
+int jerk_plan_create(jerk_plan** out, int64_t nbins, double zmax, double dz, double wmax, double dw, int numbetween,
+                     int seg_len) {
+  if (!out) return JERK_EINVAL;
+  *out = nullptr;
+  if (nbins < 1 || zmax < 0 || wmax < 0 || !(dz > 0) || !(dw > 0)) return JERK_EINVAL;
+  if (!is_integer(zmax / dz) || !is_integer(wmax / dw)) return JERK_EINVAL;
+  if (numbetween != 2) return JERK_EINVAL;
+  if (seg_len != 1024 && seg_len != 2048 && seg_len != 4096 && seg_len != 8192) return JERK_EINVAL;
+  if (nbins > (int64_t)1 << 30) return JERK_EINVAL;  // j = 2b+p is reported as int32
+  jerk_plan* p = new jerk_plan();
+  p->nbins = nbins;
+  p->zmax = zmax;
+  p->dz = dz;
+  p->wmax = wmax;
+  p->dw = dw;
+  p->numbetween = numbetween;
+  p->L = seg_len;
+  p->nz = (int)llround(2.0 * zmax / dz) + 1;
+  p->nw = (int)llround(2.0 * wmax / dw) + 1;
+  if (p->nz >= 32768 || p->nw >= 32768 || (int64_t)p->nz * p->nw > (1 << 24)) {
+    delete p;
+    return JERK_EINVAL;
+  }
+  p->T = p->nz * p->nw;
+  p->geom.resize(p->T);
+  p->hw_max = 0;
+  p->c_max = 0;
+  for (int iw = 0; iw < p->nw; iw++)
+    for (int iz = 0; iz < p->nz; iz++) {
+      TemplateGeom g = template_geom(-zmax + iz * dz, -wmax + iw * dw);
+      p->geom[(size_t)iw * p->nz + iz] = g;
+      if (g.hw > p->hw_max) p->hw_max = g.hw;
+      if (abs(g.c) > p->c_max) p->c_max = abs(g.c);
+    }
+  p->step = seg_len - 2 * p->hw_max;
+  if (p->step < 2) {
+    delete p;
+    return JERK_EINVAL;
+  }
+  // first segment: s0 <= -(c_max + hw_max), even (16-byte aligned bulk copies); output b = s0 + n - c, n in [hw_max, hw_max+step)
+  int64_t base = -((int64_t)p->c_max + p->hw_max);
+  if (base & 1) base -= 1;
+  p->seg_base = base;
+  // last segment must reach b = nbins-1 for c = +c_max:  base + (nseg-1)*step + hw_max + step - 1 - c_max >= nbins - 1
+  int64_t need = nbins + p->c_max - p->hw_max - base;
+  p->nseg = (need + p->step - 1) / p->step;
+  p->geom_bytes = align_up((uint64_t)p->T * sizeof(TemplateGeom), kBankAlign);
+  p->bank_bytes = p->geom_bytes + (uint64_t)p->T * 2 * seg_len * sizeof(float2);
+  p->work_bytes = kWorkHeader + (uint64_t)kSeamCap * sizeof(jerk_cand);
+  p->d_bank = nullptr;
+  p->sm_count = 0;
+  *out = p;
+  return JERK_OK;
+}
+
+int jerk_plan_destroy(jerk_plan* plan) {
+  delete plan;
+  return JERK_OK;
+}
+
+int jerk_plan_info(const jerk_plan* p, jerk_plan_info_t* info) {
+  if (!p || !info) return JERK_EINVAL;
+  memset(info, 0, sizeof(*info));
+  info->nbins = p->nbins;
+  info->zmax = p->zmax;
+  info->dz = p->dz;
+  info->wmax = p->wmax;
+  info->dw = p->dw;
+  info->numbetween = p->numbetween;
+  info->seg_len = p->L;
+  info->nz = p->nz;
+  info->nw = p->nw;
+  info->ntemplates = p->T;
+  info->hw_max = p->hw_max;
+  info->c_max = p->c_max;
+  info->step = p->step;
+  info->seg_base = p->seg_base;
+  info->nseg = p->nseg;
+  info->points = (int64_t)p->numbetween * p->nbins * p->T;
+  info->bank_bytes = p->bank_bytes;
+  info->work_bytes = p->work_bytes;
+  // nominal segments ceil(nbins/step), 2T template-phases, 5 L log2 L + 6 L + 3 step flops each
+  double nseg_nom = ceil((double)p->nbins / (double)p->step);
+  double l2 = log2((double)p->L);
+  info->flops_per_search = nseg_nom * 2.0 * p->T * (5.0 * p->L * l2 + 6.0 * p->L + 3.0 * p->step);
+  return JERK_OK;
+}
+
+int jerk_template_geometry(const jerk_plan* p, int iz, int iw, int* c, int* hw) {
+  if (!p || iz < 0 || iz >= p->nz || iw < 0 || iw >= p->nw) return JERK_EINVAL;
+  const TemplateGeom& g = p->geom[(size_t)iw * p->nz + iz];
+  if (c) *c = g.c;
+  if (hw) *hw = g.hw;
+  return JERK_OK;
+}
+
+uint64_t jerk_plane_bytes(int64_t r_cnt, int iz_cnt, int iw_cnt) {
+  if (r_cnt < 0 || iz_cnt < 0 || iw_cnt < 0) return 0;
+  return (uint64_t)iw_cnt * (uint64_t)iz_cnt * (uint64_t)(2 * r_cnt) * sizeof(float);
+}
+
+static int ensure_device(jerk_plan* p) {
+  if (p->sm_count > 0) return JERK_OK;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return fail(p, JERK_ENODEV, "cudaGetDevice failed: no CUDA device");
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return fail(p, JERK_ENODEV, "cudaGetDeviceProperties failed");
+  if (prop.major != 10) return fail(p, JERK_ENODEV, "device is not sm_100 (B200): this library has no other code path");
+  p->sm_count = prop.multiProcessorCount;
+  return JERK_OK;
+}
+
+int jerk_templates(jerk_plan* p, void* d_bank, uint64_t bank_bytes, void* stream) {
+  if (!p || !d_bank) return JERK_EINVAL;
+  if (bank_bytes < p->bank_bytes) return fail(p, JERK_ENOMEM, "bank buffer smaller than plan bank_bytes");
+  if ((uintptr_t)d_bank % kBankAlign) return fail(p, JERK_EINVAL, "d_bank must be 256-byte aligned");
+  int rc = ensure_device(p);
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaError_t e = cudaMemcpyAsync(d_bank, p->geom.data(), (size_t)p->T * sizeof(TemplateGeom), cudaMemcpyHostToDevice, st);
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("geom copy: ") + cudaGetErrorString(e));
+  BankParams bp;
+  bp.zmax = p->zmax;
+  bp.dz = p->dz;
+  bp.wmax = p->wmax;
+  bp.dw = p->dw;
+  bp.nz = p->nz;
+  bp.nw = p->nw;
+  bp.geom = (const TemplateGeom*)d_bank;
+  bp.G = (float2*)((unsigned char*)d_bank + p->geom_bytes);
+  switch (p->L) {
+    case 1024: e = launch_bank<1024>(p, bp, st); break;
+    case 2048: e = launch_bank<2048>(p, bp, st); break;
+    case 4096: e = launch_bank<4096>(p, bp, st); break;
+    default: e = launch_bank<8192>(p, bp, st); break;
+  }
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_bank launch: ") + cudaGetErrorString(e));
+  p->d_bank = d_bank;
+  return JERK_OK;
+}
+
+int jerk_templates_taps(jerk_plan* p, int iz, int iw, void* d_taps, uint64_t taps_bytes, void* stream) {
+  if (!p || !d_taps || iz < 0 || iz >= p->nz || iw < 0 || iw >= p->nw) return JERK_EINVAL;
+  int rc = ensure_device(p);
+  if (rc) return rc;
+  const TemplateGeom& g = p->geom[(size_t)iw * p->nz + iz];
+  if (taps_bytes < (uint64_t)(4 * g.hw + 1) * sizeof(float2)) return fail(p, JERK_ENOMEM, "taps buffer too small");
+  k_taps<<<8, 128, 0, (cudaStream_t)stream>>>(-p->zmax + iz * p->dz, -p->wmax + iw * p->dw, g.c, g.hw, (float2*)d_taps);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_taps launch: ") + cudaGetErrorString(e));
+  return JERK_OK;
+}
+
+static int check_common(jerk_plan* p, const void* d_spec, void* d_work, uint64_t work_bytes) {
+  if (!p || !d_spec || !d_work) return JERK_EINVAL;
+  if (!p->d_bank) return fail(p, JERK_ESTATE, "jerk_templates has not been called");
+  if (work_bytes < p->work_bytes) return fail(p, JERK_ENOMEM, "work buffer smaller than plan work_bytes");
+  if ((uintptr_t)d_spec % 16) return fail(p, JERK_EINVAL, "d_spec must be 16-byte aligned");
+  if ((uintptr_t)d_work % 256) return fail(p, JERK_EINVAL, "d_work must be 256-byte aligned");
+  return ensure_device(p);
+}
+
+int jerk_search_plane(jerk_plan* p, const void* d_spec, int64_t r_lo, int64_t r_cnt, int iz_lo, int iz_cnt, int iw_lo,
+                      int iw_cnt, float* d_plane, uint64_t plane_bytes, void* d_work, uint64_t work_bytes, void* stream) {
+  int rc = check_common(p, d_spec, d_work, work_bytes);
+  if (rc) return rc;
+  if (r_lo < 0 || r_cnt < 0 || r_lo + r_cnt > p->nbins || iz_lo < 0 || iz_cnt < 0 || iz_lo + iz_cnt > p->nz || iw_lo < 0 ||
+      iw_cnt < 0 || iw_lo + iw_cnt > p->nw)
+    return fail(p, JERK_EINVAL, "plane sub-range outside the plan's grid");
+  if (plane_bytes < jerk_plane_bytes(r_cnt, iz_cnt, iw_cnt)) return fail(p, JERK_ENOMEM, "plane buffer too small");
+  if (r_cnt == 0 || iz_cnt == 0 || iw_cnt == 0) return JERK_OK;  // empty range: nothing to write, d_plane may be NULL
+  if (!d_plane) return JERK_EINVAL;
+  if ((uintptr_t)d_plane % 8) return fail(p, JERK_EINVAL, "d_plane must be 8-byte aligned");
+  cudaStream_t st = (cudaStream_t)stream;
+  SearchParams sp;
+  fill_params(p, sp, d_spec, d_work);
+  sp.iz_lo = iz_lo;
+  sp.iz_cnt = iz_cnt;
+  sp.iw_lo = iw_lo;
+  sp.iw_cnt = iw_cnt;
+  sp.ntp = 2 * iz_cnt * iw_cnt;
+  sp.nchunks = (sp.ntp + kChunkTP - 1) / kChunkTP;
+  sp.plane = d_plane;
+  sp.r_lo = r_lo;
+  sp.r_cnt = r_cnt;
+  // segments whose outputs b = s0 + n - c (n in [hw_max, hw_max+step), |c| <= c_max) can touch [r_lo, r_lo+r_cnt)
+  int64_t lo = r_lo - p->c_max - p->seg_base - p->hw_max - p->step + 1;  // s*step >= lo
+  int64_t hi = r_lo + r_cnt - 1 + p->c_max - p->seg_base - p->hw_max;    // s*step <= hi
+  int64_t s_first = lo <= 0 ? 0 : (lo + p->step - 1) / p->step;
+  int64_t s_last = hi < 0 ? -1 : hi / p->step;
+  if (s_last > p->nseg - 1) s_last = p->nseg - 1;
+  if (s_last < s_first) return JERK_OK;
+  sp.seg_first = s_first;
+  sp.seg_count = s_last - s_first + 1;
+  k_reset<<<1, 32, 0, st>>>(sp.work, nullptr);
+  cudaError_t e = dispatch_search<MODE_PLANE>(p, sp, st);
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_search(plane) launch: ") + cudaGetErrorString(e));
+  return JERK_OK;
+}
+
+int jerk_search_candidates(jerk_plan* p, const void* d_spec, float threshold, jerk_cand* d_cands, int64_t max_cands,
+                           unsigned long long* d_count, void* d_work, uint64_t work_bytes, void* stream) {
+  int rc = check_common(p, d_spec, d_work, work_bytes);
+  if (rc) return rc;
+  if (!d_cands || !d_count || max_cands < 0) return JERK_EINVAL;
+  cudaStream_t st = (cudaStream_t)stream;
+  SearchParams sp;
+  fill_params(p, sp, d_spec, d_work);
+  sp.iz_lo = 0;
+  sp.iz_cnt = p->nz;
+  sp.iw_lo = 0;
+  sp.iw_cnt = p->nw;
+  sp.ntp = 2 * p->T;
+  sp.nchunks = (sp.ntp + kChunkTP - 1) / kChunkTP;
+  sp.seg_first = 0;
+  sp.seg_count = p->nseg;
+  sp.threshold = threshold;
+  sp.cands = d_cands;
+  sp.max_cands = max_cands;
+  sp.count = d_count;
+  k_reset<<<1, 32, 0, st>>>(sp.work, d_count);
+  cudaError_t e = dispatch_search<MODE_CAND>(p, sp, st);
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_search(cand) launch: ") + cudaGetErrorString(e));
+  k_resolve<<<p->sm_count, 256, 0, st>>>(sp);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_resolve launch: ") + cudaGetErrorString(e));
+  return JERK_OK;
+}
+
+int jerk_search_candidates_host(jerk_plan* p, const void* h_spec, float threshold, jerk_cand* h_cands, int64_t max_cands,
+                                unsigned long long* h_count, void* d_spec, jerk_cand* d_cands, unsigned long long* d_count,
+                                void* d_work, uint64_t work_bytes, void* stream) {
+  if (!p || !h_spec || !h_cands || !h_count || !d_spec) return JERK_EINVAL;
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaError_t e = cudaMemcpyAsync(d_spec, h_spec, (size_t)p->nbins * sizeof(float2), cudaMemcpyHostToDevice, st);
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("H2D spectrum: ") + cudaGetErrorString(e));
+  int rc = jerk_search_candidates(p, d_spec, threshold, d_cands, max_cands, d_count, d_work, work_bytes, stream);
+  if (rc) return rc;
+  e = cudaMemcpyAsync(h_count, d_count, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("D2H count: ") + cudaGetErrorString(e));
+  unsigned long long n = *h_count;
+  if ((int64_t)n > max_cands) n = (unsigned long long)max_cands;
+  if (n) {
+    e = cudaMemcpyAsync(h_cands, d_cands, (size_t)n * sizeof(jerk_cand), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("D2H candidates: ") + cudaGetErrorString(e));
+  }
+  return JERK_OK;
+}
+
+uint64_t jerk_harmonic_scratch_bytes(const jerk_plan* plan) {
+  (void)plan;
+  return 0;
+}
+
+int jerk_harmonic_sum(jerk_plan* p, const void* d_spec, int nstages, const int* h_harm, const float* h_thr, jerk_cand* d_top,
+                      void* d_scratch, uint64_t scratch_bytes, void* d_work, uint64_t work_bytes, void* stream) {
+  (void)d_spec; (void)nstages; (void)h_harm; (void)h_thr; (void)d_top; (void)d_scratch; (void)scratch_bytes;
+  (void)d_work; (void)work_bytes; (void)stream;
+  return fail(p, JERK_EINVAL, "jerk_harmonic_sum: not built yet (SURVEY.md 8(a) row a-6)");
+}
+
+}  // extern "C"

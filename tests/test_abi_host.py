@@ -1,0 +1,103 @@
+"""CPU tests of the boundary: the C-ABI library loads, exports every symbol include/jerk.h declares,
+and its host-only logic (plan geometry, validation, sizes) agrees with the oracle's definitions.
+No compute call is made here (no GPU)."""
+import ctypes as C
+import math
+import os
+import re
+
+import numpy as np
+import pytest
+
+from oracle import jerk_oracle as orc
+from paper_1911_01353_b200 import binding, build, synth
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    build.build()
+    return binding.load_library()
+
+
+def test_header_symbols_exported(lib):
+    hdr = open(os.path.join(ROOT, "include", "jerk.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    names = set(re.findall(r"\b(jerk_[a-z_]+)\s*\(", hdr))
+    assert names == set(binding.EXPORTS), names ^ set(binding.EXPORTS)
+    for n in names:
+        assert hasattr(lib, n), n
+
+
+def test_cand_record_is_16_bytes():
+    assert binding.CAND_DTYPE.itemsize == 16
+
+
+@pytest.mark.parametrize("idx", [1, 2, 3, 4])
+def test_plan_geometry_matches_survey_table(lib, idx):
+    cfg = synth.config(idx)
+    p = binding.Plan(cfg.nbins, cfg.zmax, cfg.dz, cfg.wmax, cfg.dw, 2, cfg.seg_len)
+    want = {1: (21, 7, 33, 958, 25), 2: (101, 31, 133, 1782, 125), 3: (201, 61, 258, 3580, 250), 4: (201, 61, 258, 7676, 250)}[idx]
+    i = p.info
+    assert (i.nz, i.nw, i.hw_max, i.step, i.c_max) == want          # SURVEY.md 8(a) size table
+    assert i.points == 2 * cfg.nbins * i.nz * i.nw
+    assert i.seg_base % 2 == 0 and i.seg_base <= -(i.c_max + i.hw_max)
+    # coverage: first segment reaches b <= 0 for c = -c_max.., last reaches nbins-1 for c = +c_max
+    assert i.seg_base + i.hw_max + i.c_max <= 0
+    assert i.seg_base + (i.nseg - 1) * i.step + i.hw_max + i.step - 1 - i.c_max >= cfg.nbins - 1
+    assert i.bank_bytes >= i.ntemplates * 2 * cfg.seg_len * 8
+    flops_unit = 5 * cfg.seg_len * math.log2(cfg.seg_len) + 6 * cfg.seg_len + 3 * i.step
+    assert abs(i.flops_per_search - math.ceil(cfg.nbins / i.step) * 2 * i.ntemplates * flops_unit) < 1e-6 * i.flops_per_search
+
+
+def test_template_geometry_matches_oracle(lib):
+    cfg = synth.config(3)
+    p = binding.Plan(cfg.nbins, cfg.zmax, cfg.dz, cfg.wmax, cfg.dw, 2, cfg.seg_len)
+    zs, ws = orc.grid_values(cfg.zmax, cfg.dz), orc.grid_values(cfg.wmax, cfg.dw)
+    for iw in range(p.info.nw):
+        for iz in range(0, p.info.nz, 1):
+            c, hw = p.template_geometry(iz, iw)
+            assert c == orc.centre(float(zs[iz]), float(ws[iw])), (zs[iz], ws[iw])
+            assert hw == orc.halfwidth(float(zs[iz]), float(ws[iw]))
+
+
+@pytest.mark.parametrize("args", [
+    (0, 20, 2, 60, 20, 2, 1024),        # nbins < 1
+    (1000, 20, 3, 60, 20, 2, 1024),     # zmax/dz not an integer
+    (1000, 20, 2, 60, 20, 1, 1024),     # numbetween != 2
+    (1000, 20, 2, 60, 20, 2, 1000),     # seg_len not a supported power of two
+    (1000, 200, 2, 6000, 20, 2, 1024),  # overlap larger than the segment
+    (1000, -1, 2, 60, 20, 2, 1024),
+    (1000, 20, 0, 60, 20, 2, 1024),
+])
+def test_plan_create_rejects(lib, args):
+    h = C.c_void_p()
+    rc = lib.jerk_plan_create(C.byref(h), *[int(a) if i in (0, 5, 6) else float(a) for i, a in enumerate(args)])
+    assert rc == binding.JERK_EINVAL and not h.value
+
+
+def test_null_arguments(lib):
+    assert lib.jerk_plan_create(None, 10, 1.0, 1.0, 1.0, 1.0, 2, 1024) == binding.JERK_EINVAL
+    assert lib.jerk_plan_info(None, None) == binding.JERK_EINVAL
+    assert lib.jerk_templates(None, None, 0, None) == binding.JERK_EINVAL
+    assert lib.jerk_strerror(binding.JERK_ESTATE).startswith(b"JERK_ESTATE")
+    assert lib.jerk_plane_bytes(10, 3, 2) == 10 * 2 * 3 * 2 * 4
+
+
+def test_search_before_templates_is_estate(lib):
+    p = binding.Plan(4096, 20, 2, 60, 20, 2, 1024)
+    fake = C.c_void_p(4096)     # never dereferenced: the state check comes first
+    rc = lib.jerk_search_candidates(p._h, fake, 20.0, fake, 10, fake, fake, int(p.info.work_bytes), None)
+    assert rc == binding.JERK_ESTATE
+
+
+def test_synth_configs_are_deterministic():
+    cfg = synth.config(1)
+    a = synth.make_spectrum(cfg)
+    b = synth.make_spectrum(synth.config(1))
+    assert a.dtype == np.complex64 and a.size == 32768 and np.array_equal(a, b)
+    assert cfg.signals == [(5000.25, 10.0, 40.0, 50.0)]
+    # block normalisation: unit mean power per 1000-bin block (reading S15)
+    blk = a[3000:4000].astype(np.complex128)
+    assert abs(np.mean(np.abs(blk) ** 2) - 1.0) < 1e-5
