@@ -175,6 +175,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config number 1..4 (default 3: the headline)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--log2n", type=int, default=0,
+                    help="profiling aid: shorten the time series to 2^LOG2N samples (same grid, same kernel); not the headline")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                       # timing rule: at least 3 warm-up steps
@@ -201,6 +203,9 @@ def main():
     binding.load_library()
 
     cfg = synth.config(args.config)
+    if args.log2n:
+        cfg.log2n = args.log2n
+        cfg.name += f"-reduced-2^{args.log2n}"
     X = synth.make_spectrum(cfg, trial=rank)
     plan = binding.Plan(cfg.nbins, cfg.zmax, cfg.dz, cfg.wmax, cfg.dw, 2, cfg.seg_len)
     info = plan.info

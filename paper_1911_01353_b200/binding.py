@@ -12,7 +12,8 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libjerk_b200.so")
+# JERK_B200_LIB may point at an experimental build of the same library (kernel tuning); default is the in-tree one
+LIB_PATH = os.environ.get("JERK_B200_LIB") or os.path.join(_HERE, "libjerk_b200.so")
 
 JERK_OK, JERK_EINVAL, JERK_ENOMEM, JERK_ECUDA, JERK_ESTATE, JERK_ENODEV = 0, -1, -2, -3, -4, -5
 

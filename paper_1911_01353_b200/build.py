@@ -12,7 +12,7 @@ LIB = os.path.join(HERE, "libjerk_b200.so")
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-    "-Xcompiler", "-fPIC", "-shared", "--use_fast_math=false" if False else "-Xptxas", "-v",
+    "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v",
 ]
 
 
@@ -30,16 +30,18 @@ def needs_build() -> bool:
     return any(os.path.getmtime(d) > t for d in DEPS)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not needs_build():
+def build(force: bool = False, verbose: bool = False, out: str | None = None, defs: list | None = None) -> str:
+    """Compile csrc/jerk.cu.  `out`/`defs` build an experimental variant (-D flags) to another path."""
+    if out is None and not force and not needs_build():
         return LIB
-    cmd = [nvcc_path()] + NVCC_FLAGS + ["-o", LIB, SRC]
+    target = out or LIB
+    cmd = [nvcc_path()] + NVCC_FLAGS + [f"-D{d}" for d in (defs or [])] + ["-o", target, SRC]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or res.returncode != 0:
         sys.stderr.write(res.stdout + res.stderr)
     if res.returncode != 0:
         raise RuntimeError("nvcc failed building libjerk_b200.so")
-    return LIB
+    return target
 
 
 if __name__ == "__main__":

@@ -246,8 +246,11 @@ __device__ __forceinline__ void emit_seam(const SearchParams& sp, int j, int iz,
 enum { MODE_PLANE = 0, MODE_CAND = 1 };
 enum { SEAM_LEFT = 1u, SEAM_RIGHT = 2u, SEAM_WITNESS = 4u };
 
+#ifndef JERK_MINBLOCKS_4096
+#define JERK_MINBLOCKS_4096 2
+#endif
 template <int L, int MODE>
-__global__ void __launch_bounds__(FftGeom<L>::NT) k_search(SearchParams sp) {
+__global__ void __launch_bounds__(FftGeom<L>::NT, (L == 4096 ? JERK_MINBLOCKS_4096 : 1)) k_search(SearchParams sp) {
   using Gm = FftGeom<L>;
   constexpr int NT = Gm::NT, P = Gm::P, R1 = Gm::R1;
   constexpr int NW = NT / 32;
@@ -255,8 +258,8 @@ __global__ void __launch_bounds__(FftGeom<L>::NT) k_search(SearchParams sp) {
   float2* exA = reinterpret_cast<float2*>(smem_raw);
   float2* exB = exA + L;
   float2* tw2 = exB + L;
-  float* stash = reinterpret_cast<float*>(tw2 + 256);              // [NW][P][32] (candidate mode)
-  unsigned long long* mbar = reinterpret_cast<unsigned long long*>(stash + (MODE == MODE_CAND ? NW * P * 32 : 0));
+  float* stash = reinterpret_cast<float*>(tw2 + 256);              // [NW][2][P][32]: phase-0/1 powers, rare path only
+  unsigned long long* mbar = reinterpret_cast<unsigned long long*>(stash + (MODE == MODE_CAND ? NW * 2 * P * 32 : 0));
   __shared__ long long s_item;
   const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
 
@@ -330,9 +333,8 @@ __global__ void __launch_bounds__(FftGeom<L>::NT) k_search(SearchParams sp) {
     // ---- loop over the template-phases of this chunk
     const int tp_lo = chunk * kChunkTP;
     const int tp_hi = min(sp.ntp, tp_lo + kChunkTP);
-    float p0v[P];          // phase-0 powers (plane mode keeps them to store float2 pairs)
-    bool stashed = false;  // candidate mode: phase-0 powers of this warp were stashed in smem
-    int any0 = 0;
+    float p0v[P];  // phase-0 powers (plane mode keeps them to store float2 pairs)
+    int any0 = 0;  // candidate mode: phase-0 powers of this warp exceeded the threshold and were stashed in smem
     for (int tp = tp_lo; tp < tp_hi; tp++) {
       const int trel = tp >> 1, ph = tp & 1;
       const int izr = trel % sp.iz_cnt, iwr = trel / sp.iz_cnt;
@@ -353,93 +355,82 @@ __global__ void __launch_bounds__(FftGeom<L>::NT) k_search(SearchParams sp) {
           }
       }
       fft_passes<L, 1>(v, tw1, tw2, exA, exB, t);
-      // ---- a-4: overlap discard + power.  n = b3 + 16*R1*n2 ; b = s0 + n - c ; j = 2b + ph
+      // ---- a-4: overlap discard + power.  n = b3 + 16*R1*n2 ; b = s0 + n - c ; j = 2b + ph.
+      // valid outputs: n in [n_lo, n_hi) = window [hw_max, hw_max+step) clipped to the bins this call covers
+      int n_lo, n_hi;
+      {
+        long long blo = MODE == MODE_PLANE ? sp.r_lo : 0, bhi = MODE == MODE_PLANE ? sp.r_lo + sp.r_cnt : sp.nbins;
+        long long lo = blo + c - s0, hi = bhi + c - s0;
+        n_lo = (int)max((long long)sp.hw_max, min(lo, (long long)L));
+        n_hi = (int)min((long long)(sp.hw_max + sp.step), max(hi, 0LL));
+      }
       float pw[P];
-      int anyhit = 0;
 #pragma unroll
-      for (int u = 0; u < Gm::NB2; u++)
-#pragma unroll
-        for (int n2 = 0; n2 < 16; n2++) {
-          const int n = t + NT * u + 16 * R1 * n2;
-          const int64_t b = s0 + n - c;
-          bool valid = (n >= sp.hw_max) && (n < sp.hw_max + sp.step) && (b >= 0) && (b < sp.nbins);
-          float2 y = v[u * 16 + n2];
-          float pv = fmaf(y.x, y.x, y.y * y.y);
-          if (MODE == MODE_PLANE) {
-            pw[u * 16 + n2] = pv;
-          } else {
-            pv = valid ? pv : -INFINITY;
-            pw[u * 16 + n2] = pv;
-            anyhit |= (pv > sp.threshold);
-          }
-        }
+      for (int i = 0; i < P; i++) pw[i] = fmaf(v[i].x, v[i].x, v[i].y * v[i].y);
       if (MODE == MODE_PLANE) {
         if (ph == 0) {
 #pragma unroll
           for (int i = 0; i < P; i++) p0v[i] = pw[i];
         } else {
           float* row = sp.plane + ((size_t)iwr * sp.iz_cnt + izr) * (size_t)(2 * sp.r_cnt);
+          const long long boff = s0 - c - sp.r_lo;
 #pragma unroll
           for (int u = 0; u < Gm::NB2; u++)
 #pragma unroll
             for (int n2 = 0; n2 < 16; n2++) {
               const int n = t + NT * u + 16 * R1 * n2;
-              const int64_t b = s0 + n - c;
-              bool valid = (n >= sp.hw_max) && (n < sp.hw_max + sp.step) && (b >= sp.r_lo) && (b < sp.r_lo + sp.r_cnt) &&
-                           (b >= 0) && (b < sp.nbins);
-              if (valid) *reinterpret_cast<float2*>(row + 2 * (b - sp.r_lo)) = make_float2(p0v[u * 16 + n2], pw[u * 16 + n2]);
+              if (n >= n_lo && n < n_hi)
+                *reinterpret_cast<float2*>(row + 2 * (boff + n)) = make_float2(p0v[u * 16 + n2], pw[u * 16 + n2]);
             }
         }
       } else {
-        // ---- a-5: threshold + local max.  Rare path only when some power in the warp exceeds the threshold.
-        anyhit = __any_sync(0xffffffffu, anyhit);
-        float* st = stash + (size_t)warp * P * 32;
+        // ---- a-5: threshold + local max.  Hot path: one max-reduction and a vote; everything else only when some
+        // power of this warp (valid or not) exceeds the threshold.
+        float mx = pw[0];
+#pragma unroll
+        for (int i = 1; i < P; i++) mx = fmaxf(mx, pw[i]);
+        const int anyhit = __any_sync(0xffffffffu, mx > sp.threshold);
+        float* st0 = stash + (size_t)warp * (2 * P * 32);
+        float* st1 = st0 + P * 32;
         if (ph == 0) {
           any0 = anyhit;
-          stashed = false;
           if (anyhit) {
 #pragma unroll
-            for (int i = 0; i < P; i++) st[i * 32 + lane] = pw[i];
-            stashed = true;
+            for (int i = 0; i < P; i++) st0[i * 32 + lane] = pw[i];
             __syncwarp();
           }
         } else if (anyhit | any0) {
 #pragma unroll
-          for (int u = 0; u < Gm::NB2; u++)
-#pragma unroll
-            for (int n2 = 0; n2 < 16; n2++) {
-              const int i = u * 16 + n2;
-              const int n = t + NT * u + 16 * R1 * n2;
-              const int64_t b = s0 + n - c;
-              const float p1 = pw[i];
-              const float p0 = stashed ? st[i * 32 + lane] : -INFINITY;
-              float l1 = __shfl_up_sync(0xffffffffu, p1, 1);     // P1[n-1]
-              float r0 = __shfl_down_sync(0xffffffffu, p0, 1);   // P0[n+1]
-              const bool valid = (n >= sp.hw_max) && (n < sp.hw_max + sp.step) && (b >= 0) && (b < sp.nbins);
-              if (!valid) continue;
-              // phase-0 point j = 2b: left neighbour (b-1, phase 1), right neighbour (b, phase 1)
-              if (p0 > sp.threshold) {
-                bool seamL = (lane == 0 || n == sp.hw_max) && (b > 0);
-                float left = (b > 0 && !seamL) ? l1 : -INFINITY;
-                bool okR = p0 >= p1;
-                if (seamL) {
-                  emit_seam(sp, (int)(2 * b), iz, iw, p0, SEAM_LEFT | (okR ? 0u : SEAM_WITNESS));
-                } else if (p0 > left && okR) {
-                  emit_cand(sp, (int)(2 * b), iz, iw, p0);
-                }
-              }
-              // phase-1 point j = 2b+1: left neighbour (b, phase 0), right neighbour (b+1, phase 0)
-              if (p1 > sp.threshold) {
-                bool seamR = (lane == 31 || n == sp.hw_max + sp.step - 1) && (b < sp.nbins - 1);
-                float right = (b < sp.nbins - 1 && !seamR) ? r0 : -INFINITY;
-                bool okL = p1 > p0;
-                if (seamR) {
-                  emit_seam(sp, (int)(2 * b + 1), iz, iw, p1, SEAM_RIGHT | (okL ? 0u : SEAM_WITNESS));
-                } else if (okL && p1 >= right) {
-                  emit_cand(sp, (int)(2 * b + 1), iz, iw, p1);
-                }
-              }
+          for (int i = 0; i < P; i++) st1[i * 32 + lane] = pw[i];
+          __syncwarp();
+          const float NEG = -INFINITY;
+#pragma unroll 1
+          for (int i = 0; i < P; i++) {
+            const int n = t + NT * (i >> 4) + 16 * R1 * (i & 15);
+            const bool valid = (n >= n_lo) && (n < n_hi);
+            const float p1 = valid ? st1[i * 32 + lane] : NEG;
+            const float p0 = (valid && any0) ? st0[i * 32 + lane] : NEG;
+            const float l1 = __shfl_up_sync(0xffffffffu, p1, 1);    // P1[n-1]
+            const float r0 = __shfl_down_sync(0xffffffffu, p0, 1);  // P0[n+1]
+            if (!valid) continue;
+            const long long b = s0 + n - c;
+            // phase-0 point j = 2b: left neighbour (b-1, phase 1), right neighbour (b, phase 1)
+            if (p0 > sp.threshold) {
+              const bool seamL = (lane == 0 || n == sp.hw_max) && (b > 0);
+              const float left = (b > 0 && !seamL) ? l1 : NEG;
+              const bool okR = p0 >= p1;
+              if (seamL) emit_seam(sp, (int)(2 * b), iz, iw, p0, SEAM_LEFT | (okR ? 0u : SEAM_WITNESS));
+              else if (p0 > left && okR) emit_cand(sp, (int)(2 * b), iz, iw, p0);
             }
+            // phase-1 point j = 2b+1: left neighbour (b, phase 0), right neighbour (b+1, phase 0)
+            if (p1 > sp.threshold) {
+              const bool seamR = (lane == 31 || n == sp.hw_max + sp.step - 1) && (b < sp.nbins - 1);
+              const float right = (b < sp.nbins - 1 && !seamR) ? r0 : NEG;
+              const bool okL = p1 > p0;
+              if (seamR) emit_seam(sp, (int)(2 * b + 1), iz, iw, p1, SEAM_RIGHT | (okL ? 0u : SEAM_WITNESS));
+              else if (okL && p1 >= right) emit_cand(sp, (int)(2 * b + 1), iz, iw, p1);
+            }
+          }
           __syncwarp();
         }
       }
@@ -484,7 +475,7 @@ template <int L, int MODE>
 static size_t search_smem_bytes() {
   using Gm = FftGeom<L>;
   size_t b = (size_t)2 * L * sizeof(float2) + 256 * sizeof(float2);
-  if (MODE == MODE_CAND) b += (size_t)(Gm::NT / 32) * Gm::P * 32 * sizeof(float);
+  if (MODE == MODE_CAND) b += (size_t)(Gm::NT / 32) * 2 * Gm::P * 32 * sizeof(float);
   b += 16;
   return b;
 }
