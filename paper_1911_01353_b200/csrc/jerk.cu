@@ -139,7 +139,7 @@ __global__ void __launch_bounds__(FftGeom<L>::NT) k_bank(BankParams bp) {
   float2* exA = reinterpret_cast<float2*>(smem_raw);
   float2* exB = exA + L;
   float2* tw2 = exB + L;
-  float2* lat = tw2 + 256;  // 4*hw_max+1 lattice values
+  float2* lat = tw2 + kTw2Floats2;  // 4*hw_max+1 lattice values
   const int t = threadIdx.x;
   const int ti = blockIdx.x;
   const int iz = ti % bp.nz, iw = ti / bp.nz;
@@ -258,7 +258,7 @@ __global__ void __launch_bounds__(FftGeom<L>::NT, (L == 4096 ? JERK_MINBLOCKS_40
   float2* exA = reinterpret_cast<float2*>(smem_raw);
   float2* exB = exA + L;
   float2* tw2 = exB + L;
-  float* stash = reinterpret_cast<float*>(tw2 + 256);              // [NW][2][P][32]: phase-0/1 powers, rare path only
+  float* stash = reinterpret_cast<float*>(tw2 + kTw2Floats2);              // [NW][2][P][32]: phase-0/1 powers, rare path only
   unsigned long long* mbar = reinterpret_cast<unsigned long long*>(stash + (MODE == MODE_CAND ? NW * 2 * P * 32 : 0));
   __shared__ long long s_item;
   const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
@@ -335,9 +335,13 @@ __global__ void __launch_bounds__(FftGeom<L>::NT, (L == 4096 ? JERK_MINBLOCKS_40
     const int tp_hi = min(sp.ntp, tp_lo + kChunkTP);
     float p0v[P];  // phase-0 powers (plane mode keeps them to store float2 pairs)
     int any0 = 0;  // candidate mode: phase-0 powers of this warp exceeded the threshold and were stashed in smem
+    int izr = (tp_lo >> 1) % sp.iz_cnt, iwr = (tp_lo >> 1) / sp.iz_cnt;
     for (int tp = tp_lo; tp < tp_hi; tp++) {
-      const int trel = tp >> 1, ph = tp & 1;
-      const int izr = trel % sp.iz_cnt, iwr = trel / sp.iz_cnt;
+      const int ph = tp & 1;
+      if (ph == 0 && tp != tp_lo && ++izr == sp.iz_cnt) {
+        izr = 0;
+        ++iwr;
+      }
       const int iz = sp.iz_lo + izr, iw = sp.iw_lo + iwr;
       const int ti = iw * sp.nz + iz;
       const int c = sp.geom[ti].c;
@@ -474,7 +478,7 @@ __global__ void k_reset(unsigned long long* work, unsigned long long* count) {
 template <int L, int MODE>
 static size_t search_smem_bytes() {
   using Gm = FftGeom<L>;
-  size_t b = (size_t)2 * L * sizeof(float2) + 256 * sizeof(float2);
+  size_t b = (size_t)2 * L * sizeof(float2) + kTw2Floats2 * sizeof(float2);
   if (MODE == MODE_CAND) b += (size_t)(Gm::NT / 32) * 2 * Gm::P * 32 * sizeof(float);
   b += 16;
   return b;
@@ -512,7 +516,7 @@ static cudaError_t dispatch_search(const jerk_plan* plan, const SearchParams& sp
 template <int L>
 static cudaError_t launch_bank(const jerk_plan* plan, const BankParams& bp, cudaStream_t st) {
   using Gm = FftGeom<L>;
-  size_t smem = (size_t)2 * L * sizeof(float2) + 256 * sizeof(float2) + (size_t)(4 * plan->hw_max + 1) * sizeof(float2);
+  size_t smem = (size_t)2 * L * sizeof(float2) + kTw2Floats2 * sizeof(float2) + (size_t)(4 * plan->hw_max + 1) * sizeof(float2);
   cudaError_t e = cudaFuncSetAttribute(k_bank<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   k_bank<L><<<plan->T, Gm::NT, smem, st>>>(bp);

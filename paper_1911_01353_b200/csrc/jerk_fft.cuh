@@ -8,7 +8,7 @@
 //   w_L^{kn} = w_R1^{k2 n0} * w_L^{(16 k1 + k0) n0} * w_16^{k1 n1} * w_256^{k0 n1} * w_16^{k0 n2}
 //
 //   pass 1: butterfly b1 = 16*k1 + k0  : DFT_R1 over k2,  then twiddle T1 = w_L^{b1*n0}   (per-thread registers)
-//   pass 2: butterfly b2 = 16*n0 + k0  : DFT_16 over k1,  then twiddle T2 = w_256^{k0*n1} (16x16 table, smem)
+//   pass 2: butterfly b2 = 16*n0 + k0  : DFT_16 over k1;  twiddle T2 = w_256^{k0*n1} (16x16 smem table) is applied when pass 3 loads
 //   pass 3: butterfly b3 = n0 + R1*n1  : DFT_16 over k0,  output n = b3 + 16*R1*n2
 //
 // SIGN = +1 is the unnormalised inverse transform (e^{+2 pi i kn/L}), SIGN = -1 the forward one.
@@ -163,9 +163,13 @@ __device__ __forceinline__ void make_tw1(float2 (&tw1)[FftGeom<L>::P], int t) {
   }
 }
 
-// T2 table (inverse sign) in shared memory: tw2[k0*16 + n1] = w_256^{k0*n1}
+// T2 table (inverse sign) in shared memory: tw2[n1*kTw2Stride + k0] = w_256^{k0*n1}.  It is read in pass 3, where the
+// row n1 = b3 / R1 is uniform over R1 consecutive lanes (broadcast loads); rows are padded to 18 float2 so that the
+// rows touched by one 128-bit load instruction fall in different banks.
+constexpr int kTw2Stride = 18;
+constexpr int kTw2Floats2 = 16 * kTw2Stride;
 __device__ __forceinline__ void fill_tw2(float2* tw2, int t, int nthreads) {
-  for (int i = t; i < 256; i += nthreads) tw2[i] = unit_root((i >> 4) * (i & 15), 256);
+  for (int i = t; i < 256; i += nthreads) tw2[(i >> 4) * kTw2Stride + (i & 15)] = unit_root((i >> 4) * (i & 15), 256);
 }
 
 // Passes 1..3 on the P points in v[].  On entry v[u*R1 + k2] = x[256*k2 + b1], b1 = t + NT*u.
@@ -202,20 +206,22 @@ __device__ __forceinline__ void fft_passes(float2 (&v)[FftGeom<L>::P], const flo
     Dft<16, SIGN>::run(a);
 #pragma unroll
     for (int n1 = 0; n1 < 16; n1++) {
-      float2 w = tw2[k0 * 16 + n1];
-      float2 r = n1 == 0 ? a[0] : (SIGN > 0 ? cmul(a[n1], w) : cmul_conj(a[n1], w));
       int b3 = n0 + G::R1 * n1;
-      exB[16 * b3 + ((k0 + b3) & 15)] = r;
+      exB[16 * b3 + ((k0 + b3) & 15)] = a[n1];
     }
   }
   __syncthreads();
-  // ---- pass 3
+  // ---- pass 3 (the T2 twiddle w_256^{k0*n1} is applied here, on the read side: its row n1 is lane-uniform)
 #pragma unroll
   for (int u = 0; u < G::NB2; u++) {
     int b3 = t + G::NT * u;
+    const float2* trow = tw2 + (b3 / G::R1) * kTw2Stride;
     float2 a[16];
 #pragma unroll
-    for (int q = 0; q < 16; q++) a[q] = exB[16 * b3 + ((q + b3) & 15)];
+    for (int q = 0; q < 16; q++) {
+      float2 x = exB[16 * b3 + ((q + b3) & 15)];
+      a[q] = q == 0 ? x : (SIGN > 0 ? cmul(x, trow[q]) : cmul_conj(x, trow[q]));
+    }
     Dft<16, SIGN>::run(a);
 #pragma unroll
     for (int n2 = 0; n2 < 16; n2++) v[u * 16 + n2] = a[n2];
