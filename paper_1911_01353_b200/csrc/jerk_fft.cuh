@@ -17,16 +17,22 @@
 
 namespace jerk {
 
+// Complex arithmetic on (re, im) register pairs with Blackwell's packed FP32 instructions (FADD2 / FMUL2 / FFMA2):
+// one issue slot does both halves; the half-swap, negate and scalar-broadcast operand forms are free SASS modifiers
+// (R.F32x2.LO_HI, -R.F32x2.LO_HI.NP, R.F32), so multiplying by +-i costs nothing and a complex multiply is 2 instructions.
+__device__ __forceinline__ float2 bc(float s) { return make_float2(s, s); }
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
+// a * b = a*(b.x,b.x) + (i a)*(b.y,b.y)
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
-  return make_float2(fmaf(-a.y, b.y, a.x * b.x), fmaf(a.y, b.x, a.x * b.y));
+  return __ffma2_rn(make_float2(-a.y, a.x), bc(b.y), __fmul2_rn(a, bc(b.x)));
 }
-__device__ __forceinline__ float2 cmul_conj(float2 a, float2 b) {  // a * conj(b)
-  return make_float2(fmaf(a.y, b.y, a.x * b.x), fmaf(a.y, b.x, -(a.x * b.y)));
+// a * conj(b) = a*(b.x,b.x) + (-i a)*(b.y,b.y)
+__device__ __forceinline__ float2 cmul_conj(float2 a, float2 b) {
+  return __ffma2_rn(make_float2(a.y, -a.x), bc(b.y), __fmul2_rn(a, bc(b.x)));
 }
-__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
 
-// multiply by SIGN * i
+// multiply by SIGN * i (folds into the operand modifier of the consuming packed instruction)
 template <int SIGN>
 __device__ __forceinline__ float2 rot90(float2 a) {
   return SIGN > 0 ? make_float2(-a.y, a.x) : make_float2(a.y, -a.x);
@@ -53,13 +59,10 @@ __device__ __forceinline__ float2 mul_tw(float2 v, int m) {
   int r = k & 7;                           // remainder, 0..7
   float2 t = v;
   if (r != 0) {
-    if (r == 4) {                          // (1 + SIGN i)/sqrt(2)
-      const float c = cos32(4);
-      float2 u = SIGN > 0 ? make_float2(v.x - v.y, v.x + v.y) : make_float2(v.x + v.y, v.y - v.x);
-      t = make_float2(u.x * c, u.y * c);
-    } else {
-      const float c = cos32(r), s = SIGN > 0 ? cos32(8 - r) : -cos32(8 - r);
-      t = make_float2(fmaf(-v.y, s, v.x * c), fmaf(v.x, s, v.y * c));
+    if (r == 4) {                          // (1 + SIGN i)/sqrt(2) * v = (v + SIGN i v)/sqrt(2)
+      t = __fmul2_rn(__fadd2_rn(v, rot90<SIGN>(v)), bc(cos32(4)));
+    } else {                               // (c + SIGN i s) * v = c v + s (SIGN i v)
+      t = __ffma2_rn(rot90<SIGN>(v), bc(cos32(8 - r)), __fmul2_rn(v, bc(cos32(r))));
     }
   }
   // apply quarter turns: multiply by (SIGN i)^quad
