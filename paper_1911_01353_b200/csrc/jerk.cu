@@ -9,8 +9,10 @@
 #include <math.h>
 #include <stdint.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
+#include <algorithm>
 #include <string>
 #include <vector>
 
@@ -29,6 +31,8 @@ constexpr int kChunkTP = 256;          // template-phases per work item (G chunk
 constexpr int kSeamCap = 1 << 16;      // seam records kept in d_work
 constexpr uint64_t kWorkHeader = 256;  // bytes: counters
 constexpr uint64_t kBankAlign = 256;
+constexpr int kMaxCtas = 148 * 4;      // upper bound on resident CTAs of the persistent search kernel (stash slots)
+constexpr uint64_t kStashPerCta = 2ull * 8192 * sizeof(float);  // phase-0 and phase-1 powers of one segment (L <= 8192)
 
 }  // namespace jerk
 
@@ -123,13 +127,32 @@ struct BankParams {
   float2* G;                 // device, [T][2][L] in kernel element order
 };
 
-// element order of G inside one (template, phase): thread t of the search kernel reads float4 #(u*R1/2 + k2/2)*NT + t
+// element order of G inside one (template, phase): thread t of the search kernel reads float4 #(u*R1/2 + k2/2)*NT + t,
+// which holds elements k = 256*k2 + b1_of(t,u) for k2 = 2h, 2h+1
 template <int L>
 __device__ __forceinline__ int bank_slot(int k) {
   using Gm = FftGeom<L>;
   int k2 = k >> 8, b1 = k & 255;
-  int u = b1 / Gm::NT, t = b1 % Gm::NT;
+  int k1 = b1 >> 4, k0 = b1 & 15;
+  int u = k1 / Gm::GS, t = k0 * Gm::GS + (k1 % Gm::GS);
   return (((u * (Gm::R1 / 2) + (k2 >> 1)) * Gm::NT + t) << 1) + (k2 & 1);
+}
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+// mbarrier for the split write-after-read barrier of exchange buffer B: count NT, primed so that the first wait passes
+template <int NT>
+__device__ __forceinline__ WarBarrier war_init(unsigned long long* bar, int t) {
+  if (t == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(NT));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  WarBarrier w;
+  w.bar = smem_u32(bar);
+  w.parity = 0;
+  w.arrive();
+  return w;
 }
 
 template <int L>
@@ -140,6 +163,7 @@ __global__ void __launch_bounds__(FftGeom<L>::NT) k_bank(BankParams bp) {
   float2* exB = exA + L;
   float2* tw2 = exB + L;
   float2* lat = tw2 + kTw2Floats2;  // 4*hw_max+1 lattice values
+  __shared__ unsigned long long s_war;
   const int t = threadIdx.x;
   const int ti = blockIdx.x;
   const int iz = ti % bp.nz, iw = ti / bp.nz;
@@ -148,9 +172,9 @@ __global__ void __launch_bounds__(FftGeom<L>::NT) k_bank(BankParams bp) {
   const int panels = quad_panels(z, w, g.c, g.hw);
   for (int i = t; i < 4 * g.hw + 1; i += Gm::NT) lat[i] = response_quadrature(z, w, (double)(g.c - g.hw) + 0.5 * i, panels);
   fill_tw2(tw2, t, Gm::NT);
-  float2 tw1[Gm::P];
-  make_tw1<L>(tw1, t);
-  __syncthreads();
+  Tw1Regs<L> tw1;
+  make_tw1<L>(tw1.w, t);
+  WarBarrier war = war_init<Gm::NT>(&s_war, t);
   for (int p = 0; p < 2; p++) {
     // taps h~_p[m'] = R(c + m' - p/2) at index (m' mod L): lattice index i = 2*(m'+hw) - p
     for (int k = t; k < L; k += Gm::NT) {
@@ -158,22 +182,23 @@ __global__ void __launch_bounds__(FftGeom<L>::NT) k_bank(BankParams bp) {
       float2 v = make_float2(0.f, 0.f);
       int lo = p ? -g.hw + 1 : -g.hw;
       if (mp >= lo && mp <= g.hw) v = lat[2 * (mp + g.hw) - p];
-      exB[k] = v;
+      exA[k] = v;
     }
     __syncthreads();
     float2 v[Gm::P];
 #pragma unroll
     for (int u = 0; u < Gm::NB1; u++)
 #pragma unroll
-      for (int k2 = 0; k2 < Gm::R1; k2++) v[u * Gm::R1 + k2] = exB[256 * k2 + t + Gm::NT * u];
-    fft_passes<L, -1>(v, tw1, tw2, exA, exB, t);
+      for (int k2 = 0; k2 < Gm::R1; k2++) v[u * Gm::R1 + k2] = exA[256 * k2 + Gm::b1_of(t, u)];
+    __syncthreads();
+    fft_passes<L, -1>(v, tw1, tw2, exA, exB, war, t);
     float2* out = bp.G + ((size_t)ti * 2 + p) * L;
     const float sc = 1.0f / (float)L;
 #pragma unroll
     for (int u = 0; u < Gm::NB2; u++)
 #pragma unroll
       for (int n2 = 0; n2 < 16; n2++) {
-        int k = t + Gm::NT * u + 16 * Gm::R1 * n2;
+        int k = Gm::b3_of(t, u) + 16 * Gm::R1 * n2;
         float2 x = v[u * 16 + n2];
         out[bank_slot<L>(k)] = make_float2(x.x * sc, -x.y * sc);  // conj(FFT)/L
       }
@@ -212,9 +237,8 @@ struct SearchParams {
   // scratch
   unsigned long long* work;  // [0] item counter, [1] seam count, [2] seam overflow, [3] provisional
   jerk_cand* seams;
+  float* stash;              // [kMaxCtas][2][L]: powers of the current template, written only on the rare path
 };
-
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
 __device__ __forceinline__ void emit_cand(const SearchParams& sp, int j, int iz, int iw, float pw) {
   unsigned long long slot = atomicAdd(sp.count, 1ULL);
@@ -247,32 +271,60 @@ enum { MODE_PLANE = 0, MODE_CAND = 1 };
 enum { SEAM_LEFT = 1u, SEAM_RIGHT = 2u, SEAM_WITNESS = 4u };
 
 #ifndef JERK_MINBLOCKS_4096
-#define JERK_MINBLOCKS_4096 2
+#define JERK_MINBLOCKS_4096 3
 #endif
+
+// TMEM columns per CTA: two thread-private arrays (F and T1) of 2P floats per thread, NW/4 warp groups side by side
+template <int L>
+struct TmemCols {
+  static constexpr int value = 2 * ((FftGeom<L>::NW + 3) / 4) * 2 * FftGeom<L>::P;
+};
+
 template <int L, int MODE>
-__global__ void __launch_bounds__(FftGeom<L>::NT, (L == 4096 ? JERK_MINBLOCKS_4096 : 1)) k_search(SearchParams sp) {
+__global__ void __launch_bounds__(FftGeom<L>::NT, (L == 4096 ? (MODE == MODE_CAND ? JERK_MINBLOCKS_4096 : 2) : 1))
+k_search(SearchParams sp) {
   using Gm = FftGeom<L>;
   constexpr int NT = Gm::NT, P = Gm::P, R1 = Gm::R1;
-  constexpr int NW = NT / 32;
-  extern __shared__ __align__(128) unsigned char smem_raw[];
+  constexpr int TCOLS = TmemCols<L>::value;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
   float2* exA = reinterpret_cast<float2*>(smem_raw);
   float2* exB = exA + L;
   float2* tw2 = exB + L;
-  float* stash = reinterpret_cast<float*>(tw2 + kTw2Floats2);              // [NW][2][P][32]: phase-0/1 powers, rare path only
-  unsigned long long* mbar = reinterpret_cast<unsigned long long*>(stash + (MODE == MODE_CAND ? NW * 2 * P * 32 : 0));
+  unsigned long long* mbar = reinterpret_cast<unsigned long long*>(tw2 + kTw2Floats2);  // [0] segment copy, [1] exB WAR
   __shared__ long long s_item;
+  __shared__ uint32_t s_tmem;
   const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
 
+  // ---- tensor memory: per-thread homes for F (forward-transformed segment) and the T1 twiddles
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&s_tmem)), "n"(TCOLS));
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+  }
   fill_tw2(tw2, t, NT);
-  float2 tw1[P];
-  make_tw1<L>(tw1, t);
   if (t == 0) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(mbar)));
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  __syncthreads();
+  asm volatile("tcgen05.fence::before_thread_sync;");
+  WarBarrier war = war_init<NT>(mbar + 1, t);   // contains the __syncthreads that publishes s_tmem, tw2 and mbar[0]
+  asm volatile("tcgen05.fence::after_thread_sync;");
+  const uint32_t tbase = s_tmem + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(warp >> 2) * (2 * P);
+  TmemArray<L> tmF, tmT;
+  tmF.addr = tbase;
+  tmT.addr = tbase + TCOLS / 2;
+  {
+    float2 w[P];
+    make_tw1<L>(w, t);
+#pragma unroll
+    for (int h = 0; h < P / 16; h++) {
+      float2 q[16];
+#pragma unroll
+      for (int i = 0; i < 16; i++) q[i] = w[16 * h + i];
+      tmT.store16(h, q);
+    }
+  }
   uint32_t mphase = 0;
   const long long nitems = (long long)sp.nchunks * sp.seg_count;
+  float* gstash = sp.stash + (size_t)blockIdx.x * (2 * L);   // [2][P][NT] powers of the current template (rare path)
 
   for (;;) {
     if (t == 0) s_item = (long long)atomicAdd(sp.work, 1ULL);
@@ -283,13 +335,13 @@ __global__ void __launch_bounds__(FftGeom<L>::NT, (L == 4096 ? JERK_MINBLOCKS_40
     const int64_t seg = sp.seg_first + item % sp.seg_count;
     const int64_t s0 = sp.seg_base + seg * (int64_t)sp.step;  // first bin of the segment (even)
 
-    // ---- a-2: stage the segment in shared memory (exB): TMA bulk copy when fully inside the spectrum, guarded loads at the edges
+    // ---- a-2: stage the segment in shared memory (exA): TMA bulk copy when fully inside the spectrum, guarded loads at the edges
     const bool interior = (s0 >= 0) && (s0 + L <= sp.nbins);
     if (interior) {
       if (t == 0) {
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // order earlier generic accesses to exB before the async write
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // order earlier generic accesses to exA before the async write
         asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(mbar)), "r"((uint32_t)(L * 8)) : "memory");
-        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(exB)),
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(exA)),
                      "l"(sp.spec + s0), "r"((uint32_t)(L * 8)), "r"(smem_u32(mbar))
                      : "memory");
       }
@@ -305,28 +357,35 @@ __global__ void __launch_bounds__(FftGeom<L>::NT, (L == 4096 ? JERK_MINBLOCKS_40
     } else {
       for (int k = t; k < L; k += NT) {
         int64_t b = s0 + k;
-        exB[k] = (b >= 0 && b < sp.nbins) ? sp.spec[b] : make_float2(0.f, 0.f);
+        exA[k] = (b >= 0 && b < sp.nbins) ? sp.spec[b] : make_float2(0.f, 0.f);
       }
       __syncthreads();
     }
-    // ---- forward FFT; F ends in registers in the pass-1 layout f[u*R1 + k2] = F[256*k2 + b1]
-    float2 f[P];
+    // ---- forward FFT; F goes to TMEM in the pass-1 layout F[256*k2 + b1_of(t,u)] at array index u*R1 + k2
     {
       float2 v[P];
 #pragma unroll
       for (int u = 0; u < Gm::NB1; u++)
 #pragma unroll
-        for (int k2 = 0; k2 < R1; k2++) v[u * R1 + k2] = exB[256 * k2 + t + NT * u];
-      fft_passes<L, -1>(v, tw1, tw2, exA, exB, t);
+        for (int k2 = 0; k2 < R1; k2++) v[u * R1 + k2] = exA[256 * k2 + Gm::b1_of(t, u)];
+      __syncthreads();                                   // exA is about to be reused as exchange buffer 1
+      fft_passes<L, -1>(v, tmT, tw2, exA, exB, war, t);
+      __syncthreads();                                   // all pass-2 reads of exA done (they precede the barrier inside)
 #pragma unroll
       for (int u = 0; u < Gm::NB2; u++)
 #pragma unroll
-        for (int n2 = 0; n2 < 16; n2++) exA[t + NT * u + 16 * R1 * n2] = v[u * 16 + n2];
+        for (int n2 = 0; n2 < 16; n2++) exA[Gm::b3_of(t, u) + 16 * R1 * n2] = v[u * 16 + n2];
       __syncthreads();
 #pragma unroll
-      for (int u = 0; u < Gm::NB1; u++)
+      for (int h = 0; h < P / 16; h++) {
+        float2 q[16];
 #pragma unroll
-        for (int k2 = 0; k2 < R1; k2++) f[u * R1 + k2] = exA[256 * k2 + t + NT * u];
+        for (int i = 0; i < 16; i++) {
+          const int e = 16 * h + i, u = e / R1, k2 = e % R1;
+          q[i] = exA[256 * k2 + Gm::b1_of(t, u)];
+        }
+        tmF.store16(h, q);
+      }
       __syncthreads();
     }
 
@@ -334,7 +393,7 @@ __global__ void __launch_bounds__(FftGeom<L>::NT, (L == 4096 ? JERK_MINBLOCKS_40
     const int tp_lo = chunk * kChunkTP;
     const int tp_hi = min(sp.ntp, tp_lo + kChunkTP);
     float p0v[P];  // phase-0 powers (plane mode keeps them to store float2 pairs)
-    int any0 = 0;  // candidate mode: phase-0 powers of this warp exceeded the threshold and were stashed in smem
+    int any0 = 0;  // candidate mode: phase-0 powers of this warp exceeded the threshold and were stashed
     int izr = (tp_lo >> 1) % sp.iz_cnt, iwr = (tp_lo >> 1) / sp.iz_cnt;
     for (int tp = tp_lo; tp < tp_hi; tp++) {
       const int ph = tp & 1;
@@ -345,20 +404,26 @@ __global__ void __launch_bounds__(FftGeom<L>::NT, (L == 4096 ? JERK_MINBLOCKS_40
       const int iz = sp.iz_lo + izr, iw = sp.iw_lo + iwr;
       const int ti = iw * sp.nz + iz;
       const int c = sp.geom[ti].c;
-      // ---- a-3: Y = F .* G, inverse FFT
+      // ---- a-3: Y = F .* G (G straight from L2/HBM, F from TMEM), inverse FFT
       float2 v[P];
+      __syncwarp();   // tcgen05.ld is .sync.aligned: the warp must be converged (the store / candidate paths below diverge)
       {
-        const float4* g4 = reinterpret_cast<const float4*>(sp.G + ((size_t)ti * 2 + ph) * L);
+        const float4* g4 = reinterpret_cast<const float4*>(sp.G + ((size_t)ti * 2 + ph) * L) + t;
+        float4 g[P / 2];
 #pragma unroll
-        for (int u = 0; u < Gm::NB1; u++)
+        for (int e = 0; e < P / 2; e++) g[e] = __ldg(g4 + e * NT);
 #pragma unroll
-          for (int h = 0; h < R1 / 2; h++) {
-            float4 g = __ldg(g4 + (u * (R1 / 2) + h) * NT + t);
-            v[u * R1 + 2 * h] = cmul(f[u * R1 + 2 * h], make_float2(g.x, g.y));
-            v[u * R1 + 2 * h + 1] = cmul(f[u * R1 + 2 * h + 1], make_float2(g.z, g.w));
+        for (int h = 0; h < P / 16; h++) {
+          float2 fq[16];
+          tmF.load16(h, fq);
+#pragma unroll
+          for (int i = 0; i < 8; i++) {
+            v[16 * h + 2 * i] = cmul(fq[2 * i], make_float2(g[8 * h + i].x, g[8 * h + i].y));
+            v[16 * h + 2 * i + 1] = cmul(fq[2 * i + 1], make_float2(g[8 * h + i].z, g[8 * h + i].w));
           }
+        }
       }
-      fft_passes<L, 1>(v, tw1, tw2, exA, exB, t);
+      fft_passes<L, 1>(v, tmT, tw2, exA, exB, war, t);
       // ---- a-4: overlap discard + power.  n = b3 + 16*R1*n2 ; b = s0 + n - c ; j = 2b + ph.
       // valid outputs: n in [n_lo, n_hi) = window [hw_max, hw_max+step) clipped to the bins this call covers
       int n_lo, n_hi;
@@ -382,7 +447,7 @@ __global__ void __launch_bounds__(FftGeom<L>::NT, (L == 4096 ? JERK_MINBLOCKS_40
           for (int u = 0; u < Gm::NB2; u++)
 #pragma unroll
             for (int n2 = 0; n2 < 16; n2++) {
-              const int n = t + NT * u + 16 * R1 * n2;
+              const int n = Gm::b3_of(t, u) + 16 * R1 * n2;
               if (n >= n_lo && n < n_hi)
                 *reinterpret_cast<float2*>(row + 2 * (boff + n)) = make_float2(p0v[u * 16 + n2], pw[u * 16 + n2]);
             }
@@ -394,26 +459,25 @@ __global__ void __launch_bounds__(FftGeom<L>::NT, (L == 4096 ? JERK_MINBLOCKS_40
 #pragma unroll
         for (int i = 1; i < P; i++) mx = fmaxf(mx, pw[i]);
         const int anyhit = __any_sync(0xffffffffu, mx > sp.threshold);
-        float* st0 = stash + (size_t)warp * (2 * P * 32);
-        float* st1 = st0 + P * 32;
+        float* st0 = gstash;            // [P][NT]: element i of thread t at i*NT + t (written and read by the same thread)
+        float* st1 = gstash + L;
         if (ph == 0) {
           any0 = anyhit;
           if (anyhit) {
 #pragma unroll
-            for (int i = 0; i < P; i++) st0[i * 32 + lane] = pw[i];
-            __syncwarp();
+            for (int i = 0; i < P; i++) st0[i * NT + t] = pw[i];
           }
         } else if (anyhit | any0) {
 #pragma unroll
-          for (int i = 0; i < P; i++) st1[i * 32 + lane] = pw[i];
+          for (int i = 0; i < P; i++) st1[i * NT + t] = pw[i];
           __syncwarp();
           const float NEG = -INFINITY;
 #pragma unroll 1
           for (int i = 0; i < P; i++) {
-            const int n = t + NT * (i >> 4) + 16 * R1 * (i & 15);
+            const int n = Gm::b3_of(t, i >> 4) + 16 * R1 * (i & 15);
             const bool valid = (n >= n_lo) && (n < n_hi);
-            const float p1 = valid ? st1[i * 32 + lane] : NEG;
-            const float p0 = (valid && any0) ? st0[i * 32 + lane] : NEG;
+            const float p1 = valid ? st1[i * NT + t] : NEG;
+            const float p0 = (valid && any0) ? st0[i * NT + t] : NEG;
             const float l1 = __shfl_up_sync(0xffffffffu, p1, 1);    // P1[n-1]
             const float r0 = __shfl_down_sync(0xffffffffu, p0, 1);  // P0[n+1]
             if (!valid) continue;
@@ -441,6 +505,8 @@ __global__ void __launch_bounds__(FftGeom<L>::NT, (L == 4096 ? JERK_MINBLOCKS_40
     }
     __syncthreads();
   }
+  __syncthreads();
+  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(s_tmem), "n"(TCOLS));
 }
 
 // Seam records: every above-threshold point whose left (phase 0) or right (phase 1) neighbour belongs to another
@@ -477,11 +543,7 @@ __global__ void k_reset(unsigned long long* work, unsigned long long* count) {
 // ------------------------------------------------------------------------------------------------- host helpers
 template <int L, int MODE>
 static size_t search_smem_bytes() {
-  using Gm = FftGeom<L>;
-  size_t b = (size_t)2 * L * sizeof(float2) + kTw2Floats2 * sizeof(float2);
-  if (MODE == MODE_CAND) b += (size_t)(Gm::NT / 32) * 2 * Gm::P * 32 * sizeof(float);
-  b += 16;
-  return b;
+  return (size_t)2 * L * sizeof(float2) + kTw2Floats2 * sizeof(float2) + 2 * sizeof(unsigned long long);
 }
 
 template <int L, int MODE>
@@ -490,12 +552,22 @@ static cudaError_t launch_search(const jerk_plan* plan, const SearchParams& sp, 
   size_t smem = search_smem_bytes<L, MODE>();
   cudaError_t e = cudaFuncSetAttribute(k_search<L, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  int occ = 0;
-  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_search<L, MODE>, Gm::NT, smem);
+  // Resident CTAs per SM.  cudaOccupancyMaxActiveBlocksPerMultiprocessor answers 1 for every kernel that allocates
+  // tensor memory, although CTAs do co-reside as long as their TMEM columns fit (512 per SM): compute it from the
+  // kernel's own resource use.
+  cudaFuncAttributes fa;
+  e = cudaFuncGetAttributes(&fa, k_search<L, MODE>);
   if (e != cudaSuccess) return e;
+  int regs_per_cta = ((fa.numRegs + 7) / 8 * 8) * Gm::NT;
+  int occ = 65536 / regs_per_cta;
+  occ = std::min(occ, (int)(233472 / (smem + fa.sharedSizeBytes + 1024)));
+  occ = std::min(occ, 2048 / Gm::NT);
+  occ = std::min(occ, 512 / TmemCols<L>::value);
+  if (getenv("JERK_DEBUG")) fprintf(stderr, "[jerk] k_search<%d,%d>: %d regs, smem %zu B, %d CTAs/SM\n", L, MODE, fa.numRegs, smem, occ);
   if (occ < 1) occ = 1;
   long long nitems = (long long)sp.nchunks * sp.seg_count;
   long long grid = (long long)plan->sm_count * occ;
+  if (grid > kMaxCtas) grid = kMaxCtas;
   if (grid > nitems) grid = nitems;
   if (grid < 1) grid = 1;
   k_search<L, MODE><<<(unsigned)grid, Gm::NT, smem, st>>>(sp);
@@ -539,6 +611,7 @@ static void fill_params(const jerk_plan* plan, SearchParams& sp, const void* d_s
   sp.seg_base = plan->seg_base;
   sp.work = (unsigned long long*)d_work;
   sp.seams = (jerk_cand*)((unsigned char*)d_work + kWorkHeader);
+  sp.stash = (float*)((unsigned char*)d_work + kWorkHeader + (uint64_t)kSeamCap * sizeof(jerk_cand));
 }
 
 }  // namespace jerk
@@ -610,7 +683,7 @@ int jerk_plan_create(jerk_plan** out, int64_t nbins, double zmax, double dz, dou
   p->nseg = (need + p->step - 1) / p->step;
   p->geom_bytes = align_up((uint64_t)p->T * sizeof(TemplateGeom), kBankAlign);
   p->bank_bytes = p->geom_bytes + (uint64_t)p->T * 2 * seg_len * sizeof(float2);
-  p->work_bytes = kWorkHeader + (uint64_t)kSeamCap * sizeof(jerk_cand);
+  p->work_bytes = kWorkHeader + (uint64_t)kSeamCap * sizeof(jerk_cand) + (uint64_t)kMaxCtas * kStashPerCta;
   p->d_bank = nullptr;
   p->sm_count = 0;
   *out = p;

@@ -14,6 +14,7 @@
 // SIGN = +1 is the unnormalised inverse transform (e^{+2 pi i kn/L}), SIGN = -1 the forward one.
 #pragma once
 #include <cuda_runtime.h>
+#include <stdint.h>
 
 namespace jerk {
 
@@ -142,11 +143,20 @@ struct FftGeom {
   static constexpr int NT = L / P;                   // threads per FFT
   static constexpr int NB1 = P / R1;                 // pass-1 butterflies per thread
   static constexpr int NB2 = P / 16;                 // pass-2/3 butterflies per thread
+  static constexpr int GS = NT / 16;                 // threads that share one k0 (they exchange among themselves after pass 1)
+  static constexpr int NW = NT / 32;                 // warps
   static constexpr int LOG2L = L == 1024 ? 10 : L == 2048 ? 11 : L == 4096 ? 12 : 13;
   static_assert(L == 1024 || L == 2048 || L == 4096 || L == 8192, "seg_len");
+  static_assert(NB2 * GS == R1, "pass-2 butterflies per k0 group");
+  // Thread roles.  Pass 1 and pass 2 of thread t work on the same k0 = t / GS, so exchange 1 stays inside GS consecutive
+  // lanes (GS <= 16: one half-warp) and needs only __syncwarp; exchange 2 crosses warps.
+  static __device__ __forceinline__ int k0_of(int t) { return t / GS; }
+  static __device__ __forceinline__ int b1_of(int t, int u) { return 16 * ((t % GS) + GS * u) + t / GS; }   // 16*k1 + k0
+  static __device__ __forceinline__ int n0_of(int t, int u) { return (t % GS) + GS * u; }
+  static __device__ __forceinline__ int b3_of(int t, int u) { return t + NT * u; }                           // n0 + R1*n1
 };
 
-// exp(SIGN * 2 pi i * num / den), den a power of two, num reduced exactly in integers
+// exp(2 pi i * num / den), den a power of two, num reduced exactly in integers
 __device__ __forceinline__ float2 unit_root(int num, int den) {
   int r = num & (den - 1);
   float s, c;
@@ -154,17 +164,76 @@ __device__ __forceinline__ float2 unit_root(int num, int den) {
   return make_float2(c, s);
 }
 
-// Per-thread T1 twiddles for the INVERSE transform: tw1[u*R1 + n0] = w_L^{b1*n0}, b1 = t + NT*u.
+// Per-thread T1 twiddles for the INVERSE transform: tw1[u*R1 + n0] = w_L^{b1*n0}, b1 = b1_of(t, u).
 template <int L>
 __device__ __forceinline__ void make_tw1(float2 (&tw1)[FftGeom<L>::P], int t) {
   using G = FftGeom<L>;
 #pragma unroll
   for (int u = 0; u < G::NB1; u++) {
-    int b1 = t + G::NT * u;
+    int b1 = G::b1_of(t, u);
 #pragma unroll
     for (int n0 = 0; n0 < G::R1; n0++) tw1[u * G::R1 + n0] = unit_root(b1 * n0, L);
   }
 }
+
+// T1 twiddle providers: load16(h, w) returns entries 16h..16h+15 of the thread's tw1[] array.
+template <int L>
+struct Tw1Regs {                                    // kept in registers (template-bank kernel)
+  float2 w[FftGeom<L>::P];
+  __device__ __forceinline__ void load16(int h, float2 (&o)[16]) const {
+#pragma unroll
+    for (int i = 0; i < 16; i++) o[i] = w[16 * h + i];
+  }
+};
+
+// ---- tensor memory as a per-thread register extension (32x32b shape: thread i of warp w <-> TMEM lane 32*(w%4)+i).
+// The load and its wait are ONE asm statement: tcgen05.ld fills its destination registers asynchronously, so the
+// compiler must not be able to move or spill them between the two instructions.
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, float (&r)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];\n\t"
+      "tcgen05.wait::ld.sync.aligned;"
+      : "=f"(r[0]), "=f"(r[1]), "=f"(r[2]), "=f"(r[3]), "=f"(r[4]), "=f"(r[5]), "=f"(r[6]), "=f"(r[7]), "=f"(r[8]), "=f"(r[9]),
+        "=f"(r[10]), "=f"(r[11]), "=f"(r[12]), "=f"(r[13]), "=f"(r[14]), "=f"(r[15]), "=f"(r[16]), "=f"(r[17]), "=f"(r[18]),
+        "=f"(r[19]), "=f"(r[20]), "=f"(r[21]), "=f"(r[22]), "=f"(r[23]), "=f"(r[24]), "=f"(r[25]), "=f"(r[26]), "=f"(r[27]),
+        "=f"(r[28]), "=f"(r[29]), "=f"(r[30]), "=f"(r[31])
+      : "r"(taddr)
+      : "memory");
+}
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const float (&r)[32]) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+      "{%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};\n\t"
+      "tcgen05.wait::st.sync.aligned;"
+      :: "r"(taddr), "f"(r[0]), "f"(r[1]), "f"(r[2]), "f"(r[3]), "f"(r[4]), "f"(r[5]), "f"(r[6]), "f"(r[7]), "f"(r[8]), "f"(r[9]),
+        "f"(r[10]), "f"(r[11]), "f"(r[12]), "f"(r[13]), "f"(r[14]), "f"(r[15]), "f"(r[16]), "f"(r[17]), "f"(r[18]),
+        "f"(r[19]), "f"(r[20]), "f"(r[21]), "f"(r[22]), "f"(r[23]), "f"(r[24]), "f"(r[25]), "f"(r[26]), "f"(r[27]),
+        "f"(r[28]), "f"(r[29]), "f"(r[30]), "f"(r[31])
+      : "memory");
+}
+
+// A thread-private array of P complex values (P = 16 or 32) held in TMEM columns [addr, addr + 2P) of the thread's lane.
+// load16(h, o) / store16(h, o) move entries 16h .. 16h+15.
+template <int L>
+struct TmemArray {
+  uint32_t addr;
+  __device__ __forceinline__ void load16(int h, float2 (&o)[16]) const {
+    float r[32];
+    tmem_ld32(addr + 32 * h, r);
+#pragma unroll
+    for (int i = 0; i < 16; i++) o[i] = make_float2(r[2 * i], r[2 * i + 1]);
+  }
+  __device__ __forceinline__ void store16(int h, const float2 (&o)[16]) const {
+    float r[32];
+#pragma unroll
+    for (int i = 0; i < 16; i++) {
+      r[2 * i] = o[i].x;
+      r[2 * i + 1] = o[i].y;
+    }
+    tmem_st32(addr + 32 * h, r);
+  }
+};
 
 // T2 table (inverse sign) in shared memory: tw2[n1*kTw2Stride + k0] = w_256^{k0*n1}.  It is read in pass 3, where the
 // row n1 = b3 / R1 is uniform over R1 consecutive lanes (broadcast loads); rows are padded to 18 float2 so that the
@@ -175,59 +244,110 @@ __device__ __forceinline__ void fill_tw2(float2* tw2, int t, int nthreads) {
   for (int i = t; i < 256; i += nthreads) tw2[(i >> 4) * kTw2Stride + (i & 15)] = unit_root((i >> 4) * (i & 15), 256);
 }
 
-// Passes 1..3 on the P points in v[].  On entry v[u*R1 + k2] = x[256*k2 + b1], b1 = t + NT*u.
-// On exit v[u3*16 + n2] = X[b3 + 16*R1*n2], b3 = t + NT*u3.  exA/exB: two exchange buffers of L float2 each.
-// tw1: inverse-sign per-thread twiddles (conjugated here when SIGN < 0).  Two barriers (bar id, NT threads).
-template <int L, int SIGN>
-__device__ __forceinline__ void fft_passes(float2 (&v)[FftGeom<L>::P], const float2 (&tw1)[FftGeom<L>::P],
-                                           const float2* __restrict__ tw2, float2* exA, float2* exB, int t) {
+// Shared-memory exchange layouts (float2 index), both conflict-free for 64-bit accesses when GS = 16:
+//   exchange 1 (inside the k0 group): element (k0, n0, k1) at k0*16*R1 + 16*n0 + ((k1 + n0 + GS*k0) & 15)
+//   exchange 2 (across warps):        element (b3, k0)     at 16*b3 + ((k0 + b3) & 15)
+template <int L>
+__device__ __forceinline__ int ex1_index(int k0, int n0, int k1) {
   using G = FftGeom<L>;
-  // ---- pass 1
+  return k0 * (16 * G::R1) + 16 * n0 + ((k1 + n0 + G::GS * k0) & 15);
+}
+__device__ __forceinline__ int ex2_index(int b3, int k0) { return 16 * b3 + ((k0 + b3) & 15); }
+
+// Non-blocking barrier that protects exchange buffer B against the next transform's writes: every thread arrives when
+// its pass-3 loads are done and waits (normally already complete) just before it writes B again.
+struct WarBarrier {
+  uint32_t bar;     // shared-memory address of an mbarrier initialised with count NT
+  uint32_t parity;  // phase the next wait() must see completed
+  __device__ __forceinline__ void arrive() const {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+  }
+  __device__ __forceinline__ void wait() {
+    uint32_t done = 0;
+    while (!done) {
+      asm volatile(
+          "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+          : "=r"(done)
+          : "r"(bar), "r"(parity)
+          : "memory");
+    }
+    parity ^= 1u;
+  }
+};
+
+// Passes 1..3 on the P points in v[].  On entry v[u*R1 + k2] = x[256*k2 + b1_of(t,u)].
+// On exit v[u3*16 + n2] = X[b3_of(t,u3) + 16*R1*n2].  exA/exB: exchange buffers of L float2 each.
+// tw1: inverse-sign per-thread T1 twiddles (conjugated here when SIGN < 0).  One __syncthreads per call; `war` must have
+// been arrived at by every thread after its previous use of exB (the first call after init needs a primed barrier).
+template <int L, int SIGN, class TW1>
+__device__ __forceinline__ void fft_passes(float2 (&v)[FftGeom<L>::P], const TW1& tw1, const float2* __restrict__ tw2,
+                                           float2* exA, float2* exB, WarBarrier& war, int t) {
+  using G = FftGeom<L>;
+  const int k0 = G::k0_of(t);
+  // ---- pass 1: DFT_R1 over k2, twiddle T1, exchange 1 (inside the k0 group); 16 array entries (16/R1 butterflies) at a time
 #pragma unroll
-  for (int u = 0; u < G::NB1; u++) {
-    float2 a[G::R1];
+  for (int h = 0; h < G::P / 16; h++) {
+    constexpr int BPH = 16 / G::R1 > 0 ? 16 / G::R1 : 1;     // butterflies per block of 16 entries (R1 = 32: handled below)
+    if constexpr (G::R1 <= 16) {
 #pragma unroll
-    for (int i = 0; i < G::R1; i++) a[i] = v[u * G::R1 + i];
-    Dft<G::R1, SIGN>::run(a);
-    int b1 = t + G::NT * u;
+      for (int ub = 0; ub < BPH; ub++) {
+        float2 a[G::R1];
 #pragma unroll
-    for (int n0 = 0; n0 < G::R1; n0++) {
-      float2 r = n0 == 0 ? a[0] : (SIGN > 0 ? cmul(a[n0], tw1[u * G::R1 + n0]) : cmul_conj(a[n0], tw1[u * G::R1 + n0]));
-      exA[n0 * 256 + b1] = r;
+        for (int i = 0; i < G::R1; i++) a[i] = v[16 * h + ub * G::R1 + i];
+        Dft<G::R1, SIGN>::run(a);
+#pragma unroll
+        for (int i = 0; i < G::R1; i++) v[16 * h + ub * G::R1 + i] = a[i];
+      }
+    } else if (h == 0) {
+      Dft<G::R1, SIGN>::run(v);                                // R1 = 32 = P: one butterfly over the whole array
+    }
+    float2 w[16];
+    tw1.load16(h, w);
+#pragma unroll
+    for (int i = 0; i < 16; i++) {
+      const int e = 16 * h + i, u = e / G::R1, n0 = e % G::R1;
+      const int k1 = G::n0_of(t, u);   // g + GS*u
+      float2 r = n0 == 0 ? v[e] : (SIGN > 0 ? cmul(v[e], w[i]) : cmul_conj(v[e], w[i]));
+      exA[ex1_index<L>(k0, n0, k1)] = r;
     }
   }
-  __syncthreads();
-  // ---- pass 2
-  const int k0 = t & 15;
+  __syncwarp();
+  // ---- pass 2: DFT_16 over k1, exchange 2
+  float2 b[G::NB2][16];
 #pragma unroll
   for (int u = 0; u < G::NB2; u++) {
-    int b2 = t + G::NT * u;
-    int n0 = b2 >> 4;
-    float2 a[16];
+    const int n0 = G::n0_of(t, u);
 #pragma unroll
-    for (int k1 = 0; k1 < 16; k1++) a[k1] = exA[n0 * 256 + k1 * 16 + k0];
-    Dft<16, SIGN>::run(a);
+    for (int k1 = 0; k1 < 16; k1++) b[u][k1] = exA[ex1_index<L>(k0, n0, k1)];
+  }
+  __syncwarp();                       // exA may be rewritten by this warp's next transform
 #pragma unroll
-    for (int n1 = 0; n1 < 16; n1++) {
-      int b3 = n0 + G::R1 * n1;
-      exB[16 * b3 + ((k0 + b3) & 15)] = a[n1];
-    }
+  for (int u = 0; u < G::NB2; u++) Dft<16, SIGN>::run(b[u]);
+  war.wait();                         // every thread has finished reading exB from the previous transform
+#pragma unroll
+  for (int u = 0; u < G::NB2; u++) {
+    const int n0 = G::n0_of(t, u);
+#pragma unroll
+    for (int n1 = 0; n1 < 16; n1++) exB[ex2_index(n0 + G::R1 * n1, k0)] = b[u][n1];
   }
   __syncthreads();
   // ---- pass 3 (the T2 twiddle w_256^{k0*n1} is applied here, on the read side: its row n1 is lane-uniform)
 #pragma unroll
   for (int u = 0; u < G::NB2; u++) {
-    int b3 = t + G::NT * u;
+    const int b3 = G::b3_of(t, u);
+#pragma unroll
+    for (int q = 0; q < 16; q++) b[u][q] = exB[ex2_index(b3, q)];
+  }
+  war.arrive();
+#pragma unroll
+  for (int u = 0; u < G::NB2; u++) {
+    const int b3 = G::b3_of(t, u);
     const float2* trow = tw2 + (b3 / G::R1) * kTw2Stride;
-    float2 a[16];
 #pragma unroll
-    for (int q = 0; q < 16; q++) {
-      float2 x = exB[16 * b3 + ((q + b3) & 15)];
-      a[q] = q == 0 ? x : (SIGN > 0 ? cmul(x, trow[q]) : cmul_conj(x, trow[q]));
-    }
-    Dft<16, SIGN>::run(a);
+    for (int q = 1; q < 16; q++) b[u][q] = SIGN > 0 ? cmul(b[u][q], trow[q]) : cmul_conj(b[u][q], trow[q]);
+    Dft<16, SIGN>::run(b[u]);
 #pragma unroll
-    for (int n2 = 0; n2 < 16; n2++) v[u * 16 + n2] = a[n2];
+    for (int n2 = 0; n2 < 16; n2++) v[u * 16 + n2] = b[u][n2];
   }
 }
 
