@@ -160,8 +160,8 @@ __global__ void __launch_bounds__(FftGeom<L>::NT) k_bank(BankParams bp) {
   using Gm = FftGeom<L>;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float2* exA = reinterpret_cast<float2*>(smem_raw);
-  float2* exB = exA + L;
-  float2* tw2 = exB + L;
+  float2* exB = exA + Gm::EX1;
+  float2* tw2 = exB + Gm::EX2;
   float2* lat = tw2 + kTw2Floats2;  // 4*hw_max+1 lattice values
   __shared__ unsigned long long s_war;
   const int t = threadIdx.x;
@@ -288,8 +288,8 @@ k_search(SearchParams sp) {
   constexpr int TCOLS = TmemCols<L>::value;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float2* exA = reinterpret_cast<float2*>(smem_raw);
-  float2* exB = exA + L;
-  float2* tw2 = exB + L;
+  float2* exB = exA + Gm::EX1;
+  float2* tw2 = exB + Gm::EX2;
   unsigned long long* mbar = reinterpret_cast<unsigned long long*>(tw2 + kTw2Floats2);  // [0] segment copy, [1] exB WAR
   __shared__ long long s_item;
   __shared__ uint32_t s_tmem;
@@ -543,7 +543,7 @@ __global__ void k_reset(unsigned long long* work, unsigned long long* count) {
 // ------------------------------------------------------------------------------------------------- host helpers
 template <int L, int MODE>
 static size_t search_smem_bytes() {
-  return (size_t)2 * L * sizeof(float2) + kTw2Floats2 * sizeof(float2) + 2 * sizeof(unsigned long long);
+  return (size_t)(FftGeom<L>::EX1 + FftGeom<L>::EX2 + kTw2Floats2) * sizeof(float2) + 2 * sizeof(unsigned long long);
 }
 
 template <int L, int MODE>
@@ -588,7 +588,7 @@ static cudaError_t dispatch_search(const jerk_plan* plan, const SearchParams& sp
 template <int L>
 static cudaError_t launch_bank(const jerk_plan* plan, const BankParams& bp, cudaStream_t st) {
   using Gm = FftGeom<L>;
-  size_t smem = (size_t)2 * L * sizeof(float2) + kTw2Floats2 * sizeof(float2) + (size_t)(4 * plan->hw_max + 1) * sizeof(float2);
+  size_t smem = (size_t)(Gm::EX1 + Gm::EX2 + kTw2Floats2 + 4 * plan->hw_max + 1) * sizeof(float2);
   cudaError_t e = cudaFuncSetAttribute(k_bank<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   k_bank<L><<<plan->T, Gm::NT, smem, st>>>(bp);

@@ -148,12 +148,31 @@ struct FftGeom {
   static constexpr int LOG2L = L == 1024 ? 10 : L == 2048 ? 11 : L == 4096 ? 12 : 13;
   static_assert(L == 1024 || L == 2048 || L == 4096 || L == 8192, "seg_len");
   static_assert(NB2 * GS == R1, "pass-2 butterflies per k0 group");
-  // Thread roles.  Pass 1 and pass 2 of thread t work on the same k0 = t / GS, so exchange 1 stays inside GS consecutive
-  // lanes (GS <= 16: one half-warp) and needs only __syncwarp; exchange 2 crosses warps.
+  // Thread roles.  Pass 1: thread t owns k0 = t / GS and k1 = t % GS + GS*u.  Pass 2 works on the same k0 values inside
+  // the same warp (exchange 1 never leaves the warp: __syncwarp only).  For GS = 16 the two k0 groups of a warp are
+  // interleaved over the lanes in pass 2 (lane l: k0 = 2*warp + (l & 1), n0 = l >> 1), which is what makes the padded
+  // exchange-2 layout conflict-free for 64-bit stores AND 128-bit loads; for GS < 16 the natural mapping already is.
+  static constexpr bool INTERLEAVE = GS == 16;
   static __device__ __forceinline__ int k0_of(int t) { return t / GS; }
   static __device__ __forceinline__ int b1_of(int t, int u) { return 16 * ((t % GS) + GS * u) + t / GS; }   // 16*k1 + k0
-  static __device__ __forceinline__ int n0_of(int t, int u) { return (t % GS) + GS * u; }
+  static __device__ __forceinline__ int k1_of(int t, int u) { return (t % GS) + GS * u; }
+  static __device__ __forceinline__ int k0_p2(int t) { return INTERLEAVE ? 2 * (t >> 5) + (t & 1) : t / GS; }
+  static __device__ __forceinline__ int n0_p2(int t) { return INTERLEAVE ? (t & 31) >> 1 : t % GS; }        // + GS*u
   static __device__ __forceinline__ int b3_of(int t, int u) { return t + NT * u; }                           // n0 + R1*n1
+  // Padded shared-memory exchange layouts (float2 index); every loop-variable term is a compile-time offset, so each
+  // access is base register + immediate.  Constants found by exhaustive bank-conflict search:
+  //   exchange 1: element (k0, n0, k1) at A1*k0 + B1*n0 + k1      (pass 1 stores n0 = 0..R1-1, pass 2 loads k1 = 0..15)
+  //   exchange 2: element (n0 + R1*n1, k0) at B2*n0 + C2*n1 + k0  (pass 2 stores n1 = 0..15, pass 3 loads k0 = 0..15)
+  // Even strides allow 128-bit loads of (k, k+1) pairs.  All four accesses are conflict-free for every L.
+  static constexpr int A1 = L == 1024 ? 68 : L == 2048 ? 152 : L == 4096 ? 280 : 584;
+  static constexpr int B1 = L == 1024 ? 17 : L == 2048 ? 18 : L == 4096 ? 17 : 18;
+  static constexpr int B2 = L == 1024 ? 20 : 18;
+  static constexpr int C2 = L == 1024 ? 78 : L == 2048 ? 142 : L == 4096 ? 286 : 576;
+  static constexpr bool WIDE1 = (A1 % 2 == 0) && (B1 % 2 == 0);
+  static constexpr bool WIDE2 = (B2 % 2 == 0) && (C2 % 2 == 0);
+  static constexpr int EX1 = (A1 * 15 + B1 * (R1 - 1) + 16 + 1) / 2 * 2;    // float2 slots of exchange buffer A (>= L)
+  static constexpr int EX2 = (B2 * (R1 - 1) + C2 * 15 + 16 + 1) / 2 * 2;    // float2 slots of exchange buffer B
+  static_assert(EX1 >= L && EX2 >= L, "exchange buffers double as plain L-point staging arrays");
 };
 
 // exp(2 pi i * num / den), den a power of two, num reduced exactly in integers
@@ -244,16 +263,6 @@ __device__ __forceinline__ void fill_tw2(float2* tw2, int t, int nthreads) {
   for (int i = t; i < 256; i += nthreads) tw2[(i >> 4) * kTw2Stride + (i & 15)] = unit_root((i >> 4) * (i & 15), 256);
 }
 
-// Shared-memory exchange layouts (float2 index), both conflict-free for 64-bit accesses when GS = 16:
-//   exchange 1 (inside the k0 group): element (k0, n0, k1) at k0*16*R1 + 16*n0 + ((k1 + n0 + GS*k0) & 15)
-//   exchange 2 (across warps):        element (b3, k0)     at 16*b3 + ((k0 + b3) & 15)
-template <int L>
-__device__ __forceinline__ int ex1_index(int k0, int n0, int k1) {
-  using G = FftGeom<L>;
-  return k0 * (16 * G::R1) + 16 * n0 + ((k1 + n0 + G::GS * k0) & 15);
-}
-__device__ __forceinline__ int ex2_index(int b3, int k0) { return 16 * b3 + ((k0 + b3) & 15); }
-
 // Non-blocking barrier that protects exchange buffer B against the next transform's writes: every thread arrives when
 // its pass-3 loads are done and waits (normally already complete) just before it writes B again.
 struct WarBarrier {
@@ -276,15 +285,15 @@ struct WarBarrier {
 };
 
 // Passes 1..3 on the P points in v[].  On entry v[u*R1 + k2] = x[256*k2 + b1_of(t,u)].
-// On exit v[u3*16 + n2] = X[b3_of(t,u3) + 16*R1*n2].  exA/exB: exchange buffers of L float2 each.
+// On exit v[u3*16 + n2] = X[b3_of(t,u3) + 16*R1*n2].  exA/exB: exchange buffers of FftGeom::EX1 / EX2 float2.
 // tw1: inverse-sign per-thread T1 twiddles (conjugated here when SIGN < 0).  One __syncthreads per call; `war` must have
 // been arrived at by every thread after its previous use of exB (the first call after init needs a primed barrier).
 template <int L, int SIGN, class TW1>
 __device__ __forceinline__ void fft_passes(float2 (&v)[FftGeom<L>::P], const TW1& tw1, const float2* __restrict__ tw2,
                                            float2* exA, float2* exB, WarBarrier& war, int t) {
   using G = FftGeom<L>;
-  const int k0 = G::k0_of(t);
-  // ---- pass 1: DFT_R1 over k2, twiddle T1, exchange 1 (inside the k0 group); 16 array entries (16/R1 butterflies) at a time
+  // ---- pass 1: DFT_R1 over k2, twiddle T1, exchange 1 (inside the warp); 16 array entries (16/R1 butterflies) at a time
+  float2* const w1 = exA + G::A1 * G::k0_of(t) + (t % G::GS);
 #pragma unroll
   for (int h = 0; h < G::P / 16; h++) {
     constexpr int BPH = 16 / G::R1 > 0 ? 16 / G::R1 : 1;     // butterflies per block of 16 entries (R1 = 32: handled below)
@@ -306,37 +315,60 @@ __device__ __forceinline__ void fft_passes(float2 (&v)[FftGeom<L>::P], const TW1
 #pragma unroll
     for (int i = 0; i < 16; i++) {
       const int e = 16 * h + i, u = e / G::R1, n0 = e % G::R1;
-      const int k1 = G::n0_of(t, u);   // g + GS*u
       float2 r = n0 == 0 ? v[e] : (SIGN > 0 ? cmul(v[e], w[i]) : cmul_conj(v[e], w[i]));
-      exA[ex1_index<L>(k0, n0, k1)] = r;
+      w1[G::B1 * n0 + G::GS * u] = r;                          // element (k0, n0, k1 = t%GS + GS*u)
     }
   }
   __syncwarp();
   // ---- pass 2: DFT_16 over k1, exchange 2
   float2 b[G::NB2][16];
+  const int k0p = G::k0_p2(t), n0p = G::n0_p2(t);
+  {
+    const float2* r1 = exA + G::A1 * k0p + G::B1 * n0p;
 #pragma unroll
-  for (int u = 0; u < G::NB2; u++) {
-    const int n0 = G::n0_of(t, u);
+    for (int u = 0; u < G::NB2; u++) {
+      if constexpr (G::WIDE1) {
 #pragma unroll
-    for (int k1 = 0; k1 < 16; k1++) b[u][k1] = exA[ex1_index<L>(k0, n0, k1)];
+        for (int k1 = 0; k1 < 16; k1 += 2) {
+          const float4 x = *reinterpret_cast<const float4*>(r1 + G::B1 * G::GS * u + k1);
+          b[u][k1] = make_float2(x.x, x.y);
+          b[u][k1 + 1] = make_float2(x.z, x.w);
+        }
+      } else {
+#pragma unroll
+        for (int k1 = 0; k1 < 16; k1++) b[u][k1] = r1[G::B1 * G::GS * u + k1];
+      }
+    }
   }
   __syncwarp();                       // exA may be rewritten by this warp's next transform
 #pragma unroll
   for (int u = 0; u < G::NB2; u++) Dft<16, SIGN>::run(b[u]);
   war.wait();                         // every thread has finished reading exB from the previous transform
+  {
+    float2* w2 = exB + G::B2 * n0p + k0p;
 #pragma unroll
-  for (int u = 0; u < G::NB2; u++) {
-    const int n0 = G::n0_of(t, u);
+    for (int u = 0; u < G::NB2; u++)
 #pragma unroll
-    for (int n1 = 0; n1 < 16; n1++) exB[ex2_index(n0 + G::R1 * n1, k0)] = b[u][n1];
+      for (int n1 = 0; n1 < 16; n1++) w2[G::B2 * G::GS * u + G::C2 * n1] = b[u][n1];   // element (n0 + R1*n1, k0)
   }
   __syncthreads();
   // ---- pass 3 (the T2 twiddle w_256^{k0*n1} is applied here, on the read side: its row n1 is lane-uniform)
+  {
+    const float2* r2 = exB + G::B2 * (t % G::R1) + G::C2 * (t / G::R1);              // b3 = t + NT*u: n0 = t % R1, n1 = t / R1 + (NT/R1)*u
 #pragma unroll
-  for (int u = 0; u < G::NB2; u++) {
-    const int b3 = G::b3_of(t, u);
+    for (int u = 0; u < G::NB2; u++) {
+      if constexpr (G::WIDE2) {
 #pragma unroll
-    for (int q = 0; q < 16; q++) b[u][q] = exB[ex2_index(b3, q)];
+        for (int q = 0; q < 16; q += 2) {
+          const float4 x = *reinterpret_cast<const float4*>(r2 + G::C2 * (G::NT / G::R1) * u + q);
+          b[u][q] = make_float2(x.x, x.y);
+          b[u][q + 1] = make_float2(x.z, x.w);
+        }
+      } else {
+#pragma unroll
+        for (int q = 0; q < 16; q++) b[u][q] = r2[G::C2 * (G::NT / G::R1) * u + q];
+      }
+    }
   }
   war.arrive();
 #pragma unroll
