@@ -147,17 +147,33 @@ int jerk_search_candidates_host(jerk_plan* plan, const void* h_spec, float thres
                                 uint64_t work_bytes, void* stream);
 
 /*
- * jerk_harmonic_sum — optional fused harmonic-sum stage (row a-6; BASELINE.json configs[4]):
+ * jerk_harmonic_sum — fused harmonic-sum stage (row a-6; BASELINE.json configs[4]; section 3):
  * S_h(j,iz',iw') = sum_{k=1..h} P[rnd(j k/h); rnd(iz' k/h), rnd(iw' k/h)] with signed grid indices
  * iz' = iz-(nz-1)/2, iw' = iw-(nw-1)/2 and rnd = round half away from zero (reading S13).
- * For each of nstages stages (h_harm[s] in {1,2,4,8}, thresholds h_thr[s], HOST arrays) d_top[s] receives
- * the arg-max of S_h over the whole grid (position of the top harmonic) if it exceeds the threshold, else
- * {j=-1, power=0}.  d_scratch: DEVICE, >= jerk_harmonic_scratch_bytes(plan).
+ * For each of nstages (1..4) stages (h_harm[s] in {1,2,4,8}, thresholds h_thr[s]; HOST arrays) d_top[s]
+ * (DEVICE, nstages records) receives the arg-max of S_h over the whole (j,iz,iw) grid — the position of the
+ * top harmonic, power = S_h; ties go to the smallest (iw,iz,j) — if it exceeds the threshold, else
+ * {j=-1, iz=0, iw=0, power=0}.  The volume is processed in r-chunks sized to d_scratch: for each chunk the
+ * eight sub-planes of fractions k/8 are recomputed by the fused plane-mode kernel into d_scratch and summed.
+ * d_scratch: DEVICE, 256-byte aligned, >= 1/256 of jerk_harmonic_scratch_bytes(plan) (that size gives the
+ * default 65536-bin chunk; smaller buffers give smaller chunks); d_work as for the search calls.
+ * Asynchronous on `stream`.  Errors: JERK_EINVAL, JERK_ENOMEM, JERK_ESTATE, JERK_ECUDA.
  */
 uint64_t jerk_harmonic_scratch_bytes(const jerk_plan* plan);
 int jerk_harmonic_sum(jerk_plan* plan, const void* d_spec, int nstages, const int* h_harm, const float* h_thr,
                       jerk_cand* d_top, void* d_scratch, uint64_t scratch_bytes, void* d_work,
                       uint64_t work_bytes, void* stream);
+
+/*
+ * jerk_harmonic_plane — plane-output mode of the same stage: writes S_h (h in {1,2,4,8}) for the box
+ * r_lo <= b < r_lo+r_cnt, iz_lo <= iz < iz_lo+iz_cnt, iw_lo <= iw < iw_lo+iw_cnt as
+ * d_out[iw_rel][iz_rel][j - 2*r_lo] (float32, >= jerk_plane_bytes(r_cnt, iz_cnt, iw_cnt)).  The box is handled
+ * as one chunk: JERK_ENOMEM if d_scratch cannot hold its eight sub-planes (a box no larger than the default
+ * chunk always fits in jerk_harmonic_scratch_bytes(plan)).
+ */
+int jerk_harmonic_plane(jerk_plan* plan, const void* d_spec, int h, int64_t r_lo, int64_t r_cnt, int iz_lo,
+                        int iz_cnt, int iw_lo, int iw_cnt, float* d_out, uint64_t out_bytes, void* d_scratch,
+                        uint64_t scratch_bytes, void* d_work, uint64_t work_bytes, void* stream);
 
 const char* jerk_strerror(int status);
 const char* jerk_last_error(const jerk_plan* plan);

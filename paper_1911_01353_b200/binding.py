@@ -40,7 +40,7 @@ class PlanInfo(C.Structure):
 EXPORTS = [
     "jerk_plan_create", "jerk_plan_destroy", "jerk_plan_info", "jerk_template_geometry", "jerk_plane_bytes",
     "jerk_templates", "jerk_templates_taps", "jerk_search_plane", "jerk_search_candidates",
-    "jerk_search_candidates_host", "jerk_harmonic_scratch_bytes", "jerk_harmonic_sum", "jerk_strerror",
+    "jerk_search_candidates_host", "jerk_harmonic_scratch_bytes", "jerk_harmonic_sum", "jerk_harmonic_plane", "jerk_strerror",
     "jerk_last_error",
 ]
 
@@ -71,6 +71,7 @@ def load_library() -> C.CDLL:
     lib.jerk_harmonic_scratch_bytes.argtypes = [vp]
     lib.jerk_harmonic_scratch_bytes.restype = u64
     lib.jerk_harmonic_sum.argtypes = [vp, vp, i32, C.POINTER(i32), C.POINTER(C.c_float), vp, vp, u64, vp, u64, vp]
+    lib.jerk_harmonic_plane.argtypes = [vp, vp, i32, i64, i64, i32, i32, i32, i32, vp, u64, vp, u64, vp, u64, vp]
     lib.jerk_strerror.argtypes = [i32]
     lib.jerk_strerror.restype = C.c_char_p
     lib.jerk_last_error.argtypes = [vp]
@@ -182,6 +183,45 @@ class Plan:
             C.c_void_p(h_count.data_ptr()), C.c_void_p(d_spec.data_ptr()), C.c_void_p(d_cands.data_ptr()),
             C.c_void_p(d_count.data_ptr()), C.c_void_p(work.data_ptr()), work.numel(), _stream_ptr(stream)))
         return int(h_count.item())
+
+    # ---- harmonic stage (row a-6)
+    def harmonic_scratch_bytes(self):
+        return int(self._lib.jerk_harmonic_scratch_bytes(self._h))
+
+    def _ensure_scratch(self, device, nbytes=None):
+        import torch
+        nbytes = self.harmonic_scratch_bytes() if nbytes is None else int(nbytes)
+        if getattr(self, "scratch", None) is None or self.scratch.numel() < nbytes:
+            self.scratch = torch.empty(nbytes, dtype=torch.uint8, device=device)
+        return self.scratch
+
+    def harmonic_sum(self, d_spec, harms=(1, 2, 4, 8), thresholds=(25.0, 35.0, 50.0, 75.0), scratch_bytes=None, stream=None):
+        """jerk_harmonic_sum: returns a structured numpy array (CAND_DTYPE) with one record per stage (synchronises)."""
+        import torch
+        n = len(harms)
+        d_top = torch.zeros(n * 16, dtype=torch.uint8, device=d_spec.device)
+        work = self._ensure_work(d_spec.device)
+        scratch = self._ensure_scratch(d_spec.device, scratch_bytes)
+        nbytes = scratch.numel() if scratch_bytes is None else int(scratch_bytes)
+        self._check(self._lib.jerk_harmonic_sum(
+            self._h, C.c_void_p(d_spec.data_ptr()), n, (C.c_int * n)(*[int(h) for h in harms]),
+            (C.c_float * n)(*[float(t) for t in thresholds]), C.c_void_p(d_top.data_ptr()), C.c_void_p(scratch.data_ptr()),
+            nbytes, C.c_void_p(work.data_ptr()), work.numel(), _stream_ptr(stream)))
+        return d_top.cpu().numpy().view(CAND_DTYPE).copy()
+
+    def harmonic_plane(self, d_spec, h, r_lo, r_cnt, iz_lo=0, iz_cnt=None, iw_lo=0, iw_cnt=None, stream=None):
+        """jerk_harmonic_plane: S_h[iw_cnt][iz_cnt][2*r_cnt] float32 (torch, device) for a box of top-harmonic positions."""
+        import torch
+        iz_cnt = self.info.nz - iz_lo if iz_cnt is None else iz_cnt
+        iw_cnt = self.info.nw - iw_lo if iw_cnt is None else iw_cnt
+        out = torch.empty((iw_cnt, iz_cnt, 2 * r_cnt), dtype=torch.float32, device=d_spec.device)
+        work = self._ensure_work(d_spec.device)
+        scratch = self._ensure_scratch(d_spec.device)
+        self._check(self._lib.jerk_harmonic_plane(
+            self._h, C.c_void_p(d_spec.data_ptr()), int(h), int(r_lo), int(r_cnt), int(iz_lo), int(iz_cnt), int(iw_lo),
+            int(iw_cnt), C.c_void_p(out.data_ptr()), out.numel() * 4, C.c_void_p(scratch.data_ptr()), scratch.numel(),
+            C.c_void_p(work.data_ptr()), work.numel(), _stream_ptr(stream)))
+        return out
 
     def work_counters(self):
         """Diagnostic counters the last search left in d_work (item counter, seam records, seam overflow, provisional)."""

@@ -213,6 +213,19 @@ __global__ void k_taps(double z, double w, int c, int hw, float2* out) {
 }
 
 // ------------------------------------------------------------------------------------------------- search kernel
+// One (r, iz, iw) box of the volume handled by a launch.  Candidate mode has one job (the whole grid); the harmonic
+// stage submits up to eight plane-mode boxes (one per fraction k/8) in a single launch so that small boxes share the GPU.
+struct SearchJob {
+  int64_t seg_first, seg_count;  // segments [seg_first, seg_first+seg_count)
+  int64_t r_lo, r_cnt;           // plane mode: bins [r_lo, r_lo+r_cnt) are written
+  int iz_lo, iz_cnt, iw_lo, iw_cnt;
+  int ntp;                       // template-phases selected = 2*iz_cnt*iw_cnt
+  int chunk_tp;                  // template-phases per work item (even)
+  float* plane;                  // plane mode: P[iw_rel][iz_rel][j - 2*r_lo]
+  long long item_end;            // work items of jobs 0..this one (exclusive prefix sum of nchunks*seg_count)
+};
+constexpr int kMaxJobs = 8;
+
 struct SearchParams {
   const float2* spec;  // X[nbins]
   int64_t nbins;
@@ -221,14 +234,9 @@ struct SearchParams {
   int nz;
   int hw_max, step;
   int64_t seg_base;
-  // work decomposition
-  int64_t seg_first, seg_count;  // segments [seg_first, seg_first+seg_count)
-  int iz_lo, iz_cnt, iw_lo, iw_cnt;
-  int ntp;                       // template-phases selected = 2*iz_cnt*iw_cnt
-  int nchunks;                   // ceil(ntp / kChunkTP)
-  // plane mode
-  float* plane;
-  int64_t r_lo, r_cnt;
+  int njobs;
+  long long nitems;
+  SearchJob jobs[kMaxJobs];
   // candidate mode
   float threshold;
   jerk_cand* cands;
@@ -282,7 +290,7 @@ struct TmemCols {
 
 template <int L, int MODE>
 __global__ void __launch_bounds__(FftGeom<L>::NT, (L == 4096 ? (MODE == MODE_CAND ? JERK_MINBLOCKS_4096 : 2) : 1))
-k_search(SearchParams sp) {
+k_search(const __grid_constant__ SearchParams sp) {
   using Gm = FftGeom<L>;
   constexpr int NT = Gm::NT, P = Gm::P, R1 = Gm::R1;
   constexpr int TCOLS = TmemCols<L>::value;
@@ -323,7 +331,7 @@ k_search(SearchParams sp) {
     }
   }
   uint32_t mphase = 0;
-  const long long nitems = (long long)sp.nchunks * sp.seg_count;
+  const long long nitems = sp.nitems;
   float* gstash = sp.stash + (size_t)blockIdx.x * (2 * L);   // [2][P][NT] powers of the current template (rare path)
 
   for (;;) {
@@ -331,8 +339,15 @@ k_search(SearchParams sp) {
     __syncthreads();
     const long long item = s_item;
     if (item >= nitems) break;
-    const int chunk = (int)(item / sp.seg_count);
-    const int64_t seg = sp.seg_first + item % sp.seg_count;
+    int q = 0;
+    if (MODE == MODE_PLANE) {
+      while (q + 1 < sp.njobs && item >= sp.jobs[q].item_end) q++;
+    }
+    const SearchJob& jb = sp.jobs[q];
+    const long long jitem = item - (q ? sp.jobs[q - 1].item_end : 0LL);
+    const int chunk = (int)(jitem / jb.seg_count);
+    const int64_t seg = jb.seg_first + jitem % jb.seg_count;
+    const int iz_cnt = jb.iz_cnt, iz_lo = jb.iz_lo, iw_lo = jb.iw_lo;
     const int64_t s0 = sp.seg_base + seg * (int64_t)sp.step;  // first bin of the segment (even)
 
     // ---- a-2: stage the segment in shared memory (exA): TMA bulk copy when fully inside the spectrum, guarded loads at the edges
@@ -390,18 +405,18 @@ k_search(SearchParams sp) {
     }
 
     // ---- loop over the template-phases of this chunk
-    const int tp_lo = chunk * kChunkTP;
-    const int tp_hi = min(sp.ntp, tp_lo + kChunkTP);
+    const int tp_lo = chunk * jb.chunk_tp;
+    const int tp_hi = min(jb.ntp, tp_lo + jb.chunk_tp);
     float p0v[P];  // phase-0 powers (plane mode keeps them to store float2 pairs)
     int any0 = 0;  // candidate mode: phase-0 powers of this warp exceeded the threshold and were stashed
-    int izr = (tp_lo >> 1) % sp.iz_cnt, iwr = (tp_lo >> 1) / sp.iz_cnt;
+    int izr = (tp_lo >> 1) % iz_cnt, iwr = (tp_lo >> 1) / iz_cnt;
     for (int tp = tp_lo; tp < tp_hi; tp++) {
       const int ph = tp & 1;
-      if (ph == 0 && tp != tp_lo && ++izr == sp.iz_cnt) {
+      if (ph == 0 && tp != tp_lo && ++izr == iz_cnt) {
         izr = 0;
         ++iwr;
       }
-      const int iz = sp.iz_lo + izr, iw = sp.iw_lo + iwr;
+      const int iz = iz_lo + izr, iw = iw_lo + iwr;
       const int ti = iw * sp.nz + iz;
       const int c = sp.geom[ti].c;
       // ---- a-3: Y = F .* G (G straight from L2/HBM, F from TMEM), inverse FFT
@@ -428,7 +443,7 @@ k_search(SearchParams sp) {
       // valid outputs: n in [n_lo, n_hi) = window [hw_max, hw_max+step) clipped to the bins this call covers
       int n_lo, n_hi;
       {
-        long long blo = MODE == MODE_PLANE ? sp.r_lo : 0, bhi = MODE == MODE_PLANE ? sp.r_lo + sp.r_cnt : sp.nbins;
+        long long blo = MODE == MODE_PLANE ? jb.r_lo : 0, bhi = MODE == MODE_PLANE ? jb.r_lo + jb.r_cnt : sp.nbins;
         long long lo = blo + c - s0, hi = bhi + c - s0;
         n_lo = (int)max((long long)sp.hw_max, min(lo, (long long)L));
         n_hi = (int)min((long long)(sp.hw_max + sp.step), max(hi, 0LL));
@@ -441,8 +456,8 @@ k_search(SearchParams sp) {
 #pragma unroll
           for (int i = 0; i < P; i++) p0v[i] = pw[i];
         } else {
-          float* row = sp.plane + ((size_t)iwr * sp.iz_cnt + izr) * (size_t)(2 * sp.r_cnt);
-          const long long boff = s0 - c - sp.r_lo;
+          float* row = jb.plane + ((size_t)iwr * iz_cnt + izr) * (size_t)(2 * jb.r_cnt);
+          const long long boff = s0 - c - jb.r_lo;
 #pragma unroll
           for (int u = 0; u < Gm::NB2; u++)
 #pragma unroll
@@ -540,6 +555,172 @@ __global__ void k_reset(unsigned long long* work, unsigned long long* count) {
   if (threadIdx.x == 0 && count) *count = 0ULL;
 }
 
+// ------------------------------------------------------------------------------------------------- harmonic stage
+// Row a-6 (BASELINE.json configs[4]; reading S13):  S_h(j,iz',iw') = sum_{k=1..h} P[rnd(j k/h); rnd(iz' k/h), rnd(iw' k/h)]
+// with signed grid indices and rnd = round half away from zero.  Every fraction k/h of h in {1,2,4,8} is e/8, e = 1..8, and
+// the stage sums nest:  S1 = P8;  S2 = S1 + P4;  S4 = S2 + P2 + P6;  S8 = S4 + P1 + P3 + P5 + P7   (Pe = sub-plane of e/8).
+struct HarmSub {           // sub-plane of fraction e/8 for the current box, as written by the plane-mode search kernel
+  const float* base;       // P[iw_rel][iz_rel][j - j0]
+  long long j0, nj;        // first half-bin index stored (even) and row length
+  int iz_lo, iz_cnt, iw_lo;
+};
+struct HarmParams {
+  HarmSub sub[8];          // index e-1
+  long long j_lo, nj;      // top-harmonic box along r, half-bin indices [j_lo, j_lo+nj)
+  int iz_lo, iz_cnt, iw_lo, iw_cnt;
+  int cz, cw;              // centre indices (nz-1)/2, (nw-1)/2
+  int jtile, ntiles;       // half-bin indices per block, blocks per (iz,iw) row
+  jerk_cand* blockbest;    // arg-max mode: [4][nblocks] best of each block for h = 1,2,4,8
+  float* out;              // store mode: S_h of the box, out[iw_rel][iz_rel][j - j_lo]
+  int out_stage;           // store mode: log2(h)
+};
+
+__device__ __forceinline__ int rnd_eighths(int a, int e) {          // round-half-away-from-zero of a*e/8
+  const int m = (abs(a) * e + 4) >> 3;
+  return a < 0 ? -m : m;
+}
+
+// better(a, b): a beats b as the arg-max: larger sum, ties -> smallest (iw, iz, j) in row-major order
+__device__ __forceinline__ bool harm_better(float sa, int ja, int iza, int iwa, float sb, int jb, int izb, int iwb) {
+  if (sa != sb) return sa > sb;
+  if (iwa != iwb) return iwa < iwb;
+  if (iza != izb) return iza < izb;
+  return ja < jb;
+}
+
+template <bool STORE>
+__global__ void __launch_bounds__(256) k_harm(const __grid_constant__ HarmParams hp) {
+  const int tile = blockIdx.x % hp.ntiles;
+  const int row = blockIdx.x / hp.ntiles;
+  const int izr = row % hp.iz_cnt, iwr = row / hp.iz_cnt;
+  const int iz = hp.iz_lo + izr, iw = hp.iw_lo + iwr;
+  const int az = iz - hp.cz, aw = iw - hp.cw;
+  const float* rp[8];
+#pragma unroll
+  for (int e = 1; e <= 8; e++) {
+    const HarmSub& sb = hp.sub[e - 1];
+    const int ize = rnd_eighths(az, e) + hp.cz, iwe = rnd_eighths(aw, e) + hp.cw;
+    rp[e - 1] = sb.base + ((long long)(iwe - sb.iw_lo) * sb.iz_cnt + (ize - sb.iz_lo)) * sb.nj - sb.j0;
+  }
+  const long long jb = hp.j_lo + (long long)tile * hp.jtile;
+  const long long je = min(hp.j_lo + hp.nj, jb + hp.jtile);
+  float best[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+  int bj[4] = {-1, -1, -1, -1};
+  float* orow = STORE ? hp.out + ((long long)iwr * hp.iz_cnt + izr) * hp.nj - hp.j_lo : nullptr;
+  for (long long j = jb + threadIdx.x; j < je; j += 256) {
+    float pe[8];
+#pragma unroll
+    for (int e = 1; e <= 8; e++) pe[e - 1] = __ldg(rp[e - 1] + ((j * e + 4) >> 3));
+    float sv[4];
+    sv[0] = pe[7];
+    sv[1] = sv[0] + pe[3];
+    sv[2] = sv[1] + pe[1] + pe[5];
+    sv[3] = sv[2] + pe[0] + pe[2] + pe[4] + pe[6];
+    if (STORE) {
+      orow[j] = sv[hp.out_stage];
+    } else {
+#pragma unroll
+      for (int q = 0; q < 4; q++)
+        if (sv[q] > best[q]) {        // j increases per thread: strict > keeps the smallest j among equals
+          best[q] = sv[q];
+          bj[q] = (int)j;
+        }
+    }
+  }
+  if (STORE) return;
+  __shared__ float s_best[4][8];
+  __shared__ int s_bj[4][8];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int q = 0; q < 4; q++) {
+    float b = best[q];
+    int jj = bj[q];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      const float ob = __shfl_xor_sync(0xffffffffu, b, o);
+      const int oj = __shfl_xor_sync(0xffffffffu, jj, o);
+      if (oj >= 0 && (jj < 0 || ob > b || (ob == b && oj < jj))) {
+        b = ob;
+        jj = oj;
+      }
+    }
+    if (lane == 0) {
+      s_best[q][warp] = b;
+      s_bj[q][warp] = jj;
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x < 4) {
+    const int q = threadIdx.x;
+    float b = s_best[q][0];
+    int jj = s_bj[q][0];
+    for (int w = 1; w < 8; w++) {
+      const float ob = s_best[q][w];
+      const int oj = s_bj[q][w];
+      if (oj >= 0 && (jj < 0 || ob > b || (ob == b && oj < jj))) {
+        b = ob;
+        jj = oj;
+      }
+    }
+    jerk_cand c;
+    c.j = jj;
+    c.iz = (int16_t)iz;
+    c.iw = (int16_t)iw;
+    c.power = b;
+    c.flags = 0;
+    hp.blockbest[(size_t)q * gridDim.x + blockIdx.x] = c;
+  }
+}
+
+// Folds the per-block bests of one box into the running per-stage arg-max (running[4]); one block of 256 threads.
+__global__ void __launch_bounds__(256) k_harm_fold(const jerk_cand* blockbest, int nblocks, jerk_cand* running, int first) {
+  __shared__ jerk_cand s_c[256];
+  for (int q = 0; q < 4; q++) {
+    jerk_cand b;
+    b.j = -1;
+    b.iz = b.iw = 0;
+    b.power = -INFINITY;
+    b.flags = 0;
+    for (int i = threadIdx.x; i < nblocks; i += 256) {
+      const jerk_cand c = blockbest[(size_t)q * nblocks + i];
+      if (c.j >= 0 && (b.j < 0 || harm_better(c.power, c.j, c.iz, c.iw, b.power, b.j, b.iz, b.iw))) b = c;
+    }
+    s_c[threadIdx.x] = b;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+      if (threadIdx.x < o) {
+        const jerk_cand c = s_c[threadIdx.x + o], m = s_c[threadIdx.x];
+        if (c.j >= 0 && (m.j < 0 || harm_better(c.power, c.j, c.iz, c.iw, m.power, m.j, m.iz, m.iw))) s_c[threadIdx.x] = c;
+      }
+      __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+      const jerk_cand c = s_c[0], m = running[q];
+      if (first || (c.j >= 0 && (m.j < 0 || harm_better(c.power, c.j, c.iz, c.iw, m.power, m.j, m.iz, m.iw)))) running[q] = c;
+    }
+    __syncthreads();
+  }
+}
+
+// d_top[s] = running[log2 h_s] if its sum exceeds the stage threshold, else {j = -1, power = 0}
+struct HarmEmit {
+  int nstages;
+  int stage[4];
+  float thr[4];
+};
+__global__ void k_harm_emit(const jerk_cand* running, jerk_cand* top, HarmEmit he) {
+  const int s = threadIdx.x;
+  if (s >= he.nstages) return;
+  jerk_cand c = running[he.stage[s]];
+  if (!(c.j >= 0 && c.power > he.thr[s])) {
+    c.j = -1;
+    c.iz = c.iw = 0;
+    c.power = 0.f;
+  }
+  c.flags = 0;
+  top[s] = c;
+}
+
 // ------------------------------------------------------------------------------------------------- host helpers
 template <int L, int MODE>
 static size_t search_smem_bytes() {
@@ -565,7 +746,7 @@ static cudaError_t launch_search(const jerk_plan* plan, const SearchParams& sp, 
   occ = std::min(occ, 512 / TmemCols<L>::value);
   if (getenv("JERK_DEBUG")) fprintf(stderr, "[jerk] k_search<%d,%d>: %d regs, smem %zu B, %d CTAs/SM\n", L, MODE, fa.numRegs, smem, occ);
   if (occ < 1) occ = 1;
-  long long nitems = (long long)sp.nchunks * sp.seg_count;
+  long long nitems = sp.nitems;
   long long grid = (long long)plan->sm_count * occ;
   if (grid > kMaxCtas) grid = kMaxCtas;
   if (grid > nitems) grid = nitems;
@@ -612,6 +793,47 @@ static void fill_params(const jerk_plan* plan, SearchParams& sp, const void* d_s
   sp.work = (unsigned long long*)d_work;
   sp.seams = (jerk_cand*)((unsigned char*)d_work + kWorkHeader);
   sp.stash = (float*)((unsigned char*)d_work + kWorkHeader + (uint64_t)kSeamCap * sizeof(jerk_cand));
+}
+
+// Appends the box (r, iz, iw) as a job of `sp`.  Returns false when the box is empty (nothing appended).
+// Segments whose outputs b = s0 + n - c (n in [hw_max, hw_max+step), |c| <= c_max) can touch [r_lo, r_lo+r_cnt) are selected.
+static bool add_job(const jerk_plan* p, SearchParams& sp, int64_t r_lo, int64_t r_cnt, int iz_lo, int iz_cnt, int iw_lo,
+                    int iw_cnt, float* plane, int chunk_tp) {
+  if (r_cnt <= 0 || iz_cnt <= 0 || iw_cnt <= 0 || sp.njobs >= kMaxJobs) return false;
+  int64_t lo = r_lo - p->c_max - p->seg_base - p->hw_max - p->step + 1;  // s*step >= lo
+  int64_t hi = r_lo + r_cnt - 1 + p->c_max - p->seg_base - p->hw_max;    // s*step <= hi
+  int64_t s_first = lo <= 0 ? 0 : (lo + p->step - 1) / p->step;
+  int64_t s_last = hi < 0 ? -1 : hi / p->step;
+  if (s_last > p->nseg - 1) s_last = p->nseg - 1;
+  if (s_last < s_first) return false;
+  SearchJob& jb = sp.jobs[sp.njobs];
+  jb.seg_first = s_first;
+  jb.seg_count = s_last - s_first + 1;
+  jb.r_lo = r_lo;
+  jb.r_cnt = r_cnt;
+  jb.iz_lo = iz_lo;
+  jb.iz_cnt = iz_cnt;
+  jb.iw_lo = iw_lo;
+  jb.iw_cnt = iw_cnt;
+  jb.ntp = 2 * iz_cnt * iw_cnt;
+  jb.chunk_tp = chunk_tp;
+  jb.plane = plane;
+  long long nchunks = (jb.ntp + chunk_tp - 1) / chunk_tp;
+  sp.nitems += nchunks * jb.seg_count;
+  jb.item_end = sp.nitems;
+  sp.njobs++;
+  return true;
+}
+
+// template-phases per work item: kChunkTP when the box is large; smaller (even, >= 16) when the box alone could not
+// give every resident CTA a few items
+static int pick_chunk_tp(const jerk_plan* p, int64_t r_cnt, int iz_cnt, int iw_cnt) {
+  long long ntp = 2LL * iz_cnt * iw_cnt;
+  long long segs = r_cnt / p->step + 2;
+  long long want_items = 4LL * kMaxCtas;
+  int c = kChunkTP;
+  while (c > 16 && ((ntp + c - 1) / c) * segs < want_items) c >>= 1;
+  return c;
 }
 
 }  // namespace jerk
@@ -811,24 +1033,7 @@ int jerk_search_plane(jerk_plan* p, const void* d_spec, int64_t r_lo, int64_t r_
   cudaStream_t st = (cudaStream_t)stream;
   SearchParams sp;
   fill_params(p, sp, d_spec, d_work);
-  sp.iz_lo = iz_lo;
-  sp.iz_cnt = iz_cnt;
-  sp.iw_lo = iw_lo;
-  sp.iw_cnt = iw_cnt;
-  sp.ntp = 2 * iz_cnt * iw_cnt;
-  sp.nchunks = (sp.ntp + kChunkTP - 1) / kChunkTP;
-  sp.plane = d_plane;
-  sp.r_lo = r_lo;
-  sp.r_cnt = r_cnt;
-  // segments whose outputs b = s0 + n - c (n in [hw_max, hw_max+step), |c| <= c_max) can touch [r_lo, r_lo+r_cnt)
-  int64_t lo = r_lo - p->c_max - p->seg_base - p->hw_max - p->step + 1;  // s*step >= lo
-  int64_t hi = r_lo + r_cnt - 1 + p->c_max - p->seg_base - p->hw_max;    // s*step <= hi
-  int64_t s_first = lo <= 0 ? 0 : (lo + p->step - 1) / p->step;
-  int64_t s_last = hi < 0 ? -1 : hi / p->step;
-  if (s_last > p->nseg - 1) s_last = p->nseg - 1;
-  if (s_last < s_first) return JERK_OK;
-  sp.seg_first = s_first;
-  sp.seg_count = s_last - s_first + 1;
+  if (!add_job(p, sp, r_lo, r_cnt, iz_lo, iz_cnt, iw_lo, iw_cnt, d_plane, pick_chunk_tp(p, r_cnt, iz_cnt, iw_cnt))) return JERK_OK;
   k_reset<<<1, 32, 0, st>>>(sp.work, nullptr);
   cudaError_t e = dispatch_search<MODE_PLANE>(p, sp, st);
   if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_search(plane) launch: ") + cudaGetErrorString(e));
@@ -843,14 +1048,7 @@ int jerk_search_candidates(jerk_plan* p, const void* d_spec, float threshold, je
   cudaStream_t st = (cudaStream_t)stream;
   SearchParams sp;
   fill_params(p, sp, d_spec, d_work);
-  sp.iz_lo = 0;
-  sp.iz_cnt = p->nz;
-  sp.iw_lo = 0;
-  sp.iw_cnt = p->nw;
-  sp.ntp = 2 * p->T;
-  sp.nchunks = (sp.ntp + kChunkTP - 1) / kChunkTP;
-  sp.seg_first = 0;
-  sp.seg_count = p->nseg;
+  add_job(p, sp, 0, p->nbins, 0, p->nz, 0, p->nw, nullptr, kChunkTP);
   sp.threshold = threshold;
   sp.cands = d_cands;
   sp.max_cands = max_cands;
@@ -886,16 +1084,192 @@ int jerk_search_candidates_host(jerk_plan* p, const void* h_spec, float threshol
   return JERK_OK;
 }
 
-uint64_t jerk_harmonic_scratch_bytes(const jerk_plan* plan) {
-  (void)plan;
-  return 0;
+// ---- harmonic stage (row a-6)
+}  // extern "C" (reopened below)
+
+namespace jerk {
+
+constexpr int64_t kHarmChunkBins = 1 << 16;   // default r-chunk of the top-harmonic axis
+constexpr int kHarmJTile = 8192;              // half-bin indices per k_harm block
+constexpr uint64_t kHarmHeader = 256;         // running[4] arg-max records
+
+struct HarmBox {
+  int64_t r_lo, r_cnt;
+  int iz_lo, iz_cnt, iw_lo, iw_cnt;
+};
+struct HarmSubBox {       // source box of fraction e/8
+  int64_t r_lo, r_cnt;
+  int iz_lo, iz_cnt, iw_lo, iw_cnt;
+  uint64_t offset, bytes;  // inside the scratch buffer
+};
+
+static int host_rnd_eighths(int a, int e) {
+  int m = (abs(a) * e + 4) >> 3;
+  return a < 0 ? -m : m;
+}
+
+// Source boxes of the eight fractions for a top-harmonic box (all index maps are monotone, so boxes map to boxes),
+// their placement in scratch after the header, the per-block arg-max records, and the total bytes needed.
+static uint64_t harm_layout(const jerk_plan* p, const HarmBox& bx, HarmSubBox (&sub)[8], uint64_t* blockbest_off, int* nblocks,
+                            int* ntiles) {
+  const int cz = (p->nz - 1) / 2, cw = (p->nw - 1) / 2;
+  const int64_t j_lo = 2 * bx.r_lo, j_hi = 2 * (bx.r_lo + bx.r_cnt) - 1;   // inclusive
+  uint64_t off = kHarmHeader;
+  for (int e = 1; e <= 8; e++) {
+    HarmSubBox& sb = sub[e - 1];
+    const int64_t js_lo = (j_lo * e + 4) >> 3, js_hi = (j_hi * e + 4) >> 3;
+    sb.r_lo = js_lo >> 1;
+    sb.r_cnt = (js_hi >> 1) - sb.r_lo + 1;
+    sb.iz_lo = host_rnd_eighths(bx.iz_lo - cz, e) + cz;
+    sb.iz_cnt = host_rnd_eighths(bx.iz_lo + bx.iz_cnt - 1 - cz, e) + cz - sb.iz_lo + 1;
+    sb.iw_lo = host_rnd_eighths(bx.iw_lo - cw, e) + cw;
+    sb.iw_cnt = host_rnd_eighths(bx.iw_lo + bx.iw_cnt - 1 - cw, e) + cw - sb.iw_lo + 1;
+    sb.offset = off;
+    sb.bytes = align_up((uint64_t)sb.iw_cnt * sb.iz_cnt * (uint64_t)(2 * sb.r_cnt) * sizeof(float), 256);
+    off += sb.bytes;
+  }
+  *ntiles = (int)((2 * bx.r_cnt + kHarmJTile - 1) / kHarmJTile);
+  *nblocks = bx.iw_cnt * bx.iz_cnt * *ntiles;
+  *blockbest_off = off;
+  off += align_up((uint64_t)4 * *nblocks * sizeof(jerk_cand), 256);
+  return off;
+}
+
+// Sub-planes of one box (one plane-mode launch with eight jobs), then k_harm in arg-max or store mode.
+static int harm_box(jerk_plan* p, const void* d_spec, const HarmBox& bx, unsigned char* scratch, uint64_t scratch_bytes,
+                    void* d_work, float* d_out, int out_stage, bool first, cudaStream_t st) {
+  HarmSubBox sub[8];
+  uint64_t bb_off;
+  int nblocks, ntiles;
+  if (harm_layout(p, bx, sub, &bb_off, &nblocks, &ntiles) > scratch_bytes)
+    return fail(p, JERK_ENOMEM, "harmonic scratch buffer too small for this box");
+  SearchParams sp;
+  fill_params(p, sp, d_spec, d_work);
+  HarmParams hp;
+  memset(&hp, 0, sizeof(hp));
+  for (int e = 1; e <= 8; e++) {
+    const HarmSubBox& sb = sub[e - 1];
+    float* plane = (float*)(scratch + sb.offset);
+    if (!add_job(p, sp, sb.r_lo, sb.r_cnt, sb.iz_lo, sb.iz_cnt, sb.iw_lo, sb.iw_cnt, plane, kChunkTP))
+      return fail(p, JERK_EINVAL, "harmonic stage: empty sub-box");
+    hp.sub[e - 1].base = plane;
+    hp.sub[e - 1].j0 = 2 * sb.r_lo;
+    hp.sub[e - 1].nj = 2 * sb.r_cnt;
+    hp.sub[e - 1].iz_lo = sb.iz_lo;
+    hp.sub[e - 1].iz_cnt = sb.iz_cnt;
+    hp.sub[e - 1].iw_lo = sb.iw_lo;
+  }
+  // small boxes: shrink the work items until every resident CTA gets a few
+  while (sp.nitems < 4LL * kMaxCtas && sp.jobs[0].chunk_tp > 16) {
+    sp.nitems = 0;
+    for (int q = 0; q < sp.njobs; q++) {
+      SearchJob& jb = sp.jobs[q];
+      jb.chunk_tp >>= 1;
+      sp.nitems += (long long)((jb.ntp + jb.chunk_tp - 1) / jb.chunk_tp) * jb.seg_count;
+      jb.item_end = sp.nitems;
+    }
+  }
+  k_reset<<<1, 32, 0, st>>>(sp.work, nullptr);
+  cudaError_t e = dispatch_search<MODE_PLANE>(p, sp, st);
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_search(harmonic sub-planes) launch: ") + cudaGetErrorString(e));
+  hp.j_lo = 2 * bx.r_lo;
+  hp.nj = 2 * bx.r_cnt;
+  hp.iz_lo = bx.iz_lo;
+  hp.iz_cnt = bx.iz_cnt;
+  hp.iw_lo = bx.iw_lo;
+  hp.iw_cnt = bx.iw_cnt;
+  hp.cz = (p->nz - 1) / 2;
+  hp.cw = (p->nw - 1) / 2;
+  hp.jtile = kHarmJTile;
+  hp.ntiles = ntiles;
+  hp.blockbest = (jerk_cand*)(scratch + bb_off);
+  hp.out = d_out;
+  hp.out_stage = out_stage;
+  if (d_out) {
+    k_harm<true><<<nblocks, 256, 0, st>>>(hp);
+  } else {
+    k_harm<false><<<nblocks, 256, 0, st>>>(hp);
+    k_harm_fold<<<1, 256, 0, st>>>(hp.blockbest, nblocks, (jerk_cand*)scratch, first ? 1 : 0);
+  }
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_harm launch: ") + cudaGetErrorString(e));
+  return JERK_OK;
+}
+
+static int stage_of(int h) { return h == 1 ? 0 : h == 2 ? 1 : h == 4 ? 2 : h == 8 ? 3 : -1; }
+
+// largest r-chunk (bins) of the full (iz, iw) grid whose scratch fits in `bytes` (0 if not even one 256-bin chunk fits)
+static int64_t harm_chunk_for(const jerk_plan* p, uint64_t bytes) {
+  int64_t c = std::min<int64_t>(p->nbins, kHarmChunkBins);
+  for (;;) {
+    // rounding can add a source bin per fraction depending on r_lo: size for a box 16 bins longer
+    HarmBox bx{0, c + 16, 0, p->nz, 0, p->nw};
+    HarmSubBox sub[8];
+    uint64_t bb;
+    int nb, nt;
+    if (harm_layout(p, bx, sub, &bb, &nb, &nt) <= bytes) return c;
+    if (c <= 256) return 0;
+    c = (c + 1) / 2;
+  }
+}
+
+}  // namespace jerk
+
+extern "C" {
+
+uint64_t jerk_harmonic_scratch_bytes(const jerk_plan* p) {
+  if (!p) return 0;
+  HarmBox bx{0, std::min<int64_t>(p->nbins, kHarmChunkBins) + 16, 0, p->nz, 0, p->nw};   // +16: see harm_chunk_for
+  HarmSubBox sub[8];
+  uint64_t bb;
+  int nb, nt;
+  return harm_layout(p, bx, sub, &bb, &nb, &nt);
 }
 
 int jerk_harmonic_sum(jerk_plan* p, const void* d_spec, int nstages, const int* h_harm, const float* h_thr, jerk_cand* d_top,
                       void* d_scratch, uint64_t scratch_bytes, void* d_work, uint64_t work_bytes, void* stream) {
-  (void)d_spec; (void)nstages; (void)h_harm; (void)h_thr; (void)d_top; (void)d_scratch; (void)scratch_bytes;
-  (void)d_work; (void)work_bytes; (void)stream;
-  return fail(p, JERK_EINVAL, "jerk_harmonic_sum: not built yet (SURVEY.md 8(a) row a-6)");
+  int rc = check_common(p, d_spec, d_work, work_bytes);
+  if (rc) return rc;
+  if (nstages < 1 || nstages > 4 || !h_harm || !h_thr || !d_top || !d_scratch) return JERK_EINVAL;
+  if ((uintptr_t)d_scratch % 256) return fail(p, JERK_EINVAL, "d_scratch must be 256-byte aligned");
+  HarmEmit he;
+  he.nstages = nstages;
+  for (int s = 0; s < nstages; s++) {
+    he.stage[s] = stage_of(h_harm[s]);
+    he.thr[s] = h_thr[s];
+    if (he.stage[s] < 0) return fail(p, JERK_EINVAL, "harmonic stages must be 1, 2, 4 or 8");
+  }
+  const int64_t chunk = harm_chunk_for(p, scratch_bytes);
+  if (chunk == 0) return fail(p, JERK_ENOMEM, "harmonic scratch buffer too small (see jerk_harmonic_scratch_bytes)");
+  cudaStream_t st = (cudaStream_t)stream;
+  bool first = true;
+  for (int64_t r_lo = 0; r_lo < p->nbins; r_lo += chunk) {
+    HarmBox bx{r_lo, std::min<int64_t>(chunk, p->nbins - r_lo), 0, p->nz, 0, p->nw};
+    rc = harm_box(p, d_spec, bx, (unsigned char*)d_scratch, scratch_bytes, d_work, nullptr, 0, first, st);
+    if (rc) return rc;
+    first = false;
+  }
+  k_harm_emit<<<1, 32, 0, st>>>((const jerk_cand*)d_scratch, d_top, he);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_harm_emit launch: ") + cudaGetErrorString(e));
+  return JERK_OK;
+}
+
+int jerk_harmonic_plane(jerk_plan* p, const void* d_spec, int h, int64_t r_lo, int64_t r_cnt, int iz_lo, int iz_cnt, int iw_lo,
+                        int iw_cnt, float* d_out, uint64_t out_bytes, void* d_scratch, uint64_t scratch_bytes, void* d_work,
+                        uint64_t work_bytes, void* stream) {
+  int rc = check_common(p, d_spec, d_work, work_bytes);
+  if (rc) return rc;
+  if (stage_of(h) < 0) return fail(p, JERK_EINVAL, "h must be 1, 2, 4 or 8");
+  if (r_lo < 0 || r_cnt < 0 || r_lo + r_cnt > p->nbins || iz_lo < 0 || iz_cnt < 0 || iz_lo + iz_cnt > p->nz || iw_lo < 0 ||
+      iw_cnt < 0 || iw_lo + iw_cnt > p->nw)
+    return fail(p, JERK_EINVAL, "harmonic plane sub-range outside the plan's grid");
+  if (out_bytes < jerk_plane_bytes(r_cnt, iz_cnt, iw_cnt)) return fail(p, JERK_ENOMEM, "harmonic plane buffer too small");
+  if (r_cnt == 0 || iz_cnt == 0 || iw_cnt == 0) return JERK_OK;
+  if (!d_out || !d_scratch) return JERK_EINVAL;
+  if ((uintptr_t)d_scratch % 256) return fail(p, JERK_EINVAL, "d_scratch must be 256-byte aligned");
+  HarmBox bx{r_lo, r_cnt, iz_lo, iz_cnt, iw_lo, iw_cnt};
+  return harm_box(p, d_spec, bx, (unsigned char*)d_scratch, scratch_bytes, d_work, d_out, stage_of(h), true, (cudaStream_t)stream);
 }
 
 }  // extern "C"
