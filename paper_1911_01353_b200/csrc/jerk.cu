@@ -162,7 +162,7 @@ __global__ void __launch_bounds__(FftGeom<L>::NT) k_bank(BankParams bp) {
   float2* exA = reinterpret_cast<float2*>(smem_raw);
   float2* exB = exA + Gm::EX1;
   float2* tw2 = exB + Gm::EX2;
-  float2* lat = tw2 + kTw2Floats2;  // 4*hw_max+1 lattice values
+  float2* lat = tw2 + Tw2Table<L>::FLOATS2;  // 4*hw_max+1 lattice values
   __shared__ unsigned long long s_war;
   const int t = threadIdx.x;
   const int ti = blockIdx.x;
@@ -171,9 +171,9 @@ __global__ void __launch_bounds__(FftGeom<L>::NT) k_bank(BankParams bp) {
   const TemplateGeom g = bp.geom[ti];
   const int panels = quad_panels(z, w, g.c, g.hw);
   for (int i = t; i < 4 * g.hw + 1; i += Gm::NT) lat[i] = response_quadrature(z, w, (double)(g.c - g.hw) + 0.5 * i, panels);
-  fill_tw2(tw2, t, Gm::NT);
-  Tw1Regs<L> tw1;
-  make_tw1<L>(tw1.w, t);
+  fill_tw2<L>(tw2, t, Gm::NT);
+  Tw3Regs<L> tw1;
+  make_tw3<L>(tw1.w, t);
   WarBarrier war = war_init<Gm::NT>(&s_war, t);
   for (int p = 0; p < 2; p++) {
     // taps h~_p[m'] = R(c + m' - p/2) at index (m' mod L): lattice index i = 2*(m'+hw) - p
@@ -298,7 +298,7 @@ k_search(const __grid_constant__ SearchParams sp) {
   float2* exA = reinterpret_cast<float2*>(smem_raw);
   float2* exB = exA + Gm::EX1;
   float2* tw2 = exB + Gm::EX2;
-  unsigned long long* mbar = reinterpret_cast<unsigned long long*>(tw2 + kTw2Floats2);  // [0] segment copy, [1] exB WAR
+  unsigned long long* mbar = reinterpret_cast<unsigned long long*>(tw2 + Tw2Table<L>::FLOATS2);  // [0] segment copy, [1] exB WAR
   __shared__ long long s_item;
   __shared__ uint32_t s_tmem;
   const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
@@ -308,7 +308,7 @@ k_search(const __grid_constant__ SearchParams sp) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&s_tmem)), "n"(TCOLS));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
-  fill_tw2(tw2, t, NT);
+  fill_tw2<L>(tw2, t, NT);
   if (t == 0) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(mbar)));
   }
@@ -321,7 +321,7 @@ k_search(const __grid_constant__ SearchParams sp) {
   tmT.addr = tbase + TCOLS / 2;
   {
     float2 w[P];
-    make_tw1<L>(w, t);
+    make_tw3<L>(w, t);
 #pragma unroll
     for (int h = 0; h < P / 16; h++) {
       float2 q[16];
@@ -724,7 +724,7 @@ __global__ void k_harm_emit(const jerk_cand* running, jerk_cand* top, HarmEmit h
 // ------------------------------------------------------------------------------------------------- host helpers
 template <int L, int MODE>
 static size_t search_smem_bytes() {
-  return (size_t)(FftGeom<L>::EX1 + FftGeom<L>::EX2 + kTw2Floats2) * sizeof(float2) + 2 * sizeof(unsigned long long);
+  return (size_t)(FftGeom<L>::EX1 + FftGeom<L>::EX2 + Tw2Table<L>::FLOATS2) * sizeof(float2) + 2 * sizeof(unsigned long long);
 }
 
 template <int L, int MODE>
@@ -769,7 +769,7 @@ static cudaError_t dispatch_search(const jerk_plan* plan, const SearchParams& sp
 template <int L>
 static cudaError_t launch_bank(const jerk_plan* plan, const BankParams& bp, cudaStream_t st) {
   using Gm = FftGeom<L>;
-  size_t smem = (size_t)(Gm::EX1 + Gm::EX2 + kTw2Floats2 + 4 * plan->hw_max + 1) * sizeof(float2);
+  size_t smem = (size_t)(Gm::EX1 + Gm::EX2 + Tw2Table<L>::FLOATS2 + 4 * plan->hw_max + 1) * sizeof(float2);
   cudaError_t e = cudaFuncSetAttribute(k_bank<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   k_bank<L><<<plan->T, Gm::NT, smem, st>>>(bp);

@@ -125,10 +125,97 @@ template <int SIGN>
 struct Dft<8, SIGN> {
   static __device__ __forceinline__ void run(float2 (&x)[8]) { dft_pq<2, 4, SIGN>(x); }
 };
+// ---- DFT_16 = 4 x 4 with every twiddle absorbed into fused multiply-adds.
+// A twiddle w = c + i s applied to v is written c * (v + t * (i v)), t = s / c (one FFMA2), and the factor c is applied by
+// the FFMA2 that adds the result to its butterfly partner; when both partners carry a factor, one is divided out
+// (c_b / c_a) and c_a is applied one level later.  A twiddled radix-4 butterfly costs 11 packed instructions instead of 14.
+__device__ __forceinline__ float2 cneg(float2 a) { return make_float2(-a.x, -a.y); }
+__device__ __forceinline__ float2 fma_s(float2 a, float s, float2 c) { return __ffma2_rn(a, bc(s), c); }   // a*s + c
+
+constexpr float kC1 = 0.92387953251128675613f;   // cos(pi/8)
+constexpr float kC2 = 0.70710678118654752440f;   // cos(pi/4)
+constexpr float kC3 = 0.38268343236508977173f;   // cos(3pi/8)
+constexpr float kT1 = 0.41421356237309504880f;   // tan(pi/8) = cos(3pi/8)/cos(pi/8)
+constexpr float kT3 = 2.41421356237309504880f;   // tan(3pi/8) = cos(pi/8)/cos(3pi/8)
+
+// second half of a radix-4 butterfly whose odd half (t2, t3) still carries the real factor c:
+//   o0 = t0 + c t2, o2 = t0 - c t2, o1 = t1 + c (SIGN i) t3, o3 = t1 - c (SIGN i) t3
+template <int SIGN>
+__device__ __forceinline__ void bfly4_tail(float2 t0, float2 t1, float2 t2, float2 t3, float c, float2& o0, float2& o1,
+                                           float2& o2, float2& o3) {
+  const float2 r3 = rot90<SIGN>(t3);
+  o0 = fma_s(t2, c, t0);
+  o2 = fma_s(cneg(t2), c, t0);
+  o1 = fma_s(r3, c, t1);
+  o3 = fma_s(cneg(r3), c, t1);
+}
+
+// Second layer of DFT_16: column k1 holds v[n2] = x[4 k1 + n2]; out X[k1 + 4 k2] = sum_n2 v[n2] w16^{n2 k1} i^{SIGN n2 k2}
+template <int SIGN>
+__device__ __forceinline__ void dft16_layerB(float2 (&x)[16]) {
+  float2 y[16];
+  {  // k1 = 0: plain radix-4
+    float2 t[4] = {x[0], x[1], x[2], x[3]};
+    Dft<4, SIGN>::run(t);
+    y[0] = t[0]; y[4] = t[1]; y[8] = t[2]; y[12] = t[3];
+  }
+  {  // k1 = 1: twiddles w16^1, w16^2, w16^3
+    const float2 v0 = x[4], v1 = x[5], v2 = x[6], v3 = x[7];
+    const float2 u2 = cadd(v2, rot90<SIGN>(v2));
+    const float2 t0 = fma_s(u2, kC2, v0), t1 = fma_s(cneg(u2), kC2, v0);
+    const float2 u1 = fma_s(rot90<SIGN>(v1), kT1, v1), u3 = fma_s(rot90<SIGN>(v3), kT3, v3);
+    const float2 t2 = fma_s(u3, kT1, u1), t3 = fma_s(cneg(u3), kT1, u1);           // c3/c1 = tan(pi/8)
+    bfly4_tail<SIGN>(t0, t1, t2, t3, kC1, y[1], y[5], y[9], y[13]);
+  }
+  {  // k1 = 2: twiddles w16^2, w16^4 = SIGN i, w16^6 = c2 (-1 + SIGN i)
+    const float2 v0 = x[8], v1 = x[9], v2 = x[10], v3 = x[11];
+    const float2 r2 = rot90<SIGN>(v2);
+    const float2 t0 = cadd(v0, r2), t1 = csub(v0, r2);
+    const float2 u1 = cadd(v1, rot90<SIGN>(v1)), u3 = csub(rot90<SIGN>(v3), v3);
+    const float2 t2 = cadd(u1, u3), t3 = csub(u1, u3);
+    bfly4_tail<SIGN>(t0, t1, t2, t3, kC2, y[2], y[6], y[10], y[14]);
+  }
+  {  // k1 = 3: twiddles w16^3, w16^6, w16^9 = -c1 (1 + SIGN i tan(pi/8))
+    const float2 v0 = x[12], v1 = x[13], v2 = x[14], v3 = x[15];
+    const float2 u2 = csub(rot90<SIGN>(v2), v2);
+    const float2 t0 = fma_s(u2, kC2, v0), t1 = fma_s(cneg(u2), kC2, v0);
+    const float2 u1 = fma_s(rot90<SIGN>(v1), kT3, v1), u3 = fma_s(rot90<SIGN>(v3), kT1, v3);
+    const float2 t2 = fma_s(cneg(u3), kT3, u1), t3 = fma_s(u3, kT3, u1);           // -c1/c3 = -tan(3pi/8)
+    bfly4_tail<SIGN>(t0, t1, t2, t3, kC3, y[3], y[7], y[11], y[15]);
+  }
+#pragma unroll
+  for (int i = 0; i < 16; i++) x[i] = y[i];
+}
+
 template <int SIGN>
 struct Dft<16, SIGN> {
-  static __device__ __forceinline__ void run(float2 (&x)[16]) { dft_pq<4, 4, SIGN>(x); }
+  static __device__ __forceinline__ void run(float2 (&x)[16]) {
+#pragma unroll
+    for (int n2 = 0; n2 < 4; n2++) {          // first layer: radix-4 over n1 on x[4 n1 + n2], result k1 left at x[4 k1 + n2]
+      float2 t[4] = {x[n2], x[4 + n2], x[8 + n2], x[12 + n2]};
+      Dft<4, SIGN>::run(t);
+      x[n2] = t[0]; x[4 + n2] = t[1]; x[8 + n2] = t[2]; x[12 + n2] = t[3];
+    }
+    dft16_layerB<SIGN>(x);
+  }
 };
+
+// First layer of a DFT_16 whose inputs carry the twiddles w_q (q = 4 n1 + n2), for one n2.  The four twiddles arrive in
+// "mixed form" (tw_mixed below), in the order n1 = 0..3:
+//   w[0] = (c, s)            full complex multiply (skipped when n2 == 0: w_0 = 1)
+//   w[1] = (c_a, t_a)        q = 4+n2      t = s/c
+//   w[2] = (c_b, t_b)        q = 8+n2
+//   w[3] = (c_d / c_a, t_d)  q = 12+n2
+// 13 packed instructions (11 for n2 = 0) against 16 for multiply-then-butterfly.  SIGN = -1 conjugates the twiddles.
+template <int SIGN, bool FIRST_TRIVIAL>
+__device__ __forceinline__ void dft16_layerA_tw(float2& x0, float2& x1, float2& x2, float2& x3, const float2 (&w)[4]) {
+  const float2 a0 = FIRST_TRIVIAL ? x0 : (SIGN > 0 ? cmul(x0, w[0]) : cmul_conj(x0, w[0]));
+  const float2 u2 = fma_s(rot90<SIGN>(x2), w[2].y, x2);
+  const float2 t0 = fma_s(u2, w[2].x, a0), t1 = fma_s(cneg(u2), w[2].x, a0);
+  const float2 u1 = fma_s(rot90<SIGN>(x1), w[1].y, x1), u3 = fma_s(rot90<SIGN>(x3), w[3].y, x3);
+  const float2 t2 = fma_s(u3, w[3].x, u1), t3 = fma_s(cneg(u3), w[3].x, u1);
+  bfly4_tail<SIGN>(t0, t1, t2, t3, w[1].x, x0, x1, x2, x3);
+}
 template <int SIGN>
 struct Dft<32, SIGN> {
   static __device__ __forceinline__ void run(float2 (&x)[32]) { dft_pq<2, 16, SIGN>(x); }
@@ -183,25 +270,37 @@ __device__ __forceinline__ float2 unit_root(int num, int den) {
   return make_float2(c, s);
 }
 
-// Per-thread T1 twiddles for the INVERSE transform: tw1[u*R1 + n0] = w_L^{b1*n0}, b1 = b1_of(t, u).
-template <int L>
-__device__ __forceinline__ void make_tw1(float2 (&tw1)[FftGeom<L>::P], int t) {
-  using G = FftGeom<L>;
-#pragma unroll
-  for (int u = 0; u < G::NB1; u++) {
-    int b1 = G::b1_of(t, u);
-#pragma unroll
-    for (int n0 = 0; n0 < G::R1; n0++) tw1[u * G::R1 + n0] = unit_root(b1 * n0, L);
-  }
+// Mixed-form twiddle (see dft16_layerA_tw) at table position pos = 4*n2 + n1 for the 16 input twiddles
+// w_q = exp(2 pi i * e * q / den), q = 4*n1 + n2, of one DFT_16 (inverse sign).  An exactly vanishing cosine (quarter
+// turns) is replaced by 1e-9: c * (v + (s/c) i v) then equals i s v up to 1e-9 |v|, far below fp32 rounding.
+__device__ __forceinline__ float tw_cos_safe(float c) { return c == 0.0f ? 1e-9f : c; }
+__device__ __forceinline__ float2 tw_mixed(int pos, int e, int den) {
+  const int n1 = pos & 3, q = 4 * n1 + (pos >> 2);
+  const float2 w = unit_root(e * q, den);
+  if (n1 == 0) return w;
+  const float c = tw_cos_safe(w.x);
+  const float t = w.y / c;
+  if (n1 == 3) return make_float2(c / tw_cos_safe(unit_root(e * (q - 8), den).x), t);
+  return make_float2(c, t);
 }
 
-// T1 twiddle providers: load16(h, w) returns entries 16h..16h+15 of the thread's tw1[] array.
+// Per-thread pass-3 twiddles (inverse sign): tw3[16*u + pos] = mixed form of w_L^{k0 * b3_of(t,u)}, k0 = q(pos).
 template <int L>
-struct Tw1Regs {                                    // kept in registers (template-bank kernel)
-  float2 w[FftGeom<L>::P];
-  __device__ __forceinline__ void load16(int h, float2 (&o)[16]) const {
+__device__ __forceinline__ void make_tw3(float2 (&tw3)[FftGeom<L>::P], int t) {
+  using G = FftGeom<L>;
 #pragma unroll
-    for (int i = 0; i < 16; i++) o[i] = w[16 * h + i];
+  for (int u = 0; u < G::NB2; u++)
+#pragma unroll
+    for (int pos = 0; pos < 16; pos++) tw3[16 * u + pos] = tw_mixed(pos, G::b3_of(t, u), L);
+}
+
+// Pass-3 twiddle providers: load8(i, w) returns entries 8i..8i+7 of the thread's tw3[] array.
+template <int L>
+struct Tw3Regs {                                    // kept in registers (template-bank kernel)
+  float2 w[FftGeom<L>::P];
+  __device__ __forceinline__ void load8(int i, float2 (&o)[8]) const {
+#pragma unroll
+    for (int k = 0; k < 8; k++) o[k] = w[8 * i + k];
   }
 };
 
@@ -232,11 +331,27 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const float (&r)[32]) 
       : "memory");
 }
 
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&r)[16]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];\n\t"
+      "tcgen05.wait::ld.sync.aligned;"
+      : "=f"(r[0]), "=f"(r[1]), "=f"(r[2]), "=f"(r[3]), "=f"(r[4]), "=f"(r[5]), "=f"(r[6]), "=f"(r[7]), "=f"(r[8]), "=f"(r[9]),
+        "=f"(r[10]), "=f"(r[11]), "=f"(r[12]), "=f"(r[13]), "=f"(r[14]), "=f"(r[15])
+      : "r"(taddr)
+      : "memory");
+}
+
 // A thread-private array of P complex values (P = 16 or 32) held in TMEM columns [addr, addr + 2P) of the thread's lane.
-// load16(h, o) / store16(h, o) move entries 16h .. 16h+15.
+// load16(h, o) / store16(h, o) move entries 16h .. 16h+15; load8(i, o) entries 8i .. 8i+7.
 template <int L>
 struct TmemArray {
   uint32_t addr;
+  __device__ __forceinline__ void load8(int i, float2 (&o)[8]) const {
+    float r[16];
+    tmem_ld16(addr + 16 * i, r);
+#pragma unroll
+    for (int k = 0; k < 8; k++) o[k] = make_float2(r[2 * k], r[2 * k + 1]);
+  }
   __device__ __forceinline__ void load16(int h, float2 (&o)[16]) const {
     float r[32];
     tmem_ld32(addr + 32 * h, r);
@@ -258,9 +373,17 @@ struct TmemArray {
 // row n1 = b3 / R1 is uniform over R1 consecutive lanes (broadcast loads); rows are padded to 18 float2 so that the
 // rows touched by one 128-bit load instruction fall in different banks.
 constexpr int kTw2Stride = 18;
-constexpr int kTw2Floats2 = 16 * kTw2Stride;
+// Pass-2 table (inverse sign) in shared memory: row n0 (R1 rows, padded to 18 float2) holds the 16 mixed-form input
+// twiddles w_{16 R1}^{k1 n0} of the pass-2 DFT_16 over k1, in position order (pos = 4*n2 + n1, k1 = 4*n1 + n2).  The rows
+// read by the 8 lanes of one 128-bit load phase are 4 (or 8) consecutive n0: bank group 4*n0 + const, conflict-free.
+template <int L>
+struct Tw2Table {
+  static constexpr int FLOATS2 = FftGeom<L>::R1 * kTw2Stride;
+};
+template <int L>
 __device__ __forceinline__ void fill_tw2(float2* tw2, int t, int nthreads) {
-  for (int i = t; i < 256; i += nthreads) tw2[(i >> 4) * kTw2Stride + (i & 15)] = unit_root((i >> 4) * (i & 15), 256);
+  for (int i = t; i < 16 * FftGeom<L>::R1; i += nthreads)
+    tw2[(i >> 4) * kTw2Stride + (i & 15)] = tw_mixed(i & 15, i >> 4, 16 * FftGeom<L>::R1);
 }
 
 // Non-blocking barrier that protects exchange buffer B against the next transform's writes: every thread arrives when
@@ -286,41 +409,29 @@ struct WarBarrier {
 
 // Passes 1..3 on the P points in v[].  On entry v[u*R1 + k2] = x[256*k2 + b1_of(t,u)].
 // On exit v[u3*16 + n2] = X[b3_of(t,u3) + 16*R1*n2].  exA/exB: exchange buffers of FftGeom::EX1 / EX2 float2.
-// tw1: inverse-sign per-thread T1 twiddles (conjugated here when SIGN < 0).  One __syncthreads per call; `war` must have
-// been arrived at by every thread after its previous use of exB (the first call after init needs a primed barrier).
-template <int L, int SIGN, class TW1>
-__device__ __forceinline__ void fft_passes(float2 (&v)[FftGeom<L>::P], const TW1& tw1, const float2* __restrict__ tw2,
+// All twiddles sit on the input side of a DFT_16 (decimation in time) so that they fold into its first layer:
+//   pass 1: DFT_R1 over k2, no twiddle;
+//   pass 2: input twiddle w_{16 R1}^{k1 n0} (shared-memory table tw2, row n0), DFT_16 over k1;
+//   pass 3: input twiddle w_L^{k0 b3} (per-thread table tw3: tensor memory or registers), DFT_16 over k0.
+// Tables hold the inverse-sign twiddles; SIGN < 0 conjugates them on the fly.  One __syncthreads per call; `war` must
+// have been arrived at by every thread after its previous use of exB (the first call after init needs a primed barrier).
+template <int L, int SIGN, class TW3>
+__device__ __forceinline__ void fft_passes(float2 (&v)[FftGeom<L>::P], const TW3& tw3, const float2* __restrict__ tw2,
                                            float2* exA, float2* exB, WarBarrier& war, int t) {
   using G = FftGeom<L>;
-  // ---- pass 1: DFT_R1 over k2, twiddle T1, exchange 1 (inside the warp); 16 array entries (16/R1 butterflies) at a time
+  // ---- pass 1: DFT_R1 over k2, exchange 1 (inside the warp)
   float2* const w1 = exA + G::A1 * G::k0_of(t) + (t % G::GS);
 #pragma unroll
-  for (int h = 0; h < G::P / 16; h++) {
-    constexpr int BPH = 16 / G::R1 > 0 ? 16 / G::R1 : 1;     // butterflies per block of 16 entries (R1 = 32: handled below)
-    if constexpr (G::R1 <= 16) {
+  for (int u = 0; u < G::NB1; u++) {
+    float2 a[G::R1];
 #pragma unroll
-      for (int ub = 0; ub < BPH; ub++) {
-        float2 a[G::R1];
+    for (int i = 0; i < G::R1; i++) a[i] = v[u * G::R1 + i];
+    Dft<G::R1, SIGN>::run(a);
 #pragma unroll
-        for (int i = 0; i < G::R1; i++) a[i] = v[16 * h + ub * G::R1 + i];
-        Dft<G::R1, SIGN>::run(a);
-#pragma unroll
-        for (int i = 0; i < G::R1; i++) v[16 * h + ub * G::R1 + i] = a[i];
-      }
-    } else if (h == 0) {
-      Dft<G::R1, SIGN>::run(v);                                // R1 = 32 = P: one butterfly over the whole array
-    }
-    float2 w[16];
-    tw1.load16(h, w);
-#pragma unroll
-    for (int i = 0; i < 16; i++) {
-      const int e = 16 * h + i, u = e / G::R1, n0 = e % G::R1;
-      float2 r = n0 == 0 ? v[e] : (SIGN > 0 ? cmul(v[e], w[i]) : cmul_conj(v[e], w[i]));
-      w1[G::B1 * n0 + G::GS * u] = r;                          // element (k0, n0, k1 = t%GS + GS*u)
-    }
+    for (int n0 = 0; n0 < G::R1; n0++) w1[G::B1 * n0 + G::GS * u] = a[n0];   // element (k0, n0, k1 = t%GS + GS*u)
   }
   __syncwarp();
-  // ---- pass 2: DFT_16 over k1, exchange 2
+  // ---- pass 2: twiddle + DFT_16 over k1, exchange 2
   float2 b[G::NB2][16];
   const int k0p = G::k0_p2(t), n0p = G::n0_p2(t);
   {
@@ -342,7 +453,17 @@ __device__ __forceinline__ void fft_passes(float2 (&v)[FftGeom<L>::P], const TW1
   }
   __syncwarp();                       // exA may be rewritten by this warp's next transform
 #pragma unroll
-  for (int u = 0; u < G::NB2; u++) Dft<16, SIGN>::run(b[u]);
+  for (int u = 0; u < G::NB2; u++) {
+    const float4* trow = reinterpret_cast<const float4*>(tw2 + (n0p + G::GS * u) * kTw2Stride);
+#pragma unroll
+    for (int n2 = 0; n2 < 4; n2++) {
+      const float4 wa = trow[2 * n2], wb = trow[2 * n2 + 1];
+      const float2 w[4] = {make_float2(wa.x, wa.y), make_float2(wa.z, wa.w), make_float2(wb.x, wb.y), make_float2(wb.z, wb.w)};
+      if (n2 == 0) dft16_layerA_tw<SIGN, true>(b[u][0], b[u][4], b[u][8], b[u][12], w);
+      else dft16_layerA_tw<SIGN, false>(b[u][n2], b[u][4 + n2], b[u][8 + n2], b[u][12 + n2], w);
+    }
+    dft16_layerB<SIGN>(b[u]);
+  }
   war.wait();                         // every thread has finished reading exB from the previous transform
   {
     float2* w2 = exB + G::B2 * n0p + k0p;
@@ -352,7 +473,7 @@ __device__ __forceinline__ void fft_passes(float2 (&v)[FftGeom<L>::P], const TW1
       for (int n1 = 0; n1 < 16; n1++) w2[G::B2 * G::GS * u + G::C2 * n1] = b[u][n1];   // element (n0 + R1*n1, k0)
   }
   __syncthreads();
-  // ---- pass 3 (the T2 twiddle w_256^{k0*n1} is applied here, on the read side: its row n1 is lane-uniform)
+  // ---- pass 3: twiddle + DFT_16 over k0
   {
     const float2* r2 = exB + G::B2 * (t % G::R1) + G::C2 * (t / G::R1);              // b3 = t + NT*u: n0 = t % R1, n1 = t / R1 + (NT/R1)*u
 #pragma unroll
@@ -373,11 +494,19 @@ __device__ __forceinline__ void fft_passes(float2 (&v)[FftGeom<L>::P], const TW1
   war.arrive();
 #pragma unroll
   for (int u = 0; u < G::NB2; u++) {
-    const int b3 = G::b3_of(t, u);
-    const float2* trow = tw2 + (b3 / G::R1) * kTw2Stride;
 #pragma unroll
-    for (int q = 1; q < 16; q++) b[u][q] = SIGN > 0 ? cmul(b[u][q], trow[q]) : cmul_conj(b[u][q], trow[q]);
-    Dft<16, SIGN>::run(b[u]);
+    for (int half = 0; half < 2; half++) {
+      float2 w8[8];
+      tw3.load8(2 * u + half, w8);
+#pragma unroll
+      for (int m = 0; m < 2; m++) {
+        const int n2 = 2 * half + m;
+        const float2 w[4] = {w8[4 * m], w8[4 * m + 1], w8[4 * m + 2], w8[4 * m + 3]};
+        if (n2 == 0) dft16_layerA_tw<SIGN, true>(b[u][0], b[u][4], b[u][8], b[u][12], w);
+        else dft16_layerA_tw<SIGN, false>(b[u][n2], b[u][4 + n2], b[u][8 + n2], b[u][12 + n2], w);
+      }
+    }
+    dft16_layerB<SIGN>(b[u]);
 #pragma unroll
     for (int n2 = 0; n2 < 16; n2++) v[u * 16 + n2] = b[u][n2];
   }
