@@ -18,6 +18,7 @@
 
 #include "../../include/jerk.h"
 #include "jerk_fft.cuh"
+#include "jerk_fft64.cuh"
 
 namespace jerk {
 
@@ -136,6 +137,14 @@ __device__ __forceinline__ int bank_slot(int k) {
   int k1 = b1 >> 4, k0 = b1 & 15;
   int u = k1 / Gm::GS, t = k0 * Gm::GS + (k1 % Gm::GS);
   return (((u * (Gm::R1 / 2) + (k2 >> 1)) * Gm::NT + t) << 1) + (k2 & 1);
+}
+
+// seg_len 4096 is searched by k_search64 (64 threads x 64 points per FFT): thread t reads float4 #(e*64 + t), which holds
+// elements k = 64*k1 + t for k1 = 2e, 2e+1
+template <>
+__device__ __forceinline__ int bank_slot<4096>(int k) {
+  const int k1 = k >> 6, t = k & 63;
+  return ((((k1 >> 1) << 6) + t) << 1) + (k1 & 1);
 }
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -524,6 +533,227 @@ k_search(const __grid_constant__ SearchParams sp) {
   if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(s_tmem), "n"(TCOLS));
 }
 
+// ------------------------------------------------------------------------------------------------- search kernel, seg_len 4096
+// k_search64: the same fused path (rows a-2..a-5) on the two-pass 64 x 64 FFT of jerk_fft64.cuh.  A CTA holds two
+// independent FFT groups of 64 threads (two warps each); every group takes its own work items from the global counter,
+// has its own exchange buffer, named barrier and mbarriers, and shares only the CTA's tensor-memory allocation:
+// F (the transformed segment, 64 complex per thread) in columns [0,128) and the pass-2 twiddles in [128,256) of the
+// thread's own TMEM lane.  Two CTAs per SM (TMEM 2 x 256 columns, up to 255 registers per thread).
+template <int MODE>
+__global__ void __launch_bounds__(128, 2) k_search64(const __grid_constant__ SearchParams sp) {
+  constexpr int L = 4096, NT = 64, P = 64;
+  constexpr int TCOLS = 256;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  float2* ex_all = reinterpret_cast<float2*>(smem_raw);
+  unsigned long long* mbar_all = reinterpret_cast<unsigned long long*>(ex_all + 2 * kEx64);  // [group][0] segment copy, [group][1] ex WAR
+  __shared__ long long s_item[2];
+  __shared__ uint32_t s_tmem;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, grp = warp >> 1, t = threadIdx.x & 63;
+  float2* ex = ex_all + grp * kEx64;
+  unsigned long long* mbar = mbar_all + 2 * grp;
+  const int barid = 1 + grp;
+
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&s_tmem)), "n"(TCOLS));
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+  }
+  if (t == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(mbar)));
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(mbar + 1)), "r"(NT));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;");
+  WarBarrier war;
+  war.bar = smem_u32(mbar + 1);
+  war.parity = 0;
+  war.arrive();
+  const uint32_t tbase = s_tmem + ((uint32_t)(warp * 32) << 16);
+  TmemArray<L> tmF, tmT;
+  tmF.addr = tbase;
+  tmT.addr = tbase + 128;
+#pragma unroll
+  for (int h = 0; h < 4; h++) {
+    float2 w[16];
+#pragma unroll
+    for (int i = 0; i < 16; i++) w[i] = tw64_mixed(16 * h + i, t);
+    tmT.store16(h, w);
+  }
+  uint32_t mphase = 0;
+  const long long nitems = sp.nitems;
+  float* gstash = sp.stash + ((size_t)blockIdx.x * 2 + grp) * (2 * L);   // [2][P][NT] powers of the current template (rare path)
+
+  for (;;) {
+    if (t == 0) s_item[grp] = (long long)atomicAdd(sp.work, 1ULL);
+    bar_sync_named(barid, NT);
+    const long long item = s_item[grp];
+    if (item >= nitems) break;
+    int q = 0;
+    if (MODE == MODE_PLANE) {
+      while (q + 1 < sp.njobs && item >= sp.jobs[q].item_end) q++;
+    }
+    const SearchJob& jb = sp.jobs[q];
+    const long long jitem = item - (q ? sp.jobs[q - 1].item_end : 0LL);
+    const int chunk = (int)(jitem / jb.seg_count);
+    const int64_t seg = jb.seg_first + jitem % jb.seg_count;
+    const int iz_cnt = jb.iz_cnt, iz_lo = jb.iz_lo, iw_lo = jb.iw_lo;
+    const int64_t s0 = sp.seg_base + seg * (int64_t)sp.step;  // first bin of the segment (even)
+
+    // ---- a-2: stage the segment in the exchange buffer: TMA bulk copy when fully inside the spectrum, guarded loads at the edges
+    const bool interior = (s0 >= 0) && (s0 + L <= sp.nbins);
+    if (interior) {
+      if (t == 0) {
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(mbar)), "r"((uint32_t)(L * 8)) : "memory");
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(ex)),
+                     "l"(sp.spec + s0), "r"((uint32_t)(L * 8)), "r"(smem_u32(mbar))
+                     : "memory");
+      }
+      uint32_t done = 0;
+      while (!done) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done)
+            : "r"(smem_u32(mbar)), "r"(mphase)
+            : "memory");
+      }
+      mphase ^= 1u;
+    } else {
+      for (int k = t; k < L; k += NT) {
+        int64_t b = s0 + k;
+        ex[k] = (b >= 0 && b < sp.nbins) ? sp.spec[b] : make_float2(0.f, 0.f);
+      }
+      bar_sync_named(barid, NT);
+    }
+    // ---- forward FFT; F goes to TMEM in the pass-1 layout: array index k1 holds F[64*k1 + t]
+    {
+      float2 v[P];
+#pragma unroll
+      for (int k1 = 0; k1 < 64; k1++) v[k1] = ex[64 * k1 + t];
+      bar_sync_named(barid, NT);                         // ex is about to be reused as the exchange buffer
+      fft64_passes<-1>(v, tmT, ex, war, t, barid);
+      bar_sync_named(barid, NT);                         // all pass-2 loads of ex done
+#pragma unroll
+      for (int r = 0; r < 64; r++) ex[t + 64 * dft64_out_index(r)] = v[r];
+      bar_sync_named(barid, NT);
+#pragma unroll
+      for (int h = 0; h < 4; h++) {
+        float2 fq[16];
+#pragma unroll
+        for (int i = 0; i < 16; i++) fq[i] = ex[64 * (16 * h + i) + t];
+        tmF.store16(h, fq);
+      }
+      bar_sync_named(barid, NT);
+    }
+
+    // ---- loop over the template-phases of this chunk
+    const int tp_lo = chunk * jb.chunk_tp;
+    const int tp_hi = min(jb.ntp, tp_lo + jb.chunk_tp);
+    int any0 = 0;  // candidate mode: phase-0 powers of this warp exceeded the threshold and were stashed
+    int izr = (tp_lo >> 1) % iz_cnt, iwr = (tp_lo >> 1) / iz_cnt;
+    for (int tp = tp_lo; tp < tp_hi; tp++) {
+      const int ph = tp & 1;
+      if (ph == 0 && tp != tp_lo && ++izr == iz_cnt) {
+        izr = 0;
+        ++iwr;
+      }
+      const int iz = iz_lo + izr, iw = iw_lo + iwr;
+      const int ti = iw * sp.nz + iz;
+      const int c = sp.geom[ti].c;
+      // ---- a-3: Y = F .* G (G straight from L2/HBM, F from TMEM), inverse FFT
+      float2 v[P];
+      __syncwarp();   // tcgen05.ld is .sync.aligned: the warp must be converged
+      {
+        const float4* g4 = reinterpret_cast<const float4*>(sp.G + ((size_t)ti * 2 + ph) * L) + t;
+        float4 g[P / 2];
+#pragma unroll
+        for (int e = 0; e < P / 2; e++) g[e] = __ldg(g4 + e * NT);
+#pragma unroll
+        for (int h = 0; h < 4; h++) {
+          float2 fq[16];
+          tmF.load16(h, fq);
+#pragma unroll
+          for (int i = 0; i < 8; i++) {
+            v[16 * h + 2 * i] = cmul(fq[2 * i], make_float2(g[8 * h + i].x, g[8 * h + i].y));
+            v[16 * h + 2 * i + 1] = cmul(fq[2 * i + 1], make_float2(g[8 * h + i].z, g[8 * h + i].w));
+          }
+        }
+      }
+      fft64_passes<1>(v, tmT, ex, war, t, barid);
+      // ---- a-4: overlap discard + power.  n = t + 64*n1 ; b = s0 + n - c ; j = 2b + ph.
+      int n_lo, n_hi;
+      {
+        long long blo = MODE == MODE_PLANE ? jb.r_lo : 0, bhi = MODE == MODE_PLANE ? jb.r_lo + jb.r_cnt : sp.nbins;
+        long long lo = blo + c - s0, hi = bhi + c - s0;
+        n_lo = (int)max((long long)sp.hw_max, min(lo, (long long)L));
+        n_hi = (int)min((long long)(sp.hw_max + sp.step), max(hi, 0LL));
+      }
+      float pw[P];
+#pragma unroll
+      for (int i = 0; i < P; i++) pw[i] = fmaf(v[i].x, v[i].x, v[i].y * v[i].y);
+      if (MODE == MODE_PLANE) {
+        float* row = jb.plane + ((size_t)iwr * iz_cnt + izr) * (size_t)(2 * jb.r_cnt) + ph;
+        const long long boff = s0 - c - jb.r_lo;
+#pragma unroll
+        for (int r = 0; r < P; r++) {
+          const int n = t + 64 * dft64_out_index(r);
+          if (n >= n_lo && n < n_hi) row[2 * (boff + n)] = pw[r];
+        }
+      } else {
+        // ---- a-5: threshold + local max.  Hot path: one max-reduction and a vote.
+        float mx = pw[0];
+#pragma unroll
+        for (int i = 1; i < P; i++) mx = fmaxf(mx, pw[i]);
+        const int anyhit = __any_sync(0xffffffffu, mx > sp.threshold);
+        float* st0 = gstash;            // [P][NT]: register i of thread t at i*NT + t (written and read by the same thread)
+        float* st1 = gstash + L;
+        if (ph == 0) {
+          any0 = anyhit;
+          if (anyhit) {
+#pragma unroll
+            for (int i = 0; i < P; i++) st0[i * NT + t] = pw[i];
+          }
+        } else if (anyhit | any0) {
+#pragma unroll
+          for (int i = 0; i < P; i++) st1[i * NT + t] = pw[i];
+          __syncwarp();
+          const float NEG = -INFINITY;
+#pragma unroll 1
+          for (int i = 0; i < P; i++) {
+            const int n = t + 64 * dft64_out_index(i);
+            const bool valid = (n >= n_lo) && (n < n_hi);
+            const float p1 = valid ? st1[i * NT + t] : NEG;
+            const float p0 = (valid && any0) ? st0[i * NT + t] : NEG;
+            const float l1 = __shfl_up_sync(0xffffffffu, p1, 1);    // P1[n-1]
+            const float r0 = __shfl_down_sync(0xffffffffu, p0, 1);  // P0[n+1]
+            if (!valid) continue;
+            const long long b = s0 + n - c;
+            if (p0 > sp.threshold) {
+              const bool seamL = (lane == 0 || n == sp.hw_max) && (b > 0);
+              const float left = (b > 0 && !seamL) ? l1 : NEG;
+              const bool okR = p0 >= p1;
+              if (seamL) emit_seam(sp, (int)(2 * b), iz, iw, p0, SEAM_LEFT | (okR ? 0u : SEAM_WITNESS));
+              else if (p0 > left && okR) emit_cand(sp, (int)(2 * b), iz, iw, p0);
+            }
+            if (p1 > sp.threshold) {
+              const bool seamR = (lane == 31 || n == sp.hw_max + sp.step - 1) && (b < sp.nbins - 1);
+              const float right = (b < sp.nbins - 1 && !seamR) ? r0 : NEG;
+              const bool okL = p1 > p0;
+              if (seamR) emit_seam(sp, (int)(2 * b + 1), iz, iw, p1, SEAM_RIGHT | (okL ? 0u : SEAM_WITNESS));
+              else if (okL && p1 >= right) emit_cand(sp, (int)(2 * b + 1), iz, iw, p1);
+            }
+          }
+          __syncwarp();
+        }
+      }
+    }
+    bar_sync_named(barid, NT);
+  }
+  __syncthreads();
+  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(s_tmem), "n"(TCOLS));
+}
+
 // Seam records: every above-threshold point whose left (phase 0) or right (phase 1) neighbour belongs to another
 // warp or segment.  A seam point is a candidate iff it passed its own-side test and no seam record at the missing
 // neighbour position beats it (a neighbour that emitted nothing is <= threshold < this power).
@@ -756,11 +986,30 @@ static cudaError_t launch_search(const jerk_plan* plan, const SearchParams& sp, 
 }
 
 template <int MODE>
+static cudaError_t launch_search64(const jerk_plan* plan, const SearchParams& sp, cudaStream_t st) {
+  const size_t smem = (size_t)2 * kEx64 * sizeof(float2) + 4 * sizeof(unsigned long long);
+  cudaError_t e = cudaFuncSetAttribute(k_search64<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  if (getenv("JERK_DEBUG")) {
+    cudaFuncAttributes fa;
+    if (cudaFuncGetAttributes(&fa, k_search64<MODE>) == cudaSuccess)
+      fprintf(stderr, "[jerk] k_search64<%d>: %d regs, %zu B local, smem %zu B\n", MODE, fa.numRegs, (size_t)fa.localSizeBytes, smem);
+  }
+  // two CTAs per SM (tensor memory: 2 x 256 columns), two FFT groups per CTA, one work item per group at a time
+  long long grid = (long long)plan->sm_count * 2;
+  if (2 * grid > kMaxCtas) grid = kMaxCtas / 2;   // stash slots: one per FFT group
+  if (grid > (sp.nitems + 1) / 2) grid = (sp.nitems + 1) / 2;
+  if (grid < 1) grid = 1;
+  k_search64<MODE><<<(unsigned)grid, 128, smem, st>>>(sp);
+  return cudaGetLastError();
+}
+
+template <int MODE>
 static cudaError_t dispatch_search(const jerk_plan* plan, const SearchParams& sp, cudaStream_t st) {
   switch (plan->L) {
     case 1024: return launch_search<1024, MODE>(plan, sp, st);
     case 2048: return launch_search<2048, MODE>(plan, sp, st);
-    case 4096: return launch_search<4096, MODE>(plan, sp, st);
+    case 4096: return launch_search64<MODE>(plan, sp, st);
     case 8192: return launch_search<8192, MODE>(plan, sp, st);
   }
   return cudaErrorInvalidValue;
