@@ -539,18 +539,48 @@ k_search(const __grid_constant__ SearchParams sp) {
 // has its own exchange buffer, named barrier and mbarriers, and shares only the CTA's tensor-memory allocation:
 // F (the transformed segment, 64 complex per thread) in columns [0,128) and the pass-2 twiddles in [128,256) of the
 // thread's own TMEM lane.  Two CTAs per SM (TMEM 2 x 256 columns, up to 255 registers per thread).
+//
+// G never passes through registers before it is used: while pass 2 of the current template-phase runs, one thread
+// bulk-copies (TMA) the 32 KB of the NEXT template-phase into the group's exchange buffer, which is idle from the
+// pass-2 loads of one transform to the pass-1 stores of the next; the multiply F .* G then reads G with 128-bit
+// shared-memory loads (30 cycles instead of an exposed L2 round trip with only two warps per scheduler to hide it).
+// Hazards on the buffer, per group: [1] G landed (TMA tx) -> G reads; [2] G reads done (count 64) -> pass-1 stores;
+// named barrier: stores -> loads; [3] loads done (count 64) -> next TMA.
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t done = 0;
+  while (!done) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done)
+        : "r"(bar), "r"(parity)
+        : "memory");
+  }
+}
+__device__ __forceinline__ void bulk_copy_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // earlier generic accesses to dst before the async write
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src),
+               "r"(bytes), "r"(bar)
+               : "memory");
+}
 template <int MODE>
 __global__ void __launch_bounds__(128, 2) k_search64(const __grid_constant__ SearchParams sp) {
   constexpr int L = 4096, NT = 64, P = 64;
   constexpr int TCOLS = 256;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float2* ex_all = reinterpret_cast<float2*>(smem_raw);
-  unsigned long long* mbar_all = reinterpret_cast<unsigned long long*>(ex_all + 2 * kEx64);  // [group][0] segment copy, [group][1] ex WAR
+  unsigned long long* mbar_all = reinterpret_cast<unsigned long long*>(ex_all + 2 * kEx64);  // [group][4]
   __shared__ long long s_item[2];
   __shared__ uint32_t s_tmem;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, grp = warp >> 1, t = threadIdx.x & 63;
   float2* ex = ex_all + grp * kEx64;
-  unsigned long long* mbar = mbar_all + 2 * grp;
+  const uint32_t mbS = smem_u32(mbar_all + 4 * grp);   // segment copy landed (tx)
+  const uint32_t mbG = mbS + 8;                        // G copy landed (tx)
+  const uint32_t mbR = mbS + 16;                       // all 64 threads have read G out of ex
+  const uint32_t mbW = mbS + 24;                       // all 64 threads have finished their pass-2 loads from ex
   const int barid = 1 + grp;
 
   if (warp == 0) {
@@ -558,17 +588,15 @@ __global__ void __launch_bounds__(128, 2) k_search64(const __grid_constant__ Sea
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
   if (t == 0) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(mbar)));
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(mbar + 1)), "r"(NT));
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbS));
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbG));
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mbR), "r"(NT));
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mbW), "r"(NT));
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   asm volatile("tcgen05.fence::before_thread_sync;");
   __syncthreads();
   asm volatile("tcgen05.fence::after_thread_sync;");
-  WarBarrier war;
-  war.bar = smem_u32(mbar + 1);
-  war.parity = 0;
-  war.arrive();
   const uint32_t tbase = s_tmem + ((uint32_t)(warp * 32) << 16);
   TmemArray<L> tmF, tmT;
   tmF.addr = tbase;
@@ -580,7 +608,8 @@ __global__ void __launch_bounds__(128, 2) k_search64(const __grid_constant__ Sea
     for (int i = 0; i < 16; i++) w[i] = tw64_mixed(16 * h + i, t);
     tmT.store16(h, w);
   }
-  uint32_t mphase = 0;
+  uint32_t sphase = 0, gphase = 0, rphase = 0, wphase = 0;
+  const auto nohook = [] {};
   const long long nitems = sp.nitems;
   float* gstash = sp.stash + ((size_t)blockIdx.x * 2 + grp) * (2 * L);   // [2][P][NT] powers of the current template (rare path)
 
@@ -603,22 +632,9 @@ __global__ void __launch_bounds__(128, 2) k_search64(const __grid_constant__ Sea
     // ---- a-2: stage the segment in the exchange buffer: TMA bulk copy when fully inside the spectrum, guarded loads at the edges
     const bool interior = (s0 >= 0) && (s0 + L <= sp.nbins);
     if (interior) {
-      if (t == 0) {
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(mbar)), "r"((uint32_t)(L * 8)) : "memory");
-        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(ex)),
-                     "l"(sp.spec + s0), "r"((uint32_t)(L * 8)), "r"(smem_u32(mbar))
-                     : "memory");
-      }
-      uint32_t done = 0;
-      while (!done) {
-        asm volatile(
-            "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-            : "=r"(done)
-            : "r"(smem_u32(mbar)), "r"(mphase)
-            : "memory");
-      }
-      mphase ^= 1u;
+      if (t == 0) bulk_copy_g2s(smem_u32(ex), sp.spec + s0, (uint32_t)(L * 8), mbS);
+      mbar_wait(mbS, sphase);
+      sphase ^= 1u;
     } else {
       for (int k = t; k < L; k += NT) {
         int64_t b = s0 + k;
@@ -632,7 +648,7 @@ __global__ void __launch_bounds__(128, 2) k_search64(const __grid_constant__ Sea
 #pragma unroll
       for (int k1 = 0; k1 < 64; k1++) v[k1] = ex[64 * k1 + t];
       bar_sync_named(barid, NT);                         // ex is about to be reused as the exchange buffer
-      fft64_passes<-1>(v, tmT, ex, war, t, barid);
+      fft64_passes<-1>(v, tmT, ex, t, barid, nohook, nohook);
       bar_sync_named(barid, NT);                         // all pass-2 loads of ex done
 #pragma unroll
       for (int r = 0; r < 64; r++) ex[t + 64 * dft64_out_index(r)] = v[r];
@@ -652,35 +668,56 @@ __global__ void __launch_bounds__(128, 2) k_search64(const __grid_constant__ Sea
     const int tp_hi = min(jb.ntp, tp_lo + jb.chunk_tp);
     int any0 = 0;  // candidate mode: phase-0 powers of this warp exceeded the threshold and were stashed
     int izr = (tp_lo >> 1) % iz_cnt, iwr = (tp_lo >> 1) / iz_cnt;
+    if (t == 0)   // G of the first template-phase of the item (ex is free: the barrier above)
+      bulk_copy_g2s(smem_u32(ex), sp.G + ((size_t)((iw_lo + iwr) * sp.nz + iz_lo + izr) * 2 + (tp_lo & 1)) * L, (uint32_t)(L * 8), mbG);
     for (int tp = tp_lo; tp < tp_hi; tp++) {
       const int ph = tp & 1;
-      if (ph == 0 && tp != tp_lo && ++izr == iz_cnt) {
-        izr = 0;
-        ++iwr;
-      }
       const int iz = iz_lo + izr, iw = iw_lo + iwr;
       const int ti = iw * sp.nz + iz;
       const int c = sp.geom[ti].c;
-      // ---- a-3: Y = F .* G (G straight from L2/HBM, F from TMEM), inverse FFT
+      const int izr_c = izr, iwr_c = iwr;
+      // next template-phase: the same template's phase 1, or phase 0 of the next template of the box
+      if (ph == 1 && ++izr == iz_cnt) {
+        izr = 0;
+        ++iwr;
+      }
+      const bool have_next = tp + 1 < tp_hi;
+      const float2* g_next = sp.G + ((size_t)((iw_lo + iwr) * sp.nz + iz_lo + izr) * 2 + (ph ^ 1)) * L;
+      // ---- a-3: Y = F .* G (G from the exchange buffer, F from TMEM), inverse FFT
       float2 v[P];
+      mbar_wait(mbG, gphase);
+      gphase ^= 1u;
       __syncwarp();   // tcgen05.ld is .sync.aligned: the warp must be converged
       {
-        const float4* g4 = reinterpret_cast<const float4*>(sp.G + ((size_t)ti * 2 + ph) * L) + t;
-        float4 g[P / 2];
-#pragma unroll
-        for (int e = 0; e < P / 2; e++) g[e] = __ldg(g4 + e * NT);
+        const float4* g4 = reinterpret_cast<const float4*>(ex) + t;
 #pragma unroll
         for (int h = 0; h < 4; h++) {
           float2 fq[16];
           tmF.load16(h, fq);
 #pragma unroll
           for (int i = 0; i < 8; i++) {
-            v[16 * h + 2 * i] = cmul(fq[2 * i], make_float2(g[8 * h + i].x, g[8 * h + i].y));
-            v[16 * h + 2 * i + 1] = cmul(fq[2 * i + 1], make_float2(g[8 * h + i].z, g[8 * h + i].w));
+            const float4 g = g4[(8 * h + i) * NT];
+            v[16 * h + 2 * i] = cmul(fq[2 * i], make_float2(g.x, g.y));
+            v[16 * h + 2 * i + 1] = cmul(fq[2 * i + 1], make_float2(g.z, g.w));
           }
         }
       }
-      fft64_passes<1>(v, tmT, ex, war, t, barid);
+      mbar_arrive(mbR);
+      fft64_passes<1>(
+          v, tmT, ex, t, barid,
+          [&] {
+            mbar_wait(mbR, rphase);
+          },
+          [&] {
+            mbar_arrive(mbW);
+            if (t == 0 && have_next) {
+              mbar_wait(mbW, wphase);
+              bulk_copy_g2s(smem_u32(ex), g_next, (uint32_t)(L * 8), mbG);
+            }
+            __syncwarp();
+          });
+      rphase ^= 1u;
+      wphase ^= 1u;
       // ---- a-4: overlap discard + power.  n = t + 64*n1 ; b = s0 + n - c ; j = 2b + ph.
       int n_lo, n_hi;
       {
@@ -693,7 +730,7 @@ __global__ void __launch_bounds__(128, 2) k_search64(const __grid_constant__ Sea
 #pragma unroll
       for (int i = 0; i < P; i++) pw[i] = fmaf(v[i].x, v[i].x, v[i].y * v[i].y);
       if (MODE == MODE_PLANE) {
-        float* row = jb.plane + ((size_t)iwr * iz_cnt + izr) * (size_t)(2 * jb.r_cnt) + ph;
+        float* row = jb.plane + ((size_t)iwr_c * iz_cnt + izr_c) * (size_t)(2 * jb.r_cnt) + ph;
         const long long boff = s0 - c - jb.r_lo;
 #pragma unroll
         for (int r = 0; r < P; r++) {
@@ -987,7 +1024,7 @@ static cudaError_t launch_search(const jerk_plan* plan, const SearchParams& sp, 
 
 template <int MODE>
 static cudaError_t launch_search64(const jerk_plan* plan, const SearchParams& sp, cudaStream_t st) {
-  const size_t smem = (size_t)2 * kEx64 * sizeof(float2) + 4 * sizeof(unsigned long long);
+  const size_t smem = (size_t)2 * kEx64 * sizeof(float2) + 8 * sizeof(unsigned long long);
   cudaError_t e = cudaFuncSetAttribute(k_search64<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   if (getenv("JERK_DEBUG")) {

@@ -147,10 +147,10 @@ __device__ __forceinline__ void dft64(float2 (&x)[64]) {
 }
 __device__ __forceinline__ constexpr int dft64_out_index(int reg) { return (reg >> 4) + 4 * (reg & 15); }
 
-// DFT_64 whose inputs carry runtime twiddles in mixed form (dft16_layerA_tw): tw(c, w) returns table entries 16c..16c+15,
-// entry 4 b + a belongs to input register 16 a + b.  SIGN < 0 conjugates the (inverse-sign) table on the fly.
+// First layer of a DFT_64 whose inputs carry runtime twiddles in mixed form (dft16_layerA_tw): tw(c, w) returns table
+// entries 16c..16c+15, entry 4 b + a belongs to input register 16 a + b.  SIGN < 0 conjugates the (inverse-sign) table.
 template <int SIGN, class TW>
-__device__ __forceinline__ void dft64_tw(float2 (&x)[64], const TW& tw) {
+__device__ __forceinline__ void dft64_tw_stage1(float2 (&x)[64], const TW& tw) {
 #pragma unroll
   for (int c = 0; c < 4; c++) {
     float2 w16[16];
@@ -163,7 +163,21 @@ __device__ __forceinline__ void dft64_tw(float2 (&x)[64], const TW& tw) {
       else dft16_layerA_tw<SIGN, false>(x[b], x[16 + b], x[32 + b], x[48 + b], w);
     }
   }
+}
+template <int SIGN, class TW>
+__device__ __forceinline__ void dft64_tw(float2 (&x)[64], const TW& tw) {
+  dft64_tw_stage1<SIGN>(x, tw);
   dft64_stage2<SIGN>(x);
+}
+// column A (0..3) of the second stage alone: x[16 A + b] -> X[A + 4 k2] at x[16 A + k2]
+template <int SIGN, int A>
+__device__ __forceinline__ void dft64_stage2_col(float2 (&x)[64]) {
+  float2 y[16];
+#pragma unroll
+  for (int b = 0; b < 16; b++) y[b] = x[16 * A + b];
+  dft16_ct<SIGN, A>(y);
+#pragma unroll
+  for (int b = 0; b < 16; b++) x[16 * A + b] = y[b];
 }
 
 // Pass-2 twiddle table entry pos = 4 b + a of thread n0 (inverse sign): mixed form of w_4096^{(16 a + b) n0}
@@ -183,12 +197,14 @@ __device__ __forceinline__ void bar_sync_named(int id, int nthreads) {
 }
 
 // Both passes on the 64 points of thread t (0..63) of one FFT group.  On entry v[k1] = x[64 k1 + t]; on exit register r
-// holds X[t + 64 * dft64_out_index(r)].  ex: the group's exchange buffer (kEx64 float2); barid: its named barrier;
-// war: split write-after-read barrier of ex (count 64), arrived at by every thread after its previous loads from ex.
-template <int SIGN, class TW>
-__device__ __forceinline__ void fft64_passes(float2 (&v)[64], const TW& tw, float2* ex, WarBarrier& war, int t, int barid) {
+// holds X[t + 64 * dft64_out_index(r)].  ex: the group's exchange buffer (kEx64 float2); barid: its named barrier.
+// before_store() runs before the first write to ex (the caller's write-after-read protection of ex), after_load() right
+// after the last read of ex.
+template <int SIGN, class TW, class PRE, class POST>
+__device__ __forceinline__ void fft64_passes(float2 (&v)[64], const TW& tw, float2* ex, int t, int barid, PRE before_store,
+                                             POST after_load) {
   dft64<SIGN>(v);
-  war.wait();
+  before_store();
   {
     float2* w = ex + t;
 #pragma unroll
@@ -204,7 +220,7 @@ __device__ __forceinline__ void fft64_passes(float2 (&v)[64], const TW& tw, floa
       v[2 * q + 1] = make_float2(x.z, x.w);
     }
   }
-  war.arrive();
+  after_load();
   dft64_tw<SIGN>(v, tw);
 }
 #endif
