@@ -690,15 +690,19 @@ __global__ void __launch_bounds__(128, 2) k_search64(const __grid_constant__ Sea
       __syncwarp();   // tcgen05.ld is .sync.aligned: the warp must be converged
       {
         const float4* g4 = reinterpret_cast<const float4*>(ex) + t;
+        float fa[32], fb[32];   // F chunks, double-buffered: chunk h+1 is in flight while chunk h is multiplied
+        tmF.issue16(0, fa);
 #pragma unroll
         for (int h = 0; h < 4; h++) {
-          float2 fq[16];
-          tmF.load16(h, fq);
+          float(&cur)[32] = (h & 1) ? fb : fa;
+          float(&nxt)[32] = (h & 1) ? fa : fb;
+          tmem_ld32_wait(cur);
+          if (h < 3) tmF.issue16(h + 1, nxt);
 #pragma unroll
           for (int i = 0; i < 8; i++) {
             const float4 g = g4[(8 * h + i) * NT];
-            v[16 * h + 2 * i] = cmul(fq[2 * i], make_float2(g.x, g.y));
-            v[16 * h + 2 * i + 1] = cmul(fq[2 * i + 1], make_float2(g.z, g.w));
+            v[16 * h + 2 * i] = cmul(make_float2(cur[4 * i], cur[4 * i + 1]), make_float2(g.x, g.y));
+            v[16 * h + 2 * i + 1] = cmul(make_float2(cur[4 * i + 2], cur[4 * i + 3]), make_float2(g.z, g.w));
           }
         }
       }

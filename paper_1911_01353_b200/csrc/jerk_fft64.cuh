@@ -164,6 +164,29 @@ __device__ __forceinline__ void dft64_tw_stage1(float2 (&x)[64], const TW& tw) {
     }
   }
 }
+#ifdef __CUDACC__
+// The same with the table in tensor memory, double-buffered: the load of chunk c+1 is in flight while chunk c is used.
+template <int SIGN>
+__device__ __forceinline__ void dft64_tw_stage1(float2 (&x)[64], const TmemArray<4096>& tw) {
+  float wa[32], wb[32];
+  tw.issue16(0, wa);
+#pragma unroll
+  for (int c = 0; c < 4; c++) {
+    float(&cur)[32] = (c & 1) ? wb : wa;
+    float(&nxt)[32] = (c & 1) ? wa : wb;
+    tmem_ld32_wait(cur);
+    if (c < 3) tw.issue16(c + 1, nxt);
+#pragma unroll
+    for (int m = 0; m < 4; m++) {
+      const int b = 4 * c + m;
+      const float2 w[4] = {make_float2(cur[8 * m], cur[8 * m + 1]), make_float2(cur[8 * m + 2], cur[8 * m + 3]),
+                           make_float2(cur[8 * m + 4], cur[8 * m + 5]), make_float2(cur[8 * m + 6], cur[8 * m + 7])};
+      if (b == 0) dft16_layerA_tw<SIGN, true>(x[0], x[16], x[32], x[48], w);
+      else dft16_layerA_tw<SIGN, false>(x[b], x[16 + b], x[32 + b], x[48 + b], w);
+    }
+  }
+}
+#endif
 template <int SIGN, class TW>
 __device__ __forceinline__ void dft64_tw(float2 (&x)[64], const TW& tw) {
   dft64_tw_stage1<SIGN>(x, tw);
