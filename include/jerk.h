@@ -136,6 +136,17 @@ int jerk_search_candidates(jerk_plan* plan, const void* d_spec, float threshold,
                            uint64_t work_bytes, void* stream);
 
 /*
+ * jerk_search_candidates_range — candidate mode restricted to the template box iz in [iz_lo, iz_lo+iz_cnt),
+ * iw in [iw_lo, iw_lo+iw_cnt) (all r).  This is the unit of multi-GPU sharding (partition by template,
+ * w-rows first): the candidate rule is one-dimensional along r inside a (z,w) row (reading S10), so the union of
+ * the candidates of disjoint boxes that cover the grid equals the result of jerk_search_candidates.
+ * An empty box (iz_cnt == 0 or iw_cnt == 0) sets *d_count = 0.  Other arguments and errors as jerk_search_candidates.
+ */
+int jerk_search_candidates_range(jerk_plan* plan, const void* d_spec, float threshold, int iz_lo, int iz_cnt,
+                                 int iw_lo, int iw_cnt, jerk_cand* d_cands, int64_t max_cands,
+                                 unsigned long long* d_count, void* d_work, uint64_t work_bytes, void* stream);
+
+/*
  * jerk_search_candidates_host — the same search with HOST input/output (end-to-end entry point):
  * copies h_spec (host, ideally pinned, nbins complex64) to d_spec, searches, copies the count and
  * min(count, max_cands) records back to h_count / h_cands and synchronises the stream before returning.

@@ -40,6 +40,7 @@ class PlanInfo(C.Structure):
 EXPORTS = [
     "jerk_plan_create", "jerk_plan_destroy", "jerk_plan_info", "jerk_template_geometry", "jerk_plane_bytes",
     "jerk_templates", "jerk_templates_taps", "jerk_search_plane", "jerk_search_candidates",
+    "jerk_search_candidates_range",
     "jerk_search_candidates_host", "jerk_harmonic_scratch_bytes", "jerk_harmonic_sum", "jerk_harmonic_plane", "jerk_strerror",
     "jerk_last_error",
 ]
@@ -67,6 +68,7 @@ def load_library() -> C.CDLL:
     lib.jerk_templates_taps.argtypes = [vp, i32, i32, vp, u64, vp]
     lib.jerk_search_plane.argtypes = [vp, vp, i64, i64, i32, i32, i32, i32, vp, u64, vp, u64, vp]
     lib.jerk_search_candidates.argtypes = [vp, vp, C.c_float, vp, i64, vp, vp, u64, vp]
+    lib.jerk_search_candidates_range.argtypes = [vp, vp, C.c_float, i32, i32, i32, i32, vp, i64, vp, vp, u64, vp]
     lib.jerk_search_candidates_host.argtypes = [vp, vp, C.c_float, vp, i64, vp, vp, vp, vp, vp, u64, vp]
     lib.jerk_harmonic_scratch_bytes.argtypes = [vp]
     lib.jerk_harmonic_scratch_bytes.restype = u64
@@ -172,6 +174,21 @@ class Plan:
         self._check(self._lib.jerk_search_candidates(
             self._h, C.c_void_p(d_spec.data_ptr()), float(threshold), C.c_void_p(d_cands.data_ptr()), int(max_cands),
             C.c_void_p(d_count.data_ptr()), C.c_void_p(work.data_ptr()), work.numel(), _stream_ptr(stream)))
+        return d_cands, d_count
+
+    def search_candidates_range(self, d_spec, threshold, iz_lo, iz_cnt, iw_lo, iw_cnt, max_cands=1 << 20, d_cands=None,
+                                d_count=None, stream=None):
+        """jerk_search_candidates_range: candidate mode over one template box (the unit of multi-GPU sharding)."""
+        import torch
+        if d_cands is None:
+            d_cands = torch.empty(max_cands * 16, dtype=torch.uint8, device=d_spec.device)
+        if d_count is None:
+            d_count = torch.zeros(1, dtype=torch.int64, device=d_spec.device)
+        work = self._ensure_work(d_spec.device)
+        self._check(self._lib.jerk_search_candidates_range(
+            self._h, C.c_void_p(d_spec.data_ptr()), float(threshold), int(iz_lo), int(iz_cnt), int(iw_lo), int(iw_cnt),
+            C.c_void_p(d_cands.data_ptr()), int(max_cands), C.c_void_p(d_count.data_ptr()), C.c_void_p(work.data_ptr()),
+            work.numel(), _stream_ptr(stream)))
         return d_cands, d_count
 
     def search_candidates_host(self, h_spec, threshold, h_cands, h_count, d_spec, d_cands, d_count, stream=None):

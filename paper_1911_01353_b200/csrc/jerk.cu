@@ -1330,26 +1330,39 @@ int jerk_search_plane(jerk_plan* p, const void* d_spec, int64_t r_lo, int64_t r_
   return JERK_OK;
 }
 
-int jerk_search_candidates(jerk_plan* p, const void* d_spec, float threshold, jerk_cand* d_cands, int64_t max_cands,
-                           unsigned long long* d_count, void* d_work, uint64_t work_bytes, void* stream) {
+int jerk_search_candidates_range(jerk_plan* p, const void* d_spec, float threshold, int iz_lo, int iz_cnt, int iw_lo, int iw_cnt,
+                                 jerk_cand* d_cands, int64_t max_cands, unsigned long long* d_count, void* d_work,
+                                 uint64_t work_bytes, void* stream) {
   int rc = check_common(p, d_spec, d_work, work_bytes);
   if (rc) return rc;
   if (!d_cands || !d_count || max_cands < 0) return JERK_EINVAL;
+  if (iz_lo < 0 || iz_cnt < 0 || iz_lo + iz_cnt > p->nz || iw_lo < 0 || iw_cnt < 0 || iw_lo + iw_cnt > p->nw)
+    return fail(p, JERK_EINVAL, "template box outside the plan's grid");
   cudaStream_t st = (cudaStream_t)stream;
   SearchParams sp;
   fill_params(p, sp, d_spec, d_work);
-  add_job(p, sp, 0, p->nbins, 0, p->nz, 0, p->nw, nullptr, kChunkTP);
+  const bool any = add_job(p, sp, 0, p->nbins, iz_lo, iz_cnt, iw_lo, iw_cnt, nullptr, kChunkTP);
   sp.threshold = threshold;
   sp.cands = d_cands;
   sp.max_cands = max_cands;
   sp.count = d_count;
   k_reset<<<1, 32, 0, st>>>(sp.work, d_count);
-  cudaError_t e = dispatch_search<MODE_CAND>(p, sp, st);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_reset launch: ") + cudaGetErrorString(e));
+  if (!any) return JERK_OK;   // empty box
+  e = dispatch_search<MODE_CAND>(p, sp, st);
   if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_search(cand) launch: ") + cudaGetErrorString(e));
   k_resolve<<<p->sm_count, 256, 0, st>>>(sp);
   e = cudaGetLastError();
   if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_resolve launch: ") + cudaGetErrorString(e));
   return JERK_OK;
+}
+
+int jerk_search_candidates(jerk_plan* p, const void* d_spec, float threshold, jerk_cand* d_cands, int64_t max_cands,
+                           unsigned long long* d_count, void* d_work, uint64_t work_bytes, void* stream) {
+  if (!p) return JERK_EINVAL;
+  return jerk_search_candidates_range(p, d_spec, threshold, 0, p->nz, 0, p->nw, d_cands, max_cands, d_count, d_work, work_bytes,
+                                      stream);
 }
 
 int jerk_search_candidates_host(jerk_plan* p, const void* h_spec, float threshold, jerk_cand* h_cands, int64_t max_cands,

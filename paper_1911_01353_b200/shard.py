@@ -1,0 +1,93 @@
+"""Host-side sharding of the jerk search over ranks; one process per GPU, torch.distributed plumbing.
+
+The path shards with NO data-path collective: every (segment, template) unit is independent ("processed
+independently"; PAPER.md:39 one filter per (z,w)) and the candidate rule is one-dimensional along r inside a (z,w)
+row (reading S10).  Two partitions are offered:
+
+  * by trial  (weak scaling, what bench.py --gpus N times): rank r searches spectra r, r+W, r+2W, ... (other DM
+    trials) against its own copy of the bank;
+  * by template (strong scaling of one spectrum): rank r searches a contiguous block of w-rows (a template box for
+    jerk_search_candidates_range); the spectrum is broadcast once, candidate lists are concatenated at the end.
+
+The only collectives are the ones around the search: broadcast of the spectrum, gather of the (small) candidate
+lists, max-over-ranks of device times.  This module holds no arithmetic of the method."""
+from __future__ import annotations
+
+import numpy as np
+
+CAND_FIELDS = [("j", "<i4"), ("iz", "<i2"), ("iw", "<i2"), ("power", "<f4"), ("flags", "<u4")]
+
+
+def block_range(n: int, world: int, rank: int) -> tuple[int, int]:
+    """Contiguous block partition of range(n): (lo, cnt) of `rank`; the first n % world ranks get one more."""
+    if world < 1 or not 0 <= rank < world or n < 0:
+        raise ValueError("block_range: bad arguments")
+    base, rem = divmod(n, world)
+    lo = rank * base + min(rank, rem)
+    return lo, base + (1 if rank < rem else 0)
+
+
+def template_box(nz: int, nw: int, world: int, rank: int) -> tuple[int, int, int, int]:
+    """(iz_lo, iz_cnt, iw_lo, iw_cnt) of `rank`: w-rows are split first; when there are more ranks than w-rows the
+    ranks that share a w-row block split the z axis."""
+    if world <= nw:
+        iw_lo, iw_cnt = block_range(nw, world, rank)
+        return 0, nz, iw_lo, iw_cnt
+    per, extra = divmod(world, nw)          # ranks per w-row; the first `extra` rows get one more
+    row, first = 0, 0
+    while True:
+        k = per + (1 if row < extra else 0)
+        if rank < first + k:
+            break
+        first += k
+        row += 1
+    iz_lo, iz_cnt = block_range(nz, k, rank - first)
+    return iz_lo, iz_cnt, row, 1
+
+
+def trial_indices(ntrials: int, world: int, rank: int) -> list[int]:
+    """Round-robin assignment of independent spectra (DM trials) to ranks."""
+    return list(range(rank, ntrials, world))
+
+
+def broadcast_spectrum(X, src: int = 0, group=None):
+    """Broadcast a complex64 spectrum tensor (viewed as float32 pairs) from `src` to every rank, in place."""
+    import torch
+    import torch.distributed as dist
+    buf = torch.view_as_real(X) if X.is_complex() else X
+    dist.broadcast(buf, src=src, group=group)
+    return X
+
+
+def gather_candidates(local: np.ndarray, group=None) -> np.ndarray:
+    """Concatenate every rank's candidate records (numpy structured array of jerk_cand) on every rank, sorted by
+    (iw, iz, j).  Uses all_gather of a padded byte tensor: sizes first, then payload."""
+    import torch
+    import torch.distributed as dist
+    world = dist.get_world_size(group)
+    dev = torch.device("cuda", torch.cuda.current_device()) if dist.get_backend(group) == "nccl" else torch.device("cpu")
+    n = torch.tensor([local.shape[0]], dtype=torch.int64, device=dev)
+    sizes = [torch.zeros_like(n) for _ in range(world)]
+    dist.all_gather(sizes, n, group=group)
+    counts = [int(s.item()) for s in sizes]
+    nmax = max(counts) if counts else 0
+    itemsize = local.dtype.itemsize
+    pad = np.zeros(nmax * itemsize, dtype=np.uint8)
+    pad[: local.shape[0] * itemsize] = np.frombuffer(local.tobytes(), dtype=np.uint8)
+    mine = torch.from_numpy(pad).to(dev)
+    bufs = [torch.empty_like(mine) for _ in range(world)]
+    if nmax:
+        dist.all_gather(bufs, mine, group=group)
+    parts = [np.frombuffer(b.cpu().numpy().tobytes()[: c * itemsize], dtype=local.dtype) for b, c in zip(bufs, counts)]
+    out = np.concatenate(parts) if parts else local[:0]
+    return np.sort(out, order=["iw", "iz", "j"])
+
+
+def max_over_ranks(value: float, group=None) -> float:
+    """Device-timed milliseconds -> max over ranks (the bench contract's timing rule)."""
+    import torch
+    import torch.distributed as dist
+    dev = torch.device("cuda", torch.cuda.current_device()) if dist.get_backend(group) == "nccl" else torch.device("cpu")
+    t = torch.tensor([value], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX, group=group)
+    return float(t.item())

@@ -280,3 +280,29 @@ def test_config3_injections_and_candidates():
 def test_config4_injections_and_candidates():
     """BASELINE.json configs[3]: N = 2^25, seg_len 8192; rows around each injection (two near threshold)."""
     assert _injection_check(4, half_range=400) > 0
+
+
+# ------------------------------------------------------------------------------------------------ template-box sharding (8(e))
+@pytest.mark.gpu
+@pytest.mark.parametrize("idx,world,thr", [(1, 2, 8.0), (1, 3, 8.0), (3, 2, 25.0)])
+def test_candidates_range_union(idx, world, thr):
+    """The union of jerk_search_candidates_range over the template boxes of shard.template_box is, record for record
+    (bit-exact j, iz, iw and power), the result of the whole-grid search: the property multi-GPU template sharding rests on."""
+    from paper_1911_01353_b200 import shard
+    cfg, X, plan, d_spec = _setup(idx)
+    d_c, d_n = plan.search_candidates(d_spec, thr)
+    full, n = binding.candidates_to_numpy(d_c, d_n)
+    assert n == full.size and n > 0
+    parts = []
+    for r in range(world):
+        iz_lo, iz_cnt, iw_lo, iw_cnt = shard.template_box(cfg.nz, cfg.nw, world, r)
+        d_c, d_n = plan.search_candidates_range(d_spec, thr, iz_lo, iz_cnt, iw_lo, iw_cnt)
+        c, k = binding.candidates_to_numpy(d_c, d_n)
+        assert k == c.size
+        assert np.all((c["iz"] >= iz_lo) & (c["iz"] < iz_lo + iz_cnt) & (c["iw"] >= iw_lo) & (c["iw"] < iw_lo + iw_cnt))
+        parts.append(c)
+    merged = np.sort(np.concatenate(parts), order=["iw", "iz", "j"])
+    assert np.array_equal(merged, np.sort(full, order=["iw", "iz", "j"]))
+    # empty box: count 0, no launch error
+    d_c, d_n = plan.search_candidates_range(d_spec, thr, 0, 0, 0, cfg.nw)
+    assert int(d_n.item()) == 0

@@ -1,0 +1,90 @@
+"""Host-side multi-rank logic on CPU: world_size-2 (and 3) gloo process groups.  No GPU, no kernels:
+the per-rank "search" is replaced by slicing a fixed synthetic candidate list by template box, which is exactly what
+jerk_search_candidates_range guarantees (tests/test_gpu_parity.py::test_candidates_range_union checks that on the GPU)."""
+import os
+import socket
+
+import numpy as np
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+from paper_1911_01353_b200 import shard
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _fake_candidates(nz, nw, n=500, seed=5):
+    rng = np.random.default_rng(seed)
+    c = np.zeros(n, dtype=shard.CAND_FIELDS)
+    c["j"] = rng.integers(0, 1 << 20, n)
+    c["iz"] = rng.integers(0, nz, n)
+    c["iw"] = rng.integers(0, nw, n)
+    c["power"] = rng.uniform(25, 90, n).astype(np.float32)
+    return np.unique(c)
+
+
+def _worker(rank, world, port, nz, nw, q):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        full = _fake_candidates(nz, nw)
+        iz_lo, iz_cnt, iw_lo, iw_cnt = shard.template_box(nz, nw, world, rank)
+        m = (full["iz"] >= iz_lo) & (full["iz"] < iz_lo + iz_cnt) & (full["iw"] >= iw_lo) & (full["iw"] < iw_lo + iw_cnt)
+        merged = shard.gather_candidates(full[m])
+        ok_merge = np.array_equal(merged, np.sort(full, order=["iw", "iz", "j"]))
+        # spectrum broadcast: rank 0 holds the data, the others zeros
+        X = torch.zeros(1000, dtype=torch.complex64)
+        if rank == 0:
+            X = torch.view_as_complex(torch.arange(2000, dtype=torch.float32).reshape(1000, 2).contiguous())
+        shard.broadcast_spectrum(X, src=0)
+        ok_bcast = bool(torch.view_as_real(X)[-1, 1] == 1999.0)
+        tmax = shard.max_over_ranks(10.0 + rank)
+        q.put((rank, ok_merge, ok_bcast, tmax, shard.trial_indices(7, world, rank)))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world,nz,nw", [(2, 201, 61), (3, 21, 2)])
+def test_template_sharding_gloo(world, nz, nw):
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, world, port, nz, nw, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in range(world))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    trials = []
+    for rank, ok_merge, ok_bcast, tmax, tr in res:
+        assert ok_merge and ok_bcast
+        assert tmax == 10.0 + world - 1
+        trials += tr
+    assert sorted(trials) == list(range(7))
+
+
+@pytest.mark.parametrize("nz,nw,world", [(201, 61, 1), (201, 61, 2), (201, 61, 8), (21, 7, 8), (21, 2, 3), (5, 1, 4), (3, 2, 16)])
+def test_template_boxes_partition_the_grid(nz, nw, world):
+    seen = np.zeros((nw, nz), dtype=np.int32)
+    for r in range(world):
+        iz_lo, iz_cnt, iw_lo, iw_cnt = shard.template_box(nz, nw, world, r)
+        assert 0 <= iz_lo and iz_lo + iz_cnt <= nz and 0 <= iw_lo and iw_lo + iw_cnt <= nw
+        seen[iw_lo:iw_lo + iw_cnt, iz_lo:iz_lo + iz_cnt] += 1
+    assert (seen == 1).all()
+
+
+def test_block_range_balanced():
+    for n in (0, 1, 7, 61, 201):
+        for w in (1, 2, 3, 8):
+            parts = [shard.block_range(n, w, r) for r in range(w)]
+            assert sum(c for _, c in parts) == n
+            assert max(c for _, c in parts) - min(c for _, c in parts) <= 1
+            assert all(parts[i][0] + parts[i][1] == parts[i + 1][0] for i in range(w - 1))
