@@ -577,6 +577,7 @@ __global__ void __launch_bounds__(128, 2) k_search64(const __grid_constant__ Sea
   __shared__ uint32_t s_tmem;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, grp = warp >> 1, t = threadIdx.x & 63;
   float2* ex = ex_all + grp * kEx64;
+  float* p0s = reinterpret_cast<float*>(mbar_all + 8) + grp * (P * NT);   // plane mode only: [P][NT] phase-0 powers of the group
   const uint32_t mbS = smem_u32(mbar_all + 4 * grp);   // segment copy landed (tx)
   const uint32_t mbG = mbS + 8;                        // G copy landed (tx)
   const uint32_t mbR = mbS + 16;                       // all 64 threads have read G out of ex
@@ -734,12 +735,20 @@ __global__ void __launch_bounds__(128, 2) k_search64(const __grid_constant__ Sea
 #pragma unroll
       for (int i = 0; i < P; i++) pw[i] = fmaf(v[i].x, v[i].x, v[i].y * v[i].y);
       if (MODE == MODE_PLANE) {
-        float* row = jb.plane + ((size_t)iwr_c * iz_cnt + izr_c) * (size_t)(2 * jb.r_cnt) + ph;
-        const long long boff = s0 - c - jb.r_lo;
+        // phase-0 powers wait in shared memory (written and read back by the same thread) so that both phases leave as
+        // interleaved float2 pairs: every warp store covers 256 contiguous bytes (full 32-byte sectors, no L2 fill reads)
+        if (ph == 0) {
 #pragma unroll
-        for (int r = 0; r < P; r++) {
-          const int n = t + 64 * dft64_out_index(r);
-          if (n >= n_lo && n < n_hi) row[2 * (boff + n)] = pw[r];
+          for (int r = 0; r < P; r++) p0s[r * NT + t] = pw[r];
+        } else {
+          float* row = jb.plane + ((size_t)iwr_c * iz_cnt + izr_c) * (size_t)(2 * jb.r_cnt);
+          const long long boff = s0 - c - jb.r_lo;
+#pragma unroll
+          for (int r = 0; r < P; r++) {
+            const int n = t + 64 * dft64_out_index(r);
+            const float p0 = p0s[r * NT + t];
+            if (n >= n_lo && n < n_hi) *reinterpret_cast<float2*>(row + 2 * (boff + n)) = make_float2(p0, pw[r]);
+          }
         }
       } else {
         // ---- a-5: threshold + local max.  Hot path: one max-reduction and a vote.
@@ -866,36 +875,51 @@ __global__ void __launch_bounds__(256) k_harm(const __grid_constant__ HarmParams
   const int izr = row % hp.iz_cnt, iwr = row / hp.iz_cnt;
   const int iz = hp.iz_lo + izr, iw = hp.iw_lo + iwr;
   const int az = iz - hp.cz, aw = iw - hp.cw;
+  // tile [jb, je) of half-bin indices; all index arithmetic inside the tile is 32-bit relative to j8 = jb rounded down
+  // to a multiple of 8:  (j e + 4) >> 3 = (j8 / 8) e + ((jl e + 4) >> 3),  jl = j - j8
+  const long long jb = hp.j_lo + (long long)tile * hp.jtile;
+  const long long je = min(hp.j_lo + hp.nj, jb + hp.jtile);
+  const long long j8 = jb & ~7LL;
+  const int l_lo = (int)(jb - j8), l_hi = (int)(je - j8);
   const float* rp[8];
 #pragma unroll
   for (int e = 1; e <= 8; e++) {
     const HarmSub& sb = hp.sub[e - 1];
     const int ize = rnd_eighths(az, e) + hp.cz, iwe = rnd_eighths(aw, e) + hp.cw;
-    rp[e - 1] = sb.base + ((long long)(iwe - sb.iw_lo) * sb.iz_cnt + (ize - sb.iz_lo)) * sb.nj - sb.j0;
+    rp[e - 1] = sb.base + ((long long)(iwe - sb.iw_lo) * sb.iz_cnt + (ize - sb.iz_lo)) * sb.nj - sb.j0 + (j8 >> 3) * e;
   }
-  const long long jb = hp.j_lo + (long long)tile * hp.jtile;
-  const long long je = min(hp.j_lo + hp.nj, jb + hp.jtile);
   float best[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
   int bj[4] = {-1, -1, -1, -1};
-  float* orow = STORE ? hp.out + ((long long)iwr * hp.iz_cnt + izr) * hp.nj - hp.j_lo : nullptr;
-  for (long long j = jb + threadIdx.x; j < je; j += 256) {
-    float pe[8];
+  float* orow = STORE ? hp.out + ((long long)iwr * hp.iz_cnt + izr) * hp.nj - hp.j_lo + j8 : nullptr;
+  constexpr int U = 4;   // points per thread in flight: 32 independent loads before the first use
+  for (int l0 = l_lo + (int)threadIdx.x; l0 < l_hi; l0 += 256 * U) {
+    float pe[U][8];
 #pragma unroll
-    for (int e = 1; e <= 8; e++) pe[e - 1] = __ldg(rp[e - 1] + ((j * e + 4) >> 3));
-    float sv[4];
-    sv[0] = pe[7];
-    sv[1] = sv[0] + pe[3];
-    sv[2] = sv[1] + pe[1] + pe[5];
-    sv[3] = sv[2] + pe[0] + pe[2] + pe[4] + pe[6];
-    if (STORE) {
-      orow[j] = sv[hp.out_stage];
-    } else {
+    for (int k = 0; k < U; k++) {
+      const int l = l0 + 256 * k;
+      const bool ok = l < l_hi;
 #pragma unroll
-      for (int q = 0; q < 4; q++)
-        if (sv[q] > best[q]) {        // j increases per thread: strict > keeps the smallest j among equals
-          best[q] = sv[q];
-          bj[q] = (int)j;
-        }
+      for (int e = 1; e <= 8; e++) pe[k][e - 1] = ok ? __ldg(rp[e - 1] + ((l * e + 4) >> 3)) : 0.f;
+    }
+#pragma unroll
+    for (int k = 0; k < U; k++) {
+      const int l = l0 + 256 * k;
+      if (l >= l_hi) break;
+      float sv[4];
+      sv[0] = pe[k][7];
+      sv[1] = sv[0] + pe[k][3];
+      sv[2] = sv[1] + pe[k][1] + pe[k][5];
+      sv[3] = sv[2] + pe[k][0] + pe[k][2] + pe[k][4] + pe[k][6];
+      if (STORE) {
+        orow[l] = sv[hp.out_stage];
+      } else {
+#pragma unroll
+        for (int q = 0; q < 4; q++)
+          if (sv[q] > best[q]) {        // l increases per thread: strict > keeps the smallest j among equals
+            best[q] = sv[q];
+            bj[q] = l;
+          }
+      }
     }
   }
   if (STORE) return;
@@ -934,7 +958,7 @@ __global__ void __launch_bounds__(256) k_harm(const __grid_constant__ HarmParams
       }
     }
     jerk_cand c;
-    c.j = jj;
+    c.j = jj < 0 ? -1 : (int)(j8 + jj);
     c.iz = (int16_t)iz;
     c.iw = (int16_t)iw;
     c.power = b;
@@ -943,8 +967,10 @@ __global__ void __launch_bounds__(256) k_harm(const __grid_constant__ HarmParams
   }
 }
 
-// Folds the per-block bests of one box into the running per-stage arg-max (running[4]); one block of 256 threads.
-__global__ void __launch_bounds__(256) k_harm_fold(const jerk_cand* blockbest, int nblocks, jerk_cand* running, int first) {
+// Arg-max fold of per-stage candidate lists: block b of the grid reduces in[q][b, b + gridDim.x, ...] (q = 0..3, n_in
+// records per stage).  A multi-block launch writes its partial results to out[q][blockIdx.x]; the final single-block
+// launch (running != nullptr) merges its result into running[q] (`first`: overwrite).
+__global__ void __launch_bounds__(256) k_harm_fold(const jerk_cand* in, int n_in, jerk_cand* out, jerk_cand* running, int first) {
   __shared__ jerk_cand s_c[256];
   for (int q = 0; q < 4; q++) {
     jerk_cand b;
@@ -952,8 +978,8 @@ __global__ void __launch_bounds__(256) k_harm_fold(const jerk_cand* blockbest, i
     b.iz = b.iw = 0;
     b.power = -INFINITY;
     b.flags = 0;
-    for (int i = threadIdx.x; i < nblocks; i += 256) {
-      const jerk_cand c = blockbest[(size_t)q * nblocks + i];
+    for (int i = blockIdx.x * 256 + threadIdx.x; i < n_in; i += 256 * gridDim.x) {
+      const jerk_cand c = in[(size_t)q * n_in + i];
       if (c.j >= 0 && (b.j < 0 || harm_better(c.power, c.j, c.iz, c.iw, b.power, b.j, b.iz, b.iw))) b = c;
     }
     s_c[threadIdx.x] = b;
@@ -966,8 +992,13 @@ __global__ void __launch_bounds__(256) k_harm_fold(const jerk_cand* blockbest, i
       __syncthreads();
     }
     if (threadIdx.x == 0) {
-      const jerk_cand c = s_c[0], m = running[q];
-      if (first || (c.j >= 0 && (m.j < 0 || harm_better(c.power, c.j, c.iz, c.iw, m.power, m.j, m.iz, m.iw)))) running[q] = c;
+      const jerk_cand c = s_c[0];
+      if (running) {
+        const jerk_cand m = running[q];
+        if (first || (c.j >= 0 && (m.j < 0 || harm_better(c.power, c.j, c.iz, c.iw, m.power, m.j, m.iz, m.iw)))) running[q] = c;
+      } else {
+        out[(size_t)q * gridDim.x + blockIdx.x] = c;
+      }
     }
     __syncthreads();
   }
@@ -1028,7 +1059,8 @@ static cudaError_t launch_search(const jerk_plan* plan, const SearchParams& sp, 
 
 template <int MODE>
 static cudaError_t launch_search64(const jerk_plan* plan, const SearchParams& sp, cudaStream_t st) {
-  const size_t smem = (size_t)2 * kEx64 * sizeof(float2) + 8 * sizeof(unsigned long long);
+  const size_t smem = (size_t)2 * kEx64 * sizeof(float2) + 8 * sizeof(unsigned long long) +
+                      (MODE == MODE_PLANE ? (size_t)2 * 64 * 64 * sizeof(float) : 0);
   cudaError_t e = cudaFuncSetAttribute(k_search64<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   if (getenv("JERK_DEBUG")) {
@@ -1120,9 +1152,9 @@ static bool add_job(const jerk_plan* p, SearchParams& sp, int64_t r_lo, int64_t 
 static int pick_chunk_tp(const jerk_plan* p, int64_t r_cnt, int iz_cnt, int iw_cnt) {
   long long ntp = 2LL * iz_cnt * iw_cnt;
   long long segs = r_cnt / p->step + 2;
-  long long want_items = 4LL * kMaxCtas;
+  long long want_items = 32LL * kMaxCtas;   // >= 32 rounds of work items per resident FFT group: tail < 3 %
   int c = kChunkTP;
-  while (c > 16 && ((ntp + c - 1) / c) * segs < want_items) c >>= 1;
+  while (c > 32 && ((ntp + c - 1) / c) * segs < want_items) c >>= 1;
   return c;
 }
 
@@ -1392,9 +1424,11 @@ int jerk_search_candidates_host(jerk_plan* p, const void* h_spec, float threshol
 
 namespace jerk {
 
-constexpr int64_t kHarmChunkBins = 1 << 16;   // default r-chunk of the top-harmonic axis
+constexpr int64_t kHarmChunkBins = 1 << 16;      // r-chunk of the top-harmonic axis that jerk_harmonic_scratch_bytes sizes for
+constexpr int64_t kHarmChunkBinsMax = 1 << 19;   // larger caller buffers are used up to this chunk (fewer segment-edge recomputations)
 constexpr int kHarmJTile = 8192;              // half-bin indices per k_harm block
 constexpr uint64_t kHarmHeader = 256;         // running[4] arg-max records
+constexpr int kHarmFoldBlocks = 128;          // first level of the arg-max fold
 
 struct HarmBox {
   int64_t r_lo, r_cnt;
@@ -1435,6 +1469,7 @@ static uint64_t harm_layout(const jerk_plan* p, const HarmBox& bx, HarmSubBox (&
   *nblocks = bx.iw_cnt * bx.iz_cnt * *ntiles;
   *blockbest_off = off;
   off += align_up((uint64_t)4 * *nblocks * sizeof(jerk_cand), 256);
+  off += align_up((uint64_t)4 * kHarmFoldBlocks * sizeof(jerk_cand), 256);   // partial arg-max records of the two-level fold
   return off;
 }
 
@@ -1463,7 +1498,7 @@ static int harm_box(jerk_plan* p, const void* d_spec, const HarmBox& bx, unsigne
     hp.sub[e - 1].iw_lo = sb.iw_lo;
   }
   // small boxes: shrink the work items until every resident CTA gets a few
-  while (sp.nitems < 4LL * kMaxCtas && sp.jobs[0].chunk_tp > 16) {
+  while (sp.nitems < 32LL * kMaxCtas && sp.jobs[0].chunk_tp > 32) {
     sp.nitems = 0;
     for (int q = 0; q < sp.njobs; q++) {
       SearchJob& jb = sp.jobs[q];
@@ -1492,7 +1527,9 @@ static int harm_box(jerk_plan* p, const void* d_spec, const HarmBox& bx, unsigne
     k_harm<true><<<nblocks, 256, 0, st>>>(hp);
   } else {
     k_harm<false><<<nblocks, 256, 0, st>>>(hp);
-    k_harm_fold<<<1, 256, 0, st>>>(hp.blockbest, nblocks, (jerk_cand*)scratch, first ? 1 : 0);
+    jerk_cand* partial = (jerk_cand*)(scratch + bb_off + align_up((uint64_t)4 * nblocks * sizeof(jerk_cand), 256));
+    k_harm_fold<<<kHarmFoldBlocks, 256, 0, st>>>(hp.blockbest, nblocks, partial, nullptr, 0);
+    k_harm_fold<<<1, 256, 0, st>>>(partial, kHarmFoldBlocks, nullptr, (jerk_cand*)scratch, first ? 1 : 0);
   }
   e = cudaGetLastError();
   if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_harm launch: ") + cudaGetErrorString(e));
@@ -1503,7 +1540,7 @@ static int stage_of(int h) { return h == 1 ? 0 : h == 2 ? 1 : h == 4 ? 2 : h == 
 
 // largest r-chunk (bins) of the full (iz, iw) grid whose scratch fits in `bytes` (0 if not even one 256-bin chunk fits)
 static int64_t harm_chunk_for(const jerk_plan* p, uint64_t bytes) {
-  int64_t c = std::min<int64_t>(p->nbins, kHarmChunkBins);
+  int64_t c = std::min<int64_t>(p->nbins, kHarmChunkBinsMax);
   for (;;) {
     // rounding can add a source bin per fraction depending on r_lo: size for a box 16 bins longer
     HarmBox bx{0, c + 16, 0, p->nz, 0, p->nw};
