@@ -566,18 +566,19 @@ __device__ __forceinline__ void bulk_copy_g2s(uint32_t dst, const void* src, uin
                "r"(bytes), "r"(bar)
                : "memory");
 }
-template <int MODE>
-__global__ void __launch_bounds__(128, 2) k_search64(const __grid_constant__ SearchParams sp) {
+template <int MODE, int NG>
+__global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __grid_constant__ SearchParams sp) {
   constexpr int L = 4096, NT = 64, P = 64;
-  constexpr int TCOLS = 256;
+  constexpr int NLAYER = (NG + 1) / 2;                          // groups of four warps: one TMEM lane quarter each
+  constexpr int TCOLS = 128 * (NLAYER + 1) <= 256 ? 256 : 512;  // F: 128 columns per layer; twiddles: 128 columns shared by all layers
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float2* ex_all = reinterpret_cast<float2*>(smem_raw);
-  unsigned long long* mbar_all = reinterpret_cast<unsigned long long*>(ex_all + 2 * kEx64);  // [group][4]
-  __shared__ long long s_item[2];
+  unsigned long long* mbar_all = reinterpret_cast<unsigned long long*>(ex_all + NG * kEx64);  // [group][4]
+  __shared__ long long s_item[NG];
   __shared__ uint32_t s_tmem;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, grp = warp >> 1, t = threadIdx.x & 63;
   float2* ex = ex_all + grp * kEx64;
-  float* p0s = reinterpret_cast<float*>(mbar_all + 8) + grp * (P * NT);   // plane mode only: [P][NT] phase-0 powers of the group
+  float* p0s = reinterpret_cast<float*>(mbar_all + 4 * NG) + grp * (P * NT);   // plane mode only: [P][NT] phase-0 powers of the group
   const uint32_t mbS = smem_u32(mbar_all + 4 * grp);   // segment copy landed (tx)
   const uint32_t mbG = mbS + 8;                        // G copy landed (tx)
   const uint32_t mbR = mbS + 16;                       // all 64 threads have read G out of ex
@@ -598,21 +599,26 @@ __global__ void __launch_bounds__(128, 2) k_search64(const __grid_constant__ Sea
   asm volatile("tcgen05.fence::before_thread_sync;");
   __syncthreads();
   asm volatile("tcgen05.fence::after_thread_sync;");
-  const uint32_t tbase = s_tmem + ((uint32_t)(warp * 32) << 16);
+  const uint32_t tbase = s_tmem + ((uint32_t)((warp & 3) * 32) << 16);
   TmemArray<L> tmF, tmT;
-  tmF.addr = tbase;
-  tmT.addr = tbase + 128;
+  tmF.addr = tbase + 128 * (warp >> 2);
+  tmT.addr = tbase + 128 * NLAYER;
+  if (warp < 4) {   // the twiddles depend on t = thread index mod 64 only: one copy per TMEM lane serves every layer
 #pragma unroll
-  for (int h = 0; h < 4; h++) {
-    float2 w[16];
+    for (int h = 0; h < 4; h++) {
+      float2 w[16];
 #pragma unroll
-    for (int i = 0; i < 16; i++) w[i] = tw64_mixed(16 * h + i, t);
-    tmT.store16(h, w);
+      for (int i = 0; i < 16; i++) w[i] = tw64_mixed(16 * h + i, t);
+      tmT.store16(h, w);
+    }
   }
-  uint32_t sphase = 0, gphase = 0, rphase = 0, wphase = 0;
+  asm volatile("tcgen05.fence::before_thread_sync;");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;");
+  uint32_t sphase = 0;   // parity of the segment-copy mbarrier
+  uint32_t tphase = 0;   // parity of mbG, mbR and mbW: each completes exactly one phase per template-phase
   const auto nohook = [] {};
   const long long nitems = sp.nitems;
-  float* gstash = sp.stash + ((size_t)blockIdx.x * 2 + grp) * (2 * L);   // [2][P][NT] powers of the current template (rare path)
 
   for (;;) {
     if (t == 0) s_item[grp] = (long long)atomicAdd(sp.work, 1ULL);
@@ -627,18 +633,18 @@ __global__ void __launch_bounds__(128, 2) k_search64(const __grid_constant__ Sea
     const long long jitem = item - (q ? sp.jobs[q - 1].item_end : 0LL);
     const int chunk = (int)(jitem / jb.seg_count);
     const int64_t seg = jb.seg_first + jitem % jb.seg_count;
-    const int iz_cnt = jb.iz_cnt, iz_lo = jb.iz_lo, iw_lo = jb.iw_lo;
-    const int64_t s0 = sp.seg_base + seg * (int64_t)sp.step;  // first bin of the segment (even)
+    const int iz_cnt = jb.iz_cnt;
+    const int s0 = (int)(sp.seg_base + seg * (int64_t)sp.step);  // first bin of the segment (even); |s0| < 2^31 (nbins <= 2^30)
 
     // ---- a-2: stage the segment in the exchange buffer: TMA bulk copy when fully inside the spectrum, guarded loads at the edges
-    const bool interior = (s0 >= 0) && (s0 + L <= sp.nbins);
+    const bool interior = (s0 >= 0) && ((int64_t)s0 + L <= sp.nbins);
     if (interior) {
       if (t == 0) bulk_copy_g2s(smem_u32(ex), sp.spec + s0, (uint32_t)(L * 8), mbS);
       mbar_wait(mbS, sphase);
       sphase ^= 1u;
     } else {
       for (int k = t; k < L; k += NT) {
-        int64_t b = s0 + k;
+        const int64_t b = (int64_t)s0 + k;
         ex[k] = (b >= 0 && b < sp.nbins) ? sp.spec[b] : make_float2(0.f, 0.f);
       }
       bar_sync_named(barid, NT);
@@ -668,26 +674,31 @@ __global__ void __launch_bounds__(128, 2) k_search64(const __grid_constant__ Sea
     const int tp_lo = chunk * jb.chunk_tp;
     const int tp_hi = min(jb.ntp, tp_lo + jb.chunk_tp);
     int any0 = 0;  // candidate mode: phase-0 powers of this warp exceeded the threshold and were stashed
-    int izr = (tp_lo >> 1) % iz_cnt, iwr = (tp_lo >> 1) / iz_cnt;
+    // template walk of the box, row-major: ti_n = index of the template of the NEXT template-phase, iz_left = templates
+    // left in its w-row
+    int ti_n, iz_left;
+    {
+      const int izr = (tp_lo >> 1) % iz_cnt, iwr = (tp_lo >> 1) / iz_cnt;
+      ti_n = (jb.iw_lo + iwr) * sp.nz + jb.iz_lo + izr;
+      iz_left = iz_cnt - izr;
+    }
     if (t == 0)   // G of the first template-phase of the item (ex is free: the barrier above)
-      bulk_copy_g2s(smem_u32(ex), sp.G + ((size_t)((iw_lo + iwr) * sp.nz + iz_lo + izr) * 2 + (tp_lo & 1)) * L, (uint32_t)(L * 8), mbG);
+      bulk_copy_g2s(smem_u32(ex), sp.G + ((size_t)ti_n * 2 + (tp_lo & 1)) * L, (uint32_t)(L * 8), mbG);
     for (int tp = tp_lo; tp < tp_hi; tp++) {
       const int ph = tp & 1;
-      const int iz = iz_lo + izr, iw = iw_lo + iwr;
-      const int ti = iw * sp.nz + iz;
+      const int ti = ti_n;
       const int c = sp.geom[ti].c;
-      const int izr_c = izr, iwr_c = iwr;
       // next template-phase: the same template's phase 1, or phase 0 of the next template of the box
-      if (ph == 1 && ++izr == iz_cnt) {
-        izr = 0;
-        ++iwr;
+      if (ph == 1) {
+        ++ti_n;
+        if (--iz_left == 0) {
+          iz_left = iz_cnt;
+          ti_n += sp.nz - iz_cnt;
+        }
       }
-      const bool have_next = tp + 1 < tp_hi;
-      const float2* g_next = sp.G + ((size_t)((iw_lo + iwr) * sp.nz + iz_lo + izr) * 2 + (ph ^ 1)) * L;
       // ---- a-3: Y = F .* G (G from the exchange buffer, F from TMEM), inverse FFT
       float2 v[P];
-      mbar_wait(mbG, gphase);
-      gphase ^= 1u;
+      mbar_wait(mbG, tphase);
       __syncwarp();   // tcgen05.ld is .sync.aligned: the warp must be converged
       {
         const float4* g4 = reinterpret_cast<const float4*>(ex) + t;
@@ -708,28 +719,25 @@ __global__ void __launch_bounds__(128, 2) k_search64(const __grid_constant__ Sea
         }
       }
       mbar_arrive(mbR);
-      fft64_passes<1>(
-          v, tmT, ex, t, barid,
-          [&] {
-            mbar_wait(mbR, rphase);
-          },
-          [&] {
-            mbar_arrive(mbW);
-            if (t == 0 && have_next) {
-              mbar_wait(mbW, wphase);
-              bulk_copy_g2s(smem_u32(ex), g_next, (uint32_t)(L * 8), mbG);
-            }
-            __syncwarp();
-          });
-      rphase ^= 1u;
-      wphase ^= 1u;
+      const auto pre = [&] { mbar_wait(mbR, tphase); };
+      const auto post = [&] {
+        mbar_arrive(mbW);
+        if (t == 0 && tp + 1 < tp_hi) {
+          mbar_wait(mbW, tphase);
+          bulk_copy_g2s(smem_u32(ex), sp.G + ((size_t)ti_n * 2 + (ph ^ 1)) * L, (uint32_t)(L * 8), mbG);
+        }
+        __syncwarp();
+      };
+      fft64_passes<1>(v, tmT, ex, t, barid, pre, post);
+      tphase ^= 1u;
       // ---- a-4: overlap discard + power.  n = t + 64*n1 ; b = s0 + n - c ; j = 2b + ph.
+      // valid outputs: n in [n_lo, n_hi) = window [hw_max, hw_max + step) clipped to the bins this call covers (32-bit: all
+      // bin indices are below 2^30)
       int n_lo, n_hi;
       {
-        long long blo = MODE == MODE_PLANE ? jb.r_lo : 0, bhi = MODE == MODE_PLANE ? jb.r_lo + jb.r_cnt : sp.nbins;
-        long long lo = blo + c - s0, hi = bhi + c - s0;
-        n_lo = (int)max((long long)sp.hw_max, min(lo, (long long)L));
-        n_hi = (int)min((long long)(sp.hw_max + sp.step), max(hi, 0LL));
+        const int blo = MODE == MODE_PLANE ? (int)jb.r_lo : 0, bhi = MODE == MODE_PLANE ? (int)(jb.r_lo + jb.r_cnt) : (int)sp.nbins;
+        n_lo = max(sp.hw_max, min(blo - s0 + c, L));
+        n_hi = min(sp.hw_max + sp.step, max(bhi - s0 + c, 0));
       }
       float pw[P];
 #pragma unroll
@@ -741,13 +749,13 @@ __global__ void __launch_bounds__(128, 2) k_search64(const __grid_constant__ Sea
 #pragma unroll
           for (int r = 0; r < P; r++) p0s[r * NT + t] = pw[r];
         } else {
-          float* row = jb.plane + ((size_t)iwr_c * iz_cnt + izr_c) * (size_t)(2 * jb.r_cnt);
-          const long long boff = s0 - c - jb.r_lo;
+          float* row = jb.plane + (size_t)(tp >> 1) * (size_t)(2 * jb.r_cnt);   // row-major box: row index = template-phase / 2
+          const int boff = s0 - c - (int)jb.r_lo;
 #pragma unroll
           for (int r = 0; r < P; r++) {
             const int n = t + 64 * dft64_out_index(r);
             const float p0 = p0s[r * NT + t];
-            if (n >= n_lo && n < n_hi) *reinterpret_cast<float2*>(row + 2 * (boff + n)) = make_float2(p0, pw[r]);
+            if (n >= n_lo && n < n_hi) *reinterpret_cast<float2*>(row + 2 * (ptrdiff_t)(boff + n)) = make_float2(p0, pw[r]);
           }
         }
       } else {
@@ -756,8 +764,10 @@ __global__ void __launch_bounds__(128, 2) k_search64(const __grid_constant__ Sea
 #pragma unroll
         for (int i = 1; i < P; i++) mx = fmaxf(mx, pw[i]);
         const int anyhit = __any_sync(0xffffffffu, mx > sp.threshold);
-        float* st0 = gstash;            // [P][NT]: register i of thread t at i*NT + t (written and read by the same thread)
-        float* st1 = gstash + L;
+        // rare-path stash of the group: [2][P][NT] powers of the current template; register i of thread t at i*NT + t
+        // (written and read by the same thread)
+        float* st0 = sp.stash + ((size_t)blockIdx.x * NG + grp) * (2 * L);
+        float* st1 = st0 + L;
         if (ph == 0) {
           any0 = anyhit;
           if (anyhit) {
@@ -778,20 +788,21 @@ __global__ void __launch_bounds__(128, 2) k_search64(const __grid_constant__ Sea
             const float l1 = __shfl_up_sync(0xffffffffu, p1, 1);    // P1[n-1]
             const float r0 = __shfl_down_sync(0xffffffffu, p0, 1);  // P0[n+1]
             if (!valid) continue;
-            const long long b = s0 + n - c;
+            const int b = s0 + n - c;
+            const int iz = ti % sp.nz, iw = ti / sp.nz;
             if (p0 > sp.threshold) {
               const bool seamL = (lane == 0 || n == sp.hw_max) && (b > 0);
               const float left = (b > 0 && !seamL) ? l1 : NEG;
               const bool okR = p0 >= p1;
-              if (seamL) emit_seam(sp, (int)(2 * b), iz, iw, p0, SEAM_LEFT | (okR ? 0u : SEAM_WITNESS));
-              else if (p0 > left && okR) emit_cand(sp, (int)(2 * b), iz, iw, p0);
+              if (seamL) emit_seam(sp, 2 * b, iz, iw, p0, SEAM_LEFT | (okR ? 0u : SEAM_WITNESS));
+              else if (p0 > left && okR) emit_cand(sp, 2 * b, iz, iw, p0);
             }
             if (p1 > sp.threshold) {
-              const bool seamR = (lane == 31 || n == sp.hw_max + sp.step - 1) && (b < sp.nbins - 1);
+              const bool seamR = (lane == 31 || n == sp.hw_max + sp.step - 1) && (b < (int)sp.nbins - 1);
               const float right = (b < sp.nbins - 1 && !seamR) ? r0 : NEG;
               const bool okL = p1 > p0;
-              if (seamR) emit_seam(sp, (int)(2 * b + 1), iz, iw, p1, SEAM_RIGHT | (okL ? 0u : SEAM_WITNESS));
-              else if (okL && p1 >= right) emit_cand(sp, (int)(2 * b + 1), iz, iw, p1);
+              if (seamR) emit_seam(sp, 2 * b + 1, iz, iw, p1, SEAM_RIGHT | (okL ? 0u : SEAM_WITNESS));
+              else if (okL && p1 >= right) emit_cand(sp, 2 * b + 1, iz, iw, p1);
             }
           }
           __syncwarp();
@@ -1057,23 +1068,32 @@ static cudaError_t launch_search(const jerk_plan* plan, const SearchParams& sp, 
   return cudaGetLastError();
 }
 
+#ifndef JERK_K64_NG_CAND
+#define JERK_K64_NG_CAND 2
+#endif
 template <int MODE>
 static cudaError_t launch_search64(const jerk_plan* plan, const SearchParams& sp, cudaStream_t st) {
-  const size_t smem = (size_t)2 * kEx64 * sizeof(float2) + 8 * sizeof(unsigned long long) +
-                      (MODE == MODE_PLANE ? (size_t)2 * 64 * 64 * sizeof(float) : 0);
-  cudaError_t e = cudaFuncSetAttribute(k_search64<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  // FFT groups per CTA: two (two CTAs per SM) in candidate mode, four (one CTA per SM) in plane mode: 8 warps per SM, up
+  // to 255 registers.  Six groups (12 warps, 168 registers: the register file is 16 K per scheduler, i.e. 170 registers at
+  // three warps each) measured 172 ms/search against 158 ms: the spills and the tighter schedule cost more than the
+  // third warp per scheduler hides.
+  constexpr int NG = MODE == MODE_PLANE ? 4 : JERK_K64_NG_CAND;
+  const size_t smem = (size_t)NG * kEx64 * sizeof(float2) + 4 * NG * sizeof(unsigned long long) +
+                      (MODE == MODE_PLANE ? (size_t)NG * 64 * 64 * sizeof(float) : 0);
+  cudaError_t e = cudaFuncSetAttribute(k_search64<MODE, NG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   if (getenv("JERK_DEBUG")) {
     cudaFuncAttributes fa;
-    if (cudaFuncGetAttributes(&fa, k_search64<MODE>) == cudaSuccess)
-      fprintf(stderr, "[jerk] k_search64<%d>: %d regs, %zu B local, smem %zu B\n", MODE, fa.numRegs, (size_t)fa.localSizeBytes, smem);
+    if (cudaFuncGetAttributes(&fa, k_search64<MODE, NG>) == cudaSuccess)
+      fprintf(stderr, "[jerk] k_search64<%d,%d>: %d regs, %zu B local, smem %zu B\n", MODE, NG, fa.numRegs, (size_t)fa.localSizeBytes, smem);
   }
-  // two CTAs per SM (tensor memory: 2 x 256 columns), two FFT groups per CTA, one work item per group at a time
-  long long grid = (long long)plan->sm_count * 2;
-  if (2 * grid > kMaxCtas) grid = kMaxCtas / 2;   // stash slots: one per FFT group
-  if (grid > (sp.nitems + 1) / 2) grid = (sp.nitems + 1) / 2;
+  const long long ctas_per_sm = NG == 2 ? 2 : 1;
+  long long grid = (long long)plan->sm_count * ctas_per_sm;
+  const long long slots = (long long)kMaxCtas * (long long)(kStashPerCta / (2ull * 4096 * sizeof(float)));   // stash slots of one FFT group
+  if (grid * NG > slots) grid = slots / NG;
+  if (grid > (sp.nitems + NG - 1) / NG) grid = (sp.nitems + NG - 1) / NG;
   if (grid < 1) grid = 1;
-  k_search64<MODE><<<(unsigned)grid, 128, smem, st>>>(sp);
+  k_search64<MODE, NG><<<(unsigned)grid, 64 * NG, smem, st>>>(sp);
   return cudaGetLastError();
 }
 
