@@ -268,6 +268,23 @@ def main():
     sync_all()
     e2e_ms = max(e0.elapsed_time(e1), (time.perf_counter() - t_host0) * 1e3)
 
+    # ---- upstream stage, reported beside the search: time series -> normalised spectrum on the device
+    prep_ms = None
+    if world == 1 and not args.log2n:
+        d_series = torch.from_numpy(synth.make_series(synth.config(args.config), trial=rank)).cuda()
+        d_scr = torch.empty(d_series.numel() * 4, dtype=torch.uint8, device="cuda")
+        for _ in range(3):
+            binding.prepare_spectrum(d_series, 1000, d_spec2, d_scr)
+        p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        p0.record()
+        for _ in range(10):
+            binding.prepare_spectrum(d_series, 1000, d_spec2, d_scr)
+        p1.record()
+        torch.cuda.synchronize()
+        prep_ms = p0.elapsed_time(p1) / 10
+        del d_series, d_scr
+
     t = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device="cuda")
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -298,7 +315,7 @@ def main():
                     "d2h_bytes_per_step": int(8 + min(n_e2e, max_cands) * 16), "ms_per_step": e2e_ms / args.steps},
             "gpu_launches": 3 * args.steps,
             "roofline": roofline,
-            "bank_build_ms": bank_ms, "candidates_found": n_found, "step_ms": step_ms,
+            "bank_build_ms": bank_ms, "spectrum_prep_ms": prep_ms, "candidates_found": n_found, "step_ms": step_ms,
         }
         if not args.no_cpu_baseline and world == 1:
             v, desc, pts, el = oracle_sample(cfg, X, seconds_target=15.0)

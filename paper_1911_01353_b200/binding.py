@@ -41,7 +41,8 @@ EXPORTS = [
     "jerk_plan_create", "jerk_plan_destroy", "jerk_plan_info", "jerk_template_geometry", "jerk_plane_bytes",
     "jerk_templates", "jerk_templates_taps", "jerk_search_plane", "jerk_search_candidates",
     "jerk_search_candidates_range",
-    "jerk_search_candidates_host", "jerk_harmonic_scratch_bytes", "jerk_harmonic_sum", "jerk_harmonic_plane", "jerk_strerror",
+    "jerk_search_candidates_host", "jerk_harmonic_scratch_bytes", "jerk_harmonic_sum", "jerk_harmonic_plane", "jerk_spectrum_scratch_bytes",
+    "jerk_prepare_spectrum", "jerk_strerror",
     "jerk_last_error",
 ]
 
@@ -74,6 +75,9 @@ def load_library() -> C.CDLL:
     lib.jerk_harmonic_scratch_bytes.restype = u64
     lib.jerk_harmonic_sum.argtypes = [vp, vp, i32, C.POINTER(i32), C.POINTER(C.c_float), vp, vp, u64, vp, u64, vp]
     lib.jerk_harmonic_plane.argtypes = [vp, vp, i32, i64, i64, i32, i32, i32, i32, vp, u64, vp, u64, vp, u64, vp]
+    lib.jerk_spectrum_scratch_bytes.argtypes = [i64]
+    lib.jerk_spectrum_scratch_bytes.restype = u64
+    lib.jerk_prepare_spectrum.argtypes = [vp, i64, i32, vp, vp, u64, vp]
     lib.jerk_strerror.argtypes = [i32]
     lib.jerk_strerror.restype = C.c_char_p
     lib.jerk_last_error.argtypes = [vp]
@@ -243,6 +247,24 @@ class Plan:
     def work_counters(self):
         """Diagnostic counters the last search left in d_work (item counter, seam records, seam overflow, provisional)."""
         return self.work[:64].view(dtype=__import__("torch").int64).cpu().numpy().copy()
+
+
+def prepare_spectrum(d_series, block=1000, d_spec=None, d_scratch=None, stream=None):
+    """jerk_prepare_spectrum: float32 device time series (2^11..2^25 samples) -> complex64 device spectrum of N/2 bins,
+    block-normalised; returns the spectrum as a float32 tensor of shape (N/2, 2) (the d_spec layout of the search calls)."""
+    import torch
+    lib = load_library()
+    n = d_series.numel()
+    if d_spec is None:
+        d_spec = torch.empty((n // 2, 2), dtype=torch.float32, device=d_series.device)
+    nbytes = int(lib.jerk_spectrum_scratch_bytes(n))
+    if d_scratch is None:
+        d_scratch = torch.empty(max(nbytes, 8), dtype=torch.uint8, device=d_series.device)
+    rc = lib.jerk_prepare_spectrum(C.c_void_p(d_series.data_ptr()), int(n), int(block), C.c_void_p(d_spec.data_ptr()),
+                                   C.c_void_p(d_scratch.data_ptr()), d_scratch.numel(), _stream_ptr(stream))
+    if rc != 0:
+        raise JerkError(rc, lib.jerk_strerror(rc).decode())
+    return d_spec
 
 
 def candidates_to_numpy(d_cands, d_count):

@@ -6,8 +6,9 @@ import subprocess
 import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SRC = os.path.join(HERE, "csrc", "jerk.cu")
-DEPS = [SRC, os.path.join(HERE, "csrc", "jerk_fft.cuh"), os.path.join(os.path.dirname(HERE), "include", "jerk.h")]
+SRCS = [os.path.join(HERE, "csrc", "jerk.cu"), os.path.join(HERE, "csrc", "jerk_spectrum.cu")]
+DEPS = SRCS + [os.path.join(HERE, "csrc", "jerk_fft.cuh"), os.path.join(HERE, "csrc", "jerk_fft64.cuh"),
+               os.path.join(os.path.dirname(HERE), "include", "jerk.h")]
 LIB = os.path.join(HERE, "libjerk_b200.so")
 
 NVCC_FLAGS = [
@@ -31,11 +32,11 @@ def needs_build() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False, out: str | None = None, defs: list | None = None) -> str:
-    """Compile csrc/jerk.cu.  `out`/`defs` build an experimental variant (-D flags) to another path."""
+    """Compile csrc/*.cu.  `out`/`defs` build an experimental variant (-D flags) to another path."""
     if out is None and not force and not needs_build():
         return LIB
     target = out or LIB
-    cmd = [nvcc_path()] + NVCC_FLAGS + [f"-D{d}" for d in (defs or [])] + ["-o", target, SRC]
+    cmd = [nvcc_path()] + NVCC_FLAGS + [f"-D{d}" for d in (defs or [])] + ["-o", target] + SRCS
     res = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or res.returncode != 0:
         sys.stderr.write(res.stdout + res.stderr)

@@ -147,23 +147,6 @@ __device__ __forceinline__ int bank_slot<4096>(int k) {
   return ((((k1 >> 1) << 6) + t) << 1) + (k1 & 1);
 }
 
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-// mbarrier for the split write-after-read barrier of exchange buffer B: count NT, primed so that the first wait passes
-template <int NT>
-__device__ __forceinline__ WarBarrier war_init(unsigned long long* bar, int t) {
-  if (t == 0) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(NT));
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  }
-  __syncthreads();
-  WarBarrier w;
-  w.bar = smem_u32(bar);
-  w.parity = 0;
-  w.arrive();
-  return w;
-}
-
 template <int L>
 __global__ void __launch_bounds__(FftGeom<L>::NT) k_bank(BankParams bp) {
   using Gm = FftGeom<L>;

@@ -431,6 +431,23 @@ struct WarBarrier {
   }
 };
 
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+// mbarrier for the split write-after-read barrier of exchange buffer B: count NT, primed so that the first wait passes
+template <int NT>
+__device__ __forceinline__ WarBarrier war_init(unsigned long long* bar, int t) {
+  if (t == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(NT));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  WarBarrier w;
+  w.bar = smem_u32(bar);
+  w.parity = 0;
+  w.arrive();
+  return w;
+}
+
 // Passes 1..3 on the P points in v[].  On entry v[u*R1 + k2] = x[256*k2 + b1_of(t,u)].
 // On exit v[u3*16 + n2] = X[b3_of(t,u3) + 16*R1*n2].  exA/exB: exchange buffers of FftGeom::EX1 / EX2 float2.
 // All twiddles sit on the input side of a DFT_16 (decimation in time) so that they fold into its first layer:

@@ -1,0 +1,202 @@
+// jerk_spectrum.cu — spectrum preparation upstream of the jerk search (BASELINE.json configs[0]:
+// "The real FFT gives 32768 complex bins, normalised to unit mean power per 1000-bin block"; reading S15).
+//
+//   X[k] = sum_n x[n] exp(-2 pi i k n / N), k = 0 .. N/2-1 (DC kept, Nyquist dropped);  every `block`-bin block / sqrt(mean |X|^2)
+//
+// The real series of N = 2^m samples is read as M = N/2 complex points z[j] = x[2j] + i x[2j+1]; FFT_M(z) is a four-step
+// transform M = M1 x M2 built from the register/shared-memory FFT of jerk_fft.cuh (three launches, each one read and
+// one write of the 8M-byte array, HBM-bound):
+//   k_fft_strided (A)  for every n2 < M2: Y[k1][n2] = w_M^{n2 k1} * DFT_M1 over n1 of z[M2 n1 + n2]          (columns)
+//   k_fft_strided (B)  for every k1 < M1: Z[k1 + M1 k2] = DFT_M2 over n2 of Y[k1][n2]                          (rows)
+//   k_untangle_norm    X[k] = (Z[k] + conj Z[M-k])/2 - i exp(-i pi k / M) (Z[k] - conj Z[M-k])/2, block power, scale
+// M2 = 4096 for M >= 2^22, else 1024; M1 = M / M2 in {1 .. 4096}; lengths below 1024 use a direct DFT (tiny inputs only).
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/jerk.h"
+#include "jerk_fft.cuh"
+
+namespace jerk {
+
+struct StridedFft {
+  const float2* in;
+  float2* out;
+  long long in_sb, in_se, out_sb, out_se;  // strides in float2 units: batch b, element e at in[b*in_sb + e*in_se]
+  int nbatch;                              // number of transforms
+  int per_cta;                             // consecutive batches handled by one CTA (sector reuse of the strided side)
+  int tw_den;                              // 0: none; else output k of batch b is multiplied by exp(-2 pi i b k / tw_den)
+};
+
+template <int L>
+__global__ void __launch_bounds__(FftGeom<L>::NT) k_fft_strided(StridedFft a) {
+  using Gm = FftGeom<L>;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  float2* exA = reinterpret_cast<float2*>(smem_raw);
+  float2* exB = exA + Gm::EX1;
+  float2* tw2 = exB + Gm::EX2;
+  __shared__ unsigned long long s_war;
+  const int t = threadIdx.x;
+  fill_tw2<L>(tw2, t, Gm::NT);
+  Tw3Regs<L> tw3;
+  make_tw3<L>(tw3.w, t);
+  WarBarrier war = war_init<Gm::NT>(&s_war, t);
+  for (int i = 0; i < a.per_cta; i++) {
+    const int b = blockIdx.x * a.per_cta + i;
+    if (b >= a.nbatch) break;
+    const float2* src = a.in + (long long)b * a.in_sb;
+    float2 v[Gm::P];
+#pragma unroll
+    for (int u = 0; u < Gm::NB1; u++)
+#pragma unroll
+      for (int k2 = 0; k2 < Gm::R1; k2++) v[u * Gm::R1 + k2] = src[(long long)(256 * k2 + Gm::b1_of(t, u)) * a.in_se];
+    fft_passes<L, -1>(v, tw3, tw2, exA, exB, war, t);
+    float2* dst = a.out + (long long)b * a.out_sb;
+#pragma unroll
+    for (int u = 0; u < Gm::NB2; u++)
+#pragma unroll
+      for (int n2 = 0; n2 < 16; n2++) {
+        const int k = Gm::b3_of(t, u) + 16 * Gm::R1 * n2;
+        float2 x = v[u * 16 + n2];
+        if (a.tw_den) x = cmul(x, unit_root(-(b * k), a.tw_den));
+        dst[(long long)k * a.out_se] = x;
+      }
+  }
+}
+
+// Direct DFT for lengths below 1024 (time series shorter than 2^21 samples): one thread per output.
+__global__ void __launch_bounds__(256) k_dft_direct(StridedFft a, int L) {
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (long long)a.nbatch * L) return;
+  const int b = (int)(idx % a.nbatch), k = (int)(idx / a.nbatch);   // batch fastest: neighbouring threads read neighbouring columns
+  const float2* src = a.in + (long long)b * a.in_sb;
+  double re = 0.0, im = 0.0;
+  for (int e = 0; e < L; e++) {
+    const float2 x = src[(long long)e * a.in_se];
+    const float2 w = unit_root(-(e * k), L);
+    re += (double)x.x * w.x - (double)x.y * w.y;
+    im += (double)x.x * w.y + (double)x.y * w.x;
+  }
+  float2 r = make_float2((float)re, (float)im);
+  if (a.tw_den) r = cmul(r, unit_root(-(b * k), a.tw_den));
+  a.out[(long long)b * a.out_sb + (long long)k * a.out_se] = r;
+}
+
+// One CTA per normalisation block: untangle the half-length transform into the real-input spectrum, reduce the block's
+// power in a fixed order (deterministic), scale.  Every thread re-reads only what it wrote itself.
+__global__ void __launch_bounds__(256) k_untangle_norm(const float2* __restrict__ Z, float2* __restrict__ X, int M, int block) {
+  const int k_lo = blockIdx.x * block, k_hi = min(M, k_lo + block);
+  double acc = 0.0;
+  for (int k = k_lo + threadIdx.x; k < k_hi; k += 256) {
+    float2 x;
+    if (k == 0) {
+      const float2 z0 = Z[0];
+      x = make_float2(z0.x + z0.y, 0.f);
+    } else {
+      const float2 zk = Z[k], zm = Z[M - k];
+      const float2 e = make_float2(0.5f * (zk.x + zm.x), 0.5f * (zk.y - zm.y));   // (Z[k] + conj Z[M-k]) / 2
+      const float2 o = make_float2(0.5f * (zk.x - zm.x), 0.5f * (zk.y + zm.y));   // (Z[k] - conj Z[M-k]) / 2
+      float s, c;
+      sincospif((float)k / (float)M, &s, &c);                                     // exp(-i pi k/M) = (c, -s)
+      // -i * (c - i s) * o = (-s - i c) * o
+      x = make_float2(e.x + (-s * o.x + c * o.y), e.y + (-c * o.x - s * o.y));
+    }
+    X[k] = x;
+    acc += (double)x.x * x.x + (double)x.y * x.y;
+  }
+  __shared__ double s_part[8];
+  __shared__ float s_scale;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+  if ((threadIdx.x & 31) == 0) s_part[threadIdx.x >> 5] = acc;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double tot = 0.0;
+    for (int w = 0; w < 8; w++) tot += s_part[w];
+    const double mean = tot / (double)(k_hi - k_lo);
+    s_scale = mean > 0.0 ? (float)(1.0 / sqrt(mean)) : 1.0f;
+  }
+  __syncthreads();
+  const float sc = s_scale;
+  for (int k = k_lo + threadIdx.x; k < k_hi; k += 256) {
+    const float2 x = X[k];
+    X[k] = make_float2(x.x * sc, x.y * sc);
+  }
+}
+
+template <int L>
+static cudaError_t launch_strided(const StridedFft& a, cudaStream_t st) {
+  using Gm = FftGeom<L>;
+  const size_t smem = (size_t)(Gm::EX1 + Gm::EX2 + Tw2Table<L>::FLOATS2) * sizeof(float2);
+  cudaError_t e = cudaFuncSetAttribute(k_fft_strided<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  k_fft_strided<L><<<(a.nbatch + a.per_cta - 1) / a.per_cta, Gm::NT, smem, st>>>(a);
+  return cudaGetLastError();
+}
+
+static cudaError_t run_fft(const StridedFft& a, int L, cudaStream_t st) {
+  switch (L) {
+    case 1024: return launch_strided<1024>(a, st);
+    case 2048: return launch_strided<2048>(a, st);
+    case 4096: return launch_strided<4096>(a, st);
+    case 8192: return launch_strided<8192>(a, st);
+  }
+  const long long n = (long long)a.nbatch * L;
+  k_dft_direct<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(a, L);
+  return cudaGetLastError();
+}
+
+}  // namespace jerk
+
+using namespace jerk;
+
+extern "C" {
+
+uint64_t jerk_spectrum_scratch_bytes(int64_t nsamples) {
+  if (nsamples < 2) return 0;
+  return (uint64_t)(nsamples / 2) * sizeof(float2);
+}
+
+int jerk_prepare_spectrum(const float* d_series, int64_t nsamples, int block, void* d_spec, void* d_scratch, uint64_t scratch_bytes,
+                          void* stream) {
+  if (!d_series || !d_spec || !d_scratch || block < 1) return JERK_EINVAL;
+  if (nsamples < (1 << 11) || nsamples > (1 << 25) || (nsamples & (nsamples - 1))) return JERK_EINVAL;   // 2^11 .. 2^25 samples
+  if (scratch_bytes < jerk_spectrum_scratch_bytes(nsamples)) return JERK_ENOMEM;
+  if ((uintptr_t)d_series % 8 || (uintptr_t)d_spec % 8 || (uintptr_t)d_scratch % 8) return JERK_EINVAL;
+  int dev = 0, major = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess ||
+      major != 10)
+    return JERK_ENODEV;   // sm_100 only: this library has no other code path
+  cudaStream_t st = (cudaStream_t)stream;
+  const int M = (int)(nsamples / 2);
+  const int M2 = M >= (1 << 22) ? 4096 : 1024;
+  const int M1 = M / M2;
+  float2* Y = (float2*)d_spec;       // step A output lives in the result buffer; step B writes the scratch buffer
+  float2* Z = (float2*)d_scratch;
+  StridedFft a;
+  a.in = (const float2*)d_series;
+  a.out = Y;
+  a.in_sb = 1;
+  a.in_se = M2;
+  a.out_sb = 1;
+  a.out_se = M2;
+  a.nbatch = M2;
+  a.per_cta = 4;
+  a.tw_den = M;
+  if (run_fft(a, M1, st) != cudaSuccess) return JERK_ECUDA;
+  StridedFft b;
+  b.in = Y;
+  b.out = Z;
+  b.in_sb = M2;
+  b.in_se = 1;
+  b.out_sb = 1;
+  b.out_se = M1;
+  b.nbatch = M1;
+  b.per_cta = M1 >= 4 ? 4 : 1;
+  b.tw_den = 0;
+  if (run_fft(b, M2, st) != cudaSuccess) return JERK_ECUDA;
+  k_untangle_norm<<<(M + block - 1) / block, 256, 0, st>>>(Z, (float2*)d_spec, M, block);
+  if (cudaGetLastError() != cudaSuccess) return JERK_ECUDA;
+  return JERK_OK;
+}
+
+}  // extern "C"

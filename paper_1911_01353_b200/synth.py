@@ -121,11 +121,9 @@ def chirp_series(n: int, r0: float, z0: float, w0: float, amp: float) -> np.ndar
     return amp * np.cos(2.0 * np.pi * ph)
 
 
-def make_spectrum(cfg: Config, noise: bool = True, trial: int = 0) -> np.ndarray:
-    """complex64 spectrum X[0..nbins) of config `cfg`; fills cfg.signals.
-
-    `trial` > 0 gives an independent realisation of the same workload (another "DM trial": bench.py uses one per
-    rank); trial 0 is the configuration the parity tests pin."""
+def make_series(cfg: Config, noise: bool = True, trial: int = 0) -> np.ndarray:
+    """float32 time series of config `cfg` (noise + injected signals); fills cfg.signals.  The input of the
+    spectrum-preparation stage and the first half of make_spectrum."""
     rng = np.random.Generator(np.random.PCG64(SEED_BASE + cfg.index + 1000 * trial))
     n = cfg.n
     x = rng.standard_normal(n, dtype=np.float32).astype(np.float64)
@@ -136,7 +134,16 @@ def make_spectrum(cfg: Config, noise: bool = True, trial: int = 0) -> np.ndarray
         a = np.sqrt(4.0 * p / n)
         for k in range(1, cfg.harmonics + 1):
             x += chirp_series(n, k * r0, k * z0, k * w0, a / k)
-    x = x.astype(np.float32).astype(np.float64)
+    return x.astype(np.float32)
+
+
+def make_spectrum(cfg: Config, noise: bool = True, trial: int = 0) -> np.ndarray:
+    """complex64 spectrum X[0..nbins) of config `cfg`; fills cfg.signals.
+
+    `trial` > 0 gives an independent realisation of the same workload (another "DM trial": bench.py uses one per
+    rank); trial 0 is the configuration the parity tests pin."""
+    n = cfg.n
+    x = make_series(cfg, noise, trial).astype(np.float64)
     X = np.fft.rfft(x)[: n // 2]
     if noise:
         X = block_normalise(X)

@@ -1,0 +1,87 @@
+"""GPU parity of the spectrum-preparation stage against oracle/spectrum_oracle.py, through the C-ABI.
+
+Tolerance: the fp32 four-step FFT of M = N/2 points has a relative rms error of about
+0.3 * eps * log2(M) ~ 4e-7 of the rms bin amplitude; the normalised spectrum has unit rms, and the largest of 2^22 errors
+is ~5.5 sigma, so |X_gpu - X_ref| <= 2e-5 * max(1, |X_ref|) leaves a factor ~5 of margin at the largest size."""
+import numpy as np
+import pytest
+
+from oracle import spectrum_oracle as so
+from paper_1911_01353_b200 import binding, build, synth
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+TOL = 2e-5
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    build.build()
+    binding.load_library()
+
+
+def _run(x, block=1000):
+    d = torch.from_numpy(np.ascontiguousarray(x, dtype=np.float32)).cuda()
+    out = binding.prepare_spectrum(d, block)
+    torch.cuda.synchronize()
+    assert torch.equal(d.cpu(), torch.from_numpy(np.ascontiguousarray(x, dtype=np.float32)))   # input untouched
+    return out.cpu().numpy().view(np.complex64).reshape(-1)
+
+
+def _check(x, block=1000):
+    got = _run(x, block).astype(np.complex128)
+    ref = so.prepare_spectrum(np.asarray(x, dtype=np.float32).astype(np.float64), block)
+    err = np.abs(got - ref) / np.maximum(1.0, np.abs(ref))
+    assert err.max() <= TOL, (err.max(), int(err.argmax()))
+    return got, ref
+
+
+@pytest.mark.parametrize("log2n", [11, 12, 16, 20, 21, 22, 23])
+def test_noise_series_all_decompositions(log2n):
+    """2^11 (M1 = 1), 2^12..2^20 (direct column DFT), 2^21/2^22 (1024 x 1024, 2048 x 1024), 2^23 (1024 x 4096)."""
+    rng = np.random.Generator(np.random.PCG64(1911013530 + log2n))
+    x = rng.standard_normal(1 << log2n, dtype=np.float32)
+    x[: 1 << (log2n - 1)] *= 3.0          # block means differ along the spectrum only weakly: add a coloured part
+    x += 0.5 * np.cos(2 * np.pi * 0.013 * np.arange(x.size)).astype(np.float32)
+    got, ref = _check(x)
+    m = so.block_powers(got, 1000)
+    assert np.allclose(m, 1.0, atol=2e-6)
+
+
+def test_config1_series_gives_the_search_input():
+    """The time series of BASELINE config 1 through the GPU stage equals the spectrum the search tests use."""
+    cfg = synth.config(1)
+    x = synth.make_series(cfg)
+    got, ref = _check(x)
+    want = synth.make_spectrum(synth.config(1))
+    assert np.abs(got - want).max() <= TOL * np.abs(want).max()
+
+
+def test_config4_size_2_pow_25():
+    rng = np.random.Generator(np.random.PCG64(77))
+    x = rng.standard_normal(1 << 25, dtype=np.float32)
+    _check(x)
+
+
+def test_pure_tone_and_ragged_block():
+    # a tone of normalised power ~1e4 in unit-variance noise (fp32 cannot carry a tone 10^5 times above the noise floor:
+    # its rounding error alone would exceed the tolerance relative to the other blocks' rms)
+    n, k0 = 1 << 16, 5000
+    x = np.sqrt(4.0 * 1e4 / n) * np.cos(2 * np.pi * k0 * np.arange(n) / n) + np.random.default_rng(1).standard_normal(n)
+    got, ref = _check(x, block=777)       # 32768 = 42 * 777 + 134: ragged last block
+    assert int(np.argmax(np.abs(got))) == k0
+
+
+def test_errors():
+    lib = binding.load_library()
+    d = torch.zeros(3000, dtype=torch.float32, device="cuda")
+    with pytest.raises(binding.JerkError):
+        binding.prepare_spectrum(d)                       # not a power of two
+    d = torch.zeros(1 << 10, dtype=torch.float32, device="cuda")
+    with pytest.raises(binding.JerkError):
+        binding.prepare_spectrum(d)                       # too short
+    d = torch.zeros(1 << 12, dtype=torch.float32, device="cuda")
+    with pytest.raises(binding.JerkError):
+        binding.prepare_spectrum(d, d_scratch=torch.empty(16, dtype=torch.uint8, device="cuda"))   # scratch too small
+    assert lib.jerk_spectrum_scratch_bytes(1 << 12) == (1 << 11) * 8
