@@ -306,3 +306,35 @@ def test_candidates_range_union(idx, world, thr):
     # empty box: count 0, no launch error
     d_c, d_n = plan.search_candidates_range(d_spec, thr, 0, 0, 0, cfg.nw)
     assert int(d_n.item()) == 0
+
+
+# ------------------------------------------------------------------------------------------------ FDAS-only mode (8(f) N4)
+@pytest.mark.gpu
+@pytest.mark.parametrize("seg_len", [1024, 4096])
+def test_fdas_only_mode_w0(seg_len):
+    """wmax = 0: the acceleration-only (FDAS) search the paper extends: one w-row, templates are the
+    Fresnel responses; full plane rows and candidates against the oracle."""
+    nbins = 40000
+    X = synth.random_spectrum(nbins, seed=424242)
+    # inject one accelerated signal: X += A * R_{z0,0}(k - r0) (the response itself), amplitude 9
+    z0, r0 = 36.0, 20000
+    c, hw, lattice = orc.template(z0, 0.0)
+    m, p0_taps = orc.phase_taps(c, hw, lattice, 0)
+    X = X.astype(np.complex128)
+    X[r0 + m] += 9.0 * p0_taps
+    X = X.astype(np.complex64)
+    plan = binding.Plan(nbins, 50.0, 2.0, 0.0, 20.0, 2, seg_len)
+    assert plan.info.nw == 1 and plan.info.nz == 51
+    plan.templates()
+    d_spec = binding.spectrum_to_device(X)
+    zs = orc.grid_values(50.0, 2.0)
+    b_lo, b_cnt = 19000, 2000
+    rows = [0, 7, 25, 43, 50]
+    refs = H.oracle_rows(X, [(zs[iz], 0.0) for iz in rows], b_lo, b_cnt)
+    for iz, ref in zip(rows, refs):
+        P = plan.search_plane(d_spec, b_lo, b_cnt, iz, 1, 0, 1).cpu().numpy()[0, 0]
+        H.assert_power_close(P, ref, f"fdas row iz={iz}")
+    d_c, d_n = plan.search_candidates(d_spec, 30.0)
+    cands, n = binding.candidates_to_numpy(d_c, d_n)
+    best = cands[np.argmax(cands["power"])]
+    assert (zs[best["iz"]], best["iw"], best["j"]) == (z0, 0, 2 * r0)

@@ -1,6 +1,6 @@
 """GPU parity of the spectrum-preparation stage against oracle/spectrum_oracle.py, through the C-ABI.
 
-Tolerance (DESIGN.md section 12): the fp32 four-step FFT of M = N/2 points has a relative rms error of about
+Tolerance (DESIGN.md section 11): the fp32 four-step FFT of M = N/2 points has a relative rms error of about
 0.3 * eps * log2(M) ~ 4e-7 of the rms bin amplitude; the normalised spectrum has unit rms, and the largest of 2^22 errors
 is ~5.5 sigma, so |X_gpu - X_ref| <= 2e-5 * max(1, |X_ref|) leaves a factor ~5 of margin at the largest size."""
 import numpy as np
