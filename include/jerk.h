@@ -147,6 +147,25 @@ int jerk_search_candidates_range(jerk_plan* plan, const void* d_spec, float thre
                                  unsigned long long* d_count, void* d_work, uint64_t work_bytes, void* stream);
 
 /*
+ * jerk_search_candidates_stats + jerk_snr_filter — the paper's own candidate front end (PAPER.md:43
+ * peaks "above a certain threshold" of the output plane, "mean and standard deviation along with candidate
+ * selection dominate the execution time"), fused: ONE pass of the search kernel collects local-max candidates above the
+ * absolute power `threshold` AND the per-row sums of P and P^2 over all 2*nbins points of every (z,w) row:
+ * d_rowstats (DEVICE, double[ntemplates][2], 8-byte aligned, rowstats_bytes >= 16*ntemplates) receives
+ * {sum P, sum P^2} of row ti = iw*nz + iz (zeroed by the call; fp64 atomics: the last bits depend on scheduling).
+ * jerk_snr_filter then keeps the candidates with snr = (P - mean_row)/std_row > snr_threshold (population standard
+ * deviation; rows with zero variance keep nothing), out of place into d_cands_out / d_count_out (DEVICE, zeroed by
+ * the call; unordered; overflow as in jerk_search_candidates) with the snr stored as float bits in `flags`.
+ * seg_len 4096 plans only (JERK_EINVAL otherwise).  Other arguments and errors as jerk_search_candidates.
+ */
+int jerk_search_candidates_stats(jerk_plan* plan, const void* d_spec, float threshold, jerk_cand* d_cands,
+                                 int64_t max_cands, unsigned long long* d_count, double* d_rowstats,
+                                 uint64_t rowstats_bytes, void* d_work, uint64_t work_bytes, void* stream);
+int jerk_snr_filter(jerk_plan* plan, const double* d_rowstats, const jerk_cand* d_cands_in,
+                    const unsigned long long* d_count_in, int64_t max_in, float snr_threshold,
+                    jerk_cand* d_cands_out, int64_t max_out, unsigned long long* d_count_out, void* stream);
+
+/*
  * jerk_search_candidates_host — the same search with HOST input/output (end-to-end entry point):
  * copies h_spec (host, ideally pinned, nbins complex64) to d_spec, searches, copies the count and
  * min(count, max_cands) records back to h_count / h_cands and synchronises the stream before returning.

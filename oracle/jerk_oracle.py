@@ -18,6 +18,8 @@ Notation follows PAPER.md:39 (z = fdot*T^2, w = fddot*T^3) and SURVEY.md section
   D  plane      A[j; z,w] = sum_m X[b+m] * conj(R_{z,w}(m - p/2)),  j = 2b+p ;  P = |A|^2
   E  candidates P > thr, P > P[j-1], P >= P[j+1] within one (z,w) row
   F  harmonic   S_h(j,iz',iw') = sum_{k=1..h} P[rnd(j k/h); rnd(iz' k/h), rnd(iw' k/h)]
+  G  row S/N    mean and (population) standard deviation of P over the 2*nbins points of one (z,w) row;
+                snr = (P - mean) / std; a candidate is kept iff snr > snr_threshold
 
 Pins (tests/test_oracle_pins.py): closed-form sinc (z=w=0), Fresnel closed form (w=0),
 conjugate symmetry, Parseval unit energy, quadrature refinement, exact-grid recovery of a
@@ -220,3 +222,36 @@ def harmonic_sum_volume(P: np.ndarray, h: int) -> np.ndarray:
                 izk = rnd_frac(iz - cz, k, h) + cz
                 S[iw, iz] += P[iwk, izk, js]
     return S
+
+
+# --------------------------------------------------------------------------- G: row statistics and S/N
+def row_stats(P) -> tuple[float, float]:
+    """(sum of P, sum of P^2) over every point of one (z,w) row, float64 (what the fused kernel accumulates)."""
+    P = np.asarray(P, dtype=np.float64)
+    return float(np.sum(P)), float(np.sum(P * P))
+
+
+def row_mean_std(P) -> tuple[float, float]:
+    """Mean and population standard deviation of the row: the paper's "mean and standard deviation" of the output
+    (PAPER.md:45), taken per (z,w) row over all 2*nbins points."""
+    P = np.asarray(P, dtype=np.float64)
+    s1, s2 = row_stats(P)
+    mean = s1 / P.size
+    var = s2 / P.size - mean * mean
+    return mean, math.sqrt(var) if var > 0.0 else 0.0
+
+
+def snr(power, mean: float, std: float):
+    """(P - mean) / std."""
+    return (np.asarray(power, dtype=np.float64) - mean) / std
+
+
+def snr_filter(j, power, mean: float, std: float, snr_threshold: float):
+    """Candidates of one row (arrays j, power) with snr > snr_threshold: (j, power, snr).  A row with std = 0 keeps nothing."""
+    j = np.asarray(j)
+    power = np.asarray(power, dtype=np.float64)
+    if not std > 0.0:
+        return j[:0], power[:0], power[:0]
+    s = snr(power, mean, std)
+    keep = s > snr_threshold
+    return j[keep], power[keep], s[keep]

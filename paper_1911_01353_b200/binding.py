@@ -40,7 +40,7 @@ class PlanInfo(C.Structure):
 EXPORTS = [
     "jerk_plan_create", "jerk_plan_destroy", "jerk_plan_info", "jerk_template_geometry", "jerk_plane_bytes",
     "jerk_templates", "jerk_templates_taps", "jerk_search_plane", "jerk_search_candidates",
-    "jerk_search_candidates_range",
+    "jerk_search_candidates_range", "jerk_search_candidates_stats", "jerk_snr_filter",
     "jerk_search_candidates_host", "jerk_harmonic_scratch_bytes", "jerk_harmonic_sum", "jerk_harmonic_plane", "jerk_spectrum_scratch_bytes",
     "jerk_prepare_spectrum", "jerk_strerror",
     "jerk_last_error",
@@ -70,6 +70,8 @@ def load_library() -> C.CDLL:
     lib.jerk_search_plane.argtypes = [vp, vp, i64, i64, i32, i32, i32, i32, vp, u64, vp, u64, vp]
     lib.jerk_search_candidates.argtypes = [vp, vp, C.c_float, vp, i64, vp, vp, u64, vp]
     lib.jerk_search_candidates_range.argtypes = [vp, vp, C.c_float, i32, i32, i32, i32, vp, i64, vp, vp, u64, vp]
+    lib.jerk_search_candidates_stats.argtypes = [vp, vp, C.c_float, vp, i64, vp, vp, u64, vp, u64, vp]
+    lib.jerk_snr_filter.argtypes = [vp, vp, vp, vp, i64, C.c_float, vp, i64, vp, vp]
     lib.jerk_search_candidates_host.argtypes = [vp, vp, C.c_float, vp, i64, vp, vp, vp, vp, vp, u64, vp]
     lib.jerk_harmonic_scratch_bytes.argtypes = [vp]
     lib.jerk_harmonic_scratch_bytes.restype = u64
@@ -194,6 +196,30 @@ class Plan:
             C.c_void_p(d_cands.data_ptr()), int(max_cands), C.c_void_p(d_count.data_ptr()), C.c_void_p(work.data_ptr()),
             work.numel(), _stream_ptr(stream)))
         return d_cands, d_count
+
+    def search_candidates_stats(self, d_spec, threshold, max_cands=1 << 20, stream=None):
+        """jerk_search_candidates_stats: (d_cands, d_count, d_rowstats float64[T, 2] = {sum P, sum P^2} per (z,w) row)."""
+        import torch
+        d_cands = torch.empty(max_cands * 16, dtype=torch.uint8, device=d_spec.device)
+        d_count = torch.zeros(1, dtype=torch.int64, device=d_spec.device)
+        d_stats = torch.empty((self.info.ntemplates, 2), dtype=torch.float64, device=d_spec.device)
+        work = self._ensure_work(d_spec.device)
+        self._check(self._lib.jerk_search_candidates_stats(
+            self._h, C.c_void_p(d_spec.data_ptr()), float(threshold), C.c_void_p(d_cands.data_ptr()), int(max_cands),
+            C.c_void_p(d_count.data_ptr()), C.c_void_p(d_stats.data_ptr()), d_stats.numel() * 8, C.c_void_p(work.data_ptr()),
+            work.numel(), _stream_ptr(stream)))
+        return d_cands, d_count, d_stats
+
+    def snr_filter(self, d_stats, d_cands, d_count, snr_threshold, max_out=1 << 20, stream=None):
+        """jerk_snr_filter: (d_out, d_count_out); records carry the snr as float bits in `flags`."""
+        import torch
+        d_out = torch.empty(max_out * 16, dtype=torch.uint8, device=d_cands.device)
+        d_nout = torch.zeros(1, dtype=torch.int64, device=d_cands.device)
+        self._check(self._lib.jerk_snr_filter(
+            self._h, C.c_void_p(d_stats.data_ptr()), C.c_void_p(d_cands.data_ptr()), C.c_void_p(d_count.data_ptr()),
+            d_cands.numel() // 16, float(snr_threshold), C.c_void_p(d_out.data_ptr()), int(max_out),
+            C.c_void_p(d_nout.data_ptr()), _stream_ptr(stream)))
+        return d_out, d_nout
 
     def search_candidates_host(self, h_spec, threshold, h_cands, h_count, d_spec, d_cands, d_count, stream=None):
         """jerk_search_candidates_host: pinned host tensors in/out, device staging caller-owned; synchronous."""

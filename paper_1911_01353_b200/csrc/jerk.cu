@@ -238,6 +238,7 @@ struct SearchParams {
   unsigned long long* work;  // [0] item counter, [1] seam count, [2] seam overflow, [3] provisional
   jerk_cand* seams;
   float* stash;              // [kMaxCtas][2][L]: powers of the current template, written only on the rare path
+  double* rowstats;          // MODE_CAND_STATS: [T][2] running sum of P and of P^2 over the valid points of every (z,w) row
 };
 
 __device__ __forceinline__ void emit_cand(const SearchParams& sp, int j, int iz, int iw, float pw) {
@@ -267,7 +268,7 @@ __device__ __forceinline__ void emit_seam(const SearchParams& sp, int j, int iz,
   }
 }
 
-enum { MODE_PLANE = 0, MODE_CAND = 1 };
+enum { MODE_PLANE = 0, MODE_CAND = 1, MODE_CAND_STATS = 2 };   // 2: candidate mode + per-row power statistics (seg_len 4096)
 enum { SEAM_LEFT = 1u, SEAM_RIGHT = 2u, SEAM_WITNESS = 4u };
 
 #ifndef JERK_MINBLOCKS_4096
@@ -742,6 +743,27 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
           }
         }
       } else {
+        if (MODE == MODE_CAND_STATS) {
+          // SURVEY.md 8(f) N2 / PAPER.md:43,45: mean and standard deviation of every (z,w) row, fused: sum of P and P^2
+          // over the valid points of this unit, one fp64 atomic pair per warp
+          float s1 = 0.f, s2 = 0.f;
+#pragma unroll
+          for (int r = 0; r < P; r++) {
+            const int n = t + 64 * dft64_out_index(r);
+            const float p = (n >= n_lo && n < n_hi) ? pw[r] : 0.f;
+            s1 += p;
+            s2 = fmaf(p, p, s2);
+          }
+#pragma unroll
+          for (int o = 16; o > 0; o >>= 1) {
+            s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+            s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+          }
+          if (lane == 0) {
+            atomicAdd(sp.rowstats + 2 * (size_t)ti, (double)s1);
+            atomicAdd(sp.rowstats + 2 * (size_t)ti + 1, (double)s2);
+          }
+        }
         // ---- a-5: threshold + local max.  Hot path: one max-reduction and a vote.
         float mx = pw[0];
 #pragma unroll
@@ -820,6 +842,31 @@ __global__ void k_resolve(SearchParams sp) {
     if (ok) {
       atomicAdd(sp.work + 3, 1ULL);
       emit_cand(sp, a.j, a.iz, a.iw, a.power);
+    }
+  }
+}
+
+// S/N filter of a candidate list ("above a certain threshold" in units of the output's
+// standard deviation): snr = (P - mean_row) / std_row with the row statistics of k_search64<MODE_CAND_STATS>.
+__global__ void k_snr_filter(const double* __restrict__ rowstats, int nz, double npts_row, const jerk_cand* __restrict__ in,
+                             const unsigned long long* __restrict__ count_in, long long max_in, float snr_thr, jerk_cand* out,
+                             long long max_out, unsigned long long* count_out) {
+  unsigned long long n = *count_in;
+  if (n > (unsigned long long)max_in) n = (unsigned long long)max_in;
+  for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i < n;
+       i += (unsigned long long)gridDim.x * blockDim.x) {
+    jerk_cand c = in[i];
+    const size_t ti = (size_t)c.iw * nz + c.iz;
+    const double mean = rowstats[2 * ti] / npts_row;
+    const double var = rowstats[2 * ti + 1] / npts_row - mean * mean;
+    if (!(var > 0.0)) continue;
+    const float snr = (float)(((double)c.power - mean) / sqrt(var));
+    if (snr > snr_thr) {
+      const unsigned long long slot = atomicAdd(count_out, 1ULL);
+      if ((long long)slot < max_out) {
+        c.flags = __float_as_uint(snr);
+        out[slot] = c;
+      }
     }
   }
 }
@@ -1398,6 +1445,52 @@ int jerk_search_candidates(jerk_plan* p, const void* d_spec, float threshold, je
   if (!p) return JERK_EINVAL;
   return jerk_search_candidates_range(p, d_spec, threshold, 0, p->nz, 0, p->nw, d_cands, max_cands, d_count, d_work, work_bytes,
                                       stream);
+}
+
+int jerk_search_candidates_stats(jerk_plan* p, const void* d_spec, float threshold, jerk_cand* d_cands, int64_t max_cands,
+                                 unsigned long long* d_count, double* d_rowstats, uint64_t rowstats_bytes, void* d_work,
+                                 uint64_t work_bytes, void* stream) {
+  int rc = check_common(p, d_spec, d_work, work_bytes);
+  if (rc) return rc;
+  if (!d_cands || !d_count || !d_rowstats || max_cands < 0) return JERK_EINVAL;
+  if (p->L != 4096) return fail(p, JERK_EINVAL, "row statistics are fused into the seg_len 4096 kernel only");
+  if (rowstats_bytes < (uint64_t)p->T * 2 * sizeof(double)) return fail(p, JERK_ENOMEM, "row statistics buffer smaller than 16 bytes per template");
+  if ((uintptr_t)d_rowstats % 8) return fail(p, JERK_EINVAL, "d_rowstats must be 8-byte aligned");
+  cudaStream_t st = (cudaStream_t)stream;
+  SearchParams sp;
+  fill_params(p, sp, d_spec, d_work);
+  add_job(p, sp, 0, p->nbins, 0, p->nz, 0, p->nw, nullptr, kChunkTP);
+  sp.threshold = threshold;
+  sp.cands = d_cands;
+  sp.max_cands = max_cands;
+  sp.count = d_count;
+  sp.rowstats = d_rowstats;
+  cudaError_t e = cudaMemsetAsync(d_rowstats, 0, (size_t)p->T * 2 * sizeof(double), st);
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("row statistics memset: ") + cudaGetErrorString(e));
+  k_reset<<<1, 32, 0, st>>>(sp.work, d_count);
+  e = launch_search64<MODE_CAND_STATS>(p, sp, st);
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_search64(cand+stats) launch: ") + cudaGetErrorString(e));
+  k_resolve<<<p->sm_count, 256, 0, st>>>(sp);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_resolve launch: ") + cudaGetErrorString(e));
+  return JERK_OK;
+}
+
+int jerk_snr_filter(jerk_plan* p, const double* d_rowstats, const jerk_cand* d_cands_in, const unsigned long long* d_count_in,
+                    int64_t max_in, float snr_threshold, jerk_cand* d_cands_out, int64_t max_out, unsigned long long* d_count_out,
+                    void* stream) {
+  if (!p || !d_rowstats || !d_cands_in || !d_count_in || !d_cands_out || !d_count_out || max_in < 0 || max_out < 0) return JERK_EINVAL;
+  if (d_cands_in == d_cands_out) return fail(p, JERK_EINVAL, "jerk_snr_filter is out of place");
+  int rc = ensure_device(p);
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaError_t e = cudaMemsetAsync(d_count_out, 0, sizeof(unsigned long long), st);
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("count memset: ") + cudaGetErrorString(e));
+  k_snr_filter<<<p->sm_count, 256, 0, st>>>(d_rowstats, p->nz, 2.0 * (double)p->nbins, d_cands_in, d_count_in, max_in, snr_threshold,
+                                            d_cands_out, max_out, d_count_out);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_snr_filter launch: ") + cudaGetErrorString(e));
+  return JERK_OK;
 }
 
 int jerk_search_candidates_host(jerk_plan* p, const void* h_spec, float threshold, jerk_cand* h_cands, int64_t max_cands,

@@ -1,0 +1,82 @@
+"""GPU parity of the fused row statistics + S/N candidate filter against oracle/jerk_oracle.py section G."""
+import numpy as np
+import pytest
+
+from oracle import jerk_oracle as orc
+from paper_1911_01353_b200 import binding, build, synth
+from tests import helpers as H
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+NBINS, ZMAX, DZ, WMAX, DW, THR, SNR_THR = 30000, 20.0, 2.0, 60.0, 20.0, 8.0, 9.0
+
+
+@pytest.fixture(scope="module")
+def setup():
+    build.build()
+    binding.load_library()
+    X = synth.random_spectrum(NBINS, seed=20251104).astype(np.complex128)
+    c, hw, lattice = orc.template(10.0, 40.0)
+    m, taps = orc.phase_taps(c, hw, lattice, 0)
+    X[12345 + m] += 8.0 * taps                      # one strong jerk signal at (r, z, w) = (12345, 10, 40)
+    X[:1500] *= 3.0                                 # and a loud band: S/N must be judged against the row's own statistics
+    X = X.astype(np.complex64)
+    plan = binding.Plan(NBINS, ZMAX, DZ, WMAX, DW, 2, 4096)
+    plan.templates()
+    d_spec = binding.spectrum_to_device(X)
+    zs, ws = orc.grid_values(ZMAX, DZ), orc.grid_values(WMAX, DW)
+    zw = [(zs[iz], ws[iw]) for iw in range(ws.size) for iz in range(zs.size)]
+    rows = H.oracle_rows(X, zw, 0, NBINS)            # every row of the plane: 147 x 60000 points
+    return X, plan, d_spec, zs, ws, rows
+
+
+def test_row_statistics_match_the_oracle(setup):
+    X, plan, d_spec, zs, ws, rows = setup
+    d_c, d_n, d_stats = plan.search_candidates_stats(d_spec, THR)
+    stats = d_stats.cpu().numpy()
+    want = np.array([orc.row_stats(P) for P in rows])
+    # every power is within 1e-3 * max(1, P) (north_star); the sums of 60000 of them average the error down
+    assert np.abs(stats[:, 0] / want[:, 0] - 1.0).max() < 2e-5
+    assert np.abs(stats[:, 1] / want[:, 1] - 1.0).max() < 1e-4
+    # the candidates of the fused pass are those of the plain candidate search, record for record
+    plain, n0 = binding.candidates_to_numpy(*plan.search_candidates(d_spec, THR))
+    fused, n1 = binding.candidates_to_numpy(d_c, d_n)
+    assert n0 == n1 and np.array_equal(np.sort(plain, order=["iw", "iz", "j"]), np.sort(fused, order=["iw", "iz", "j"]))
+
+
+def test_snr_filter_matches_the_oracle(setup):
+    X, plan, d_spec, zs, ws, rows = setup
+    d_c, d_n, d_stats = plan.search_candidates_stats(d_spec, THR)
+    d_o, d_no = plan.snr_filter(d_stats, d_c, d_n, SNR_THR)
+    kept, nk = binding.candidates_to_numpy(d_o, d_no)
+    cands, n = binding.candidates_to_numpy(d_c, d_n)
+    assert 0 < nk < n
+    kept_keys = {(int(c["iw"]), int(c["iz"]), int(c["j"])): c for c in kept}
+    nz = zs.size
+    strong = 0
+    for c in cands:
+        P = rows[int(c["iw"]) * nz + int(c["iz"])]
+        mean, std = orc.row_mean_std(P)
+        s_ref = float(orc.snr(P[int(c["j"])], mean, std))
+        key = (int(c["iw"]), int(c["iz"]), int(c["j"]))
+        if s_ref > 1.02 * SNR_THR:
+            strong += 1
+            assert key in kept_keys, (key, s_ref)
+        if s_ref < 0.98 * SNR_THR:
+            assert key not in kept_keys, (key, s_ref)
+        if key in kept_keys:
+            s_gpu = float(np.array(kept_keys[key]["flags"], dtype=np.uint32).view(np.float32))
+            assert abs(s_gpu - s_ref) <= 2e-3 * max(1.0, abs(s_ref))
+    assert strong > 0
+    # the injected signal survives at its grid point
+    iz0, iw0 = int(np.argmin(np.abs(zs - 10.0))), int(np.argmin(np.abs(ws - 40.0)))
+    assert (iw0, iz0, 2 * 12345) in kept_keys
+
+
+def test_stats_mode_needs_seg_len_4096(setup):
+    X, plan, d_spec, zs, ws, rows = setup
+    p2 = binding.Plan(NBINS, ZMAX, DZ, WMAX, DW, 2, 1024)
+    p2.templates()
+    with pytest.raises(binding.JerkError):
+        p2.search_candidates_stats(d_spec, THR)

@@ -320,3 +320,40 @@ def test_p10_harmonic_injection_noise_free():
         # moving the top harmonic off by one grid step in any coordinate lowers the sum
         for dj, da, db in ((2, 0, 0), (-2, 0, 0), (0, 1, 0), (0, 0, 1)):
             assert orc.harmonic_sum_point(P_lookup, h * j0 + dj, h * a0 + da, h * b0 + db, h) < s
+
+
+# ------------------------------------------------------------------------------------------------ G: row statistics, S/N
+def test_row_mean_std_against_textbook_routines():
+    import statistics
+    rng = np.random.default_rng(11)
+    P = rng.exponential(1.0, 500)
+    mean, std = orc.row_mean_std(P)
+    assert abs(mean - statistics.fmean(P.tolist())) < 1e-12
+    assert abs(std - statistics.pstdev(P.tolist())) < 1e-12
+    s1, s2 = orc.row_stats(P)
+    assert abs(s1 - math.fsum(P.tolist())) < 1e-9 and abs(s2 - math.fsum((P * P).tolist())) < 1e-9
+    assert orc.row_mean_std(np.full(10, 3.0)) == (3.0, 0.0)
+
+
+def test_noise_row_has_std_equal_to_mean():
+    """Unit-variance complex Gaussian X: P is exponential (pin P7), whose standard deviation equals its mean = sum |h|^2."""
+    X = synth.random_spectrum(60000, seed=99)
+    P = orc.power_row(X, 10.0, 40.0, 0, 60000)
+    mean, std = orc.row_mean_std(P)
+    assert abs(mean - 0.9925) < 0.015            # SURVEY.md 8(c) P7: mean 0.9925 for (10, 40)
+    assert abs(std / mean - 1.0) < 0.03
+
+
+def test_snr_is_scale_invariant_and_filter_is_a_plain_comparison():
+    X = synth.random_spectrum(8000, seed=5)
+    P = orc.power_row(X, 4.0, 20.0, 0, 8000)
+    P9 = orc.power_row(X.astype(np.complex128) * 3.0, 4.0, 20.0, 0, 8000)
+    m1, s1 = orc.row_mean_std(P)
+    m9, s9 = orc.row_mean_std(P9)
+    assert abs(m9 / m1 - 9.0) < 1e-9 and abs(s9 / s1 - 9.0) < 1e-9
+    assert np.allclose(orc.snr(P, m1, s1), orc.snr(P9, m9, s9), atol=1e-9)
+    j = np.arange(P.size)
+    kj, kp, ks = orc.snr_filter(j, P, m1, s1, 4.0)
+    want = [int(i) for i in range(P.size) if (P[i] - m1) / s1 > 4.0]
+    assert kj.tolist() == want and np.allclose(ks, (kp - m1) / s1)
+    assert orc.snr_filter(j, P, m1, 0.0, 4.0)[0].size == 0
