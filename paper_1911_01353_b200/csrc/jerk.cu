@@ -746,14 +746,32 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
         if (MODE == MODE_CAND_STATS) {
           // SURVEY.md 8(f) N2 / PAPER.md:43,45: mean and standard deviation of every (z,w) row, fused: sum of P and P^2
           // over the valid points of this unit, one fp64 atomic pair per warp
-          float s1 = 0.f, s2 = 0.f;
+          // four independent accumulator pairs (no 64-long dependent chains); registers whose n1 = n / 64 lies in [8, 56)
+          // are valid for every thread of an interior segment (hw_max <= 512) and are summed without a predicate
+          float a1[4] = {0.f, 0.f, 0.f, 0.f}, a2[4] = {0.f, 0.f, 0.f, 0.f};
+          const bool inner_valid = __all_sync(0xffffffffu, n_lo <= t + 64 * 8 && n_hi >= t + 64 * 56);
+          if (inner_valid) {
 #pragma unroll
-          for (int r = 0; r < P; r++) {
-            const int n = t + 64 * dft64_out_index(r);
-            const float p = (n >= n_lo && n < n_hi) ? pw[r] : 0.f;
-            s1 += p;
-            s2 = fmaf(p, p, s2);
+            for (int r = 0; r < P; r++) {
+              const int n1 = dft64_out_index(r);
+              float p = pw[r];
+              if (n1 < 8 || n1 >= 56) {
+                const int n = t + 64 * n1;
+                p = (n >= n_lo && n < n_hi) ? p : 0.f;
+              }
+              a1[r & 3] += p;
+              a2[r & 3] = fmaf(p, p, a2[r & 3]);
+            }
+          } else {
+#pragma unroll
+            for (int r = 0; r < P; r++) {
+              const int n = t + 64 * dft64_out_index(r);
+              const float p = (n >= n_lo && n < n_hi) ? pw[r] : 0.f;
+              a1[r & 3] += p;
+              a2[r & 3] = fmaf(p, p, a2[r & 3]);
+            }
           }
+          float s1 = (a1[0] + a1[1]) + (a1[2] + a1[3]), s2 = (a2[0] + a2[1]) + (a2[2] + a2[3]);
 #pragma unroll
           for (int o = 16; o > 0; o >>= 1) {
             s1 += __shfl_xor_sync(0xffffffffu, s1, o);
