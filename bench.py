@@ -213,6 +213,8 @@ def main():
     plan = binding.Plan(cfg.nbins, cfg.zmax, cfg.dz, cfg.wmax, cfg.dw, 2, cfg.seg_len)
     info = plan.info
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    plan.templates()                      # first build: includes the lazy load of the CUDA module
+    torch.cuda.synchronize()
     ev0.record()
     plan.templates()
     ev1.record()
