@@ -166,6 +166,18 @@ int jerk_snr_filter(jerk_plan* plan, const double* d_rowstats, const jerk_cand* 
                     jerk_cand* d_cands_out, int64_t max_out, unsigned long long* d_count_out, void* stream);
 
 /*
+ * jerk_sift_candidates — cross-row sifting of a candidate list (PAPER.md:47 future work): a strong
+ * signal gives one local-max candidate in every nearby (z,w) row (reading S10); this keeps a candidate iff no
+ * other candidate of the list with |dj| <= wj, |diz| <= wz and |diw| <= ww beats it (larger power; equal powers:
+ * smaller (iw, iz, j)).  The result does not depend on the order of the list and is a fixed point of the operation.
+ * Out of place into d_cands_out / d_count_out (DEVICE; zeroed by the call; unordered; records unchanged); at most
+ * 2^20 input records (O(n^2) pair tests).  Errors: JERK_EINVAL, JERK_ENODEV, JERK_ECUDA.
+ */
+int jerk_sift_candidates(jerk_plan* plan, const jerk_cand* d_cands_in, const unsigned long long* d_count_in,
+                         int64_t max_in, int wj, int wz, int ww, jerk_cand* d_cands_out, int64_t max_out,
+                         unsigned long long* d_count_out, void* stream);
+
+/*
  * jerk_search_candidates_host — the same search with HOST input/output (end-to-end entry point):
  * copies h_spec (host, ideally pinned, nbins complex64) to d_spec, searches, copies the count and
  * min(count, max_cands) records back to h_count / h_cands and synchronises the stream before returning.

@@ -20,6 +20,8 @@ Notation follows PAPER.md:39 (z = fdot*T^2, w = fddot*T^3) and SURVEY.md section
   F  harmonic   S_h(j,iz',iw') = sum_{k=1..h} P[rnd(j k/h); rnd(iz' k/h), rnd(iw' k/h)]
   G  row S/N    mean and (population) standard deviation of P over the 2*nbins points of one (z,w) row;
                 snr = (P - mean) / std; a candidate is kept iff snr > snr_threshold
+  H  sifting    a candidate is kept iff no other candidate within |dj|<=wj, |diz|<=wz, |diw|<=ww beats it
+                (larger power; ties -> smaller (iw, iz, j))
 
 Pins (tests/test_oracle_pins.py): closed-form sinc (z=w=0), Fresnel closed form (w=0),
 conjugate symmetry, Parseval unit energy, quadrature refinement, exact-grid recovery of a
@@ -255,3 +257,25 @@ def snr_filter(j, power, mean: float, std: float, snr_threshold: float):
     s = snr(power, mean, std)
     keep = s > snr_threshold
     return j[keep], power[keep], s[keep]
+
+
+# --------------------------------------------------------------------------- H: cross-row sifting
+def sift(cands, wj: int, wz: int, ww: int) -> list:
+    """Non-maximum suppression over a list of (j, iz, iw, power) tuples, written as the plain double loop.
+
+    A candidate survives iff no OTHER candidate with |dj| <= wj, |diz| <= wz, |diw| <= ww beats it: larger power, or
+    equal power and smaller (iw, iz, j).  Returns the survivors sorted by (iw, iz, j)."""
+    cands = [(int(j), int(iz), int(iw), float(p)) for (j, iz, iw, p) in cands]
+    out = []
+    for a_i, a in enumerate(cands):
+        alive = True
+        for b_i, b in enumerate(cands):
+            if b_i == a_i:
+                continue
+            if abs(b[0] - a[0]) <= wj and abs(b[1] - a[1]) <= wz and abs(b[2] - a[2]) <= ww:
+                if b[3] > a[3] or (b[3] == a[3] and (b[2], b[1], b[0]) < (a[2], a[1], a[0])):
+                    alive = False
+                    break
+        if alive:
+            out.append(a)
+    return sorted(out, key=lambda c: (c[2], c[1], c[0]))

@@ -41,6 +41,7 @@ EXPORTS = [
     "jerk_plan_create", "jerk_plan_destroy", "jerk_plan_info", "jerk_template_geometry", "jerk_plane_bytes",
     "jerk_templates", "jerk_templates_taps", "jerk_search_plane", "jerk_search_candidates",
     "jerk_search_candidates_range", "jerk_search_candidates_stats", "jerk_snr_filter",
+    "jerk_sift_candidates",
     "jerk_search_candidates_host", "jerk_harmonic_scratch_bytes", "jerk_harmonic_sum", "jerk_harmonic_plane", "jerk_spectrum_scratch_bytes",
     "jerk_prepare_spectrum", "jerk_strerror",
     "jerk_last_error",
@@ -72,6 +73,7 @@ def load_library() -> C.CDLL:
     lib.jerk_search_candidates_range.argtypes = [vp, vp, C.c_float, i32, i32, i32, i32, vp, i64, vp, vp, u64, vp]
     lib.jerk_search_candidates_stats.argtypes = [vp, vp, C.c_float, vp, i64, vp, vp, u64, vp, u64, vp]
     lib.jerk_snr_filter.argtypes = [vp, vp, vp, vp, i64, C.c_float, vp, i64, vp, vp]
+    lib.jerk_sift_candidates.argtypes = [vp, vp, vp, i64, i32, i32, i32, vp, i64, vp, vp]
     lib.jerk_search_candidates_host.argtypes = [vp, vp, C.c_float, vp, i64, vp, vp, vp, vp, vp, u64, vp]
     lib.jerk_harmonic_scratch_bytes.argtypes = [vp]
     lib.jerk_harmonic_scratch_bytes.restype = u64
@@ -219,6 +221,16 @@ class Plan:
             self._h, C.c_void_p(d_stats.data_ptr()), C.c_void_p(d_cands.data_ptr()), C.c_void_p(d_count.data_ptr()),
             d_cands.numel() // 16, float(snr_threshold), C.c_void_p(d_out.data_ptr()), int(max_out),
             C.c_void_p(d_nout.data_ptr()), _stream_ptr(stream)))
+        return d_out, d_nout
+
+    def sift_candidates(self, d_cands, d_count, wj, wz, ww, max_out=1 << 20, stream=None):
+        """jerk_sift_candidates: non-maximum suppression across (j, iz, iw); returns (d_out, d_count_out)."""
+        import torch
+        d_out = torch.empty(max_out * 16, dtype=torch.uint8, device=d_cands.device)
+        d_nout = torch.zeros(1, dtype=torch.int64, device=d_cands.device)
+        self._check(self._lib.jerk_sift_candidates(
+            self._h, C.c_void_p(d_cands.data_ptr()), C.c_void_p(d_count.data_ptr()), d_cands.numel() // 16, int(wj), int(wz),
+            int(ww), C.c_void_p(d_out.data_ptr()), int(max_out), C.c_void_p(d_nout.data_ptr()), _stream_ptr(stream)))
         return d_out, d_nout
 
     def search_candidates_host(self, h_spec, threshold, h_cands, h_count, d_spec, d_cands, d_count, stream=None):

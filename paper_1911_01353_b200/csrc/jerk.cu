@@ -889,6 +889,47 @@ __global__ void k_snr_filter(const double* __restrict__ rowstats, int nz, double
   }
 }
 
+// Cross-row sifting (second half; PAPER.md:47 names it as future work): a strong signal yields one
+// local-max candidate in every nearby (z,w) row.  Non-maximum suppression over the candidate list: a candidate is dropped
+// iff another one within |dj| <= wj, |diz| <= wz, |diw| <= ww beats it (larger power; ties -> smaller (iw, iz, j)).
+// The rule does not depend on the order of the list.  O(n^2) pair tests, tiled through shared memory.
+__device__ __forceinline__ bool sift_beats(const jerk_cand& b, const jerk_cand& a) {
+  if (b.power != a.power) return b.power > a.power;
+  if (b.iw != a.iw) return b.iw < a.iw;
+  if (b.iz != a.iz) return b.iz < a.iz;
+  return b.j < a.j;
+}
+__global__ void __launch_bounds__(256) k_sift(const jerk_cand* __restrict__ in, const unsigned long long* __restrict__ count_in,
+                                              long long max_in, int wj, int wz, int ww, jerk_cand* out, long long max_out,
+                                              unsigned long long* count_out) {
+  __shared__ jerk_cand tile[256];
+  unsigned long long n64 = *count_in;
+  if (n64 > (unsigned long long)max_in) n64 = (unsigned long long)max_in;
+  const int n = (int)n64;
+  for (int base = blockIdx.x * 256; base < n; base += gridDim.x * 256) {
+    const int i = base + threadIdx.x;
+    jerk_cand a;
+    a.j = 0; a.iz = a.iw = 0; a.power = 0.f; a.flags = 0;
+    if (i < n) a = in[i];
+    bool alive = i < n;
+    for (int t0 = 0; t0 < n; t0 += 256) {
+      __syncthreads();
+      if (t0 + (int)threadIdx.x < n) tile[threadIdx.x] = in[t0 + threadIdx.x];
+      __syncthreads();
+      const int m = min(256, n - t0);
+      for (int k = 0; k < m; k++) {
+        const jerk_cand b = tile[k];
+        const bool near = abs(b.j - a.j) <= wj && abs((int)b.iz - (int)a.iz) <= wz && abs((int)b.iw - (int)a.iw) <= ww;
+        if (near && (t0 + k != i) && sift_beats(b, a)) alive = false;
+      }
+    }
+    if (alive) {
+      const unsigned long long slot = atomicAdd(count_out, 1ULL);
+      if ((long long)slot < max_out) out[slot] = a;
+    }
+  }
+}
+
 __global__ void k_reset(unsigned long long* work, unsigned long long* count) {
   if (threadIdx.x < 8) work[threadIdx.x] = 0ULL;
   if (threadIdx.x == 0 && count) *count = 0ULL;
@@ -1508,6 +1549,23 @@ int jerk_snr_filter(jerk_plan* p, const double* d_rowstats, const jerk_cand* d_c
                                             d_cands_out, max_out, d_count_out);
   e = cudaGetLastError();
   if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_snr_filter launch: ") + cudaGetErrorString(e));
+  return JERK_OK;
+}
+
+int jerk_sift_candidates(jerk_plan* p, const jerk_cand* d_cands_in, const unsigned long long* d_count_in, int64_t max_in, int wj, int wz,
+                         int ww, jerk_cand* d_cands_out, int64_t max_out, unsigned long long* d_count_out, void* stream) {
+  if (!p || !d_cands_in || !d_count_in || !d_cands_out || !d_count_out || max_in < 0 || max_out < 0 || wj < 0 || wz < 0 || ww < 0)
+    return JERK_EINVAL;
+  if (max_in > (1 << 20)) return fail(p, JERK_EINVAL, "jerk_sift_candidates handles lists of at most 2^20 records (pair tests are O(n^2))");
+  if (d_cands_in == d_cands_out) return fail(p, JERK_EINVAL, "jerk_sift_candidates is out of place");
+  int rc = ensure_device(p);
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaError_t e = cudaMemsetAsync(d_count_out, 0, sizeof(unsigned long long), st);
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("count memset: ") + cudaGetErrorString(e));
+  k_sift<<<p->sm_count * 4, 256, 0, st>>>(d_cands_in, d_count_in, max_in, wj, wz, ww, d_cands_out, max_out, d_count_out);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_sift launch: ") + cudaGetErrorString(e));
   return JERK_OK;
 }
 

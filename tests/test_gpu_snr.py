@@ -80,3 +80,48 @@ def test_stats_mode_needs_seg_len_4096(setup):
     p2.templates()
     with pytest.raises(binding.JerkError):
         p2.search_candidates_stats(d_spec, THR)
+
+
+# ------------------------------------------------------------------------------------------------ cross-row sifting
+def _to_tuples(a):
+    return [(int(c["j"]), int(c["iz"]), int(c["iw"]), float(c["power"])) for c in a]
+
+
+@pytest.mark.parametrize("windows", [(4, 1, 1), (40, 3, 2), (0, 0, 0)])
+def test_sift_matches_the_oracle_on_search_output(setup, windows):
+    X, plan, d_spec, zs, ws, rows = setup
+    d_c, d_n = plan.search_candidates(d_spec, 45.0)          # the loud band and the injected signal: ~1e3 candidates
+    cands, n = binding.candidates_to_numpy(d_c, d_n)
+    assert 100 < n < 5000, n
+    d_o, d_no = plan.sift_candidates(d_c, d_n, *windows)
+    kept, nk = binding.candidates_to_numpy(d_o, d_no)
+    want = orc.sift(_to_tuples(cands), *windows)
+    assert sorted(_to_tuples(kept), key=lambda c: (c[2], c[1], c[0])) == want     # bit-exact: index and byte work only
+    if windows == (0, 0, 0):
+        assert nk == n
+    else:
+        assert nk < n
+    # the injected signal's cluster collapses to its grid point
+    iz0, iw0 = int(np.argmin(np.abs(zs - 10.0))), int(np.argmin(np.abs(ws - 40.0)))
+    assert (2 * 12345, iz0, iw0) in {(c[0], c[1], c[2]) for c in want}
+
+
+def test_sift_ties_and_empty_list(setup):
+    X, plan, d_spec, zs, ws, rows = setup
+    rng = np.random.default_rng(8)
+    n = 3000
+    a = np.zeros(n, dtype=binding.CAND_DTYPE)
+    keys = set()
+    while len(keys) < n:
+        keys.add((int(rng.integers(0, 3000)), int(rng.integers(0, 21)), int(rng.integers(0, 7))))
+    for i, (j, iz, iw) in enumerate(sorted(keys)):
+        a[i] = (j, iz, iw, float(rng.integers(4, 9)) * 5.0, 0)           # five distinct power values: many exact ties
+    a = a[rng.permutation(n)]
+    d_c = torch.from_numpy(a.view(np.uint8).reshape(-1).copy()).cuda()
+    d_n = torch.tensor([n], dtype=torch.int64, device="cuda")
+    d_o, d_no = plan.sift_candidates(d_c, d_n, 8, 2, 1)
+    kept, nk = binding.candidates_to_numpy(d_o, d_no)
+    assert sorted(_to_tuples(kept), key=lambda c: (c[2], c[1], c[0])) == orc.sift(_to_tuples(a), 8, 2, 1)
+    d_n.zero_()
+    d_o, d_no = plan.sift_candidates(d_c, d_n, 8, 2, 1)
+    assert int(d_no.item()) == 0

@@ -357,3 +357,53 @@ def test_snr_is_scale_invariant_and_filter_is_a_plain_comparison():
     want = [int(i) for i in range(P.size) if (P[i] - m1) / s1 > 4.0]
     assert kj.tolist() == want and np.allclose(ks, (kp - m1) / s1)
     assert orc.snr_filter(j, P, m1, 0.0, 4.0)[0].size == 0
+
+
+# ------------------------------------------------------------------------------------------------ H: sifting
+def _random_cands(rng, n, nj=4000, nz=21, nw=7, quant=None):
+    seen, out = set(), []
+    while len(out) < n:
+        key = (int(rng.integers(0, nj)), int(rng.integers(0, nz)), int(rng.integers(0, nw)))
+        if key in seen:
+            continue
+        seen.add(key)
+        p = float(rng.uniform(20, 90))
+        out.append(key + ((round(p / quant) * quant) if quant else p,))
+    return out
+
+
+def test_sift_hand_worked_cases():
+    # one cluster: the strongest wins; an isolated weak candidate survives; windows are inclusive
+    c = [(100, 5, 3, 50.0), (101, 5, 3, 40.0), (100, 6, 3, 45.0), (100, 5, 4, 30.0), (500, 5, 3, 21.0)]
+    assert orc.sift(c, 2, 1, 1) == [(100, 5, 3, 50.0), (500, 5, 3, 21.0)]
+    assert orc.sift(c, 0, 0, 0) == sorted(c, key=lambda x: (x[2], x[1], x[0]))
+    assert orc.sift([(10, 0, 0, 5.0), (13, 0, 0, 6.0)], 3, 0, 0) == [(13, 0, 0, 6.0)]
+    assert orc.sift([(10, 0, 0, 5.0), (14, 0, 0, 6.0)], 3, 0, 0) == [(10, 0, 0, 5.0), (14, 0, 0, 6.0)]
+    # suppression is not transitive clustering: b kills a, c kills b, a is not within reach of c but stays dead
+    chain = [(0, 0, 0, 1.0), (2, 0, 0, 2.0), (4, 0, 0, 3.0)]
+    assert orc.sift(chain, 2, 0, 0) == [(4, 0, 0, 3.0)]
+    # equal powers: the smaller (iw, iz, j) wins
+    assert orc.sift([(7, 2, 1, 9.0), (7, 2, 0, 9.0)], 0, 0, 1) == [(7, 2, 0, 9.0)]
+    assert orc.sift([], 1, 1, 1) == []
+
+
+def test_sift_invariants():
+    rng = np.random.default_rng(2024)
+    for quant in (None, 5.0):                      # continuous powers, and heavily tied ones
+        c = _random_cands(rng, 400, quant=quant)
+        kept = orc.sift(c, 6, 2, 1)
+        assert 0 < len(kept) < len(c)
+        # order independence
+        perm = [c[i] for i in rng.permutation(len(c))]
+        assert orc.sift(perm, 6, 2, 1) == kept
+        # fixed point
+        assert orc.sift(kept, 6, 2, 1) == kept
+        # the global best (with the tie rule) survives; every dropped candidate has a surviving-or-not better neighbour
+        best = min(c, key=lambda x: (-x[3], x[2], x[1], x[0]))
+        assert best in kept
+        # no two survivors are within one window of each other
+        for i, a in enumerate(kept):
+            for b in kept[i + 1:]:
+                assert not (abs(a[0] - b[0]) <= 6 and abs(a[1] - b[1]) <= 2 and abs(a[2] - b[2]) <= 1)
+        # larger windows never keep more
+        assert len(orc.sift(c, 12, 4, 2)) <= len(kept)
