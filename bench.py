@@ -170,6 +170,60 @@ def _config_dict(cfg, note=None):
     return d
 
 
+def run_row(args):
+    """--row harmonic|spectrum|stats|plane: time one of the OTHER rows of the path (not the headline line; one GPU).
+
+    harmonic: jerk_harmonic_sum on BASELINE config 5; spectrum: jerk_prepare_spectrum on the config's time series;
+    stats: jerk_search_candidates_stats + jerk_snr_filter on config 3; plane: jerk_search_plane of the whole config-2 volume."""
+    import torch
+    from paper_1911_01353_b200 import binding, build, synth
+    build.build()
+    binding.load_library()
+    torch.cuda.set_device(0)
+    idx = {"harmonic": 5, "plane": 2}.get(args.row, args.config)
+    cfg = synth.config(idx)
+    out = {"row": args.row, "config": _config_dict(cfg)["workload"], "steps": args.steps, "warmup": args.warmup, "data": "synthetic"}
+    if args.row == "spectrum":
+        d_series = torch.from_numpy(synth.make_series(cfg)).cuda()
+        d_spec = torch.empty((cfg.nbins, 2), dtype=torch.float32, device="cuda")
+        d_scr = torch.empty(cfg.n * 4, dtype=torch.uint8, device="cuda")
+        fn = lambda: binding.prepare_spectrum(d_series, 1000, d_spec, d_scr)
+        out["algorithmic_bytes"] = cfg.n * 4 + 5 * cfg.nbins * 8
+    else:
+        X = synth.make_spectrum(cfg)
+        plan = binding.Plan(cfg.nbins, cfg.zmax, cfg.dz, cfg.wmax, cfg.dw, 2, cfg.seg_len)
+        plan.templates()
+        d_spec = binding.spectrum_to_device(X)
+        if args.row == "harmonic":
+            fn = lambda: plan.harmonic_sum(d_spec)
+        elif args.row == "stats":
+            def fn():
+                d_c, d_n, d_s = plan.search_candidates_stats(d_spec, cfg.threshold)
+                return plan.snr_filter(d_s, d_c, d_n, 20.0)
+        else:
+            plane = torch.empty((cfg.nw, cfg.nz, 2 * cfg.nbins), dtype=torch.float32, device="cuda")
+            fn = lambda: plan.search_plane(d_spec, 0, cfg.nbins, out=plane)
+            out["algorithmic_bytes"] = plane.numel() * 4
+        out["algorithmic_flops"] = plan.info.flops_per_search
+    for _ in range(args.warmup):
+        fn()
+    torch.cuda.synchronize()
+    ts = []
+    for _ in range(args.steps):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        fn()
+        b.record()
+        torch.cuda.synchronize()
+        ts.append(a.elapsed_time(b))
+    out["ms"] = ts
+    out["ms_best"] = min(ts)
+    if "algorithmic_bytes" in out:
+        out["GBps_algorithmic"] = out["algorithmic_bytes"] / min(ts) / 1e6
+    print(json.dumps(out))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -178,12 +232,16 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config number 1..4 (default 3: the headline)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--row", default="search", choices=["search", "harmonic", "spectrum", "stats", "plane"],
+                    help="search (default) = the headline bench line; the others time another row of the path and print their own line")
     ap.add_argument("--log2n", type=int, default=0,
                     help="profiling aid: shorten the time series to 2^LOG2N samples (same grid, same kernel); not the headline")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                       # timing rule: at least 3 warm-up steps
 
+    if args.row != "search":
+        return run_row(args)
     if args.impl == "reference":
         return run_reference(args, args.config)
 
