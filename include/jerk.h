@@ -222,7 +222,7 @@ int jerk_harmonic_plane(jerk_plan* plan, const void* d_spec, int h, int64_t r_lo
  * gives 32768 complex bins, normalised to unit mean power per 1000-bin block"; reading S15):
  *   X[k] = sum_n x[n] exp(-2 pi i k n / N), k = 0 .. N/2-1 (DC kept, Nyquist dropped), then every consecutive block of
  *   `block` bins (the last one may be shorter) divided by sqrt(mean |X|^2) of that block (an all-zero block is left).
- * d_series: DEVICE float32[nsamples], 8-byte aligned, nsamples a power of two in [2^11, 2^25]; d_spec: DEVICE
+ * d_series: DEVICE float32[nsamples], 16-byte aligned (as d_spec and d_scratch), nsamples a power of two in [2^11, 2^25]; d_spec: DEVICE
  * complex64[nsamples/2] (the d_spec of the search calls); d_scratch: DEVICE, jerk_spectrum_scratch_bytes(nsamples)
  * bytes; all caller-owned.  Asynchronous on `stream`; no plan is needed.  d_series is not modified.
  * Errors: JERK_EINVAL (size, alignment, null), JERK_ENOMEM (scratch too small), JERK_ENODEV, JERK_ECUDA.

@@ -10,6 +10,7 @@
 //   k_fft_strided (B)  for every k1 < M1: Z[k1 + M1 k2] = DFT_M2 over n2 of Y[k1][n2]                          (rows)
 //   k_untangle_norm    X[k] = (Z[k] + conj Z[M-k])/2 - i exp(-i pi k / M) (Z[k] - conj Z[M-k])/2, block power, scale
 // M2 = 4096 for M >= 2^22, else 1024; M1 = M / M2 in {1 .. 4096}; lengths below 1024 use a direct DFT (tiny inputs only).
+// Both FFT launches stage their transforms through a shared-memory tile so that the strided side moves whole sectors.
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -27,30 +28,67 @@ struct StridedFft {
   int tw_den;                              // 0: none; else output k of batch b is multiplied by exp(-2 pi i b k / tw_den)
 };
 
+// C transforms (consecutive batch indices) per CTA, staged through a shared-memory tile so that every global access moves
+// whole 32-byte sectors whichever of the two index directions is contiguous in memory: when the elements of a transform
+// are contiguous (stride 1) a thread moves 16 bytes of one transform, when the batches are contiguous it moves the C
+// neighbouring values of one element index (C * 8 bytes).  The tile is padded by one slot per 16 so that the FFT's
+// register layout (stride-16 gathers) reads it without bank conflicts.
+template <int L>
+struct TileGeom {
+  static constexpr int C = L <= 2048 ? 4 : 2;            // transforms per CTA
+  static constexpr int ROW = L + L / 16;                 // padded row length in float2
+  static __device__ __forceinline__ int at(int e) { return e + (e >> 4); }
+};
+
 template <int L>
 __global__ void __launch_bounds__(FftGeom<L>::NT) k_fft_strided(StridedFft a) {
   using Gm = FftGeom<L>;
+  using Tg = TileGeom<L>;
+  constexpr int C = Tg::C, NT = Gm::NT;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float2* exA = reinterpret_cast<float2*>(smem_raw);
   float2* exB = exA + Gm::EX1;
   float2* tw2 = exB + Gm::EX2;
+  float2* tile = tw2 + Tw2Table<L>::FLOATS2;             // [C][ROW]
   __shared__ unsigned long long s_war;
   const int t = threadIdx.x;
-  fill_tw2<L>(tw2, t, Gm::NT);
+  fill_tw2<L>(tw2, t, NT);
   Tw3Regs<L> tw3;
   make_tw3<L>(tw3.w, t);
-  WarBarrier war = war_init<Gm::NT>(&s_war, t);
-  for (int i = 0; i < a.per_cta; i++) {
-    const int b = blockIdx.x * a.per_cta + i;
-    if (b >= a.nbatch) break;
-    const float2* src = a.in + (long long)b * a.in_sb;
+  WarBarrier war = war_init<NT>(&s_war, t);
+  const int b0 = blockIdx.x * C;                          // nbatch is a multiple of C (host checks)
+  // ---- load
+  if (a.in_se == 1) {
+    for (int c = 0; c < C; c++) {
+      const float4* src = reinterpret_cast<const float4*>(a.in + (long long)(b0 + c) * a.in_sb);
+      for (int e2 = t; e2 < L / 2; e2 += NT) {
+        const float4 x = src[e2];
+        tile[c * Tg::ROW + Tg::at(2 * e2)] = make_float2(x.x, x.y);
+        tile[c * Tg::ROW + Tg::at(2 * e2 + 1)] = make_float2(x.z, x.w);
+      }
+    }
+  } else {                                                // in_sb == 1
+    for (int e = t; e < L; e += NT) {
+      const float4* src = reinterpret_cast<const float4*>(a.in + b0 + (long long)e * a.in_se);
+#pragma unroll
+      for (int h = 0; h < C / 2; h++) {
+        const float4 x = src[h];
+        tile[(2 * h) * Tg::ROW + Tg::at(e)] = make_float2(x.x, x.y);
+        tile[(2 * h + 1) * Tg::ROW + Tg::at(e)] = make_float2(x.z, x.w);
+      }
+    }
+  }
+  __syncthreads();
+  // ---- transforms, in place in the tile
+  for (int c = 0; c < C; c++) {
+    float2* row = tile + c * Tg::ROW;
     float2 v[Gm::P];
 #pragma unroll
     for (int u = 0; u < Gm::NB1; u++)
 #pragma unroll
-      for (int k2 = 0; k2 < Gm::R1; k2++) v[u * Gm::R1 + k2] = src[(long long)(256 * k2 + Gm::b1_of(t, u)) * a.in_se];
-    fft_passes<L, -1>(v, tw3, tw2, exA, exB, war, t);
-    float2* dst = a.out + (long long)b * a.out_sb;
+      for (int k2 = 0; k2 < Gm::R1; k2++) v[u * Gm::R1 + k2] = row[Tg::at(256 * k2 + Gm::b1_of(t, u))];
+    fft_passes<L, -1>(v, tw3, tw2, exA, exB, war, t);     // its block barrier orders every read of `row` before the writes below
+    const int b = b0 + c;
 #pragma unroll
     for (int u = 0; u < Gm::NB2; u++)
 #pragma unroll
@@ -58,8 +96,28 @@ __global__ void __launch_bounds__(FftGeom<L>::NT) k_fft_strided(StridedFft a) {
         const int k = Gm::b3_of(t, u) + 16 * Gm::R1 * n2;
         float2 x = v[u * 16 + n2];
         if (a.tw_den) x = cmul(x, unit_root(-(b * k), a.tw_den));
-        dst[(long long)k * a.out_se] = x;
+        row[Tg::at(k)] = x;
       }
+  }
+  __syncthreads();
+  // ---- store
+  if (a.out_se == 1) {
+    for (int c = 0; c < C; c++) {
+      float4* dst = reinterpret_cast<float4*>(a.out + (long long)(b0 + c) * a.out_sb);
+      for (int e2 = t; e2 < L / 2; e2 += NT) {
+        const float2 p = tile[c * Tg::ROW + Tg::at(2 * e2)], q = tile[c * Tg::ROW + Tg::at(2 * e2 + 1)];
+        dst[e2] = make_float4(p.x, p.y, q.x, q.y);
+      }
+    }
+  } else {                                                // out_sb == 1
+    for (int e = t; e < L; e += NT) {
+      float4* dst = reinterpret_cast<float4*>(a.out + b0 + (long long)e * a.out_se);
+#pragma unroll
+      for (int h = 0; h < C / 2; h++) {
+        const float2 p = tile[(2 * h) * Tg::ROW + Tg::at(e)], q = tile[(2 * h + 1) * Tg::ROW + Tg::at(e)];
+        dst[h] = make_float4(p.x, p.y, q.x, q.y);
+      }
+    }
   }
 }
 
@@ -126,19 +184,23 @@ __global__ void __launch_bounds__(256) k_untangle_norm(const float2* __restrict_
 template <int L>
 static cudaError_t launch_strided(const StridedFft& a, cudaStream_t st) {
   using Gm = FftGeom<L>;
-  const size_t smem = (size_t)(Gm::EX1 + Gm::EX2 + Tw2Table<L>::FLOATS2) * sizeof(float2);
+  using Tg = TileGeom<L>;
+  if (a.nbatch % Tg::C) return cudaErrorInvalidValue;
+  if (!((a.in_se == 1 || a.in_sb == 1) && (a.out_se == 1 || a.out_sb == 1))) return cudaErrorInvalidValue;
+  const size_t smem = (size_t)(Gm::EX1 + Gm::EX2 + Tw2Table<L>::FLOATS2 + Tg::C * Tg::ROW) * sizeof(float2);
   cudaError_t e = cudaFuncSetAttribute(k_fft_strided<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  k_fft_strided<L><<<(a.nbatch + a.per_cta - 1) / a.per_cta, Gm::NT, smem, st>>>(a);
+  k_fft_strided<L><<<a.nbatch / Tg::C, Gm::NT, smem, st>>>(a);
   return cudaGetLastError();
 }
 
 static cudaError_t run_fft(const StridedFft& a, int L, cudaStream_t st) {
-  switch (L) {
+  const bool tiled = (L == 1024 && a.nbatch % TileGeom<1024>::C == 0) || (L == 2048 && a.nbatch % TileGeom<2048>::C == 0) ||
+                     (L == 4096 && a.nbatch % TileGeom<4096>::C == 0);   // one or two transforms only (2^11, 2^12 samples): direct DFT
+  switch (tiled ? L : 0) {
     case 1024: return launch_strided<1024>(a, st);
     case 2048: return launch_strided<2048>(a, st);
     case 4096: return launch_strided<4096>(a, st);
-    case 8192: return launch_strided<8192>(a, st);
   }
   const long long n = (long long)a.nbatch * L;
   k_dft_direct<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(a, L);
@@ -161,7 +223,7 @@ int jerk_prepare_spectrum(const float* d_series, int64_t nsamples, int block, vo
   if (!d_series || !d_spec || !d_scratch || block < 1) return JERK_EINVAL;
   if (nsamples < (1 << 11) || nsamples > (1 << 25) || (nsamples & (nsamples - 1))) return JERK_EINVAL;   // 2^11 .. 2^25 samples
   if (scratch_bytes < jerk_spectrum_scratch_bytes(nsamples)) return JERK_ENOMEM;
-  if ((uintptr_t)d_series % 8 || (uintptr_t)d_spec % 8 || (uintptr_t)d_scratch % 8) return JERK_EINVAL;
+  if ((uintptr_t)d_series % 16 || (uintptr_t)d_spec % 16 || (uintptr_t)d_scratch % 16) return JERK_EINVAL;   // 128-bit accesses
   int dev = 0, major = 0;
   if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess ||
       major != 10)
