@@ -170,6 +170,70 @@ def _config_dict(cfg, note=None):
     return d
 
 
+def run_cufft_comparator(args, cfg, out):
+    """--row cufft (PAPER.md:45 compares its shared-memory FFT with a cuFFT-based convolution): the
+    UNFUSED pipeline on the same GPU, built from library calls only (torch.fft = cuFFT, torch elementwise kernels): for a
+    block of segments x template-phases  Y = F * G  ->  batched inverse FFT  ->  |y|^2 over the valid window  ->  row max.
+    It is a comparator, not a product path: it uses this library's bank (re-ordered to natural order), is checked
+    against jerk_search_plane on one block, is timed on a bounded sample of the config-3 workload and extrapolated."""
+    import torch
+    from paper_1911_01353_b200 import binding, synth
+    L = cfg.seg_len
+    assert L == 4096, "the comparator re-orders the seg_len-4096 bank layout"
+    X = synth.make_spectrum(cfg)
+    plan = binding.Plan(cfg.nbins, cfg.zmax, cfg.dz, cfg.wmax, cfg.dw, 2, L)
+    plan.templates()
+    info = plan.info
+    d_spec = binding.spectrum_to_device(X)
+    spec = torch.view_as_complex(d_spec)
+    # bank in natural order: element k = 64*k1 + t of a (template, phase) sits at float2 slot 2*((k1>>1)*64 + t) + (k1&1)
+    k = torch.arange(L, device="cuda")
+    k1, t = k >> 6, k & 63
+    slot = 2 * ((k1 >> 1) * 64 + t) + (k1 & 1)
+    geom_bytes = (info.ntemplates * 8 + 255) // 256 * 256
+    bank = plan.bank[geom_bytes:geom_bytes + info.ntemplates * 2 * L * 8].view(torch.float32).view(-1, L, 2)
+    ntp_blk, nseg_blk = 512, 64                      # 512 template-phases x 64 segments per block: 1 GB of complex64
+    G = torch.view_as_complex(bank[:ntp_blk][:, slot, :].contiguous())           # [ntp, L] natural order
+    seg0 = info.nseg // 2
+    starts = info.seg_base + (seg0 + torch.arange(nseg_blk, device="cuda")) * info.step
+    idx = starts[:, None] + torch.arange(L, device="cuda")[None, :]
+    lo, hi = info.hw_max, info.hw_max + info.step
+
+    def block():
+        F = torch.fft.fft(spec[idx], dim=1)                                    # [nseg, L]   (a-2)
+        Y = F[:, None, :] * G[None, :, :]                                      # [nseg, ntp, L]   (a-3, written to HBM)
+        y = torch.fft.ifft(Y, dim=2, norm="forward")                           # unnormalised inverse FFT (cuFFT, batched)
+        P = (y.real * y.real + y.imag * y.imag)[:, :, lo:hi]                   # (a-4)
+        return P, P.amax(dim=2)                                                # (a-5, reduced to a row maximum)
+
+    P, mx = block()
+    # check one template-phase row of the block against the fused kernel's plane output
+    geom_c = int(plan.template_geometry(0, 0)[0])
+    b_first = int(starts[0].item()) + lo - geom_c
+    ours = plan.search_plane(d_spec, b_first, info.step, 0, 1, 0, 1)[0, 0]     # P[j], j = 2*(b - b_first) + p
+    theirs = torch.stack([P[0, 0], P[0, 1]], dim=1).reshape(-1)
+    err = float(((ours - theirs).abs() / torch.clamp(ours, min=1.0)).max())
+    assert err < 1e-3, err
+    for _ in range(max(1, args.warmup)):
+        block()
+    torch.cuda.synchronize()
+    ts = []
+    for _ in range(args.steps):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        block()
+        b.record()
+        torch.cuda.synchronize()
+        ts.append(a.elapsed_time(b))
+    units = ntp_blk * nseg_blk
+    total_units = 2 * info.ntemplates * info.nseg
+    out.update({"ms_block": ts, "units_per_block": units, "max_rel_diff_vs_fused_plane": err,
+                "extrapolated_ms_per_search": min(ts) * total_units / units,
+                "note": "library-only unfused pipeline (cuFFT through torch.fft + elementwise kernels); comparator, not a product path"})
+    print(json.dumps(out))
+    return 0
+
+
 def run_row(args):
     """--row harmonic|spectrum|stats|plane: time one of the OTHER rows of the path (not the headline line; one GPU).
 
@@ -183,6 +247,8 @@ def run_row(args):
     idx = {"harmonic": 5, "plane": 2}.get(args.row, args.config)
     cfg = synth.config(idx)
     out = {"row": args.row, "config": _config_dict(cfg)["workload"], "steps": args.steps, "warmup": args.warmup, "data": "synthetic"}
+    if args.row == "cufft":
+        return run_cufft_comparator(args, cfg, out)
     if args.row == "spectrum":
         d_series = torch.from_numpy(synth.make_series(cfg)).cuda()
         d_spec = torch.empty((cfg.nbins, 2), dtype=torch.float32, device="cuda")
@@ -232,7 +298,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config number 1..4 (default 3: the headline)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--row", default="search", choices=["search", "harmonic", "spectrum", "stats", "plane"],
+    ap.add_argument("--row", default="search", choices=["search", "harmonic", "spectrum", "stats", "plane", "cufft"],
                     help="search (default) = the headline bench line; the others time another row of the path and print their own line")
     ap.add_argument("--log2n", type=int, default=0,
                     help="profiling aid: shorten the time series to 2^LOG2N samples (same grid, same kernel); not the headline")
