@@ -77,7 +77,8 @@ typedef struct jerk_plan_info_t {
  * jerk_plan_create — host only (BASELINE.json north_star: jerk_plan_create(nbins, zmax, dz, wmax, dw,
  * numbetween, seg_len)).  Validates the grid and derives nz, nw, c(z,w), hw(z,w), hw_max, step, nseg.
  * Requirements: nbins >= 1; zmax, wmax >= 0; dz, dw > 0 with zmax/dz and wmax/dw integers;
- * numbetween == 2; seg_len in {1024, 2048, 4096, 8192} and seg_len - 2*hw_max >= 2; nz, nw < 32768.
+ * numbetween == 2; seg_len in {1024, 2048, 4096, 8192} and seg_len - 2*hw_max >= 2, or seg_len == 0 for the library's
+ * choice (4096, the fastest kernel, whenever it leaves a positive step; the result does not depend on seg_len); nz, nw < 32768.
  * *out receives a plan that jerk_plan_destroy frees.  Errors: JERK_EINVAL.
  */
 int jerk_plan_create(jerk_plan** out, int64_t nbins, double zmax, double dz, double wmax, double dw,

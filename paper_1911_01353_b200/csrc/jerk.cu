@@ -1295,7 +1295,7 @@ int jerk_plan_create(jerk_plan** out, int64_t nbins, double zmax, double dz, dou
   if (nbins < 1 || zmax < 0 || wmax < 0 || !(dz > 0) || !(dw > 0)) return JERK_EINVAL;
   if (!is_integer(zmax / dz) || !is_integer(wmax / dw)) return JERK_EINVAL;
   if (numbetween != 2) return JERK_EINVAL;
-  if (seg_len != 1024 && seg_len != 2048 && seg_len != 4096 && seg_len != 8192) return JERK_EINVAL;
+  if (seg_len != 0 && seg_len != 1024 && seg_len != 2048 && seg_len != 4096 && seg_len != 8192) return JERK_EINVAL;
   if (nbins > (int64_t)1 << 30) return JERK_EINVAL;  // j = 2b+p is reported as int32
   jerk_plan* p = new jerk_plan();
   p->nbins = nbins;
@@ -1322,6 +1322,10 @@ int jerk_plan_create(jerk_plan** out, int64_t nbins, double zmax, double dz, dou
       if (g.hw > p->hw_max) p->hw_max = g.hw;
       if (abs(g.c) > p->c_max) p->c_max = abs(g.c);
     }
+  // seg_len 0: the library's choice.  The result does not depend on the segment length (SURVEY.md 8(c) pin P9); 4096 is
+  // the length of the two-pass kernel (k_search64) and is taken whenever the templates leave a positive step.
+  if (seg_len == 0) seg_len = 4096 - 2 * p->hw_max >= 2 ? 4096 : 8192;
+  p->L = seg_len;
   p->step = seg_len - 2 * p->hw_max;
   if (p->step < 2) {
     delete p;

@@ -101,3 +101,10 @@ def test_synth_configs_are_deterministic():
     # block normalisation: unit mean power per 1000-bin block (reading S15)
     blk = a[3000:4000].astype(np.complex128)
     assert abs(np.mean(np.abs(blk) ** 2) - 1.0) < 1e-5
+
+
+def test_seg_len_zero_is_the_library_choice(lib):
+    p = binding.Plan(1 << 20, 200.0, 2.0, 600.0, 20.0, 2, 0)
+    assert p.info.seg_len == 4096 and p.info.step == 4096 - 2 * 258
+    with pytest.raises(binding.JerkError):
+        binding.Plan(1 << 20, 200.0, 2.0, 600.0, 20.0, 2, 512)
