@@ -550,7 +550,10 @@ __device__ __forceinline__ void bulk_copy_g2s(uint32_t dst, const void* src, uin
                "r"(bytes), "r"(bar)
                : "memory");
 }
-template <int MODE, int NG>
+// PRUNE (hw_max >= 256): outputs n < 256 and n >= 3840 lie outside the valid window [hw_max, 4096 - hw_max) of every
+// template; they are outputs 0 and 15 of each last-stage DFT_16 (registers 16a and 16a + 15), whose final butterfly
+// operations and power are then never computed (their power is reported as 0).
+template <int MODE, int NG, bool PRUNE>
 __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __grid_constant__ SearchParams sp) {
   constexpr int L = 4096, NT = 64, P = 64;
   constexpr int NLAYER = (NG + 1) / 2;                          // groups of four warps: one TMEM lane quarter each
@@ -725,7 +728,8 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
       }
       float pw[P];
 #pragma unroll
-      for (int i = 0; i < P; i++) pw[i] = fmaf(v[i].x, v[i].x, v[i].y * v[i].y);
+      for (int i = 0; i < P; i++)
+        pw[i] = (PRUNE && ((i & 15) == 0 || (i & 15) == 15)) ? 0.f : fmaf(v[i].x, v[i].x, v[i].y * v[i].y);
       if (MODE == MODE_PLANE) {
         // phase-0 powers wait in shared memory (written and read back by the same thread) so that both phases leave as
         // interleaved float2 pairs: every warp store covers 256 contiguous bytes (full 32-byte sectors, no L2 fill reads)
@@ -1160,8 +1164,8 @@ static cudaError_t launch_search(const jerk_plan* plan, const SearchParams& sp, 
 #ifndef JERK_K64_NG_CAND
 #define JERK_K64_NG_CAND 2
 #endif
-template <int MODE>
-static cudaError_t launch_search64(const jerk_plan* plan, const SearchParams& sp, cudaStream_t st) {
+template <int MODE, bool PRUNE>
+static cudaError_t launch_search64p(const jerk_plan* plan, const SearchParams& sp, cudaStream_t st) {
   // FFT groups per CTA: two (two CTAs per SM) in candidate mode, four (one CTA per SM) in plane mode: 8 warps per SM, up
   // to 255 registers.  Six groups (12 warps, 168 registers: the register file is 16 K per scheduler, i.e. 170 registers at
   // three warps each) measured 172 ms/search against 158 ms: the spills and the tighter schedule cost more than the
@@ -1169,12 +1173,12 @@ static cudaError_t launch_search64(const jerk_plan* plan, const SearchParams& sp
   constexpr int NG = MODE == MODE_PLANE ? 4 : JERK_K64_NG_CAND;
   const size_t smem = (size_t)NG * kEx64 * sizeof(float2) + 4 * NG * sizeof(unsigned long long) +
                       (MODE == MODE_PLANE ? (size_t)NG * 64 * 64 * sizeof(float) : 0);
-  cudaError_t e = cudaFuncSetAttribute(k_search64<MODE, NG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaError_t e = cudaFuncSetAttribute(k_search64<MODE, NG, PRUNE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   if (getenv("JERK_DEBUG")) {
     cudaFuncAttributes fa;
-    if (cudaFuncGetAttributes(&fa, k_search64<MODE, NG>) == cudaSuccess)
-      fprintf(stderr, "[jerk] k_search64<%d,%d>: %d regs, %zu B local, smem %zu B\n", MODE, NG, fa.numRegs, (size_t)fa.localSizeBytes, smem);
+    if (cudaFuncGetAttributes(&fa, k_search64<MODE, NG, PRUNE>) == cudaSuccess)
+      fprintf(stderr, "[jerk] k_search64<%d,%d,%d>: %d regs, %zu B local, smem %zu B\n", MODE, NG, (int)PRUNE, fa.numRegs, (size_t)fa.localSizeBytes, smem);
   }
   const long long ctas_per_sm = NG == 2 ? 2 : 1;
   long long grid = (long long)plan->sm_count * ctas_per_sm;
@@ -1182,8 +1186,13 @@ static cudaError_t launch_search64(const jerk_plan* plan, const SearchParams& sp
   if (grid * NG > slots) grid = slots / NG;
   if (grid > (sp.nitems + NG - 1) / NG) grid = (sp.nitems + NG - 1) / NG;
   if (grid < 1) grid = 1;
-  k_search64<MODE, NG><<<(unsigned)grid, 64 * NG, smem, st>>>(sp);
+  k_search64<MODE, NG, PRUNE><<<(unsigned)grid, 64 * NG, smem, st>>>(sp);
   return cudaGetLastError();
+}
+
+template <int MODE>
+static cudaError_t launch_search64(const jerk_plan* plan, const SearchParams& sp, cudaStream_t st) {
+  return plan->hw_max >= 256 ? launch_search64p<MODE, true>(plan, sp, st) : launch_search64p<MODE, false>(plan, sp, st);
 }
 
 template <int MODE>
