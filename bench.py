@@ -33,9 +33,9 @@ import numpy as np
 METRIC = "ffdot_points_per_sec"
 UNIT = "points/s"
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12     # 74.45: SMs x FP32 lanes x 2 (FMA) x max SM clock
-# dram__bytes_read.sum + dram__bytes_write.sum of one full-size config-3 k_search64<cand> launch (profiles/r1_03_k_search64_cand_full.md);
+# dram__bytes_read.sum + dram__bytes_write.sum of one full-size config-3 k_search64<cand> launch (profiles/r1_05_k_search64_cand_full.md);
 # algorithmic minimum = bank + spectrum once = 0.837 GB
-NCU_DRAM_BYTES_PER_LAUNCH = {3: 1061323520 + 8599040}
+NCU_DRAM_BYTES_PER_LAUNCH = {3: 1055630080 + 8592896}
 
 
 def _measured_peaks():
@@ -426,7 +426,7 @@ def main():
         roofline = {
             "bound": "alu", "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
             "traffic": None if args.log2n else NCU_DRAM_BYTES_PER_LAUNCH.get(args.config),
-            "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1_03)",
+            "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1_05)",
             "kernel": "k_search64<cand>" if cfg.seg_len == 4096 else f"k_search<{cfg.seg_len},cand>", "kernel_ms": kernel_ms,
             "algorithmic_flops_per_launch": info.flops_per_search,
             "peak_source": "FP32 FMA nominal: 148 SMs x 128 lanes x 2 x 1.965 GHz (DESIGN.md); MEASURED_PEAKS.json has no fp32 entry"
