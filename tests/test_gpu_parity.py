@@ -360,3 +360,42 @@ def test_repeated_searches_are_bit_identical():
         if p_ref is None:
             p_ref = P
         assert P.tobytes() == p_ref.tobytes()
+
+
+# ------------------------------------------------------------------------------------------------ k_search64 edge cases
+class _Cfg:
+    """Minimal stand-in for synth.Config in _check_candidates (grid + nbins)."""
+    def __init__(self, nbins, zmax, dz, wmax, dw):
+        self.nbins, self.zmax, self.dz, self.wmax, self.dw = nbins, zmax, dz, wmax, dw
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("nbins", [100, 3579, 3581, 9000])
+def test_seg_len_4096_low_threshold_seams_and_edges(nbins):
+    """The two-pass kernel (seg_len 4096) on spectra shorter than a segment, one bin either side of one step (3580), and
+    several ragged segments: full plane of sampled rows and ALL low-threshold candidates (hundreds on warp/segment seams
+    and at both spectrum edges) against the oracle."""
+    X = synth.random_spectrum(nbins, 1000 + nbins)
+    cfg = _Cfg(nbins, 20.0, 2.0, 60.0, 20.0)
+    plan = binding.Plan(nbins, 20, 2, 60, 20, 2, 4096)
+    plan.templates()
+    d_spec = binding.spectrum_to_device(X)
+    zs, ws = orc.grid_values(20, 2), orc.grid_values(60, 20)
+    rows = [(0, 0), (20, 6), (10, 3), (3, 5), (17, 1), (20, 0), (0, 6)]
+    ref = H.oracle_rows(X, [(zs[iz], ws[iw]) for iz, iw in rows], 0, nbins)
+    P = plan.search_plane(d_spec, 0, nbins).cpu().numpy()
+    for (iz, iw), r in zip(rows, ref):
+        H.assert_power_close(P[iw, iz], r, f"nbins={nbins} row {(iz, iw)}")
+    # sub-box == slice of the full plane, bit for bit
+    r_lo, r_cnt = nbins // 3, max(1, nbins // 5)
+    sub = plan.search_plane(d_spec, r_lo, r_cnt, 5, 4, 2, 3).cpu().numpy()
+    assert np.array_equal(sub, P[2:5, 5:9, 2 * r_lo:2 * (r_lo + r_cnt)])
+    thr = 5.0
+    d_c, d_n = plan.search_candidates(d_spec, thr, max_cands=1 << 18)
+    cands, n = binding.candidates_to_numpy(d_c, d_n)
+    assert n == cands.size and len({(c["j"], c["iz"], c["iw"]) for c in cands}) == n
+    assert plan.work_counters()[2] == 0                                       # no seam overflow
+    m, s = _check_candidates(cfg, X, cands, rows, 0, nbins, thr)
+    assert m == s and (s > 0 or nbins < 1000)
+    # first and last half-bin of a row can be candidates (P[-1] = P[2 nbins] = -inf)
+    assert cands["j"].min() >= 0 and cands["j"].max() <= 2 * nbins - 1
