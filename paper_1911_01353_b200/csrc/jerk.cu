@@ -995,16 +995,25 @@ __global__ void __launch_bounds__(256) k_harm(const __grid_constant__ HarmParams
   float best[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
   int bj[4] = {-1, -1, -1, -1};
   float* orow = STORE ? hp.out + ((long long)iwr * hp.iz_cnt + izr) * hp.nj - hp.j_lo + j8 : nullptr;
+  // Strength-reduced gathers: for l = l0 + 256 k the source index ((l e + 4) >> 3) = ((l0 e + 4) >> 3) + 32 k e exactly, and
+  // l0 advances by 1024 per iteration, so every thread keeps one pointer per fraction, reads at compile-time offsets
+  // and bumps the pointer by 128 e floats per iteration (the kernel was issue-bound on index arithmetic: 107
+  // instructions per point, ALU pipe 71 % busy).
   constexpr int U = 4;   // points per thread in flight: 32 independent loads before the first use
-  for (int l0 = l_lo + (int)threadIdx.x; l0 < l_hi; l0 += 256 * U) {
+  const int l_first = l_lo + (int)threadIdx.x;
+  const float* pe_ptr[8];
+#pragma unroll
+  for (int e = 1; e <= 8; e++) pe_ptr[e - 1] = rp[e - 1] + ((l_first * e + 4) >> 3);
+  for (int l0 = l_first; l0 < l_hi; l0 += 256 * U) {
     float pe[U][8];
 #pragma unroll
     for (int k = 0; k < U; k++) {
-      const int l = l0 + 256 * k;
-      const bool ok = l < l_hi;
+      const bool ok = l0 + 256 * k < l_hi;
 #pragma unroll
-      for (int e = 1; e <= 8; e++) pe[k][e - 1] = ok ? __ldg(rp[e - 1] + ((l * e + 4) >> 3)) : 0.f;
+      for (int e = 1; e <= 8; e++) pe[k][e - 1] = ok ? __ldg(pe_ptr[e - 1] + 32 * k * e) : 0.f;
     }
+#pragma unroll
+    for (int e = 1; e <= 8; e++) pe_ptr[e - 1] += 32 * U * e;
 #pragma unroll
     for (int k = 0; k < U; k++) {
       const int l = l0 + 256 * k;
