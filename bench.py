@@ -423,12 +423,17 @@ def main():
         kernel_ms = float(np.mean(step_ms))                   # k_search is > 99.9 % of a step (profiles/)
         achieved = info.flops_per_search / (kernel_ms * 1e-3) / 1e12
         peaks = _measured_peaks()
+        try:
+            measured_fp32 = binding.probe_fp32_tflops()
+        except Exception:
+            measured_fp32 = None
         roofline = {
             "bound": "alu", "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
             "traffic": None if args.log2n else NCU_DRAM_BYTES_PER_LAUNCH.get(args.config),
             "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1_05)",
             "kernel": "k_search64<cand>" if cfg.seg_len == 4096 else f"k_search<{cfg.seg_len},cand>", "kernel_ms": kernel_ms,
             "algorithmic_flops_per_launch": info.flops_per_search,
+            "peak_measured_ffma": measured_fp32, "frac_of_measured_ffma": (achieved / measured_fp32) if measured_fp32 else None,
             "peak_source": "FP32 FMA nominal: 148 SMs x 128 lanes x 2 x 1.965 GHz (DESIGN.md); MEASURED_PEAKS.json has no fp32 entry"
                            + (f"; hbm_gbs={peaks.get('hbm_gbs')} (not the bound here)" if peaks else ""),
         }

@@ -232,6 +232,14 @@ uint64_t jerk_spectrum_scratch_bytes(int64_t nsamples);
 int jerk_prepare_spectrum(const float* d_series, int64_t nsamples, int block, void* d_spec, void* d_scratch,
                           uint64_t scratch_bytes, void* stream);
 
+/*
+ * jerk_probe_fma — measurement aid for the roofline denominator: launches a kernel of nothing but
+ * independent FP32 fused multiply-add chains (2048 threads per SM, 16 chains per thread, `iters` iterations) on
+ * `stream` and returns in *flops (HOST) the number of floating-point operations it executes; the caller times it.
+ * d_out: DEVICE, >= 4 bytes (never written in practice).  Errors: JERK_EINVAL, JERK_ENODEV, JERK_ECUDA.
+ */
+int jerk_probe_fma(void* d_out, int iters, double* flops, void* stream);
+
 const char* jerk_strerror(int status);
 const char* jerk_last_error(const jerk_plan* plan);
 

@@ -43,7 +43,7 @@ EXPORTS = [
     "jerk_search_candidates_range", "jerk_search_candidates_stats", "jerk_snr_filter",
     "jerk_sift_candidates",
     "jerk_search_candidates_host", "jerk_harmonic_scratch_bytes", "jerk_harmonic_sum", "jerk_harmonic_plane", "jerk_spectrum_scratch_bytes",
-    "jerk_prepare_spectrum", "jerk_strerror",
+    "jerk_prepare_spectrum", "jerk_probe_fma", "jerk_strerror",
     "jerk_last_error",
 ]
 
@@ -82,6 +82,7 @@ def load_library() -> C.CDLL:
     lib.jerk_spectrum_scratch_bytes.argtypes = [i64]
     lib.jerk_spectrum_scratch_bytes.restype = u64
     lib.jerk_prepare_spectrum.argtypes = [vp, i64, i32, vp, vp, u64, vp]
+    lib.jerk_probe_fma.argtypes = [vp, i32, C.POINTER(dbl), vp]
     lib.jerk_strerror.argtypes = [i32]
     lib.jerk_strerror.restype = C.c_char_p
     lib.jerk_last_error.argtypes = [vp]
@@ -303,6 +304,27 @@ def prepare_spectrum(d_series, block=1000, d_spec=None, d_scratch=None, stream=N
     if rc != 0:
         raise JerkError(rc, lib.jerk_strerror(rc).decode())
     return d_spec
+
+
+def probe_fp32_tflops(iters=1 << 15, reps=5):
+    """Measured FP32 FMA throughput of the current device in TFLOP/s (jerk_probe_fma timed with CUDA events, best of reps)."""
+    import torch
+    lib = load_library()
+    d = torch.zeros(4, dtype=torch.float32, device="cuda")
+    fl = C.c_double(0.0)
+    best = None
+    for i in range(reps + 1):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        rc = lib.jerk_probe_fma(C.c_void_p(d.data_ptr()), int(iters), C.byref(fl), _stream_ptr(None))
+        b.record()
+        torch.cuda.synchronize()
+        if rc != 0:
+            raise JerkError(rc, lib.jerk_strerror(rc).decode())
+        ms = a.elapsed_time(b)
+        if i > 0:
+            best = ms if best is None else min(best, ms)
+    return fl.value / (best * 1e-3) / 1e12
 
 
 def candidates_to_numpy(d_cands, d_count):

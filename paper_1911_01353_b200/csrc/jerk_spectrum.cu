@@ -207,6 +207,23 @@ static cudaError_t run_fft(const StridedFft& a, int L, cudaStream_t st) {
   return cudaGetLastError();
 }
 
+// Measurement aid ("the bench must also run a pure-FFMA micro-kernel"): 16 independent fused multiply-add
+// chains per thread, nothing else; flops = threads * iters * 16 * 2.
+__global__ void __launch_bounds__(256) k_ffma_probe(float* out, int iters) {
+  float a[16];
+#pragma unroll
+  for (int i = 0; i < 16; i++) a[i] = 1.0f + 1e-3f * (float)(threadIdx.x + i);
+  const float m = 0.999f + 1e-6f * (float)(blockIdx.x & 7), c = 1e-3f;
+  for (int it = 0; it < iters; it++) {
+#pragma unroll
+    for (int i = 0; i < 16; i++) a[i] = fmaf(a[i], m, c);
+  }
+  float s = 0.f;
+#pragma unroll
+  for (int i = 0; i < 16; i++) s += a[i];
+  if (s == 12345.678f) out[0] = s;   // never true: keeps the chains alive without memory traffic
+}
+
 }  // namespace jerk
 
 using namespace jerk;
@@ -258,6 +275,17 @@ int jerk_prepare_spectrum(const float* d_series, int64_t nsamples, int block, vo
   if (run_fft(b, M2, st) != cudaSuccess) return JERK_ECUDA;
   k_untangle_norm<<<(M + block - 1) / block, 256, 0, st>>>(Z, (float2*)d_spec, M, block);
   if (cudaGetLastError() != cudaSuccess) return JERK_ECUDA;
+  return JERK_OK;
+}
+
+int jerk_probe_fma(void* d_out, int iters, double* flops, void* stream) {
+  if (!d_out || iters < 1 || !flops) return JERK_EINVAL;
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return JERK_ENODEV;
+  const int blocks = sms * 8;   // 2048 threads per SM
+  k_ffma_probe<<<blocks, 256, 0, (cudaStream_t)stream>>>((float*)d_out, iters);
+  if (cudaGetLastError() != cudaSuccess) return JERK_ECUDA;
+  *flops = (double)blocks * 256.0 * (double)iters * 16.0 * 2.0;
   return JERK_OK;
 }
 
