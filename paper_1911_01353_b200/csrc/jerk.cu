@@ -735,15 +735,23 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
         // interleaved float2 pairs: every warp store covers 256 contiguous bytes (full 32-byte sectors, no L2 fill reads)
         if (ph == 0) {
 #pragma unroll
-          for (int r = 0; r < P; r++) p0s[r * NT + t] = pw[r];
+          for (int r = 0; r < P; r++)
+            if (!(PRUNE && ((r & 15) == 0 || (r & 15) == 15))) p0s[r * NT + t] = pw[r];
         } else {
           float* row = jb.plane + (size_t)(tp >> 1) * (size_t)(2 * jb.r_cnt);   // row-major box: row index = template-phase / 2
           const int boff = s0 - c - (int)jb.r_lo;
+          float2* dst = reinterpret_cast<float2*>(row + 2 * (ptrdiff_t)(boff + t));   // + 64 n1 float2 per register
+          // registers with n1 = n / 64 in [8, 56) are valid for every thread of a segment inside the box (hw_max <= 512):
+          // no predicate; registers known to be outside every window (PRUNE) are skipped
+          const bool inner_valid = __all_sync(0xffffffffu, n_lo <= t + 64 * 8 && n_hi >= t + 64 * 56);
 #pragma unroll
           for (int r = 0; r < P; r++) {
-            const int n = t + 64 * dft64_out_index(r);
+            if (PRUNE && ((r & 15) == 0 || (r & 15) == 15)) continue;
+            const int n1 = dft64_out_index(r);
+            const int n = t + 64 * n1;
             const float p0 = p0s[r * NT + t];
-            if (n >= n_lo && n < n_hi) *reinterpret_cast<float2*>(row + 2 * (ptrdiff_t)(boff + n)) = make_float2(p0, pw[r]);
+            const bool ok = (inner_valid && n1 >= 8 && n1 < 56) || (n >= n_lo && n < n_hi);
+            if (ok) dst[64 * n1] = make_float2(p0, pw[r]);
           }
         }
       } else {
