@@ -28,7 +28,10 @@ struct TemplateGeom {
   int32_t hw;
 };
 
-constexpr int kChunkTP = 256;          // template-phases per work item (G chunk = kChunkTP * L * 8 bytes, L2-resident)
+#ifndef JERK_CHUNK_TP
+#define JERK_CHUNK_TP 256
+#endif
+constexpr int kChunkTP = JERK_CHUNK_TP;          // template-phases per work item (G chunk = kChunkTP * L * 8 bytes, L2-resident)
 constexpr int kSeamCap = 1 << 16;      // seam records kept in d_work
 constexpr uint64_t kWorkHeader = 256;  // bytes: counters
 constexpr uint64_t kBankAlign = 256;
