@@ -91,3 +91,26 @@ def max_over_ranks(value: float, group=None) -> float:
     t = torch.tensor([value], dtype=torch.float64, device=dev)
     dist.all_reduce(t, op=dist.ReduceOp.MAX, group=group)
     return float(t.item())
+
+
+def search_candidates_sharded(plan, d_spec, threshold, max_cands: int = 1 << 20, group=None, src: int = 0) -> np.ndarray:
+    """Strong-scaling search of ONE spectrum over the ranks of `group` (partition by template):
+    the spectrum is broadcast from `src`, every rank searches its template box with jerk_search_candidates_range
+    against its own bank, and the candidate lists are concatenated on every rank (sorted by (iw, iz, j)).
+    Without an initialised process group it is the whole-grid search on this rank.  No collective touches the search
+    itself: the candidate rule is one-dimensional along r inside a (z,w) row (reading S10)."""
+    import torch.distributed as dist
+    from . import binding
+    sharded = dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1
+    world = dist.get_world_size(group) if sharded else 1
+    rank = dist.get_rank(group) if sharded else 0
+    if sharded:
+        broadcast_spectrum(d_spec, src=src, group=group)
+    iz_lo, iz_cnt, iw_lo, iw_cnt = template_box(plan.info.nz, plan.info.nw, world, rank)
+    d_c, d_n = plan.search_candidates_range(d_spec, threshold, iz_lo, iz_cnt, iw_lo, iw_cnt, max_cands)
+    local, n = binding.candidates_to_numpy(d_c, d_n)
+    if n > max_cands:
+        raise RuntimeError(f"candidate buffer overflow on rank {rank}: {n} > {max_cands}")
+    if sharded:
+        return gather_candidates(local, group=group)
+    return np.sort(local, order=["iw", "iz", "j"])

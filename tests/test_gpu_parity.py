@@ -399,3 +399,14 @@ def test_seg_len_4096_low_threshold_seams_and_edges(nbins):
     assert m == s and (s > 0 or nbins < 1000)
     # first and last half-bin of a row can be candidates (P[-1] = P[2 nbins] = -inf)
     assert cands["j"].min() >= 0 and cands["j"].max() <= 2 * nbins - 1
+
+
+@pytest.mark.gpu
+def test_sharded_search_entry_point_single_rank():
+    """shard.search_candidates_sharded without a process group == the whole-grid search (the N = 1 end of SURVEY.md 8(e);
+    the multi-rank host logic runs under gloo in tests/test_shard_gloo.py, the box property in test_candidates_range_union)."""
+    from paper_1911_01353_b200 import shard
+    cfg, X, plan, d_spec = _setup(1)
+    got = shard.search_candidates_sharded(plan, d_spec, 8.0)
+    full, n = binding.candidates_to_numpy(*plan.search_candidates(d_spec, 8.0))
+    assert np.array_equal(got, np.sort(full, order=["iw", "iz", "j"]))
