@@ -45,6 +45,24 @@ def _worker(rank, world, port, nz, nw, q):
             X = torch.view_as_complex(torch.arange(2000, dtype=torch.float32).reshape(1000, 2).contiguous())
         shard.broadcast_spectrum(X, src=0)
         ok_bcast = bool(torch.view_as_real(X)[-1, 1] == 1999.0)
+        # the whole strong-scaling entry point against a stand-in plan whose "search" slices the fixed list by box
+        class _Info:
+            pass
+
+        class _FakePlan:
+            info = _Info()
+
+            def search_candidates_range(self, d_spec, thr, iz_lo, iz_cnt, iw_lo, iw_cnt, max_cands):
+                sel = full[(full["iz"] >= iz_lo) & (full["iz"] < iz_lo + iz_cnt) & (full["iw"] >= iw_lo) &
+                           (full["iw"] < iw_lo + iw_cnt) & (full["power"] > thr)]
+                buf = np.zeros(max_cands * 16, dtype=np.uint8)
+                buf[: sel.size * 16] = np.frombuffer(sel.tobytes(), dtype=np.uint8)
+                return torch.from_numpy(buf), torch.tensor([sel.size], dtype=torch.int64)
+
+        _FakePlan.info.nz, _FakePlan.info.nw = nz, nw
+        merged2 = shard.search_candidates_sharded(_FakePlan(), X, 40.0, max_cands=4096)
+        want2 = np.sort(full[full["power"] > 40.0], order=["iw", "iz", "j"])
+        ok_merge = ok_merge and np.array_equal(merged2, want2) and bool(torch.view_as_real(X)[-1, 1] == 1999.0)
         tmax = shard.max_over_ranks(10.0 + rank)
         q.put((rank, ok_merge, ok_bcast, tmax, shard.trial_indices(7, world, rank)))
     finally:
