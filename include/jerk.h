@@ -190,6 +190,18 @@ int jerk_search_candidates_host(jerk_plan* plan, const void* h_spec, float thres
                                 uint64_t work_bytes, void* stream);
 
 /*
+ * jerk_search_series_host — the whole pipeline from a HOST time series: copies h_series (host, ideally pinned, float32,
+ * nsamples = 2*nbins) to d_series, jerk_prepare_spectrum (block-normalised spectrum into d_spec), jerk_search_candidates,
+ * copies the count and min(count, max_cands) records back and synchronises the stream.  All device buffers are
+ * caller-owned staging (d_series: nsamples floats, 16-byte aligned; d_spec: nbins complex64; d_scratch:
+ * jerk_spectrum_scratch_bytes(nsamples)); errors as the calls it is made of.
+ */
+int jerk_search_series_host(jerk_plan* plan, const float* h_series, int64_t nsamples, int block, float threshold,
+                            jerk_cand* h_cands, int64_t max_cands, unsigned long long* h_count, float* d_series,
+                            void* d_spec, void* d_scratch, uint64_t scratch_bytes, jerk_cand* d_cands,
+                            unsigned long long* d_count, void* d_work, uint64_t work_bytes, void* stream);
+
+/*
  * jerk_harmonic_sum — fused harmonic-sum stage (row a-6; BASELINE.json configs[4]; section 3):
  * S_h(j,iz',iw') = sum_{k=1..h} P[rnd(j k/h); rnd(iz' k/h), rnd(iw' k/h)] with signed grid indices
  * iz' = iz-(nz-1)/2, iw' = iw-(nw-1)/2 and rnd = round half away from zero (reading S13).

@@ -42,7 +42,7 @@ EXPORTS = [
     "jerk_templates", "jerk_templates_taps", "jerk_search_plane", "jerk_search_candidates",
     "jerk_search_candidates_range", "jerk_search_candidates_stats", "jerk_snr_filter",
     "jerk_sift_candidates",
-    "jerk_search_candidates_host", "jerk_harmonic_scratch_bytes", "jerk_harmonic_sum", "jerk_harmonic_plane", "jerk_spectrum_scratch_bytes",
+    "jerk_search_candidates_host", "jerk_search_series_host", "jerk_harmonic_scratch_bytes", "jerk_harmonic_sum", "jerk_harmonic_plane", "jerk_spectrum_scratch_bytes",
     "jerk_prepare_spectrum", "jerk_probe_fma", "jerk_strerror",
     "jerk_last_error",
 ]
@@ -75,6 +75,7 @@ def load_library() -> C.CDLL:
     lib.jerk_snr_filter.argtypes = [vp, vp, vp, vp, i64, C.c_float, vp, i64, vp, vp]
     lib.jerk_sift_candidates.argtypes = [vp, vp, vp, i64, i32, i32, i32, vp, i64, vp, vp]
     lib.jerk_search_candidates_host.argtypes = [vp, vp, C.c_float, vp, i64, vp, vp, vp, vp, vp, u64, vp]
+    lib.jerk_search_series_host.argtypes = [vp, vp, i64, i32, C.c_float, vp, i64, vp, vp, vp, vp, u64, vp, vp, vp, u64, vp]
     lib.jerk_harmonic_scratch_bytes.argtypes = [vp]
     lib.jerk_harmonic_scratch_bytes.restype = u64
     lib.jerk_harmonic_sum.argtypes = [vp, vp, i32, C.POINTER(i32), C.POINTER(C.c_float), vp, vp, u64, vp, u64, vp]
@@ -241,6 +242,18 @@ class Plan:
         self._check(self._lib.jerk_search_candidates_host(
             self._h, C.c_void_p(h_spec.data_ptr()), float(threshold), C.c_void_p(h_cands.data_ptr()), int(max_cands),
             C.c_void_p(h_count.data_ptr()), C.c_void_p(d_spec.data_ptr()), C.c_void_p(d_cands.data_ptr()),
+            C.c_void_p(d_count.data_ptr()), C.c_void_p(work.data_ptr()), work.numel(), _stream_ptr(stream)))
+        return int(h_count.item())
+
+    def search_series_host(self, h_series, threshold, h_cands, h_count, d_series, d_spec, d_scratch, d_cands, d_count, block=1000,
+                           stream=None):
+        """jerk_search_series_host: pinned host time series in, candidates out; device staging caller-owned; synchronous."""
+        work = self._ensure_work(d_spec.device)
+        max_cands = d_cands.numel() // 16
+        self._check(self._lib.jerk_search_series_host(
+            self._h, C.c_void_p(h_series.data_ptr()), int(h_series.numel()), int(block), float(threshold),
+            C.c_void_p(h_cands.data_ptr()), int(max_cands), C.c_void_p(h_count.data_ptr()), C.c_void_p(d_series.data_ptr()),
+            C.c_void_p(d_spec.data_ptr()), C.c_void_p(d_scratch.data_ptr()), d_scratch.numel(), C.c_void_p(d_cands.data_ptr()),
             C.c_void_p(d_count.data_ptr()), C.c_void_p(work.data_ptr()), work.numel(), _stream_ptr(stream)))
         return int(h_count.item())
 

@@ -1624,6 +1624,32 @@ int jerk_search_candidates_host(jerk_plan* p, const void* h_spec, float threshol
   return JERK_OK;
 }
 
+int jerk_search_series_host(jerk_plan* p, const float* h_series, int64_t nsamples, int block, float threshold, jerk_cand* h_cands,
+                            int64_t max_cands, unsigned long long* h_count, float* d_series, void* d_spec, void* d_scratch,
+                            uint64_t scratch_bytes, jerk_cand* d_cands, unsigned long long* d_count, void* d_work, uint64_t work_bytes,
+                            void* stream) {
+  if (!p || !h_series || !h_cands || !h_count || !d_series || !d_spec || !d_scratch) return JERK_EINVAL;
+  if (nsamples != 2 * p->nbins) return fail(p, JERK_EINVAL, "the series must have 2 * nbins samples");
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaError_t e = cudaMemcpyAsync(d_series, h_series, (size_t)nsamples * sizeof(float), cudaMemcpyHostToDevice, st);
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("H2D series: ") + cudaGetErrorString(e));
+  int rc = jerk_prepare_spectrum(d_series, nsamples, block, d_spec, d_scratch, scratch_bytes, stream);
+  if (rc) return fail(p, rc, "jerk_prepare_spectrum failed (size, alignment or scratch)");
+  rc = jerk_search_candidates(p, d_spec, threshold, d_cands, max_cands, d_count, d_work, work_bytes, stream);
+  if (rc) return rc;
+  e = cudaMemcpyAsync(h_count, d_count, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("D2H count: ") + cudaGetErrorString(e));
+  unsigned long long n = *h_count;
+  if ((int64_t)n > max_cands) n = (unsigned long long)max_cands;
+  if (n) {
+    e = cudaMemcpyAsync(h_cands, d_cands, (size_t)n * sizeof(jerk_cand), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("D2H candidates: ") + cudaGetErrorString(e));
+  }
+  return JERK_OK;
+}
+
 // ---- harmonic stage (row a-6)
 }  // extern "C" (reopened below)
 

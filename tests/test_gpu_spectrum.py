@@ -85,3 +85,29 @@ def test_errors():
     with pytest.raises(binding.JerkError):
         binding.prepare_spectrum(d, d_scratch=torch.empty(16, dtype=torch.uint8, device="cuda"))   # scratch too small
     assert lib.jerk_spectrum_scratch_bytes(1 << 12) == (1 << 11) * 8
+
+
+def test_pipeline_from_host_series_equals_the_separate_calls():
+    """jerk_search_series_host (H2D series -> jerk_prepare_spectrum -> jerk_search_candidates -> D2H) returns, record for
+    record, what the separate calls return, and recovers the config-1 injection at the oracle's grid point."""
+    cfg = synth.config(1)
+    x = synth.make_series(cfg)
+    plan = binding.Plan(cfg.nbins, cfg.zmax, cfg.dz, cfg.wmax, cfg.dw, 2, 4096)
+    plan.templates()
+    max_cands = 1 << 16
+    h_series = torch.from_numpy(x).pin_memory()
+    h_cands = torch.empty(max_cands * 16, dtype=torch.uint8).pin_memory()
+    h_count = torch.zeros(1, dtype=torch.int64).pin_memory()
+    d_series = torch.empty(cfg.n, dtype=torch.float32, device="cuda")
+    d_spec = torch.empty((cfg.nbins, 2), dtype=torch.float32, device="cuda")
+    d_scr = torch.empty(cfg.n * 4, dtype=torch.uint8, device="cuda")
+    d_cands = torch.empty(max_cands * 16, dtype=torch.uint8, device="cuda")
+    d_count = torch.zeros(1, dtype=torch.int64, device="cuda")
+    n = plan.search_series_host(h_series, cfg.threshold, h_cands, h_count, d_series, d_spec, d_scr, d_cands, d_count)
+    got = np.sort(h_cands.numpy()[: n * 16].view(binding.CAND_DTYPE), order=["iw", "iz", "j"])
+    spec2 = binding.prepare_spectrum(torch.from_numpy(x).cuda())
+    want, n2 = binding.candidates_to_numpy(*plan.search_candidates(spec2, cfg.threshold))
+    assert n == n2 and np.array_equal(got, np.sort(want, order=["iw", "iz", "j"]))
+    best = got[np.argmax(got["power"])]
+    zs, ws = np.arange(-cfg.zmax, cfg.zmax + 1e-9, cfg.dz), np.arange(-cfg.wmax, cfg.wmax + 1e-9, cfg.dw)
+    assert (zs[best["iz"]], ws[best["iw"]]) == (10.0, 40.0) and best["j"] / 2.0 in (5000.0, 5000.5)
