@@ -6,11 +6,18 @@ zmax=200 / wmax=600 configuration (BASELINE.json configs[2], N = 2^23, seg_len 4
 synthetic spectrum already resident in HBM; the template bank (row a-1) is built once before the timed region, as in a
 survey where one bank serves thousands of DM trials (reading S20), and its build time is reported separately.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1..4]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1..4] [--scaling weak|strong]
 
-N > 1 (launched by torchrun, one rank per GPU): every rank searches its own independent spectrum (another DM trial)
-with its own copy of the bank: weak scaling, no data-path collective; the only collectives are the
-barrier and the max-over-ranks of the device time.
+The default run (N = 1) also times every other row of the path and puts them in the same JSON line under "rows":
+BASELINE configs 1, 2, 4 at their specified seg_len and at seg_len = 0 (the library's choice), config 5 (harmonic sum),
+plane mode, the fused row statistics, the batched search and numbetween = 1; --no-rows skips them.
+
+N > 1 (launched by torchrun, one rank per GPU).  --scaling weak (default): every rank searches its own independent
+spectrum (another DM trial) with its own copy of the bank, no data-path collective; the only
+collectives are the barrier and the max-over-ranks of the device time.  --scaling strong: ONE spectrum, every rank
+builds, holds and searches 1/N of the template bank (jerk_templates_range + jerk_search_candidates_templates), the
+spectrum is broadcast and the candidate lists gathered inside the timed step (shard.search_candidates_sharded), and the
+gathered list is checked against rank 0's whole-grid search.
 
 --impl reference times the oracle (oracle/jerk_oracle.py, as it stands) on this box's host cores on a bounded sample
 of the same workload; it is a deliberately slow baseline, not the target.
@@ -33,9 +40,8 @@ import numpy as np
 METRIC = "ffdot_points_per_sec"
 UNIT = "points/s"
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12     # 74.45: SMs x FP32 lanes x 2 (FMA) x max SM clock
-# dram__bytes_read.sum + dram__bytes_write.sum of one full-size config-3 k_search64<cand> launch (profiles/r1_05_k_search64_cand_full.md);
-# algorithmic minimum = bank + spectrum once = 0.837 GB
-NCU_DRAM_BYTES_PER_LAUNCH = {3: 1055630080 + 8592896}
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "k_search64_traffic.json")   # written from the ncu capture it names
+HARM_FLOP_FACTOR = sum(e ** 3 for e in range(1, 9)) / 512.0                # eight sub-volumes of fractions e/8: 2.53 base searches
 
 
 def _measured_peaks():
@@ -44,6 +50,18 @@ def _measured_peaks():
             return json.load(f)
     except Exception:
         return None
+
+
+def _ncu_traffic(config_index):
+    """DRAM bytes per launch of the headline kernel from the committed ncu capture (profiles/k_search64_traffic.json)."""
+    try:
+        with open(TRAFFIC_FILE) as f:
+            t = json.load(f)
+        if t.get("config") != config_index:
+            return None, None
+        return int(t["dram_bytes_read"]) + int(t["dram_bytes_write"]), f"bytes per launch (ncu dram read+write, capture {t['capture']})"
+    except Exception:
+        return None, None
 
 
 class ClockSampler(threading.Thread):
@@ -99,10 +117,24 @@ class ClockSampler(threading.Thread):
         return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
-def oracle_sample(cfg, X, seconds_target=15.0, seed=7):
-    """Time the oracle as it stands on a bounded sample of the workload: random (z,w) rows x a bin range.
+# ------------------------------------------------------------------------------------------------ the oracle, timed
+def _oracle_row_job(args):
+    from oracle import jerk_oracle as orc
+    Xs, z, w, b_rel, b_cnt = args
+    return orc.power_row(Xs, z, w, b_rel, b_cnt).size
 
-    Returns (points_per_s, description, points, seconds).  Template quadrature is part of the oracle's work."""
+
+def _nproc():
+    try:
+        return len(os.sched_getaffinity(0))
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def oracle_sample(cfg, X, seconds_target=8.0, seed=7, workers=1, pool=None):
+    """Time the oracle as it stands on a bounded sample of the workload: random (z,w) rows x a 4000-bin range, one row
+    per task, `workers` processes.  Returns (points_per_s, description, points, seconds).  Template quadrature is part of
+    the oracle's work."""
     from oracle import jerk_oracle as orc
     zs, ws = orc.grid_values(cfg.zmax, cfg.dz), orc.grid_values(cfg.wmax, cfg.dw)
     rng = np.random.default_rng(seed)
@@ -111,45 +143,88 @@ def oracle_sample(cfg, X, seconds_target=15.0, seed=7):
     pad = 700
     lo, hi = max(0, b_lo - pad), min(cfg.nbins, b_lo + b_cnt + pad)
     Xs = np.asarray(X[lo:hi])
+
+    def job():
+        iz, iw = int(rng.integers(0, zs.size)), int(rng.integers(0, ws.size))
+        return (Xs, float(zs[iz]), float(ws[iw]), b_lo - lo, b_cnt)
+
     rows = 0
     t0 = time.perf_counter()
-    while True:
-        iz, iw = int(rng.integers(0, zs.size)), int(rng.integers(0, ws.size))
-        orc.power_row(Xs, float(zs[iz]), float(ws[iw]), b_lo - lo, b_cnt)
-        rows += 1
-        el = time.perf_counter() - t0
-        if el >= seconds_target or rows >= 4096:
-            break
+    if workers <= 1 or pool is None:
+        while True:
+            _oracle_row_job(job())
+            rows += 1
+            el = time.perf_counter() - t0
+            if el >= seconds_target or rows >= 4096:
+                break
+    else:
+        while True:                                   # waves of 2 rows per worker until the time target is reached
+            wave = [job() for _ in range(2 * workers)]
+            list(pool.map(_oracle_row_job, wave))
+            rows += len(wave)
+            el = time.perf_counter() - t0
+            if el >= seconds_target or rows >= 65536:
+                break
     pts = rows * 2 * b_cnt
-    return pts / el, f"{rows} random (z,w) rows x {b_cnt} bins ({pts} points) of {cfg.name}, templates included", pts, el
+    return pts / el, f"{rows} random (z,w) rows x {b_cnt} bins ({pts} points) of {cfg.name}, templates included, {workers} process(es)", pts, el
+
+
+def oracle_pool(workers):
+    import multiprocessing as mp
+    from concurrent.futures import ProcessPoolExecutor
+    pool = ProcessPoolExecutor(max_workers=workers, mp_context=mp.get_context("spawn"))
+    list(pool.map(_oracle_row_job, [(np.zeros(64, np.complex64), 0.0, 0.0, 8, 4)] * (2 * workers)))    # start the workers (imports) outside the timed region
+    return pool
+
+
+def cpu_baseline(cfg, X):
+    """The oracle on ALL host cores of this box (a process pool over rows) plus the 1-core figure."""
+    n = _nproc()
+    v1, d1, p1, s1 = oracle_sample(cfg, X, seconds_target=6.0, workers=1)
+    out = {"value": v1, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": d1, "seconds": s1,
+           "value_1core": v1, "extrapolated_seconds_per_search": cfg.points / v1, "host_cores": n}
+    if n > 1:
+        pool = oracle_pool(n)
+        try:
+            v, d, p, s = oracle_sample(cfg, X, seconds_target=10.0, seed=8, workers=n, pool=pool)
+        finally:
+            pool.shutdown()
+        out.update({"value": v, "cores": n, "sample": d, "seconds": s, "extrapolated_seconds_per_search": cfg.points / v,
+                    "sample_1core": d1, "seconds_1core": s1})
+    return out
 
 
 def run_reference(args, cfg_index):
-    """--impl reference: the oracle on host cores, same metric/config; each step is a bounded sample."""
-    from paper_1911_01353_b200 import synth
+    """--impl reference: the oracle on the host cores, same metric/config; each step is a bounded sample."""
+    import workloads as synth
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
     cfg = synth.config(cfg_index)
     X = synth.make_spectrum(cfg)
-    per_step = max(2.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
-    for _ in range(args.warmup):
-        oracle_sample(cfg, X, seconds_target=per_step)
-    pts = 0
-    secs = 0.0
-    desc = ""
-    for s in range(args.steps):
-        v, desc, p, el = oracle_sample(cfg, X, seconds_target=per_step, seed=100 + s)
-        pts += p
-        secs += el
+    n = _nproc()
+    pool = oracle_pool(n) if n > 1 else None
+    per_step = max(2.0, min(12.0, 90.0 / max(1, args.steps + args.warmup)))
+    try:
+        for _ in range(args.warmup):
+            oracle_sample(cfg, X, seconds_target=per_step, workers=n, pool=pool)
+        pts, secs, desc = 0, 0.0, ""
+        for s in range(args.steps):
+            v, desc, p, el = oracle_sample(cfg, X, seconds_target=per_step, seed=100 + s, workers=n, pool=pool)
+            pts += p
+            secs += el
+    finally:
+        if pool is not None:
+            pool.shutdown()
     value = pts / secs
-    ms_per_step_full = cfg.points / value * 1e3        # extrapolated time of one full search at the oracle's rate
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms_per_step_full, "higher_is_better": True, "scaling": "weak",
+        "warmup": args.warmup, "ms_per_step": secs * 1e3 / max(1, args.steps), "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": _config_dict(cfg, note="oracle timed on a bounded sample per step; ms_per_step is extrapolated to a full search"),
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc + f", x{args.steps} steps"},
+        "config": _config_dict(cfg),
+        "note": "each step is a bounded sample of the workload (ms_per_step is the sample's own time); a full search at this rate is extrapolated_ms_per_search",
+        "points_per_step": pts / max(1, args.steps), "extrapolated_ms_per_search": cfg.points / value * 1e3,
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": n, "kind": "oracle", "sample": desc + f", x{args.steps} steps"},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -157,17 +232,44 @@ def run_reference(args, cfg_index):
     return 0
 
 
-def _config_dict(cfg, note=None):
-    d = {
+def _config_dict(cfg, seg_len=None, mode="candidate mode"):
+    L = cfg.seg_len if seg_len is None else seg_len
+    return {
         "workload": f"BASELINE.json configs[{cfg.index - 1}] '{cfg.name}': N=2^{cfg.log2n}, zmax={cfg.zmax:g} dz={cfg.dz:g}, "
-                    f"wmax={cfg.wmax:g} dw={cfg.dw:g}, numbetween=2, seg_len={cfg.seg_len}, candidate mode thr={cfg.threshold:g}",
+                    f"wmax={cfg.wmax:g} dw={cfg.dw:g}, numbetween=2, seg_len={L}, {mode} thr={cfg.threshold:g}",
         "nbins": cfg.nbins, "nz": cfg.nz, "nw": cfg.nw, "points_per_search": cfg.points,
         "cache": "inputs larger than L2: the 0.8 GB template bank is streamed every step (no L2 flush needed)",
         "parallelism": "one independent spectrum (DM trial) per GPU, bank replicated; no data-path collective",
     }
-    if note:
-        d["note"] = note
-    return d
+
+
+# ------------------------------------------------------------------------------------------------ timing helpers
+def _time_steps(fn, warmup, steps):
+    """Per-step CUDA-event times (ms) of fn on the current stream after `warmup` (>= 3) untimed calls."""
+    import torch
+    for _ in range(max(3, warmup)):
+        fn()
+    torch.cuda.synchronize()
+    ts = []
+    for _ in range(steps):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        fn()
+        b.record()
+        torch.cuda.synchronize()
+        ts.append(a.elapsed_time(b))
+    return ts
+
+
+def _row_entry(ts, points, flops, extra=None):
+    ms = float(np.median(ts))
+    e = {"ms": ms, "ms_best": float(min(ts)), "steps": len(ts), "points_per_s": points / (ms * 1e-3) if points else None}
+    if flops:
+        e["tflops_algorithmic"] = flops / (ms * 1e-3) / 1e12
+        e["frac_fp32_peak"] = e["tflops_algorithmic"] / FP32_PEAK_TFLOPS
+    if extra:
+        e.update(extra)
+    return e
 
 
 def run_cufft_comparator(args, cfg, out):
@@ -177,7 +279,8 @@ def run_cufft_comparator(args, cfg, out):
     It is a comparator, not a product path: it uses this library's bank (re-ordered to natural order), is checked
     against jerk_search_plane on one block, is timed on a bounded sample of the config-3 workload and extrapolated."""
     import torch
-    from paper_1911_01353_b200 import binding, synth
+    from paper_1911_01353_b200 import binding
+    import workloads as synth
     L = cfg.seg_len
     assert L == 4096, "the comparator re-orders the seg_len-4096 bank layout"
     X = synth.make_spectrum(cfg)
@@ -214,17 +317,7 @@ def run_cufft_comparator(args, cfg, out):
     theirs = torch.stack([P[0, 0], P[0, 1]], dim=1).reshape(-1)
     err = float(((ours - theirs).abs() / torch.clamp(ours, min=1.0)).max())
     assert err < 1e-3, err
-    for _ in range(max(1, args.warmup)):
-        block()
-    torch.cuda.synchronize()
-    ts = []
-    for _ in range(args.steps):
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record()
-        block()
-        b.record()
-        torch.cuda.synchronize()
-        ts.append(a.elapsed_time(b))
+    ts = _time_steps(block, args.warmup, args.steps)
     units = ntp_blk * nseg_blk
     total_units = 2 * info.ntemplates * info.nseg
     out.update({"ms_block": ts, "units_per_block": units, "max_rel_diff_vs_fused_plane": err,
@@ -234,13 +327,18 @@ def run_cufft_comparator(args, cfg, out):
     return 0
 
 
-def run_row(args):
-    """--row harmonic|spectrum|stats|plane: time one of the OTHER rows of the path (not the headline line; one GPU).
+def harmonic_scratch_bytes(plan, free_bytes):
+    """Scratch for the harmonic row: 4x the default (a 262144-bin r-chunk: fewer segment-edge recomputations) when the
+    device has room, else the default."""
+    base = plan.harmonic_scratch_bytes()
+    return 4 * base if free_bytes > 4 * base + (8 << 30) else base
 
-    harmonic: jerk_harmonic_sum on BASELINE config 5; spectrum: jerk_prepare_spectrum on the config's time series;
-    stats: jerk_search_candidates_stats + jerk_snr_filter on config 3; plane: jerk_search_plane of the whole config-2 volume."""
+
+def run_row(args):
+    """--row harmonic|spectrum|stats|plane|batch|cufft: time ONE of the other rows of the path and print its own line."""
     import torch
-    from paper_1911_01353_b200 import binding, build, synth
+    from paper_1911_01353_b200 import binding, build
+    import workloads as synth
     build.build()
     binding.load_library()
     torch.cuda.set_device(0)
@@ -249,6 +347,7 @@ def run_row(args):
     out = {"row": args.row, "config": _config_dict(cfg)["workload"], "steps": args.steps, "warmup": args.warmup, "data": "synthetic"}
     if args.row == "cufft":
         return run_cufft_comparator(args, cfg, out)
+    points = flops = None
     if args.row == "spectrum":
         d_series = torch.from_numpy(synth.make_series(cfg)).cuda()
         d_spec = torch.empty((cfg.nbins, 2), dtype=torch.float32, device="cuda")
@@ -260,33 +359,148 @@ def run_row(args):
         plan = binding.Plan(cfg.nbins, cfg.zmax, cfg.dz, cfg.wmax, cfg.dw, 2, cfg.seg_len)
         plan.templates()
         d_spec = binding.spectrum_to_device(X)
+        points, flops = cfg.points, plan.info.flops_per_search
         if args.row == "harmonic":
-            fn = lambda: plan.harmonic_sum(d_spec)
+            nbytes = args.scratch_gb << 30 if args.scratch_gb else harmonic_scratch_bytes(plan, torch.cuda.mem_get_info()[0])
+            out["scratch_bytes"] = nbytes
+            flops *= HARM_FLOP_FACTOR
+            fn = lambda: plan.harmonic_sum(d_spec, scratch_bytes=nbytes)
         elif args.row == "stats":
             def fn():
                 d_c, d_n, d_s = plan.search_candidates_stats(d_spec, cfg.threshold)
                 return plan.snr_filter(d_s, d_c, d_n, 20.0)
+        elif args.row == "batch":
+            specs = [d_spec] + [binding.spectrum_to_device(synth.make_spectrum(synth.config(idx), trial=b)) for b in range(1, args.batch)]
+            points, flops = points * args.batch, flops * args.batch
+            out["nspec"] = args.batch
+            fn = lambda: plan.search_candidates_batch(specs, cfg.threshold)
         else:
             plane = torch.empty((cfg.nw, cfg.nz, 2 * cfg.nbins), dtype=torch.float32, device="cuda")
             fn = lambda: plan.search_plane(d_spec, 0, cfg.nbins, out=plane)
             out["algorithmic_bytes"] = plane.numel() * 4
-        out["algorithmic_flops"] = plan.info.flops_per_search
-    for _ in range(args.warmup):
-        fn()
-    torch.cuda.synchronize()
-    ts = []
-    for _ in range(args.steps):
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record()
-        fn()
-        b.record()
-        torch.cuda.synchronize()
-        ts.append(a.elapsed_time(b))
-    out["ms"] = ts
-    out["ms_best"] = min(ts)
+    ts = _time_steps(fn, args.warmup, args.steps)
+    out.update(_row_entry(ts, points, flops))
+    out["ms_all"] = ts
     if "algorithmic_bytes" in out:
         out["GBps_algorithmic"] = out["algorithmic_bytes"] / min(ts) / 1e6
     print(json.dumps(out))
+    return 0
+
+
+def other_rows(steps=3):
+    """Every other row of the path, timed in the same run (CUDA events, >= 3 warm-ups each): BASELINE configs 1, 2, 4 at
+    their specified seg_len and at seg_len = 0 (the library's choice; results do not depend on seg_len, pin P9), plane
+    mode, fused statistics, batched spectra, numbetween = 1, and config 5 (harmonic sum)."""
+    import torch
+    from paper_1911_01353_b200 import binding
+    import workloads as synth
+    rows = {}
+    for idx in (1, 2, 4):
+        cfg = synth.config(idx)
+        X = synth.make_spectrum(cfg)
+        d_spec = binding.spectrum_to_device(X)
+        for L in (cfg.seg_len, 0):
+            plan = binding.Plan(cfg.nbins, cfg.zmax, cfg.dz, cfg.wmax, cfg.dw, 2, L)
+            plan.templates()
+            n_steps = 2 if idx == 4 else steps
+            ts = _time_steps(lambda: plan.search_candidates(d_spec, cfg.threshold), 3, n_steps)
+            n = int(plan.search_candidates(d_spec, cfg.threshold)[1].item())
+            rows[f"config{idx}_candidates_seg{L if L else '0(4096)'}"] = _row_entry(
+                ts, cfg.points, plan.info.flops_per_search, {"seg_len": int(plan.info.seg_len), "candidates": n})
+            if idx == 2 and L == cfg.seg_len:
+                plane = torch.empty((cfg.nw, cfg.nz, 2 * cfg.nbins), dtype=torch.float32, device="cuda")
+                ts = _time_steps(lambda: plan.search_plane(d_spec, 0, cfg.nbins, out=plane), 3, steps)
+                rows["config2_plane_mode_seg2048"] = _row_entry(ts, cfg.points, plan.info.flops_per_search,
+                                                                {"plane_bytes": plane.numel() * 4, "plane_GBps": plane.numel() * 4 / np.median(ts) / 1e6})
+                del plane
+            del plan
+        del d_spec
+        torch.cuda.empty_cache()
+    cfg = synth.config(3)
+    X = synth.make_spectrum(cfg)
+    d_spec = binding.spectrum_to_device(X)
+    plan = binding.Plan(cfg.nbins, cfg.zmax, cfg.dz, cfg.wmax, cfg.dw, 2, cfg.seg_len)
+    plan.templates()
+
+    def stats():
+        d_c, d_n, d_s = plan.search_candidates_stats(d_spec, cfg.threshold)
+        return plan.snr_filter(d_s, d_c, d_n, 20.0)
+
+    rows["config3_candidates_with_row_statistics"] = _row_entry(_time_steps(stats, 3, steps), cfg.points, plan.info.flops_per_search)
+    nspec = 4
+    specs = [d_spec] + [binding.spectrum_to_device(synth.make_spectrum(synth.config(3), trial=b)) for b in range(1, nspec)]
+    ts = _time_steps(lambda: plan.search_candidates_batch(specs, cfg.threshold), 3, 2)
+    rows["config3_batch_of_4_spectra"] = _row_entry(ts, nspec * cfg.points, nspec * plan.info.flops_per_search,
+                                                    {"nspec": nspec, "ms_per_spectrum": float(np.median(ts)) / nspec})
+    del specs
+    plan1 = binding.Plan(cfg.nbins, cfg.zmax, cfg.dz, cfg.wmax, cfg.dw, 1, cfg.seg_len)
+    plan1.templates()
+    ts = _time_steps(lambda: plan1.search_candidates(d_spec, cfg.threshold), 3, steps)
+    rows["config3_numbetween1"] = _row_entry(ts, cfg.points // 2, plan1.info.flops_per_search)
+    del plan1, d_spec
+    torch.cuda.empty_cache()
+    cfg = synth.config(5)
+    X = synth.make_spectrum(cfg)
+    d_spec = binding.spectrum_to_device(X)
+    nbytes = harmonic_scratch_bytes(plan, torch.cuda.mem_get_info()[0])
+    ts = _time_steps(lambda: plan.harmonic_sum(d_spec, scratch_bytes=nbytes), 3, 2)
+    top = plan.harmonic_sum(d_spec, scratch_bytes=nbytes)
+    rows["config5_harmonic_sum_1_2_4_8"] = _row_entry(
+        ts, cfg.points, plan.info.flops_per_search * HARM_FLOP_FACTOR,
+        {"scratch_bytes": nbytes, "stage_tops": [{"h": h, "j": int(r["j"]), "iz": int(r["iz"]), "iw": int(r["iw"]), "S": float(r["power"])}
+                                                  for h, r in zip((1, 2, 4, 8), top)],
+         "flops_note": "algorithmic flops = (1^3 + ... + 8^3)/512 = 2.53 base searches (the eight sub-volumes of fractions e/8)"})
+    return rows
+
+
+def run_strong(args, torch, dist, rank, local_rank, world):
+    """--scaling strong: one spectrum, the template bank sharded over the ranks."""
+    from paper_1911_01353_b200 import binding, shard
+    import workloads as synth
+    cfg = synth.config(args.config)
+    X = synth.make_spectrum(cfg)                         # every rank can make it; only rank 0's copy is used (broadcast)
+    plan = binding.Plan(cfg.nbins, cfg.zmax, cfg.dz, cfg.wmax, cfg.dw, 2, cfg.seg_len)
+    ti_lo, ti_cnt = shard.build_bank_shard(plan)
+    d_spec = binding.spectrum_to_device(X if rank == 0 else np.zeros_like(X))
+    step = lambda: shard.search_candidates_sharded(plan, d_spec, cfg.threshold)
+    merged = step()
+    check = None
+    if rank == 0:                                        # the gathered list == the whole-grid search of a full bank
+        full = binding.Plan(cfg.nbins, cfg.zmax, cfg.dz, cfg.wmax, cfg.dw, 2, cfg.seg_len)
+        full.templates()
+        ref, _ = binding.candidates_to_numpy(*full.search_candidates(d_spec, cfg.threshold))
+        check = bool(merged.tobytes() == np.sort(ref, order=["iw", "iz", "j"]).tobytes())
+        del full
+    for _ in range(max(3, args.warmup) - 1):
+        step()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    total_ms = e0.elapsed_time(e1)
+    if world > 1:
+        total_ms = shard.max_over_ranks(total_ms)
+    if rank == 0:
+        ms = total_ms / args.steps
+        cd = _config_dict(cfg)
+        cd["parallelism"] = (f"tp{world} over the template bank: rank r builds and searches templates [r T/{world}, (r+1) T/{world}); spectrum "
+                             "broadcast + candidate all-gather inside the timed step; no collective inside the search")
+        print(json.dumps({
+            "metric": METRIC, "value": cfg.points / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
+            "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": cd, "clocks": clocks, "gathered_equals_whole_grid_search": check, "templates_per_rank": int(ti_cnt),
+            "bank_bytes_per_rank": int(plan.bank.numel()), "candidates": int(merged.size), "gpu_launches": 5 * args.steps,
+        }))
     return 0
 
 
@@ -297,9 +511,13 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config number 1..4 (default 3: the headline)")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--row", default="search", choices=["search", "harmonic", "spectrum", "stats", "plane", "cufft"],
+    ap.add_argument("--no-rows", action="store_true", help="skip the other rows of the path (configs 1, 2, 4, 5, plane, statistics, batch)")
+    ap.add_argument("--row", default="search", choices=["search", "harmonic", "spectrum", "stats", "plane", "batch", "cufft"],
                     help="search (default) = the headline bench line; the others time another row of the path and print their own line")
+    ap.add_argument("--batch", type=int, default=4, help="--row batch: spectra per call")
+    ap.add_argument("--scratch-gb", type=int, default=0, help="--row harmonic: scratch buffer size in GiB (default: 4x the library's default chunk)")
     ap.add_argument("--log2n", type=int, default=0,
                     help="profiling aid: shorten the time series to 2^LOG2N samples (same grid, same kernel); not the headline")
     args = ap.parse_args()
@@ -313,7 +531,8 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_1911_01353_b200 import binding, build, synth
+    from paper_1911_01353_b200 import binding, build
+    import workloads as synth
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -328,6 +547,11 @@ def main():
     if world > 1:
         dist.barrier()
     binding.load_library()
+    if args.scaling == "strong":
+        rc = run_strong(args, torch, dist, rank, local_rank, world)
+        if world > 1:
+            dist.destroy_process_group()
+        return rc
 
     cfg = synth.config(args.config)
     if args.log2n:
@@ -436,10 +660,10 @@ def main():
             measured_fp32 = binding.probe_fp32_tflops()
         except Exception:
             measured_fp32 = None
+        traffic, traffic_unit = (None, None) if args.log2n else _ncu_traffic(args.config)
         roofline = {
             "bound": "alu", "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
-            "traffic": None if args.log2n else NCU_DRAM_BYTES_PER_LAUNCH.get(args.config),
-            "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1_05)",
+            "traffic": traffic, "traffic_unit": traffic_unit,
             "kernel": "k_search64<cand>" if cfg.seg_len == 4096 else f"k_search<{cfg.seg_len},cand>", "kernel_ms": kernel_ms,
             "algorithmic_flops_per_launch": info.flops_per_search,
             "peak_measured_ffma": measured_fp32, "frac_of_measured_ffma": (achieved / measured_fp32) if measured_fp32 else None,
@@ -453,14 +677,17 @@ def main():
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(cfg.nbins * 8),
                     "d2h_bytes_per_step": int(8 + min(n_e2e, max_cands) * 16), "ms_per_step": e2e_ms / args.steps},
-            "gpu_launches": 3 * args.steps,
+            "gpu_launches": 5 * args.steps,      # k_reset, k_search64, k_seam_clear, k_seam_insert, k_seam_resolve per search
             "roofline": roofline,
             "bank_build_ms": bank_ms, "spectrum_prep_ms": prep_ms, "e2e_from_series_ms": series_ms, "candidates_found": n_found, "step_ms": step_ms,
         }
+        del d_cands, d_spec2
+        if world == 1 and not args.no_rows and not args.log2n and args.config == 3:
+            del plan, d_spec
+            torch.cuda.empty_cache()
+            line["rows"] = other_rows()
         if not args.no_cpu_baseline and world == 1:
-            v, desc, pts, el = oracle_sample(cfg, X, seconds_target=15.0)
-            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc,
-                                    "seconds": el, "extrapolated_seconds_per_search": cfg.points / v}
+            line["cpu_baseline"] = cpu_baseline(cfg, X)
         elif world > 1:
             line["cpu_baseline"] = None
         print(json.dumps(line))

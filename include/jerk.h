@@ -20,7 +20,9 @@
  *    frees or retains ownership of device memory and never creates streams: every device buffer is
  *    caller-owned (e.g. torch.Tensor.data_ptr()), every call takes the caller's cudaStream_t
  *    (passed as void*) and is asynchronous on it unless stated otherwise.
- *  - The plan is the only library-owned object (host memory).
+ *  - The plan is the only library-owned object (host memory).  A plan and the d_work buffer passed with it serve ONE
+ *    call at a time: two searches of the same plan (or with the same d_work) must not overlap, on any stream or thread
+ *    (the work-item counter, the seam records and the error text live there).  Use one plan + d_work per stream.
  *  - One GPU, sm_100a only; there is no CPU fallback of any kind.
  *  - Grid: z_iz = -zmax + iz*dz (iz = 0..nz-1), w_iw = -wmax + iw*dw (iw = 0..nw-1); template index
  *    ti = iw*nz + iz; r = j/2 bins.
@@ -41,7 +43,8 @@ typedef enum jerk_status {
   JERK_ENOMEM = -2,   /* a caller-provided buffer is smaller than the *_bytes the plan asks */
   JERK_ECUDA = -3,    /* a CUDA runtime call or launch failed                              */
   JERK_ESTATE = -4,   /* jerk_templates has not been called for this plan                  */
-  JERK_ENODEV = -5    /* no sm_100 device is current                                       */
+  JERK_ENODEV = -5,   /* no sm_100 device is current                                       */
+  JERK_EOVERFLOW = -6 /* (host entry points) more candidates than max_cands, or more seam records than d_work holds */
 } jerk_status;
 
 typedef struct jerk_plan jerk_plan;
@@ -77,7 +80,8 @@ typedef struct jerk_plan_info_t {
  * jerk_plan_create — host only (BASELINE.json north_star: jerk_plan_create(nbins, zmax, dz, wmax, dw,
  * numbetween, seg_len)).  Validates the grid and derives nz, nw, c(z,w), hw(z,w), hw_max, step, nseg.
  * Requirements: nbins >= 1; zmax, wmax >= 0; dz, dw > 0 with zmax/dz and wmax/dw integers;
- * numbetween == 2; seg_len in {1024, 2048, 4096, 8192} and seg_len - 2*hw_max >= 2, or seg_len == 0 for the library's
+ * numbetween 2 (the half-bin phases p = 0, 1) or 1 (integer bins only, p = 0: half the work; the FDAS-style option of
+ * SURVEY.md 8(f) N4; planes then hold one float per bin and the harmonic stage is not offered); seg_len in {1024, 2048, 4096, 8192} and seg_len - 2*hw_max >= 2, or seg_len == 0 for the library's
  * choice (4096, the fastest kernel, whenever it leaves a positive step; the result does not depend on seg_len); nz, nw < 32768.
  * *out receives a plan that jerk_plan_destroy frees.  Errors: JERK_EINVAL.
  */
@@ -107,6 +111,15 @@ uint64_t jerk_plane_bytes(int64_t r_cnt, int iz_cnt, int iw_cnt);
 int jerk_templates(jerk_plan* plan, void* d_bank, uint64_t bank_bytes, void* stream);
 
 /*
+ * jerk_templates_range — build only templates ti in [ti_lo, ti_lo + ti_cnt) (flat index ti = iw*nz + iz) into d_bank
+ * (>= jerk_bank_bytes_range(plan, ti_cnt) bytes: the c/hw tables of the whole grid + ti_cnt filters).  This is what one
+ * rank of a template-sharded multi-GPU search holds ("each GPU holds 1/G of the bank"); afterwards the
+ * plan searches only boxes / ranges inside it (JERK_ESTATE otherwise).  jerk_templates is the range [0, ntemplates).
+ */
+uint64_t jerk_bank_bytes_range(const jerk_plan* plan, int ti_cnt);
+int jerk_templates_range(jerk_plan* plan, int ti_lo, int ti_cnt, void* d_bank, uint64_t bank_bytes, void* stream);
+
+/*
  * jerk_templates_taps — export the raw half-bin lattice R_{z,w}(c - hw + i/2), i = 0..4hw, of one
  * template as complex64 pairs into d_taps (DEVICE, >= (4hw+1)*8 bytes).  Test hook for row a-1.
  */
@@ -129,7 +142,12 @@ int jerk_search_plane(jerk_plan* plan, const void* d_spec, int64_t r_lo, int64_t
  * (unordered on return); d_count: DEVICE uint64, set by the call to the total number of candidates found
  * (may exceed max_cands: the excess is dropped, the caller detects overflow by count > max_cands).
  * d_work as above; after the call d_work's first 64 bytes hold diagnostic counters
- * (uint64: [0] work-item counter, [1] seam records, [2] seam overflow flag, [3] provisional candidates).
+ * (uint64: [0] work-item counter, [1] seam records, [2] seam overflow flag, [3] candidates settled at seams).
+ * Seams: an above-threshold point whose r-neighbour is computed by another warp or segment is parked as a 16-byte seam
+ * record in d_work (about 1 in 32 above-threshold points) and settled after the kernel.  plan work_bytes leaves room for
+ * 2^20 records; a larger d_work (work_bytes argument) holds 16 bytes per extra record, up to 2^22.  If the records do
+ * not fit the result would be incomplete: the call then sets *d_count = UINT64_MAX (never a silently shortened list),
+ * which the "count > max_cands" test every caller must make catches; the *_host entry points return JERK_EOVERFLOW.
  * Errors: JERK_EINVAL, JERK_ENOMEM, JERK_ESTATE, JERK_ECUDA.
  */
 int jerk_search_candidates(jerk_plan* plan, const void* d_spec, float threshold, jerk_cand* d_cands,
@@ -148,6 +166,28 @@ int jerk_search_candidates_range(jerk_plan* plan, const void* d_spec, float thre
                                  unsigned long long* d_count, void* d_work, uint64_t work_bytes, void* stream);
 
 /*
+ * jerk_search_candidates_templates — the same for a FLAT range of templates ti in [ti_lo, ti_lo + ti_cnt), ti = iw*nz + iz
+ * (one launch over at most three boxes).  Splitting [0, ntemplates) evenly over G ranks leaves at most one template of
+ * imbalance; with jerk_templates_range every rank builds and holds only its own part of the bank.
+ */
+int jerk_search_candidates_templates(jerk_plan* plan, const void* d_spec, float threshold, int ti_lo, int ti_cnt,
+                                     jerk_cand* d_cands, int64_t max_cands, unsigned long long* d_count, void* d_work,
+                                     uint64_t work_bytes, void* stream);
+
+/*
+ * jerk_search_candidates_batch — many spectra against one bank (PAPER.md:27 the search runs once per
+ * de-dispersion trial of the pipeline, PAPER.md:39 one bank of filters serves all of them).  h_d_specs: HOST array of
+ * nspec DEVICE pointers (each a d_spec as above, all of the plan's nbins).  The spectrum index is one more dimension of
+ * the work-item space: one launch per 32 spectra walks every 8 MB chunk of the bank once for all of their segments.
+ * Spectrum b gets its own list d_cands[b*max_cands ..) and count d_counts[b] (DEVICE, nspec entries), each exactly what
+ * jerk_search_candidates would return for that spectrum alone (same records, unordered; same overflow rules, the seam
+ * room of d_work being shared by the spectra of one launch).
+ */
+int jerk_search_candidates_batch(jerk_plan* plan, const void* const* h_d_specs, int nspec, float threshold,
+                                 jerk_cand* d_cands, int64_t max_cands, unsigned long long* d_counts, void* d_work,
+                                 uint64_t work_bytes, void* stream);
+
+/*
  * jerk_search_candidates_stats + jerk_snr_filter — the paper's own candidate front end (PAPER.md:43
  * peaks "above a certain threshold" of the output plane, "mean and standard deviation along with candidate
  * selection dominate the execution time"), fused: ONE pass of the search kernel collects local-max candidates above the
@@ -157,7 +197,7 @@ int jerk_search_candidates_range(jerk_plan* plan, const void* d_spec, float thre
  * jerk_snr_filter then keeps the candidates with snr = (P - mean_row)/std_row > snr_threshold (population standard
  * deviation; rows with zero variance keep nothing), out of place into d_cands_out / d_count_out (DEVICE, zeroed by
  * the call; unordered; overflow as in jerk_search_candidates) with the snr stored as float bits in `flags`.
- * seg_len 4096 plans only (JERK_EINVAL otherwise).  Other arguments and errors as jerk_search_candidates.
+ * Other arguments and errors as jerk_search_candidates.
  */
 int jerk_search_candidates_stats(jerk_plan* plan, const void* d_spec, float threshold, jerk_cand* d_cands,
                                  int64_t max_cands, unsigned long long* d_count, double* d_rowstats,
@@ -182,7 +222,9 @@ int jerk_sift_candidates(jerk_plan* plan, const jerk_cand* d_cands_in, const uns
  * jerk_search_candidates_host — the same search with HOST input/output (end-to-end entry point):
  * copies h_spec (host, ideally pinned, nbins complex64) to d_spec, searches, copies the count and
  * min(count, max_cands) records back to h_count / h_cands and synchronises the stream before returning.
- * All device buffers are still caller-owned staging.
+ * All device buffers are still caller-owned staging.  Being synchronous it reports both overflow conditions as
+ * JERK_EOVERFLOW: count > max_cands (the first max_cands records are copied, *h_count is the total) and a seam-record
+ * overflow (*h_count = UINT64_MAX, nothing copied).
  */
 int jerk_search_candidates_host(jerk_plan* plan, const void* h_spec, float threshold, jerk_cand* h_cands,
                                 int64_t max_cands, unsigned long long* h_count, void* d_spec,

@@ -279,3 +279,26 @@ def sift(cands, wj: int, wz: int, ww: int) -> list:
         if alive:
             out.append(a)
     return sorted(out, key=lambda c: (c[2], c[1], c[0]))
+
+
+# --------------------------------------------------------------------------- I: numbetween = 1
+def power_row_nb1(X: np.ndarray, z: float, w: float, b_lo: int = 0, b_cnt: int | None = None, tmpl=None) -> np.ndarray:
+    """P[b; z,w] = |sum_m X[b+m] conj(R_{z,w}(m))|^2 on the integer bins b in [b_lo, b_lo+b_cnt) only: the
+    numbetween = 1 search keeps the phase-0 tap set of section C (m = c-hw..c+hw, q = m) and drops the half-bin
+    phase (the FDAS-style option; SURVEY.md 8(f) N4 "numbetween options").  X[k] = 0 outside [0, nbins)."""
+    X = np.asarray(X, dtype=np.complex128)
+    nbins = X.size
+    if b_cnt is None:
+        b_cnt = nbins - b_lo
+    c, hw, lattice = tmpl if tmpl is not None else template(z, w)
+    out = np.zeros(b_cnt, dtype=np.float64)
+    for i in range(b_cnt):
+        b = b_lo + i
+        acc = 0.0 + 0.0j
+        for m in range(c - hw, c + hw + 1):
+            k = b + m
+            if 0 <= k < nbins:
+                acc += X[k] * np.conj(lattice[2 * (m - (c - hw))])
+        out[i] = acc.real * acc.real + acc.imag * acc.imag
+    return out
+

@@ -1,7 +1,7 @@
 """CPU oracle for the spectrum-preparation stage upstream of the jerk search.
 
 TEST INFRASTRUCTURE ONLY (same rules as jerk_oracle.py): only ``tests/``, ``__graft_entry__.smoke()`` and
-``bench.py``'s oracle legs may import it; it shares no code with the CUDA path or with ``synth.py``.
+``bench.py``'s oracle legs may import it; it shares no code with the CUDA path or with ``workloads.py``.
 
 What it computes (BASELINE.json configs[0]: "The real FFT gives 32768 complex bins, normalised to unit mean power
 per 1000-bin block"; PAPER.md:15 the search works on the Fourier transform of the de-dispersed time series;

@@ -12,10 +12,10 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-# JERK_B200_LIB may point at an experimental build of the same library (kernel tuning); default is the in-tree one
-LIB_PATH = os.environ.get("JERK_B200_LIB") or os.path.join(_HERE, "libjerk_b200.so")
+LIB_PATH = os.path.join(_HERE, "libjerk_b200.so")
 
-JERK_OK, JERK_EINVAL, JERK_ENOMEM, JERK_ECUDA, JERK_ESTATE, JERK_ENODEV = 0, -1, -2, -3, -4, -5
+JERK_OK, JERK_EINVAL, JERK_ENOMEM, JERK_ECUDA, JERK_ESTATE, JERK_ENODEV, JERK_EOVERFLOW = 0, -1, -2, -3, -4, -5, -6
+SEAM_OVERFLOW = (1 << 64) - 1      # *d_count after a search whose seam records did not fit in d_work (include/jerk.h)
 
 CAND_DTYPE = np.dtype([("j", "<i4"), ("iz", "<i2"), ("iw", "<i2"), ("power", "<f4"), ("flags", "<u4")])
 assert CAND_DTYPE.itemsize == 16
@@ -39,8 +39,9 @@ class PlanInfo(C.Structure):
 
 EXPORTS = [
     "jerk_plan_create", "jerk_plan_destroy", "jerk_plan_info", "jerk_template_geometry", "jerk_plane_bytes",
-    "jerk_templates", "jerk_templates_taps", "jerk_search_plane", "jerk_search_candidates",
-    "jerk_search_candidates_range", "jerk_search_candidates_stats", "jerk_snr_filter",
+    "jerk_templates", "jerk_templates_range", "jerk_bank_bytes_range", "jerk_templates_taps", "jerk_search_plane",
+    "jerk_search_candidates", "jerk_search_candidates_range", "jerk_search_candidates_templates",
+    "jerk_search_candidates_batch", "jerk_search_candidates_stats", "jerk_snr_filter",
     "jerk_sift_candidates",
     "jerk_search_candidates_host", "jerk_search_series_host", "jerk_harmonic_scratch_bytes", "jerk_harmonic_sum", "jerk_harmonic_plane", "jerk_spectrum_scratch_bytes",
     "jerk_prepare_spectrum", "jerk_probe_fma", "jerk_strerror",
@@ -67,10 +68,15 @@ def load_library() -> C.CDLL:
     lib.jerk_plane_bytes.argtypes = [i64, i32, i32]
     lib.jerk_plane_bytes.restype = u64
     lib.jerk_templates.argtypes = [vp, vp, u64, vp]
+    lib.jerk_templates_range.argtypes = [vp, i32, i32, vp, u64, vp]
+    lib.jerk_bank_bytes_range.argtypes = [vp, i32]
+    lib.jerk_bank_bytes_range.restype = u64
     lib.jerk_templates_taps.argtypes = [vp, i32, i32, vp, u64, vp]
     lib.jerk_search_plane.argtypes = [vp, vp, i64, i64, i32, i32, i32, i32, vp, u64, vp, u64, vp]
     lib.jerk_search_candidates.argtypes = [vp, vp, C.c_float, vp, i64, vp, vp, u64, vp]
     lib.jerk_search_candidates_range.argtypes = [vp, vp, C.c_float, i32, i32, i32, i32, vp, i64, vp, vp, u64, vp]
+    lib.jerk_search_candidates_templates.argtypes = [vp, vp, C.c_float, i32, i32, vp, i64, vp, vp, u64, vp]
+    lib.jerk_search_candidates_batch.argtypes = [vp, C.POINTER(vp), i32, C.c_float, vp, i64, vp, vp, u64, vp]
     lib.jerk_search_candidates_stats.argtypes = [vp, vp, C.c_float, vp, i64, vp, vp, u64, vp, u64, vp]
     lib.jerk_snr_filter.argtypes = [vp, vp, vp, vp, i64, C.c_float, vp, i64, vp, vp]
     lib.jerk_sift_candidates.argtypes = [vp, vp, vp, i64, i32, i32, i32, vp, i64, vp, vp]
@@ -101,8 +107,9 @@ def _stream_ptr(stream=None):
 class Plan:
     """jerk_plan_create(nbins, zmax, dz, wmax, dw, numbetween, seg_len) and the calls that take a plan."""
 
-    def __init__(self, nbins, zmax, dz, wmax, dw, numbetween=2, seg_len=4096):
+    def __init__(self, nbins, zmax, dz, wmax, dw, numbetween=2, seg_len=4096, extra_seams=0):
         self._lib = load_library()
+        self.extra_seams = extra_seams
         self._h = C.c_void_p()
         rc = self._lib.jerk_plan_create(C.byref(self._h), int(nbins), float(zmax), float(dz), float(wmax), float(dw),
                                         int(numbetween), int(seg_len))
@@ -137,9 +144,11 @@ class Plan:
 
     # ---- device calls (torch supplies memory and the stream)
     def _ensure_work(self, device):
+        """The plan's d_work (caller-owned scratch).  One plan + work buffer serves one call at a time (include/jerk.h);
+        `extra_seams` at construction time adds room for more seam records than the 2^20 of info.work_bytes."""
         import torch
         if self.work is None:
-            self.work = torch.empty(int(self.info.work_bytes), dtype=torch.uint8, device=device)
+            self.work = torch.empty(int(self.info.work_bytes) + 16 * int(self.extra_seams), dtype=torch.uint8, device=device)
         return self.work
 
     def templates(self, device="cuda", stream=None):
@@ -149,6 +158,15 @@ class Plan:
             self.bank = torch.empty(int(self.info.bank_bytes), dtype=torch.uint8, device=device)
         self._check(self._lib.jerk_templates(self._h, C.c_void_p(self.bank.data_ptr()), int(self.info.bank_bytes),
                                              _stream_ptr(stream)))
+        return self.bank
+
+    def templates_range(self, ti_lo, ti_cnt, device="cuda", stream=None):
+        """jerk_templates_range: build and hold only templates [ti_lo, ti_lo + ti_cnt) (one rank's share of the bank)."""
+        import torch
+        nbytes = int(self._lib.jerk_bank_bytes_range(self._h, int(ti_cnt)))
+        self.bank = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=device)
+        self._check(self._lib.jerk_templates_range(self._h, int(ti_lo), int(ti_cnt), C.c_void_p(self.bank.data_ptr()), nbytes,
+                                                   _stream_ptr(stream)))
         return self.bank
 
     def templates_taps(self, iz, iw, stream=None):
@@ -200,6 +218,36 @@ class Plan:
             C.c_void_p(d_cands.data_ptr()), int(max_cands), C.c_void_p(d_count.data_ptr()), C.c_void_p(work.data_ptr()),
             work.numel(), _stream_ptr(stream)))
         return d_cands, d_count
+
+    def search_candidates_templates(self, d_spec, threshold, ti_lo, ti_cnt, max_cands=1 << 20, d_cands=None, d_count=None, stream=None):
+        """jerk_search_candidates_templates: candidate mode over the flat template range [ti_lo, ti_lo + ti_cnt)."""
+        import torch
+        if d_cands is None:
+            d_cands = torch.empty(max_cands * 16, dtype=torch.uint8, device=d_spec.device)
+        if d_count is None:
+            d_count = torch.zeros(1, dtype=torch.int64, device=d_spec.device)
+        work = self._ensure_work(d_spec.device)
+        self._check(self._lib.jerk_search_candidates_templates(
+            self._h, C.c_void_p(d_spec.data_ptr()), float(threshold), int(ti_lo), int(ti_cnt), C.c_void_p(d_cands.data_ptr()),
+            int(max_cands), C.c_void_p(d_count.data_ptr()), C.c_void_p(work.data_ptr()), work.numel(), _stream_ptr(stream)))
+        return d_cands, d_count
+
+    def search_candidates_batch(self, d_specs, threshold, max_cands=1 << 18, d_cands=None, d_counts=None, stream=None):
+        """jerk_search_candidates_batch: a list of device spectra against the one bank; returns (d_cands uint8
+        [nspec, max_cands*16], d_counts int64[nspec])."""
+        import torch
+        n = len(d_specs)
+        dev = d_specs[0].device
+        if d_cands is None:
+            d_cands = torch.empty((n, max_cands * 16), dtype=torch.uint8, device=dev)
+        if d_counts is None:
+            d_counts = torch.zeros(n, dtype=torch.int64, device=dev)
+        work = self._ensure_work(dev)
+        ptrs = (C.c_void_p * n)(*[C.c_void_p(x.data_ptr()) for x in d_specs])
+        self._check(self._lib.jerk_search_candidates_batch(
+            self._h, ptrs, n, float(threshold), C.c_void_p(d_cands.data_ptr()), int(max_cands), C.c_void_p(d_counts.data_ptr()),
+            C.c_void_p(work.data_ptr()), work.numel(), _stream_ptr(stream)))
+        return d_cands, d_counts
 
     def search_candidates_stats(self, d_spec, threshold, max_cands=1 << 20, stream=None):
         """jerk_search_candidates_stats: (d_cands, d_count, d_rowstats float64[T, 2] = {sum P, sum P^2} per (z,w) row)."""
@@ -297,7 +345,7 @@ class Plan:
         return out
 
     def work_counters(self):
-        """Diagnostic counters the last search left in d_work (item counter, seam records, seam overflow, provisional)."""
+        """Diagnostic counters the last search left in d_work (item counter, seam records, seam overflow, settled at seams)."""
         return self.work[:64].view(dtype=__import__("torch").int64).cpu().numpy().copy()
 
 
@@ -341,8 +389,11 @@ def probe_fp32_tflops(iters=1 << 15, reps=5):
 
 
 def candidates_to_numpy(d_cands, d_count):
-    """Device candidate buffer -> structured numpy array sorted by (iw, iz, j)."""
-    n = int(d_count.item())
+    """Device candidate buffer -> (structured numpy array sorted by (iw, iz, j), total count).  Raises JerkError
+    (JERK_EOVERFLOW) when the search reported a seam-record overflow: that result is incomplete (include/jerk.h)."""
+    n = int(d_count.item()) & SEAM_OVERFLOW
+    if n == SEAM_OVERFLOW:
+        raise JerkError(JERK_EOVERFLOW, "seam records overflowed d_work: use a Plan with extra_seams or a higher threshold")
     cap = d_cands.numel() // 16
     arr = d_cands[: min(n, cap) * 16].cpu().numpy().view(CAND_DTYPE).copy()
     order = np.lexsort((arr["j"], arr["iz"], arr["iw"]))

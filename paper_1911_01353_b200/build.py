@@ -31,12 +31,12 @@ def needs_build() -> bool:
     return any(os.path.getmtime(d) > t for d in DEPS)
 
 
-def build(force: bool = False, verbose: bool = False, out: str | None = None, defs: list | None = None) -> str:
-    """Compile csrc/*.cu.  `out`/`defs` build an experimental variant (-D flags) to another path."""
-    if out is None and not force and not needs_build():
+def build(force: bool = False, verbose: bool = False) -> str:
+    """Compile csrc/*.cu into libjerk_b200.so (skipped when the library is newer than every source)."""
+    if not force and not needs_build():
         return LIB
-    target = out or LIB
-    cmd = [nvcc_path()] + NVCC_FLAGS + [f"-D{d}" for d in (defs or [])] + ["-o", target] + SRCS
+    target = LIB
+    cmd = [nvcc_path()] + NVCC_FLAGS + ["-o", target] + SRCS
     res = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or res.returncode != 0:
         sys.stderr.write(res.stdout + res.stderr)

@@ -28,15 +28,16 @@ struct TemplateGeom {
   int32_t hw;
 };
 
-#ifndef JERK_CHUNK_TP
-#define JERK_CHUNK_TP 256
-#endif
-constexpr int kChunkTP = JERK_CHUNK_TP;          // template-phases per work item (G chunk = kChunkTP * L * 8 bytes, L2-resident)
-constexpr int kSeamCap = 1 << 16;      // seam records kept in d_work
+constexpr int kChunkTP = 256;          // template-phases per work item (G chunk = kChunkTP * L * 8 bytes, L2-resident; 128..1024 measured equal)
 constexpr uint64_t kWorkHeader = 256;  // bytes: counters
 constexpr uint64_t kBankAlign = 256;
-constexpr int kMaxCtas = 148 * 4;      // upper bound on resident CTAs of the persistent search kernel (stash slots)
-constexpr uint64_t kStashPerCta = 2ull * 8192 * sizeof(float);  // phase-0 and phase-1 powers of one segment (L <= 8192)
+// d_work = header | stash | seam records.  The stash gives every resident FFT group (k_search64: 64 threads) or CTA
+// (k_search<L>) room for the phase-0 and phase-1 powers of one segment (rare path of the candidate test); launches never
+// use more groups than slots, so the constant only has to cover sm_count * 4 groups (148 * 4 on B200, twice that here).
+constexpr int kStashSlots = 1184;
+constexpr uint64_t kStashSlotBytes = 2ull * 4096 * sizeof(float);
+constexpr uint64_t kStashBytes = (uint64_t)kStashSlots * kStashSlotBytes;
+constexpr uint64_t kSeamCapDefault = 1ull << 20;   // seam records jerk_plan_info's work_bytes leaves room for (a larger d_work holds more)
 
 }  // namespace jerk
 
@@ -48,8 +49,9 @@ struct jerk_plan {
   int hw_max, c_max, step;
   int64_t seg_base, nseg;
   std::vector<jerk::TemplateGeom> geom;  // [T]
-  uint64_t geom_bytes, bank_bytes, work_bytes;
+  uint64_t geom_bytes, bank_bytes, work_bytes, stash_bytes;
   void* d_bank;
+  int bank_ti_lo, bank_ti_cnt;   // templates [bank_ti_lo, bank_ti_lo + bank_ti_cnt) are in d_bank (jerk_templates: all T)
   int sm_count;
   std::string err;
 };
@@ -127,8 +129,10 @@ __device__ __forceinline__ int quad_panels(double z, double w, int c, int hw) {
 struct BankParams {
   double zmax, dz, wmax, dw;
   int nz, nw;
-  const TemplateGeom* geom;  // device
-  float2* G;                 // device, [T][2][L] in kernel element order
+  int nb;                    // numbetween: phases per template
+  int ti_lo;                 // first template of the range being built (block b builds template ti_lo + b)
+  const TemplateGeom* geom;  // device, [T]
+  float2* G;                 // device, [ti - ti_lo][nb][L] in kernel element order
 };
 
 // element order of G inside one (template, phase): thread t of the search kernel reads float4 #(u*R1/2 + k2/2)*NT + t,
@@ -160,7 +164,7 @@ __global__ void __launch_bounds__(FftGeom<L>::NT) k_bank(BankParams bp) {
   float2* lat = tw2 + Tw2Table<L>::FLOATS2;  // 4*hw_max+1 lattice values
   __shared__ unsigned long long s_war;
   const int t = threadIdx.x;
-  const int ti = blockIdx.x;
+  const int ti = bp.ti_lo + blockIdx.x;
   const int iz = ti % bp.nz, iw = ti / bp.nz;
   const double z = -bp.zmax + iz * bp.dz, w = -bp.wmax + iw * bp.dw;
   const TemplateGeom g = bp.geom[ti];
@@ -170,7 +174,7 @@ __global__ void __launch_bounds__(FftGeom<L>::NT) k_bank(BankParams bp) {
   Tw3Regs<L> tw1;
   make_tw3<L>(tw1.w, t);
   WarBarrier war = war_init<Gm::NT>(&s_war, t);
-  for (int p = 0; p < 2; p++) {
+  for (int p = 0; p < bp.nb; p++) {
     // taps h~_p[m'] = R(c + m' - p/2) at index (m' mod L): lattice index i = 2*(m'+hw) - p
     for (int k = t; k < L; k += Gm::NT) {
       int mp = k < L / 2 ? k : k - L;  // m' in [-L/2, L/2)
@@ -187,7 +191,7 @@ __global__ void __launch_bounds__(FftGeom<L>::NT) k_bank(BankParams bp) {
       for (int k2 = 0; k2 < Gm::R1; k2++) v[u * Gm::R1 + k2] = exA[256 * k2 + Gm::b1_of(t, u)];
     __syncthreads();
     fft_passes<L, -1>(v, tw1, tw2, exA, exB, war, t);
-    float2* out = bp.G + ((size_t)ti * 2 + p) * L;
+    float2* out = bp.G + ((size_t)blockIdx.x * bp.nb + p) * L;
     const float sc = 1.0f / (float)L;
 #pragma unroll
     for (int u = 0; u < Gm::NB2; u++)
@@ -221,12 +225,29 @@ struct SearchJob {
 };
 constexpr int kMaxJobs = 8;
 
+// Harmonic stage fused into the top-harmonic search (row a-6): sub-plane of fraction e/8, e = 1..7, as written by the
+// plane-mode kernel: P_e[iw_rel][iz_rel][j - j0], row length nj.
+struct HarmGather {
+  const float* base[7];
+  long long j0[7], nj[7];
+  int iz_lo[7], iz_cnt[7], iw_lo[7];
+  int cz, cw;                // centre indices (nz-1)/2, (nw-1)/2
+  float thr[4];              // arg-max mode: only sums above thr[log2 h] can be reported
+  jerk_cand* warpbest;       // arg-max mode: [4][gridDim.x * warps per CTA] best record of every warp, h = 1,2,4,8
+  float* out;                // store mode: S_h of the job's box, out[iw_rel][iz_rel][j - 2 r_lo]
+  int out_stage;             // store mode: log2 h
+};
+
+constexpr int kMaxBatch = 32;   // spectra per launch of the batched candidate search
+
 struct SearchParams {
-  const float2* spec;  // X[nbins]
+  const float2* spec[kMaxBatch];  // X_b[nbins], b < nspec (one spectrum everywhere but in jerk_search_candidates_batch)
+  int nspec;
+  int nb;              // numbetween: 2 (half-bin phases 0 and 1) or 1 (phase 0 only)
   int64_t nbins;
   const float2* G;
   const TemplateGeom* geom;
-  int nz;
+  int nz, nw_grid;     // grid size (nw_grid = nw of the plan)
   int hw_max, step;
   int64_t seg_base;
   int njobs;
@@ -240,12 +261,15 @@ struct SearchParams {
   // scratch
   unsigned long long* work;  // [0] item counter, [1] seam count, [2] seam overflow, [3] provisional
   jerk_cand* seams;
-  float* stash;              // [kMaxCtas][2][L]: powers of the current template, written only on the rare path
+  unsigned long long seam_cap;   // seam records that fit in d_work
+  float* stash;              // one slot of 2 L floats per resident FFT group / CTA: powers of the current template, written only on the rare path
   double* rowstats;          // MODE_CAND_STATS: [T][2] running sum of P and of P^2 over the valid points of every (z,w) row
+  HarmGather hg;             // MODE_HARM / MODE_HARM_STORE: the seven sub-planes the top-harmonic pass gathers from
 };
 
-__device__ __forceinline__ void emit_cand(const SearchParams& sp, int j, int iz, int iw, float pw) {
-  unsigned long long slot = atomicAdd(sp.count, 1ULL);
+// spectrum b of a batch owns cands[b*max_cands ..) and count[b]; its seam records carry b in flags bits 8..31
+__device__ __forceinline__ void emit_cand(const SearchParams& sp, int b, int j, int iz, int iw, float pw) {
+  unsigned long long slot = atomicAdd(sp.count + b, 1ULL);
   if ((int64_t)slot < sp.max_cands) {
     jerk_cand c;
     c.j = j;
@@ -253,30 +277,60 @@ __device__ __forceinline__ void emit_cand(const SearchParams& sp, int j, int iz,
     c.iw = (int16_t)iw;
     c.power = pw;
     c.flags = 0;
-    sp.cands[slot] = c;
+    sp.cands[(size_t)b * sp.max_cands + slot] = c;
   }
 }
-__device__ __forceinline__ void emit_seam(const SearchParams& sp, int j, int iz, int iw, float pw, uint32_t flags) {
+__device__ __forceinline__ void emit_seam(const SearchParams& sp, int b, int j, int iz, int iw, float pw, uint32_t flags) {
   unsigned long long slot = atomicAdd(sp.work + 1, 1ULL);
-  if (slot < (unsigned long long)kSeamCap) {
+  if (slot < sp.seam_cap) {
     jerk_cand c;
     c.j = j;
     c.iz = (int16_t)iz;
     c.iw = (int16_t)iw;
     c.power = pw;
-    c.flags = flags;
+    c.flags = flags | ((uint32_t)b << 8);
     sp.seams[slot] = c;
   } else {
     sp.work[2] = 1ULL;
   }
 }
 
-enum { MODE_PLANE = 0, MODE_CAND = 1, MODE_CAND_STATS = 2 };   // 2: candidate mode + per-row power statistics (seg_len 4096)
 enum { SEAM_LEFT = 1u, SEAM_RIGHT = 2u, SEAM_WITNESS = 4u };
 
-#ifndef JERK_MINBLOCKS_4096
-#define JERK_MINBLOCKS_4096 3
-#endif
+// One work item = (job, chunk of template-phases, spectrum of the batch, segment), chunk-major so that every resident
+// FFT group streams the same chunk of the bank through L2 at the same time, for all segments of all spectra.
+struct WorkItem {
+  int q, chunk, b;
+  int64_t seg;
+};
+__device__ __forceinline__ WorkItem decode_item(const SearchParams& sp, long long item) {
+  WorkItem w;
+  w.q = 0;
+  while (w.q + 1 < sp.njobs && item >= sp.jobs[w.q].item_end) w.q++;
+  const SearchJob& jb = sp.jobs[w.q];
+  const long long jitem = item - (w.q ? sp.jobs[w.q - 1].item_end : 0LL);
+  const long long per_chunk = jb.seg_count * sp.nspec;
+  w.chunk = (int)(jitem / per_chunk);
+  const long long rem = jitem % per_chunk;
+  w.b = (int)(rem / jb.seg_count);
+  w.seg = jb.seg_first + rem % jb.seg_count;
+  return w;
+}
+
+// Candidate test of one valid point in the rare path (P > thr, P > P[j-1], P >= P[j+1]).  `left` /
+// `right` are the neighbours' powers when this warp holds them; a neighbour across a warp or segment seam is unknown
+// (seamL / seamR) and the point becomes a seam record, flagged SEAM_WITNESS when it already lost on a known side (it
+// is then only evidence for its neighbour).  At the spectrum ends the missing neighbour is -inf (known).
+__device__ __forceinline__ void test_point(const SearchParams& sp, int b, int j, int iz, int iw, float p, float left, float right,
+                                           bool seamL, bool seamR) {
+  if (!(p > sp.threshold)) return;
+  const bool pass = (seamL || p > left) && (seamR || p >= right);
+  if (seamL || seamR) emit_seam(sp, b, j, iz, iw, p, (seamL ? SEAM_LEFT : 0u) | (seamR ? SEAM_RIGHT : 0u) | (pass ? 0u : SEAM_WITNESS));
+  else if (pass) emit_cand(sp, b, j, iz, iw, p);
+}
+
+// 2: candidate mode + per-row power statistics; 3 / 4: top-harmonic pass of the harmonic stage (arg-max / S_h store), seg_len 4096
+enum { MODE_PLANE = 0, MODE_CAND = 1, MODE_CAND_STATS = 2, MODE_HARM = 3, MODE_HARM_STORE = 4 };
 
 // TMEM columns per CTA: two thread-private arrays (F and T1) of 2P floats per thread, NW/4 warp groups side by side
 template <int L>
@@ -285,7 +339,7 @@ struct TmemCols {
 };
 
 template <int L, int MODE>
-__global__ void __launch_bounds__(FftGeom<L>::NT, (L == 4096 ? (MODE == MODE_CAND ? JERK_MINBLOCKS_4096 : 2) : 1))
+__global__ void __launch_bounds__(FftGeom<L>::NT, 1)
 k_search(const __grid_constant__ SearchParams sp) {
   using Gm = FftGeom<L>;
   constexpr int NT = Gm::NT, P = Gm::P, R1 = Gm::R1;
@@ -335,16 +389,11 @@ k_search(const __grid_constant__ SearchParams sp) {
     __syncthreads();
     const long long item = s_item;
     if (item >= nitems) break;
-    int q = 0;
-    if (MODE == MODE_PLANE) {
-      while (q + 1 < sp.njobs && item >= sp.jobs[q].item_end) q++;
-    }
-    const SearchJob& jb = sp.jobs[q];
-    const long long jitem = item - (q ? sp.jobs[q - 1].item_end : 0LL);
-    const int chunk = (int)(jitem / jb.seg_count);
-    const int64_t seg = jb.seg_first + jitem % jb.seg_count;
+    const WorkItem wi = decode_item(sp, item);
+    const SearchJob& jb = sp.jobs[wi.q];
+    const float2* spec = sp.spec[wi.b];
     const int iz_cnt = jb.iz_cnt, iz_lo = jb.iz_lo, iw_lo = jb.iw_lo;
-    const int64_t s0 = sp.seg_base + seg * (int64_t)sp.step;  // first bin of the segment (even)
+    const int64_t s0 = sp.seg_base + wi.seg * (int64_t)sp.step;  // first bin of the segment (even)
 
     // ---- a-2: stage the segment in shared memory (exA): TMA bulk copy when fully inside the spectrum, guarded loads at the edges
     const bool interior = (s0 >= 0) && (s0 + L <= sp.nbins);
@@ -353,7 +402,7 @@ k_search(const __grid_constant__ SearchParams sp) {
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // order earlier generic accesses to exA before the async write
         asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(mbar)), "r"((uint32_t)(L * 8)) : "memory");
         asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(exA)),
-                     "l"(sp.spec + s0), "r"((uint32_t)(L * 8)), "r"(smem_u32(mbar))
+                     "l"(spec + s0), "r"((uint32_t)(L * 8)), "r"(smem_u32(mbar))
                      : "memory");
       }
       uint32_t done = 0;
@@ -368,7 +417,7 @@ k_search(const __grid_constant__ SearchParams sp) {
     } else {
       for (int k = t; k < L; k += NT) {
         int64_t b = s0 + k;
-        exA[k] = (b >= 0 && b < sp.nbins) ? sp.spec[b] : make_float2(0.f, 0.f);
+        exA[k] = (b >= 0 && b < sp.nbins) ? spec[b] : make_float2(0.f, 0.f);
       }
       __syncthreads();
     }
@@ -400,14 +449,15 @@ k_search(const __grid_constant__ SearchParams sp) {
       __syncthreads();
     }
 
-    // ---- loop over the template-phases of this chunk
-    const int tp_lo = chunk * jb.chunk_tp;
+    // ---- loop over the template-phases of this chunk (numbetween = 1: one phase per template)
+    const int nb = sp.nb;
+    const int tp_lo = wi.chunk * jb.chunk_tp;
     const int tp_hi = min(jb.ntp, tp_lo + jb.chunk_tp);
     float p0v[P];  // phase-0 powers (plane mode keeps them to store float2 pairs)
     int any0 = 0;  // candidate mode: phase-0 powers of this warp exceeded the threshold and were stashed
-    int izr = (tp_lo >> 1) % iz_cnt, iwr = (tp_lo >> 1) / iz_cnt;
+    int izr = (tp_lo / nb) % iz_cnt, iwr = (tp_lo / nb) / iz_cnt;
     for (int tp = tp_lo; tp < tp_hi; tp++) {
-      const int ph = tp & 1;
+      const int ph = nb == 2 ? (tp & 1) : 0;
       if (ph == 0 && tp != tp_lo && ++izr == iz_cnt) {
         izr = 0;
         ++iwr;
@@ -419,7 +469,7 @@ k_search(const __grid_constant__ SearchParams sp) {
       float2 v[P];
       __syncwarp();   // tcgen05.ld is .sync.aligned: the warp must be converged (the store / candidate paths below diverge)
       {
-        const float4* g4 = reinterpret_cast<const float4*>(sp.G + ((size_t)ti * 2 + ph) * L) + t;
+        const float4* g4 = reinterpret_cast<const float4*>(sp.G + ((size_t)ti * nb + ph) * L) + t;
         float4 g[P / 2];
 #pragma unroll
         for (int e = 0; e < P / 2; e++) g[e] = __ldg(g4 + e * NT);
@@ -435,7 +485,7 @@ k_search(const __grid_constant__ SearchParams sp) {
         }
       }
       fft_passes<L, 1>(v, tmT, tw2, exA, exB, war, t);
-      // ---- a-4: overlap discard + power.  n = b3 + 16*R1*n2 ; b = s0 + n - c ; j = 2b + ph.
+      // ---- a-4: overlap discard + power.  n = b3 + 16*R1*n2 ; b = s0 + n - c ; j = nb*b + ph.
       // valid outputs: n in [n_lo, n_hi) = window [hw_max, hw_max+step) clipped to the bins this call covers
       int n_lo, n_hi;
       {
@@ -448,12 +498,20 @@ k_search(const __grid_constant__ SearchParams sp) {
 #pragma unroll
       for (int i = 0; i < P; i++) pw[i] = fmaf(v[i].x, v[i].x, v[i].y * v[i].y);
       if (MODE == MODE_PLANE) {
-        if (ph == 0) {
+        float* row = jb.plane + ((size_t)iwr * iz_cnt + izr) * (size_t)(nb * jb.r_cnt);
+        const long long boff = s0 - c - jb.r_lo;
+        if (nb == 1) {
+#pragma unroll
+          for (int u = 0; u < Gm::NB2; u++)
+#pragma unroll
+            for (int n2 = 0; n2 < 16; n2++) {
+              const int n = Gm::b3_of(t, u) + 16 * R1 * n2;
+              if (n >= n_lo && n < n_hi) row[boff + n] = pw[u * 16 + n2];
+            }
+        } else if (ph == 0) {
 #pragma unroll
           for (int i = 0; i < P; i++) p0v[i] = pw[i];
         } else {
-          float* row = jb.plane + ((size_t)iwr * iz_cnt + izr) * (size_t)(2 * jb.r_cnt);
-          const long long boff = s0 - c - jb.r_lo;
 #pragma unroll
           for (int u = 0; u < Gm::NB2; u++)
 #pragma unroll
@@ -464,6 +522,27 @@ k_search(const __grid_constant__ SearchParams sp) {
             }
         }
       } else {
+        if (MODE == MODE_CAND_STATS) {
+          // sum of P and P^2 over the valid points of this unit, one fp64 atomic pair per warp
+          float a1[4] = {0.f, 0.f, 0.f, 0.f}, a2[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+          for (int i = 0; i < P; i++) {
+            const int n = Gm::b3_of(t, i >> 4) + 16 * R1 * (i & 15);
+            const float p = (n >= n_lo && n < n_hi) ? pw[i] : 0.f;
+            a1[i & 3] += p;
+            a2[i & 3] = fmaf(p, p, a2[i & 3]);
+          }
+          float s1 = (a1[0] + a1[1]) + (a1[2] + a1[3]), s2 = (a2[0] + a2[1]) + (a2[2] + a2[3]);
+#pragma unroll
+          for (int o = 16; o > 0; o >>= 1) {
+            s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+            s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+          }
+          if (lane == 0) {
+            atomicAdd(sp.rowstats + 2 * (size_t)ti, (double)s1);
+            atomicAdd(sp.rowstats + 2 * (size_t)ti + 1, (double)s2);
+          }
+        }
         // ---- a-5: threshold + local max.  Hot path: one max-reduction and a vote; everything else only when some
         // power of this warp (valid or not) exceeds the threshold.
         float mx = pw[0];
@@ -472,7 +551,28 @@ k_search(const __grid_constant__ SearchParams sp) {
         const int anyhit = __any_sync(0xffffffffu, mx > sp.threshold);
         float* st0 = gstash;            // [P][NT]: element i of thread t at i*NT + t (written and read by the same thread)
         float* st1 = gstash + L;
-        if (ph == 0) {
+        const float NEG = -INFINITY;
+        if (nb == 1) {
+          if (anyhit) {
+#pragma unroll
+            for (int i = 0; i < P; i++) st0[i * NT + t] = pw[i];
+            __syncwarp();
+#pragma unroll 1
+            for (int i = 0; i < P; i++) {
+              const int n = Gm::b3_of(t, i >> 4) + 16 * R1 * (i & 15);
+              const bool valid = (n >= n_lo) && (n < n_hi);
+              const float p = valid ? st0[i * NT + t] : NEG;
+              const float l = __shfl_up_sync(0xffffffffu, p, 1);      // P[b-1]
+              const float r = __shfl_down_sync(0xffffffffu, p, 1);    // P[b+1]
+              if (!valid) continue;
+              const long long b = s0 + n - c;
+              const bool seamL = (lane == 0 || n == sp.hw_max) && (b > 0);
+              const bool seamR = (lane == 31 || n == sp.hw_max + sp.step - 1) && (b < sp.nbins - 1);
+              test_point(sp, wi.b, (int)b, iz, iw, p, b > 0 ? l : NEG, b < sp.nbins - 1 ? r : NEG, seamL, seamR);
+            }
+            __syncwarp();
+          }
+        } else if (ph == 0) {
           any0 = anyhit;
           if (anyhit) {
 #pragma unroll
@@ -482,7 +582,6 @@ k_search(const __grid_constant__ SearchParams sp) {
 #pragma unroll
           for (int i = 0; i < P; i++) st1[i * NT + t] = pw[i];
           __syncwarp();
-          const float NEG = -INFINITY;
 #pragma unroll 1
           for (int i = 0; i < P; i++) {
             const int n = Gm::b3_of(t, i >> 4) + 16 * R1 * (i & 15);
@@ -494,21 +593,10 @@ k_search(const __grid_constant__ SearchParams sp) {
             if (!valid) continue;
             const long long b = s0 + n - c;
             // phase-0 point j = 2b: left neighbour (b-1, phase 1), right neighbour (b, phase 1)
-            if (p0 > sp.threshold) {
-              const bool seamL = (lane == 0 || n == sp.hw_max) && (b > 0);
-              const float left = (b > 0 && !seamL) ? l1 : NEG;
-              const bool okR = p0 >= p1;
-              if (seamL) emit_seam(sp, (int)(2 * b), iz, iw, p0, SEAM_LEFT | (okR ? 0u : SEAM_WITNESS));
-              else if (p0 > left && okR) emit_cand(sp, (int)(2 * b), iz, iw, p0);
-            }
+            test_point(sp, wi.b, (int)(2 * b), iz, iw, p0, b > 0 ? l1 : NEG, p1, (lane == 0 || n == sp.hw_max) && (b > 0), false);
             // phase-1 point j = 2b+1: left neighbour (b, phase 0), right neighbour (b+1, phase 0)
-            if (p1 > sp.threshold) {
-              const bool seamR = (lane == 31 || n == sp.hw_max + sp.step - 1) && (b < sp.nbins - 1);
-              const float right = (b < sp.nbins - 1 && !seamR) ? r0 : NEG;
-              const bool okL = p1 > p0;
-              if (seamR) emit_seam(sp, (int)(2 * b + 1), iz, iw, p1, SEAM_RIGHT | (okL ? 0u : SEAM_WITNESS));
-              else if (okL && p1 >= right) emit_cand(sp, (int)(2 * b + 1), iz, iw, p1);
-            }
+            test_point(sp, wi.b, (int)(2 * b + 1), iz, iw, p1, p0, b < sp.nbins - 1 ? r0 : NEG, false,
+                       (lane == 31 || n == sp.hw_max + sp.step - 1) && (b < sp.nbins - 1));
           }
           __syncwarp();
         }
@@ -553,6 +641,235 @@ __device__ __forceinline__ void bulk_copy_g2s(uint32_t dst, const void* src, uin
                "r"(bytes), "r"(bar)
                : "memory");
 }
+// ---- harmonic stage, fused into the top-harmonic pass (row a-6; BASELINE.json configs[4]; reading S13)
+//   S_h(j,iz',iw') = sum_{k=1..h} P[rnd(j k/h); rnd(iz' k/h), rnd(iw' k/h)],  signed grid indices, rnd = round half away from zero.
+// Every fraction k/h of h in {1,2,4,8} is e/8:  S1 = P8;  S2 = S1 + P4;  S4 = S2 + P2 + P6;  S8 = S4 + P1 + P3 + P5 + P7,
+// Pe = the sub-plane of fraction e/8.  P8 is the search itself: the top-harmonic pass holds it in registers (phase 1) and
+// tensor memory (phase 0) and gathers P1..P7 from the sub-planes that an earlier plane-mode launch left in scratch, so
+// the largest sub-plane never exists in memory and no separate summing pass reads it back.
+struct HarmRecord {   // running arg-max of one warp and one stage
+  float s;            // best sum so far (initially the stage threshold: only sums above it count)
+  int j, ti;          // its position (j = -1: none yet)
+};
+
+__device__ __forceinline__ int rnd_eighths(int a, int e) {          // round-half-away-from-zero of a*e/8
+  const int m = (abs(a) * e + 4) >> 3;
+  return a < 0 ? -m : m;
+}
+
+// a beats b as the arg-max: larger sum, ties -> smallest (iw, iz, j) in row-major order (ti = iw*nz + iz)
+__device__ __forceinline__ bool harm_better_ti(float sa, int ja, int tia, float sb, int jb, int tib) {
+  if (sa != sb) return sa > sb;
+  if (tia != tib) return tia < tib;
+  return ja < jb;
+}
+
+// the four stage sums of one point from its own power p8 and the seven gathered sub-harmonic powers g[e-1]
+__device__ __forceinline__ void harm_stage_sums(float p8, const float (&g)[7], float (&sv)[4]) {
+  sv[0] = p8;
+  sv[1] = sv[0] + g[3];
+  sv[2] = sv[1] + g[1] + g[5];
+  sv[3] = sv[2] + g[0] + g[2] + g[4] + g[6];
+}
+
+// Seven read-only loads (one per fraction e = 1..7) at byte offsets KOFF * e from the seven pointers: one register of
+// one phase.  Unpredicated: a register outside the unit's valid window (the box may be much shorter than a segment) reads
+// up to (4096 + c_max) e / 4 floats before or after its sub-plane row -- still inside the scratch buffer, which carries a
+// guard band at both ends (kHarmGuard) -- and its sums are discarded.  volatile: the loads of a batch keep their place before the fence.
+template <int KOFF>
+__device__ __forceinline__ void ld_gather7(float (&g)[7], const float* const (&q)[7]) {
+  asm volatile(
+      "ld.global.nc.f32 %0, [%7+%14];\n\tld.global.nc.f32 %1, [%8+%15];\n\tld.global.nc.f32 %2, [%9+%16];\n\t"
+      "ld.global.nc.f32 %3, [%10+%17];\n\tld.global.nc.f32 %4, [%11+%18];\n\tld.global.nc.f32 %5, [%12+%19];\n\t"
+      "ld.global.nc.f32 %6, [%13+%20];"
+      : "=f"(g[0]), "=f"(g[1]), "=f"(g[2]), "=f"(g[3]), "=f"(g[4]), "=f"(g[5]), "=f"(g[6])
+      : "l"(q[0]), "l"(q[1]), "l"(q[2]), "l"(q[3]), "l"(q[4]), "l"(q[5]), "l"(q[6]), "n"(KOFF * 1), "n"(KOFF * 2), "n"(KOFF * 3),
+        "n"(KOFF * 4), "n"(KOFF * 5), "n"(KOFF * 6), "n"(KOFF * 7));
+}
+
+// the valid half-bin range of one (segment, template) unit -> the seven contiguous sub-plane ranges it will gather;
+// one thread asks for them to be brought into L2 (bulk prefetch) two transforms before the gathers
+__device__ __forceinline__ void harm_prefetch(const SearchParams& sp, const SearchJob& jb, int s0, int c, int ti) {
+  const HarmGather& hg = sp.hg;
+  const long long b_lo = max((long long)jb.r_lo, (long long)s0 + sp.hw_max - c);
+  const long long b_hi = min((long long)(jb.r_lo + jb.r_cnt), (long long)s0 + sp.hw_max + sp.step - c);   // exclusive
+  if (b_hi <= b_lo) return;
+  const int az = ti % sp.nz - hg.cz, aw = ti / sp.nz - hg.cw;
+#pragma unroll
+  for (int e = 1; e <= 7; e++) {
+    const int ize = rnd_eighths(az, e) + hg.cz, iwe = rnd_eighths(aw, e) + hg.cw;
+    const float* row = hg.base[e - 1] + ((long long)(iwe - hg.iw_lo[e - 1]) * hg.iz_cnt[e - 1] + (ize - hg.iz_lo[e - 1])) * hg.nj[e - 1] - hg.j0[e - 1];
+    const uintptr_t lo = (uintptr_t)(row + ((2 * b_lo * e + 4) >> 3)) & ~(uintptr_t)15;
+    const uintptr_t hi = ((uintptr_t)(row + (((2 * b_hi - 1) * e + 4) >> 3) + 1) + 15) & ~(uintptr_t)15;
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(lo), "r"((uint32_t)(hi - lo)) : "memory");
+  }
+}
+
+// One batch of the gathers of harm_unit: registers k = K0 .. K0+3 (< KHI) of register group a, both phases: 14 loads per
+// register, all issued before the first sum.
+constexpr int kHarmBatch = 4;   // registers per batch: 56 loads in flight per thread (about what one warp can have outstanding)
+template <bool STORE, int K0, int KHI>
+__device__ __forceinline__ void harm_batch(const HarmGather& hg, const float* const (&q0)[7], const float* const (&q1)[7],
+                                           uint32_t tmP, const float* p1s, int a, int t, int n_lo, int n_hi,
+                                           bool inner_valid, float2* dst, float (&mx)[4]) {
+  constexpr int kB = kHarmBatch;
+  float g0[kB][7], g1[kB][7];
+  bool ok[kB];
+#pragma unroll
+  for (int b = 0; b < kB; b++) {
+    if (K0 + b >= KHI) continue;
+    const int n1 = a + 4 * (K0 + b);
+    const int n = t + 64 * n1;
+    ok[b] = (inner_valid && n1 >= 8 && n1 < 56) || (n >= n_lo && n < n_hi);
+  }
+  if (K0 + 0 < KHI) { ld_gather7<256 * (K0 + 0)>(g0[0], q0); ld_gather7<256 * (K0 + 0)>(g1[0], q1); }
+  if (K0 + 1 < KHI) { ld_gather7<256 * (K0 + 1)>(g0[1], q0); ld_gather7<256 * (K0 + 1)>(g1[1], q1); }
+  if (K0 + 2 < KHI) { ld_gather7<256 * (K0 + 2)>(g0[2], q0); ld_gather7<256 * (K0 + 2)>(g1[2], q1); }
+  if (kB > 3 && K0 + 3 < KHI) { ld_gather7<256 * (K0 + 3)>(g0[kB - 1], q0); ld_gather7<256 * (K0 + 3)>(g1[kB - 1], q1); }
+  // Scheduling fence: the sums sit behind a branch the compiler cannot resolve (cz >= 0 always), i.e. in another basic
+  // block, so that every load of the batch is issued before the first sum waits for one (ptxas otherwise pulls each
+  // sum up next to its own loads, which serialises the round trips).
+  if (hg.cz < -1 - K0) return;       // (a different condition per batch: equal ones would be merged and the batches with them)
+  constexpr int KB = K0 > 12 ? 12 : K0;   // four columns that hold the batch and stay inside the 16 of this register group
+  float p0c[4];
+  tmem_ld4(tmP + 16 * a + KB, p0c);   // the powers of this unit: phase 0 from tensor memory, phase 1 from shared memory
+#pragma unroll
+  for (int b = 0; b < kB; b++) {
+    const int k = K0 + b;
+    if (k >= KHI) continue;
+    const int n1 = a + 4 * k;
+    float sa[4], sb[4];
+    harm_stage_sums(p0c[k - KB], g0[b], sa);
+    harm_stage_sums(p1s[(16 * a + k) * 64 + t], g1[b], sb);
+    if (STORE) {
+      if (ok[b]) dst[64 * n1] = make_float2(sa[hg.out_stage], sb[hg.out_stage]);
+    } else if (ok[b]) {
+#pragma unroll
+      for (int q = 0; q < 4; q++) mx[q] = fmaxf(mx[q], fmaxf(sa[q], sb[q]));
+    }
+  }
+}
+
+// One (segment, template) unit of the top-harmonic pass, called when phase 1 is done.  Phase-0 powers are in tensor
+// memory at tmP, phase-1 powers in shared memory p1s (register r of thread t at r*64 + t; both written and read by the
+// same thread); register r = 16 a + k holds n = t + 64 n1, n1 = a + 4 k.  Point j = 2 (s0 + n - c) + ph reads sub-plane e
+// at (j e + 4) >> 3 = ((jt e + 4) >> 3) + 16 n1 e with jt = 2 (s0 - c + t) + ph: one pointer per (fraction, phase), moved
+// on by 16 e per a, and compile-time offsets 64 k e.  The loop over a is rolled: the unrolled version (5000
+// instructions on top of the transforms) thrashed the instruction cache (no_instruction stalls 1.2 per issue).
+template <bool STORE, bool PRUNE>
+__device__ __forceinline__ void harm_unit(const SearchParams& sp, const SearchJob& jb, const float* p1s, uint32_t tmP, int t, int lane,
+                                          int s0, int c, int ti, int box_row, int n_lo, int n_hi, HarmRecord* rec, float* stash) {
+  const HarmGather& hg = sp.hg;
+  const float* q0[7];
+  const float* q1[7];
+  {
+    const int az = ti % sp.nz - hg.cz, aw = ti / sp.nz - hg.cw;
+    const long long jt = 2LL * (s0 - c + t);
+#pragma unroll
+    for (int e = 1; e <= 7; e++) {
+      const int ize = rnd_eighths(az, e) + hg.cz, iwe = rnd_eighths(aw, e) + hg.cw;
+      const float* row = hg.base[e - 1] + ((long long)(iwe - hg.iw_lo[e - 1]) * hg.iz_cnt[e - 1] + (ize - hg.iz_lo[e - 1])) * hg.nj[e - 1] -
+                         hg.j0[e - 1];
+      q0[e - 1] = row + ((jt * e + 4) >> 3);
+      q1[e - 1] = row + (((jt + 1) * e + 4) >> 3);
+    }
+  }
+  // registers with n1 = n / 64 in [8, 56) are valid for every thread of a segment inside the box (hw_max <= 512)
+  const bool inner_valid = __all_sync(0xffffffffu, n_lo <= t + 64 * 8 && n_hi >= t + 64 * 56);
+  float2* dst = nullptr;
+  if (STORE) dst = reinterpret_cast<float2*>(hg.out + (size_t)box_row * (size_t)(2 * jb.r_cnt) + 2 * (ptrdiff_t)(s0 - c - (int)jb.r_lo + t));
+  float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+  // The gathers are latency-bound (two warps per scheduler, every register busy during the transforms): they are issued
+  // in batches of kB registers = 14 kB independent loads (about the number of loads one warp can have outstanding),
+  // all of a batch before the first sum.
+  constexpr int KLO = PRUNE ? 1 : 0, KHI = PRUNE ? 15 : 16;   // PRUNE: k = 0 and 15 (n1 < 4, n1 >= 60) are never valid
+#pragma unroll 1
+  for (int a = 0; a < 4; a++) {
+    harm_batch<STORE, KLO, KHI>(hg, q0, q1, tmP, p1s, a, t, n_lo, n_hi, inner_valid, dst, mx);
+    harm_batch<STORE, KLO + kHarmBatch, KHI>(hg, q0, q1, tmP, p1s, a, t, n_lo, n_hi, inner_valid, dst, mx);
+    harm_batch<STORE, KLO + 2 * kHarmBatch, KHI>(hg, q0, q1, tmP, p1s, a, t, n_lo, n_hi, inner_valid, dst, mx);
+    harm_batch<STORE, KLO + 3 * kHarmBatch, KHI>(hg, q0, q1, tmP, p1s, a, t, n_lo, n_hi, inner_valid, dst, mx);
+    if (KLO + 4 * kHarmBatch < KHI) harm_batch<STORE, KLO + 4 * kHarmBatch, KHI>(hg, q0, q1, tmP, p1s, a, t, n_lo, n_hi, inner_valid, dst, mx);
+    if (KLO + 5 * kHarmBatch < KHI) harm_batch<STORE, KLO + 5 * kHarmBatch, KHI>(hg, q0, q1, tmP, p1s, a, t, n_lo, n_hi, inner_valid, dst, mx);
+#pragma unroll
+    for (int e = 1; e <= 7; e++) {
+      q0[e - 1] += 16 * e;
+      q1[e - 1] += 16 * e;
+    }
+  }
+  if (STORE) return;
+  // Arg-max.  Hot path: four running maxima per thread and one vote per unit.  Only when some sum of this warp reaches
+  // the warp's record (initially the stage threshold) is the unit rescanned for the position.
+  bool trig = false;
+#pragma unroll
+  for (int q = 0; q < 4; q++) trig |= mx[q] >= rec[q].s;
+  if (!__any_sync(0xffffffffu, trig)) return;
+#pragma unroll
+  for (int e = 1; e <= 7; e++) {
+    q0[e - 1] -= 64 * e;
+    q1[e - 1] -= 64 * e;
+  }
+  float* st0 = stash;          // [64][64] phase-0 powers, register r of thread t at r*64 + t (written and read by the same thread)
+#pragma unroll 1
+  for (int a = 0; a < 4; a++) {
+    float p0c[16];
+    tmem_ld16(tmP + 16 * a, p0c);
+#pragma unroll
+    for (int k = 0; k < 16; k++) st0[(16 * a + k) * 64 + t] = p0c[k];
+  }
+  __syncwarp();
+  float bs[4];
+  int bj[4] = {-1, -1, -1, -1};
+#pragma unroll
+  for (int q = 0; q < 4; q++) bs[q] = hg.thr[q];
+  const int jt = 2 * (s0 - c + t);
+#pragma unroll 1
+  for (int r = 0; r < 64; r++) {
+    const int n1 = dft64_out_index(r);
+    const int n = t + 64 * n1;
+    if (n < n_lo || n >= n_hi) continue;
+#pragma unroll 1
+    for (int ph = 0; ph < 2; ph++) {
+      const float p8 = ph ? p1s[r * 64 + t] : st0[r * 64 + t];
+      float g[7];
+#pragma unroll
+      for (int e = 1; e <= 7; e++) g[e - 1] = __ldg((ph ? q1[e - 1] : q0[e - 1]) + 16 * n1 * e);
+      float sv[4];
+      harm_stage_sums(p8, g, sv);
+      const int j = jt + 128 * n1 + ph;
+#pragma unroll
+      for (int q = 0; q < 4; q++)
+        if (sv[q] > bs[q] || (sv[q] == bs[q] && bj[q] >= 0 && j < bj[q])) {   // only sums above the threshold; ties -> smallest j
+          bs[q] = sv[q];
+          bj[q] = j;
+        }
+    }
+  }
+#pragma unroll
+  for (int q = 0; q < 4; q++) {
+    float b = bs[q];
+    int jj = bj[q];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      const float ob = __shfl_xor_sync(0xffffffffu, b, o);
+      const int oj = __shfl_xor_sync(0xffffffffu, jj, o);
+      if (oj >= 0 && (jj < 0 || ob > b || (ob == b && oj < jj))) {
+        b = ob;
+        jj = oj;
+      }
+    }
+    if (lane == 0 && jj >= 0) {
+      const HarmRecord cur = rec[q];
+      if (cur.j < 0 || harm_better_ti(b, jj, ti, cur.s, cur.j, cur.ti)) {
+        rec[q].s = b;
+        rec[q].j = jj;
+        rec[q].ti = ti;
+      }
+    }
+  }
+  __syncwarp();
+}
+
 // PRUNE (hw_max >= 256): outputs n < 256 and n >= 3840 lie outside the valid window [hw_max, 4096 - hw_max) of every
 // template; they are outputs 0 and 15 of each last-stage DFT_16 (registers 16a and 16a + 15), whose final butterfly
 // operations and power are then never computed (their power is reported as 0).
@@ -561,14 +878,20 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
   constexpr int L = 4096, NT = 64, P = 64;
   constexpr int NLAYER = (NG + 1) / 2;                          // groups of four warps: one TMEM lane quarter each
   constexpr int TCOLS = 128 * (NLAYER + 1) <= 256 ? 256 : 512;  // F: 128 columns per layer; twiddles: 128 columns shared by all layers
+  // plane and harmonic modes park the phase-0 powers of the current template in tensor memory (64 columns of the
+  // thread's own lane) until phase 1 is done: both phases then leave together (interleaved float2 pairs / harmonic sums)
+  constexpr bool kStashP0 = MODE == MODE_PLANE || MODE == MODE_HARM || MODE == MODE_HARM_STORE;
+  constexpr bool kBox = kStashP0;                               // the job is an (r, iz, iw) box, not the whole grid
+  static_assert(!kStashP0 || NG == 4, "the phase-0 stash needs the 512-column layout");
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float2* ex_all = reinterpret_cast<float2*>(smem_raw);
   unsigned long long* mbar_all = reinterpret_cast<unsigned long long*>(ex_all + NG * kEx64);  // [group][4]
   __shared__ long long s_item[NG];
   __shared__ uint32_t s_tmem;
+  __shared__ HarmRecord s_rec[2 * NG][4];   // MODE_HARM: running arg-max of every warp, h = 1,2,4,8
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, grp = warp >> 1, t = threadIdx.x & 63;
   float2* ex = ex_all + grp * kEx64;
-  float* p0s = reinterpret_cast<float*>(mbar_all + 4 * NG) + grp * (P * NT);   // plane mode only: [P][NT] phase-0 powers of the group
+  float* p1s = reinterpret_cast<float*>(mbar_all + 4 * NG) + grp * (P * NT);   // harmonic modes: [P][NT] phase-1 powers of the group
   const uint32_t mbS = smem_u32(mbar_all + 4 * grp);   // segment copy landed (tx)
   const uint32_t mbG = mbS + 8;                        // G copy landed (tx)
   const uint32_t mbR = mbS + 16;                       // all 64 threads have read G out of ex
@@ -593,6 +916,12 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
   TmemArray<L> tmF, tmT;
   tmF.addr = tbase + 128 * (warp >> 2);
   tmT.addr = tbase + 128 * NLAYER;
+  const uint32_t tmP = tbase + 128 * (NLAYER + 1) + 64 * (warp >> 2);   // phase-0 power stash (kStashP0)
+  if (MODE == MODE_HARM && lane < 4) {
+    s_rec[warp][lane].s = sp.hg.thr[lane];
+    s_rec[warp][lane].j = -1;
+    s_rec[warp][lane].ti = 0;
+  }
   if (warp < 4) {   // the twiddles depend on t = thread index mod 64 only: one copy per TMEM lane serves every layer
 #pragma unroll
     for (int h = 0; h < 4; h++) {
@@ -615,27 +944,22 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
     bar_sync_named(barid, NT);
     const long long item = s_item[grp];
     if (item >= nitems) break;
-    int q = 0;
-    if (MODE == MODE_PLANE) {
-      while (q + 1 < sp.njobs && item >= sp.jobs[q].item_end) q++;
-    }
-    const SearchJob& jb = sp.jobs[q];
-    const long long jitem = item - (q ? sp.jobs[q - 1].item_end : 0LL);
-    const int chunk = (int)(jitem / jb.seg_count);
-    const int64_t seg = jb.seg_first + jitem % jb.seg_count;
+    const WorkItem wi = decode_item(sp, item);
+    const SearchJob& jb = sp.jobs[wi.q];
+    const float2* spec = sp.spec[wi.b];
     const int iz_cnt = jb.iz_cnt;
-    const int s0 = (int)(sp.seg_base + seg * (int64_t)sp.step);  // first bin of the segment (even); |s0| < 2^31 (nbins <= 2^30)
+    const int s0 = (int)(sp.seg_base + wi.seg * (int64_t)sp.step);  // first bin of the segment (even); |s0| < 2^31 (nbins <= 2^30)
 
     // ---- a-2: stage the segment in the exchange buffer: TMA bulk copy when fully inside the spectrum, guarded loads at the edges
     const bool interior = (s0 >= 0) && ((int64_t)s0 + L <= sp.nbins);
     if (interior) {
-      if (t == 0) bulk_copy_g2s(smem_u32(ex), sp.spec + s0, (uint32_t)(L * 8), mbS);
+      if (t == 0) bulk_copy_g2s(smem_u32(ex), spec + s0, (uint32_t)(L * 8), mbS);
       mbar_wait(mbS, sphase);
       sphase ^= 1u;
     } else {
       for (int k = t; k < L; k += NT) {
         const int64_t b = (int64_t)s0 + k;
-        ex[k] = (b >= 0 && b < sp.nbins) ? sp.spec[b] : make_float2(0.f, 0.f);
+        ex[k] = (b >= 0 && b < sp.nbins) ? spec[b] : make_float2(0.f, 0.f);
       }
       bar_sync_named(barid, NT);
     }
@@ -660,32 +984,35 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
       bar_sync_named(barid, NT);
     }
 
-    // ---- loop over the template-phases of this chunk
-    const int tp_lo = chunk * jb.chunk_tp;
+    // ---- loop over the template-phases of this chunk (numbetween = 1: one phase per template, tp = template)
+    const bool two = sp.nb == 2;
+    const int tp_lo = wi.chunk * jb.chunk_tp;
     const int tp_hi = min(jb.ntp, tp_lo + jb.chunk_tp);
     int any0 = 0;  // candidate mode: phase-0 powers of this warp exceeded the threshold and were stashed
     // template walk of the box, row-major: ti_n = index of the template of the NEXT template-phase, iz_left = templates
     // left in its w-row
     int ti_n, iz_left;
     {
-      const int izr = (tp_lo >> 1) % iz_cnt, iwr = (tp_lo >> 1) / iz_cnt;
+      const int tl = two ? tp_lo >> 1 : tp_lo;
+      const int izr = tl % iz_cnt, iwr = tl / iz_cnt;
       ti_n = (jb.iw_lo + iwr) * sp.nz + jb.iz_lo + izr;
       iz_left = iz_cnt - izr;
     }
-    if (t == 0)   // G of the first template-phase of the item (ex is free: the barrier above)
-      bulk_copy_g2s(smem_u32(ex), sp.G + ((size_t)ti_n * 2 + (tp_lo & 1)) * L, (uint32_t)(L * 8), mbG);
+    if (t == 0)   // G of the first template-phase of the item (ex is free: the barrier above; chunks start at phase 0)
+      bulk_copy_g2s(smem_u32(ex), sp.G + (size_t)ti_n * sp.nb * L, (uint32_t)(L * 8), mbG);
     for (int tp = tp_lo; tp < tp_hi; tp++) {
-      const int ph = tp & 1;
+      const int ph = two ? (tp & 1) : 0;
       const int ti = ti_n;
       const int c = sp.geom[ti].c;
       // next template-phase: the same template's phase 1, or phase 0 of the next template of the box
-      if (ph == 1) {
+      if (ph == 1 || !two) {
         ++ti_n;
         if (--iz_left == 0) {
           iz_left = iz_cnt;
           ti_n += sp.nz - iz_cnt;
         }
       }
+      if ((MODE == MODE_HARM || MODE == MODE_HARM_STORE) && ph == 0 && t == 0) harm_prefetch(sp, jb, s0, c, ti);
       // ---- a-3: Y = F .* G (G from the exchange buffer, F from TMEM), inverse FFT
       float2 v[P];
       mbar_wait(mbG, tphase);
@@ -714,7 +1041,7 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
         mbar_arrive(mbW);
         if (t == 0 && tp + 1 < tp_hi) {
           mbar_wait(mbW, tphase);
-          bulk_copy_g2s(smem_u32(ex), sp.G + ((size_t)ti_n * 2 + (ph ^ 1)) * L, (uint32_t)(L * 8), mbG);
+          bulk_copy_g2s(smem_u32(ex), sp.G + ((size_t)ti_n * sp.nb + (two ? ph ^ 1 : 0)) * L, (uint32_t)(L * 8), mbG);
         }
         __syncwarp();
       };
@@ -725,7 +1052,7 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
       // bin indices are below 2^30)
       int n_lo, n_hi;
       {
-        const int blo = MODE == MODE_PLANE ? (int)jb.r_lo : 0, bhi = MODE == MODE_PLANE ? (int)(jb.r_lo + jb.r_cnt) : (int)sp.nbins;
+        const int blo = kBox ? (int)jb.r_lo : 0, bhi = kBox ? (int)(jb.r_lo + jb.r_cnt) : (int)sp.nbins;
         n_lo = max(sp.hw_max, min(blo - s0 + c, L));
         n_hi = min(sp.hw_max + sp.step, max(bhi - s0 + c, 0));
       }
@@ -733,30 +1060,52 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
 #pragma unroll
       for (int i = 0; i < P; i++)
         pw[i] = (PRUNE && ((i & 15) == 0 || (i & 15) == 15)) ? 0.f : fmaf(v[i].x, v[i].x, v[i].y * v[i].y);
-      if (MODE == MODE_PLANE) {
-        // phase-0 powers wait in shared memory (written and read back by the same thread) so that both phases leave as
-        // interleaved float2 pairs: every warp store covers 256 contiguous bytes (full 32-byte sectors, no L2 fill reads)
-        if (ph == 0) {
+      if (kStashP0 && two && ph == 0) {
 #pragma unroll
-          for (int r = 0; r < P; r++)
-            if (!(PRUNE && ((r & 15) == 0 || (r & 15) == 15))) p0s[r * NT + t] = pw[r];
-        } else {
-          float* row = jb.plane + (size_t)(tp >> 1) * (size_t)(2 * jb.r_cnt);   // row-major box: row index = template-phase / 2
-          const int boff = s0 - c - (int)jb.r_lo;
-          float2* dst = reinterpret_cast<float2*>(row + 2 * (ptrdiff_t)(boff + t));   // + 64 n1 float2 per register
-          // registers with n1 = n / 64 in [8, 56) are valid for every thread of a segment inside the box (hw_max <= 512):
-          // no predicate; registers known to be outside every window (PRUNE) are skipped
-          const bool inner_valid = __all_sync(0xffffffffu, n_lo <= t + 64 * 8 && n_hi >= t + 64 * 56);
+        for (int h = 0; h < 2; h++) {
+          float q32[32];
 #pragma unroll
-          for (int r = 0; r < P; r++) {
+          for (int i = 0; i < 32; i++) q32[i] = pw[32 * h + i];
+          tmem_st32(tmP + 32 * h, q32);
+        }
+      } else if (MODE == MODE_PLANE && !two) {
+        // numbetween = 1: one float per bin, row index = template
+        float* dst = jb.plane + (size_t)tp * (size_t)jb.r_cnt + (ptrdiff_t)(s0 - c - (int)jb.r_lo + t);
+#pragma unroll
+        for (int r = 0; r < P; r++) {
+          if (PRUNE && ((r & 15) == 0 || (r & 15) == 15)) continue;
+          const int n1 = dft64_out_index(r);
+          const int n = t + 64 * n1;
+          if (n >= n_lo && n < n_hi) dst[64 * n1] = pw[r];
+        }
+      } else if (MODE == MODE_PLANE) {
+        // both phases leave as interleaved float2 pairs: every warp store covers 256 contiguous bytes (full 32-byte
+        // sectors, no L2 fill reads)
+        float* row = jb.plane + (size_t)(tp >> 1) * (size_t)(2 * jb.r_cnt);   // row-major box: row index = template-phase / 2
+        const int boff = s0 - c - (int)jb.r_lo;
+        float2* dst = reinterpret_cast<float2*>(row + 2 * (ptrdiff_t)(boff + t));   // + 64 n1 float2 per register
+        // registers with n1 = n / 64 in [8, 56) are valid for every thread of a segment inside the box (hw_max <= 512):
+        // no predicate; registers known to be outside every window (PRUNE) are skipped
+        const bool inner_valid = __all_sync(0xffffffffu, n_lo <= t + 64 * 8 && n_hi >= t + 64 * 56);
+#pragma unroll
+        for (int h = 0; h < 2; h++) {
+          float p0c[32];
+          tmem_ld32(tmP + 32 * h, p0c);
+#pragma unroll
+          for (int i = 0; i < 32; i++) {
+            const int r = 32 * h + i;
             if (PRUNE && ((r & 15) == 0 || (r & 15) == 15)) continue;
             const int n1 = dft64_out_index(r);
             const int n = t + 64 * n1;
-            const float p0 = p0s[r * NT + t];
             const bool ok = (inner_valid && n1 >= 8 && n1 < 56) || (n >= n_lo && n < n_hi);
-            if (ok) dst[64 * n1] = make_float2(p0, pw[r]);
+            if (ok) dst[64 * n1] = make_float2(p0c[i], pw[r]);
           }
         }
+      } else if (MODE == MODE_HARM || MODE == MODE_HARM_STORE) {
+#pragma unroll
+        for (int r = 0; r < P; r++) p1s[r * NT + t] = pw[r];
+        harm_unit<MODE == MODE_HARM_STORE, PRUNE>(sp, jb, p1s, tmP, t, lane, s0, c, ti, tp >> 1, n_lo, n_hi, s_rec[warp],
+                                                   sp.stash + ((size_t)blockIdx.x * NG + grp) * (2 * L));
       } else {
         if (MODE == MODE_CAND_STATS) {
           // SURVEY.md 8(f) N2 / PAPER.md:43,45: mean and standard deviation of every (z,w) row, fused: sum of P and P^2
@@ -806,7 +1155,28 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
         // (written and read by the same thread)
         float* st0 = sp.stash + ((size_t)blockIdx.x * NG + grp) * (2 * L);
         float* st1 = st0 + L;
-        if (ph == 0) {
+        const float NEG = -INFINITY;
+        if (!two) {
+          if (anyhit) {       // numbetween = 1: the neighbours of bin b are bins b - 1 and b + 1 of the same phase
+#pragma unroll
+            for (int i = 0; i < P; i++) st0[i * NT + t] = pw[i];
+            __syncwarp();
+            const int iz = ti % sp.nz, iw = ti / sp.nz;
+#pragma unroll 1
+            for (int i = 0; i < P; i++) {
+              const int n = t + 64 * dft64_out_index(i);
+              const bool valid = (n >= n_lo) && (n < n_hi);
+              const float p = valid ? st0[i * NT + t] : NEG;
+              const float l = __shfl_up_sync(0xffffffffu, p, 1);      // P[b-1]
+              const float r = __shfl_down_sync(0xffffffffu, p, 1);    // P[b+1]
+              if (!valid) continue;
+              const int b = s0 + n - c;
+              test_point(sp, wi.b, b, iz, iw, p, b > 0 ? l : NEG, b < (int)sp.nbins - 1 ? r : NEG,
+                         (lane == 0 || n == sp.hw_max) && (b > 0), (lane == 31 || n == sp.hw_max + sp.step - 1) && (b < (int)sp.nbins - 1));
+            }
+            __syncwarp();
+          }
+        } else if (ph == 0) {
           any0 = anyhit;
           if (anyhit) {
 #pragma unroll
@@ -816,7 +1186,7 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
 #pragma unroll
           for (int i = 0; i < P; i++) st1[i * NT + t] = pw[i];
           __syncwarp();
-          const float NEG = -INFINITY;
+          const int iz = ti % sp.nz, iw = ti / sp.nz;
 #pragma unroll 1
           for (int i = 0; i < P; i++) {
             const int n = t + 64 * dft64_out_index(i);
@@ -827,21 +1197,11 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
             const float r0 = __shfl_down_sync(0xffffffffu, p0, 1);  // P0[n+1]
             if (!valid) continue;
             const int b = s0 + n - c;
-            const int iz = ti % sp.nz, iw = ti / sp.nz;
-            if (p0 > sp.threshold) {
-              const bool seamL = (lane == 0 || n == sp.hw_max) && (b > 0);
-              const float left = (b > 0 && !seamL) ? l1 : NEG;
-              const bool okR = p0 >= p1;
-              if (seamL) emit_seam(sp, 2 * b, iz, iw, p0, SEAM_LEFT | (okR ? 0u : SEAM_WITNESS));
-              else if (p0 > left && okR) emit_cand(sp, 2 * b, iz, iw, p0);
-            }
-            if (p1 > sp.threshold) {
-              const bool seamR = (lane == 31 || n == sp.hw_max + sp.step - 1) && (b < (int)sp.nbins - 1);
-              const float right = (b < sp.nbins - 1 && !seamR) ? r0 : NEG;
-              const bool okL = p1 > p0;
-              if (seamR) emit_seam(sp, 2 * b + 1, iz, iw, p1, SEAM_RIGHT | (okL ? 0u : SEAM_WITNESS));
-              else if (okL && p1 >= right) emit_cand(sp, 2 * b + 1, iz, iw, p1);
-            }
+            // phase-0 point j = 2b: left neighbour (b-1, phase 1), right neighbour (b, phase 1)
+            test_point(sp, wi.b, 2 * b, iz, iw, p0, b > 0 ? l1 : NEG, p1, (lane == 0 || n == sp.hw_max) && (b > 0), false);
+            // phase-1 point j = 2b+1: left neighbour (b, phase 0), right neighbour (b+1, phase 0)
+            test_point(sp, wi.b, 2 * b + 1, iz, iw, p1, p0, b < (int)sp.nbins - 1 ? r0 : NEG, false,
+                       (lane == 31 || n == sp.hw_max + sp.step - 1) && (b < (int)sp.nbins - 1));
           }
           __syncwarp();
         }
@@ -849,32 +1209,106 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
     }
     bar_sync_named(barid, NT);
   }
+  if (MODE == MODE_HARM) {
+    __syncwarp();
+    if (lane < 4) {
+      const HarmRecord rc = s_rec[warp][lane];
+      jerk_cand c;
+      c.j = rc.j;
+      c.iz = (int16_t)(rc.ti % sp.nz);
+      c.iw = (int16_t)(rc.ti / sp.nz);
+      c.power = rc.s;
+      c.flags = 0;
+      sp.hg.warpbest[(size_t)lane * (gridDim.x * 2 * NG) + blockIdx.x * 2 * NG + warp] = c;
+    }
+  }
   __syncthreads();
   if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(s_tmem), "n"(TCOLS));
 }
 
 // Seam records: every above-threshold point whose left (phase 0) or right (phase 1) neighbour belongs to another
 // warp or segment.  A seam point is a candidate iff it passed its own-side test and no seam record at the missing
-// neighbour position beats it (a neighbour that emitted nothing is <= threshold < this power).
-__global__ void k_resolve(SearchParams sp) {
-  unsigned long long ns = sp.work[1];
-  if (ns > (unsigned long long)kSeamCap) ns = kSeamCap;
+// neighbour position beats it (a neighbour that emitted nothing is <= threshold < this power).  A point is owned by
+// exactly one (segment, warp), so a position appears at most once in the list.  Short lists are settled by direct
+// comparison; longer ones through an open-addressing hash table on (template, j) built in the stash region, which is
+// idle once the search kernel has finished.  A list that did not fit in d_work cannot be settled: the call then reports
+// *d_count = UINT64_MAX (include/jerk.h), never a silently shortened result.
+constexpr unsigned long long kSeamDirect = 512;        // lists up to this length: O(n^2) scan in k_seam_resolve alone
+constexpr unsigned long long kSeamHashMaxSlots = 1ull << 23;   // 32 MB of the 37 MB stash; seam_cap <= slots / 2
+
+__device__ __forceinline__ unsigned long long seam_count(const SearchParams& sp) {
+  const unsigned long long ns = sp.work[1];
+  return ns > sp.seam_cap ? sp.seam_cap : ns;
+}
+__device__ __forceinline__ uint32_t seam_slots(unsigned long long ns) {      // power of two >= 4 ns, at most kSeamHashMaxSlots (>= 2 ns: seam_cap)
+  uint32_t m = 2048;
+  while ((unsigned long long)m < 4 * ns && m < kSeamHashMaxSlots) m <<= 1;
+  return m;
+}
+__device__ __forceinline__ uint32_t seam_hash(int ti, int j, uint32_t mask) {
+  unsigned long long k = ((unsigned long long)(uint32_t)ti << 32) | (uint32_t)j;
+  k *= 0x9E3779B97F4A7C15ull;
+  return (uint32_t)(k >> 32) & mask;
+}
+__global__ void k_seam_clear(SearchParams sp) {
+  const unsigned long long ns = seam_count(sp);
+  if (ns <= kSeamDirect || sp.work[2]) return;
+  uint32_t* table = reinterpret_cast<uint32_t*>(sp.stash);
+  const uint32_t m = seam_slots(ns);
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < m; i += gridDim.x * blockDim.x) table[i] = 0u;
+}
+__device__ __forceinline__ int seam_row(const SearchParams& sp, const jerk_cand& a) {   // (spectrum, template) of a record
+  return (int)(a.flags >> 8) * (sp.nz * sp.nw_grid) + a.iw * sp.nz + a.iz;
+}
+__global__ void k_seam_insert(SearchParams sp) {
+  const unsigned long long ns = seam_count(sp);
+  if (ns <= kSeamDirect || sp.work[2]) return;
+  uint32_t* table = reinterpret_cast<uint32_t*>(sp.stash);
+  const uint32_t mask = seam_slots(ns) - 1;
   for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i < ns;
        i += (unsigned long long)gridDim.x * blockDim.x) {
-    jerk_cand a = sp.seams[i];
-    if (a.flags & SEAM_WITNESS) continue;
-    const int jn = (a.flags & SEAM_LEFT) ? a.j - 1 : a.j + 1;
-    bool ok = true;
-    for (unsigned long long k = 0; k < ns && ok; k++) {
-      jerk_cand b = sp.seams[k];
-      if (b.j == jn && b.iz == a.iz && b.iw == a.iw) {
-        if (a.flags & SEAM_LEFT) ok = a.power > b.power;   // P > P[j-1]
-        else ok = a.power >= b.power;                      // P >= P[j+1]
-      }
+    const jerk_cand a = sp.seams[i];
+    uint32_t h = seam_hash(seam_row(sp, a), a.j, mask);
+    while (atomicCAS(table + h, 0u, (uint32_t)i + 1u) != 0u) h = (h + 1) & mask;
+  }
+}
+// power of the seam record at (row, j), -inf when there is none (that point was not above the threshold)
+__device__ __forceinline__ float seam_lookup(const SearchParams& sp, unsigned long long ns, bool direct, const uint32_t* table,
+                                             uint32_t mask, int row, int j) {
+  if (direct) {
+    for (unsigned long long k = 0; k < ns; k++) {
+      const jerk_cand b = sp.seams[k];
+      if (b.j == j && seam_row(sp, b) == row) return b.power;
     }
+    return -INFINITY;
+  }
+  uint32_t h = seam_hash(row, j, mask);
+  for (uint32_t e; (e = table[h]) != 0u; h = (h + 1) & mask) {
+    const jerk_cand b = sp.seams[e - 1];
+    if (b.j == j && seam_row(sp, b) == row) return b.power;
+  }
+  return -INFINITY;
+}
+__global__ void k_seam_resolve(SearchParams sp) {
+  if (sp.work[2]) {      // the seam list overflowed d_work: the result would be incomplete
+    if (blockIdx.x == 0 && threadIdx.x < sp.nspec) sp.count[threadIdx.x] = ~0ULL;
+    return;
+  }
+  const unsigned long long ns = seam_count(sp);
+  const bool direct = ns <= kSeamDirect;
+  const uint32_t* table = reinterpret_cast<const uint32_t*>(sp.stash);
+  const uint32_t mask = seam_slots(ns) - 1;
+  for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i < ns;
+       i += (unsigned long long)gridDim.x * blockDim.x) {
+    const jerk_cand a = sp.seams[i];
+    if (a.flags & SEAM_WITNESS) continue;
+    const int row = seam_row(sp, a);
+    bool ok = true;
+    if (a.flags & SEAM_LEFT) ok = a.power > seam_lookup(sp, ns, direct, table, mask, row, a.j - 1);            // P > P[j-1]
+    if (ok && (a.flags & SEAM_RIGHT)) ok = a.power >= seam_lookup(sp, ns, direct, table, mask, row, a.j + 1);   // P >= P[j+1]
     if (ok) {
       atomicAdd(sp.work + 3, 1ULL);
-      emit_cand(sp, a.j, a.iz, a.iw, a.power);
+      emit_cand(sp, (int)(a.flags >> 8), a.j, a.iz, a.iw, a.power);
     }
   }
 }
@@ -945,9 +1379,9 @@ __global__ void __launch_bounds__(256) k_sift(const jerk_cand* __restrict__ in, 
   }
 }
 
-__global__ void k_reset(unsigned long long* work, unsigned long long* count) {
+__global__ void k_reset(unsigned long long* work, unsigned long long* count, int ncount) {
   if (threadIdx.x < 8) work[threadIdx.x] = 0ULL;
-  if (threadIdx.x == 0 && count) *count = 0ULL;
+  if (count && (int)threadIdx.x < ncount) count[threadIdx.x] = 0ULL;
 }
 
 // ------------------------------------------------------------------------------------------------- harmonic stage
@@ -969,11 +1403,6 @@ struct HarmParams {
   float* out;              // store mode: S_h of the box, out[iw_rel][iz_rel][j - j_lo]
   int out_stage;           // store mode: log2(h)
 };
-
-__device__ __forceinline__ int rnd_eighths(int a, int e) {          // round-half-away-from-zero of a*e/8
-  const int m = (abs(a) * e + 4) >> 3;
-  return a < 0 ? -m : m;
-}
 
 // better(a, b): a beats b as the arg-max: larger sum, ties -> smallest (iw, iz, j) in row-major order
 __device__ __forceinline__ bool harm_better(float sa, int ja, int iza, int iwa, float sb, int jb, int izb, int iwb) {
@@ -1170,43 +1599,48 @@ static cudaError_t launch_search(const jerk_plan* plan, const SearchParams& sp, 
   occ = std::min(occ, (int)(233472 / (smem + fa.sharedSizeBytes + 1024)));
   occ = std::min(occ, 2048 / Gm::NT);
   occ = std::min(occ, 512 / TmemCols<L>::value);
-  if (getenv("JERK_DEBUG")) fprintf(stderr, "[jerk] k_search<%d,%d>: %d regs, smem %zu B, %d CTAs/SM\n", L, MODE, fa.numRegs, smem, occ);
   if (occ < 1) occ = 1;
   long long nitems = sp.nitems;
   long long grid = (long long)plan->sm_count * occ;
-  if (grid > kMaxCtas) grid = kMaxCtas;
+  const long long slots = (long long)(plan->stash_bytes / (2ull * L * sizeof(float)));   // one stash slot per CTA
+  if (grid > slots) grid = slots;
   if (grid > nitems) grid = nitems;
   if (grid < 1) grid = 1;
   k_search<L, MODE><<<(unsigned)grid, Gm::NT, smem, st>>>(sp);
   return cudaGetLastError();
 }
 
-#ifndef JERK_K64_NG_CAND
-#define JERK_K64_NG_CAND 2
-#endif
+// FFT groups per CTA of k_search64: two (two CTAs per SM, 256 TMEM columns each) in the candidate modes, four (one CTA
+// per SM, all 512 columns: the phase-0 stash) in the plane and harmonic modes: 8 warps per SM either way, up to 255
+// registers.  Six groups (12 warps, 168 registers: the register file is 16 K per scheduler, i.e. 170 registers at three
+// warps each) measured 172 ms/search against 158 ms: the spills and the tighter schedule cost more than the third warp
+// per scheduler hides.
+template <int MODE>
+struct K64 {
+  static constexpr int NG = (MODE == MODE_CAND || MODE == MODE_CAND_STATS) ? 2 : 4;
+  static constexpr int CTAS_PER_SM = NG == 2 ? 2 : 1;
+  static constexpr size_t SMEM = (size_t)NG * kEx64 * sizeof(float2) + 4 * NG * sizeof(unsigned long long) +
+                                 ((MODE == MODE_HARM || MODE == MODE_HARM_STORE) ? (size_t)NG * 64 * 64 * sizeof(float) : 0);   // + phase-1 powers
+};
+
+// CTAs of a k_search64 launch: every SM full, never more FFT groups than stash slots or work items
+template <int MODE>
+static unsigned search64_grid(const jerk_plan* plan, long long nitems) {
+  constexpr int NG = K64<MODE>::NG;
+  long long grid = (long long)plan->sm_count * K64<MODE>::CTAS_PER_SM;
+  const long long slots = (long long)(plan->stash_bytes / (2ull * 4096 * sizeof(float)));   // stash slots of one FFT group
+  if (grid * NG > slots) grid = slots / NG;
+  if (grid > (nitems + NG - 1) / NG) grid = (nitems + NG - 1) / NG;
+  if (grid < 1) grid = 1;
+  return (unsigned)grid;
+}
+
 template <int MODE, bool PRUNE>
 static cudaError_t launch_search64p(const jerk_plan* plan, const SearchParams& sp, cudaStream_t st) {
-  // FFT groups per CTA: two (two CTAs per SM) in candidate mode, four (one CTA per SM) in plane mode: 8 warps per SM, up
-  // to 255 registers.  Six groups (12 warps, 168 registers: the register file is 16 K per scheduler, i.e. 170 registers at
-  // three warps each) measured 172 ms/search against 158 ms: the spills and the tighter schedule cost more than the
-  // third warp per scheduler hides.
-  constexpr int NG = MODE == MODE_PLANE ? 4 : JERK_K64_NG_CAND;
-  const size_t smem = (size_t)NG * kEx64 * sizeof(float2) + 4 * NG * sizeof(unsigned long long) +
-                      (MODE == MODE_PLANE ? (size_t)NG * 64 * 64 * sizeof(float) : 0);
-  cudaError_t e = cudaFuncSetAttribute(k_search64<MODE, NG, PRUNE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  constexpr int NG = K64<MODE>::NG;
+  cudaError_t e = cudaFuncSetAttribute(k_search64<MODE, NG, PRUNE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K64<MODE>::SMEM);
   if (e != cudaSuccess) return e;
-  if (getenv("JERK_DEBUG")) {
-    cudaFuncAttributes fa;
-    if (cudaFuncGetAttributes(&fa, k_search64<MODE, NG, PRUNE>) == cudaSuccess)
-      fprintf(stderr, "[jerk] k_search64<%d,%d,%d>: %d regs, %zu B local, smem %zu B\n", MODE, NG, (int)PRUNE, fa.numRegs, (size_t)fa.localSizeBytes, smem);
-  }
-  const long long ctas_per_sm = NG == 2 ? 2 : 1;
-  long long grid = (long long)plan->sm_count * ctas_per_sm;
-  const long long slots = (long long)kMaxCtas * (long long)(kStashPerCta / (2ull * 4096 * sizeof(float)));   // stash slots of one FFT group
-  if (grid * NG > slots) grid = slots / NG;
-  if (grid > (sp.nitems + NG - 1) / NG) grid = (sp.nitems + NG - 1) / NG;
-  if (grid < 1) grid = 1;
-  k_search64<MODE, NG, PRUNE><<<(unsigned)grid, 64 * NG, smem, st>>>(sp);
+  k_search64<MODE, NG, PRUNE><<<search64_grid<MODE>(plan, sp.nitems), 64 * NG, K64<MODE>::SMEM, st>>>(sp);
   return cudaGetLastError();
 }
 
@@ -1227,12 +1661,12 @@ static cudaError_t dispatch_search(const jerk_plan* plan, const SearchParams& sp
 }
 
 template <int L>
-static cudaError_t launch_bank(const jerk_plan* plan, const BankParams& bp, cudaStream_t st) {
+static cudaError_t launch_bank(const jerk_plan* plan, const BankParams& bp, int ti_cnt, cudaStream_t st) {
   using Gm = FftGeom<L>;
   size_t smem = (size_t)(Gm::EX1 + Gm::EX2 + Tw2Table<L>::FLOATS2 + 4 * plan->hw_max + 1) * sizeof(float2);
   cudaError_t e = cudaFuncSetAttribute(k_bank<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  k_bank<L><<<plan->T, Gm::NT, smem, st>>>(bp);
+  k_bank<L><<<ti_cnt, Gm::NT, smem, st>>>(bp);
   return cudaGetLastError();
 }
 
@@ -1240,22 +1674,53 @@ static bool is_integer(double v) { return fabs(v - round(v)) < 1e-9; }
 
 static uint64_t align_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
 
-static void fill_params(const jerk_plan* plan, SearchParams& sp, const void* d_spec, void* d_work) {
+static void fill_params(const jerk_plan* plan, SearchParams& sp, const void* d_spec, void* d_work, uint64_t work_bytes) {
   memset(&sp, 0, sizeof(sp));
-  sp.spec = (const float2*)d_spec;
+  sp.spec[0] = (const float2*)d_spec;
   sp.nbins = plan->nbins;
   sp.geom = (const TemplateGeom*)plan->d_bank;
-  sp.G = (const float2*)((const unsigned char*)plan->d_bank + plan->geom_bytes);
+  // template ti's filters are at G + ti * nb * L: for a partial bank (jerk_templates_range) the base is moved back by the
+  // templates that are not there (never dereferenced outside the range: bank_covers is checked by every entry point)
+  sp.G = (const float2*)((const unsigned char*)plan->d_bank + plan->geom_bytes) - (ptrdiff_t)plan->bank_ti_lo * plan->numbetween * plan->L;
   sp.nz = plan->nz;
+  sp.nw_grid = plan->nw;
+  sp.nspec = 1;
+  sp.nb = plan->numbetween;
   sp.hw_max = plan->hw_max;
   sp.step = plan->step;
   sp.seg_base = plan->seg_base;
   sp.work = (unsigned long long*)d_work;
-  sp.seams = (jerk_cand*)((unsigned char*)d_work + kWorkHeader);
-  sp.stash = (float*)((unsigned char*)d_work + kWorkHeader + (uint64_t)kSeamCap * sizeof(jerk_cand));
+  sp.stash = (float*)((unsigned char*)d_work + kWorkHeader);
+  sp.seams = (jerk_cand*)((unsigned char*)d_work + kWorkHeader + plan->stash_bytes);
+  sp.seam_cap = std::min<uint64_t>((work_bytes - kWorkHeader - plan->stash_bytes) / sizeof(jerk_cand), kSeamHashMaxSlots / 2);
 }
 
-// Appends the box (r, iz, iw) as a job of `sp`.  Returns false when the box is empty (nothing appended).
+// k_reset, the candidate-mode search launch `search`, then the seam kernels
+template <class F>
+static int run_candidate_search(jerk_plan* p, const SearchParams& sp, cudaStream_t st, const char* what, F search) {
+  k_reset<<<1, 32, 0, st>>>(sp.work, sp.count, sp.nspec);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_reset launch: ") + cudaGetErrorString(e));
+  if (sp.nitems == 0) return JERK_OK;   // empty box
+  e = search();
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string(what) + " launch: " + cudaGetErrorString(e));
+  const int blocks = p->sm_count * 2;
+  k_seam_clear<<<blocks, 256, 0, st>>>(sp);
+  k_seam_insert<<<blocks, 256, 0, st>>>(sp);
+  k_seam_resolve<<<blocks, 256, 0, st>>>(sp);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("seam kernels launch: ") + cudaGetErrorString(e));
+  return JERK_OK;
+}
+
+// true iff every template of the box is in the bank the plan holds
+static bool bank_covers(const jerk_plan* p, int iz_lo, int iz_cnt, int iw_lo, int iw_cnt) {
+  if (iz_cnt <= 0 || iw_cnt <= 0) return true;
+  const int first = iw_lo * p->nz + iz_lo, last = (iw_lo + iw_cnt - 1) * p->nz + iz_lo + iz_cnt - 1;
+  return first >= p->bank_ti_lo && last < p->bank_ti_lo + p->bank_ti_cnt;
+}
+
+// Appends the box (r, iz, iw) as a job of `sp` (sp.nb and sp.nspec must be set).  Returns false when the box is empty (nothing appended).
 // Segments whose outputs b = s0 + n - c (n in [hw_max, hw_max+step), |c| <= c_max) can touch [r_lo, r_lo+r_cnt) are selected.
 static bool add_job(const jerk_plan* p, SearchParams& sp, int64_t r_lo, int64_t r_cnt, int iz_lo, int iz_cnt, int iw_lo,
                     int iw_cnt, float* plane, int chunk_tp) {
@@ -1275,11 +1740,11 @@ static bool add_job(const jerk_plan* p, SearchParams& sp, int64_t r_lo, int64_t 
   jb.iz_cnt = iz_cnt;
   jb.iw_lo = iw_lo;
   jb.iw_cnt = iw_cnt;
-  jb.ntp = 2 * iz_cnt * iw_cnt;
+  jb.ntp = sp.nb * iz_cnt * iw_cnt;
   jb.chunk_tp = chunk_tp;
   jb.plane = plane;
   long long nchunks = (jb.ntp + chunk_tp - 1) / chunk_tp;
-  sp.nitems += nchunks * jb.seg_count;
+  sp.nitems += nchunks * jb.seg_count * sp.nspec;
   jb.item_end = sp.nitems;
   sp.njobs++;
   return true;
@@ -1290,7 +1755,7 @@ static bool add_job(const jerk_plan* p, SearchParams& sp, int64_t r_lo, int64_t 
 static int pick_chunk_tp(const jerk_plan* p, int64_t r_cnt, int iz_cnt, int iw_cnt) {
   long long ntp = 2LL * iz_cnt * iw_cnt;
   long long segs = r_cnt / p->step + 2;
-  long long want_items = 32LL * kMaxCtas;   // >= 32 rounds of work items per resident FFT group: tail < 3 %
+  long long want_items = 32LL * 4 * 148;    // >= 32 rounds of work items per resident FFT group of a B200: tail < 3 %
   int c = kChunkTP;
   while (c > 32 && ((ntp + c - 1) / c) * segs < want_items) c >>= 1;
   return c;
@@ -1311,6 +1776,7 @@ const char* jerk_strerror(int status) {
     case JERK_ECUDA: return "JERK_ECUDA: CUDA error";
     case JERK_ESTATE: return "JERK_ESTATE: template bank not built";
     case JERK_ENODEV: return "JERK_ENODEV: no sm_100 device";
+    case JERK_EOVERFLOW: return "JERK_EOVERFLOW: more candidates or seam records than the caller's buffers hold";
   }
   return "unknown jerk status";
 }
@@ -1323,7 +1789,7 @@ int jerk_plan_create(jerk_plan** out, int64_t nbins, double zmax, double dz, dou
   *out = nullptr;
   if (nbins < 1 || zmax < 0 || wmax < 0 || !(dz > 0) || !(dw > 0)) return JERK_EINVAL;
   if (!is_integer(zmax / dz) || !is_integer(wmax / dw)) return JERK_EINVAL;
-  if (numbetween != 2) return JERK_EINVAL;
+  if (numbetween != 1 && numbetween != 2) return JERK_EINVAL;
   if (seg_len != 0 && seg_len != 1024 && seg_len != 2048 && seg_len != 4096 && seg_len != 8192) return JERK_EINVAL;
   if (nbins > (int64_t)1 << 30) return JERK_EINVAL;  // j = 2b+p is reported as int32
   jerk_plan* p = new jerk_plan();
@@ -1368,9 +1834,11 @@ int jerk_plan_create(jerk_plan** out, int64_t nbins, double zmax, double dz, dou
   int64_t need = nbins + p->c_max - p->hw_max - base;
   p->nseg = (need + p->step - 1) / p->step;
   p->geom_bytes = align_up((uint64_t)p->T * sizeof(TemplateGeom), kBankAlign);
-  p->bank_bytes = p->geom_bytes + (uint64_t)p->T * 2 * seg_len * sizeof(float2);
-  p->work_bytes = kWorkHeader + (uint64_t)kSeamCap * sizeof(jerk_cand) + (uint64_t)kMaxCtas * kStashPerCta;
+  p->bank_bytes = p->geom_bytes + (uint64_t)p->T * numbetween * seg_len * sizeof(float2);
+  p->stash_bytes = kStashBytes;
+  p->work_bytes = kWorkHeader + p->stash_bytes + kSeamCapDefault * sizeof(jerk_cand);
   p->d_bank = nullptr;
+  p->bank_ti_lo = p->bank_ti_cnt = 0;
   p->sm_count = 0;
   *out = p;
   return JERK_OK;
@@ -1405,7 +1873,7 @@ int jerk_plan_info(const jerk_plan* p, jerk_plan_info_t* info) {
   // nominal segments ceil(nbins/step), 2T template-phases, 5 L log2 L + 6 L + 3 step flops each
   double nseg_nom = ceil((double)p->nbins / (double)p->step);
   double l2 = log2((double)p->L);
-  info->flops_per_search = nseg_nom * 2.0 * p->T * (5.0 * p->L * l2 + 6.0 * p->L + 3.0 * p->step);
+  info->flops_per_search = nseg_nom * (double)p->numbetween * p->T * (5.0 * p->L * l2 + 6.0 * p->L + 3.0 * p->step);
   return JERK_OK;
 }
 
@@ -1433,9 +1901,15 @@ static int ensure_device(jerk_plan* p) {
   return JERK_OK;
 }
 
-int jerk_templates(jerk_plan* p, void* d_bank, uint64_t bank_bytes, void* stream) {
+uint64_t jerk_bank_bytes_range(const jerk_plan* p, int ti_cnt) {
+  if (!p || ti_cnt < 0 || ti_cnt > p->T) return 0;
+  return p->geom_bytes + (uint64_t)ti_cnt * p->numbetween * p->L * sizeof(float2);
+}
+
+int jerk_templates_range(jerk_plan* p, int ti_lo, int ti_cnt, void* d_bank, uint64_t bank_bytes, void* stream) {
   if (!p || !d_bank) return JERK_EINVAL;
-  if (bank_bytes < p->bank_bytes) return fail(p, JERK_ENOMEM, "bank buffer smaller than plan bank_bytes");
+  if (ti_lo < 0 || ti_cnt < 1 || ti_lo + ti_cnt > p->T) return fail(p, JERK_EINVAL, "template range outside [0, ntemplates)");
+  if (bank_bytes < jerk_bank_bytes_range(p, ti_cnt)) return fail(p, JERK_ENOMEM, "bank buffer smaller than jerk_bank_bytes_range");
   if ((uintptr_t)d_bank % kBankAlign) return fail(p, JERK_EINVAL, "d_bank must be 256-byte aligned");
   int rc = ensure_device(p);
   if (rc) return rc;
@@ -1449,17 +1923,26 @@ int jerk_templates(jerk_plan* p, void* d_bank, uint64_t bank_bytes, void* stream
   bp.dw = p->dw;
   bp.nz = p->nz;
   bp.nw = p->nw;
+  bp.nb = p->numbetween;
+  bp.ti_lo = ti_lo;
   bp.geom = (const TemplateGeom*)d_bank;
   bp.G = (float2*)((unsigned char*)d_bank + p->geom_bytes);
   switch (p->L) {
-    case 1024: e = launch_bank<1024>(p, bp, st); break;
-    case 2048: e = launch_bank<2048>(p, bp, st); break;
-    case 4096: e = launch_bank<4096>(p, bp, st); break;
-    default: e = launch_bank<8192>(p, bp, st); break;
+    case 1024: e = launch_bank<1024>(p, bp, ti_cnt, st); break;
+    case 2048: e = launch_bank<2048>(p, bp, ti_cnt, st); break;
+    case 4096: e = launch_bank<4096>(p, bp, ti_cnt, st); break;
+    default: e = launch_bank<8192>(p, bp, ti_cnt, st); break;
   }
   if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_bank launch: ") + cudaGetErrorString(e));
   p->d_bank = d_bank;
+  p->bank_ti_lo = ti_lo;
+  p->bank_ti_cnt = ti_cnt;
   return JERK_OK;
+}
+
+int jerk_templates(jerk_plan* p, void* d_bank, uint64_t bank_bytes, void* stream) {
+  if (!p) return JERK_EINVAL;
+  return jerk_templates_range(p, 0, p->T, d_bank, bank_bytes, stream);
 }
 
 int jerk_templates_taps(jerk_plan* p, int iz, int iw, void* d_taps, uint64_t taps_bytes, void* stream) {
@@ -1490,16 +1973,19 @@ int jerk_search_plane(jerk_plan* p, const void* d_spec, int64_t r_lo, int64_t r_
   if (r_lo < 0 || r_cnt < 0 || r_lo + r_cnt > p->nbins || iz_lo < 0 || iz_cnt < 0 || iz_lo + iz_cnt > p->nz || iw_lo < 0 ||
       iw_cnt < 0 || iw_lo + iw_cnt > p->nw)
     return fail(p, JERK_EINVAL, "plane sub-range outside the plan's grid");
-  if (plane_bytes < jerk_plane_bytes(r_cnt, iz_cnt, iw_cnt)) return fail(p, JERK_ENOMEM, "plane buffer too small");
+  if (plane_bytes < jerk_plane_bytes(r_cnt, iz_cnt, iw_cnt) / 2 * p->numbetween) return fail(p, JERK_ENOMEM, "plane buffer too small");
   if (r_cnt == 0 || iz_cnt == 0 || iw_cnt == 0) return JERK_OK;  // empty range: nothing to write, d_plane may be NULL
   if (!d_plane) return JERK_EINVAL;
   if ((uintptr_t)d_plane % 8) return fail(p, JERK_EINVAL, "d_plane must be 8-byte aligned");
+  if (!bank_covers(p, iz_lo, iz_cnt, iw_lo, iw_cnt)) return fail(p, JERK_ESTATE, "the template box is not inside the range jerk_templates_range built");
   cudaStream_t st = (cudaStream_t)stream;
   SearchParams sp;
-  fill_params(p, sp, d_spec, d_work);
+  fill_params(p, sp, d_spec, d_work, work_bytes);
   if (!add_job(p, sp, r_lo, r_cnt, iz_lo, iz_cnt, iw_lo, iw_cnt, d_plane, pick_chunk_tp(p, r_cnt, iz_cnt, iw_cnt))) return JERK_OK;
-  k_reset<<<1, 32, 0, st>>>(sp.work, nullptr);
-  cudaError_t e = dispatch_search<MODE_PLANE>(p, sp, st);
+  k_reset<<<1, 32, 0, st>>>(sp.work, nullptr, 0);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_reset launch: ") + cudaGetErrorString(e));
+  e = dispatch_search<MODE_PLANE>(p, sp, st);
   if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_search(plane) launch: ") + cudaGetErrorString(e));
   return JERK_OK;
 }
@@ -1512,24 +1998,16 @@ int jerk_search_candidates_range(jerk_plan* p, const void* d_spec, float thresho
   if (!d_cands || !d_count || max_cands < 0) return JERK_EINVAL;
   if (iz_lo < 0 || iz_cnt < 0 || iz_lo + iz_cnt > p->nz || iw_lo < 0 || iw_cnt < 0 || iw_lo + iw_cnt > p->nw)
     return fail(p, JERK_EINVAL, "template box outside the plan's grid");
+  if (!bank_covers(p, iz_lo, iz_cnt, iw_lo, iw_cnt)) return fail(p, JERK_ESTATE, "the template box is not inside the range jerk_templates_range built");
   cudaStream_t st = (cudaStream_t)stream;
   SearchParams sp;
-  fill_params(p, sp, d_spec, d_work);
-  const bool any = add_job(p, sp, 0, p->nbins, iz_lo, iz_cnt, iw_lo, iw_cnt, nullptr, kChunkTP);
+  fill_params(p, sp, d_spec, d_work, work_bytes);
+  add_job(p, sp, 0, p->nbins, iz_lo, iz_cnt, iw_lo, iw_cnt, nullptr, kChunkTP);   // an empty box adds nothing: *d_count = 0
   sp.threshold = threshold;
   sp.cands = d_cands;
   sp.max_cands = max_cands;
   sp.count = d_count;
-  k_reset<<<1, 32, 0, st>>>(sp.work, d_count);
-  cudaError_t e = cudaGetLastError();
-  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_reset launch: ") + cudaGetErrorString(e));
-  if (!any) return JERK_OK;   // empty box
-  e = dispatch_search<MODE_CAND>(p, sp, st);
-  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_search(cand) launch: ") + cudaGetErrorString(e));
-  k_resolve<<<p->sm_count, 256, 0, st>>>(sp);
-  e = cudaGetLastError();
-  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_resolve launch: ") + cudaGetErrorString(e));
-  return JERK_OK;
+  return run_candidate_search(p, sp, st, "k_search(cand)", [&] { return dispatch_search<MODE_CAND>(p, sp, st); });
 }
 
 int jerk_search_candidates(jerk_plan* p, const void* d_spec, float threshold, jerk_cand* d_cands, int64_t max_cands,
@@ -1539,18 +2017,77 @@ int jerk_search_candidates(jerk_plan* p, const void* d_spec, float threshold, je
                                       stream);
 }
 
+int jerk_search_candidates_templates(jerk_plan* p, const void* d_spec, float threshold, int ti_lo, int ti_cnt, jerk_cand* d_cands,
+                                     int64_t max_cands, unsigned long long* d_count, void* d_work, uint64_t work_bytes, void* stream) {
+  int rc = check_common(p, d_spec, d_work, work_bytes);
+  if (rc) return rc;
+  if (!d_cands || !d_count || max_cands < 0) return JERK_EINVAL;
+  if (ti_lo < 0 || ti_cnt < 0 || ti_lo + ti_cnt > p->T) return fail(p, JERK_EINVAL, "template range outside [0, ntemplates)");
+  if (ti_cnt && (ti_lo < p->bank_ti_lo || ti_lo + ti_cnt > p->bank_ti_lo + p->bank_ti_cnt))
+    return fail(p, JERK_ESTATE, "the template range is not inside the range jerk_templates_range built");
+  cudaStream_t st = (cudaStream_t)stream;
+  SearchParams sp;
+  fill_params(p, sp, d_spec, d_work, work_bytes);
+  // a flat range of templates is at most three boxes: the rest of the first w-row, whole w-rows, the start of the last one
+  int ti = ti_lo, left = ti_cnt;
+  if (left && ti % p->nz) {
+    const int n = std::min(left, p->nz - ti % p->nz);
+    add_job(p, sp, 0, p->nbins, ti % p->nz, n, ti / p->nz, 1, nullptr, kChunkTP);
+    ti += n;
+    left -= n;
+  }
+  if (left >= p->nz) {
+    const int rows = left / p->nz;
+    add_job(p, sp, 0, p->nbins, 0, p->nz, ti / p->nz, rows, nullptr, kChunkTP);
+    ti += rows * p->nz;
+    left -= rows * p->nz;
+  }
+  if (left) add_job(p, sp, 0, p->nbins, 0, left, ti / p->nz, 1, nullptr, kChunkTP);
+  sp.threshold = threshold;
+  sp.cands = d_cands;
+  sp.max_cands = max_cands;
+  sp.count = d_count;
+  return run_candidate_search(p, sp, st, "k_search(cand)", [&] { return dispatch_search<MODE_CAND>(p, sp, st); });
+}
+
+int jerk_search_candidates_batch(jerk_plan* p, const void* const* h_d_specs, int nspec, float threshold, jerk_cand* d_cands,
+                                 int64_t max_cands, unsigned long long* d_counts, void* d_work, uint64_t work_bytes, void* stream) {
+  if (!p || !h_d_specs || nspec < 0 || !d_cands || !d_counts || max_cands < 0) return JERK_EINVAL;
+  if (!bank_covers(p, 0, p->nz, 0, p->nw)) return fail(p, JERK_ESTATE, "the batched search needs the whole bank (jerk_templates)");
+  cudaStream_t st = (cudaStream_t)stream;
+  for (int b0 = 0; b0 < nspec; b0 += kMaxBatch) {      // one launch per kMaxBatch spectra: the bank is streamed once for all of them
+    const int nb = std::min(kMaxBatch, nspec - b0);
+    for (int b = 0; b < nb; b++) {
+      int rc = check_common(p, h_d_specs[b0 + b], d_work, work_bytes);
+      if (rc) return rc;
+    }
+    SearchParams sp;
+    fill_params(p, sp, h_d_specs[b0], d_work, work_bytes);
+    for (int b = 0; b < nb; b++) sp.spec[b] = (const float2*)h_d_specs[b0 + b];
+    sp.nspec = nb;
+    add_job(p, sp, 0, p->nbins, 0, p->nz, 0, p->nw, nullptr, kChunkTP);
+    sp.threshold = threshold;
+    sp.cands = d_cands + (size_t)b0 * max_cands;
+    sp.max_cands = max_cands;
+    sp.count = d_counts + b0;
+    int rc = run_candidate_search(p, sp, st, "k_search(cand, batch)", [&] { return dispatch_search<MODE_CAND>(p, sp, st); });
+    if (rc) return rc;
+  }
+  return JERK_OK;
+}
+
 int jerk_search_candidates_stats(jerk_plan* p, const void* d_spec, float threshold, jerk_cand* d_cands, int64_t max_cands,
                                  unsigned long long* d_count, double* d_rowstats, uint64_t rowstats_bytes, void* d_work,
                                  uint64_t work_bytes, void* stream) {
   int rc = check_common(p, d_spec, d_work, work_bytes);
   if (rc) return rc;
   if (!d_cands || !d_count || !d_rowstats || max_cands < 0) return JERK_EINVAL;
-  if (p->L != 4096) return fail(p, JERK_EINVAL, "row statistics are fused into the seg_len 4096 kernel only");
   if (rowstats_bytes < (uint64_t)p->T * 2 * sizeof(double)) return fail(p, JERK_ENOMEM, "row statistics buffer smaller than 16 bytes per template");
   if ((uintptr_t)d_rowstats % 8) return fail(p, JERK_EINVAL, "d_rowstats must be 8-byte aligned");
+  if (!bank_covers(p, 0, p->nz, 0, p->nw)) return fail(p, JERK_ESTATE, "row statistics need the whole bank (jerk_templates)");
   cudaStream_t st = (cudaStream_t)stream;
   SearchParams sp;
-  fill_params(p, sp, d_spec, d_work);
+  fill_params(p, sp, d_spec, d_work, work_bytes);
   add_job(p, sp, 0, p->nbins, 0, p->nz, 0, p->nw, nullptr, kChunkTP);
   sp.threshold = threshold;
   sp.cands = d_cands;
@@ -1559,13 +2096,7 @@ int jerk_search_candidates_stats(jerk_plan* p, const void* d_spec, float thresho
   sp.rowstats = d_rowstats;
   cudaError_t e = cudaMemsetAsync(d_rowstats, 0, (size_t)p->T * 2 * sizeof(double), st);
   if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("row statistics memset: ") + cudaGetErrorString(e));
-  k_reset<<<1, 32, 0, st>>>(sp.work, d_count);
-  e = launch_search64<MODE_CAND_STATS>(p, sp, st);
-  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_search64(cand+stats) launch: ") + cudaGetErrorString(e));
-  k_resolve<<<p->sm_count, 256, 0, st>>>(sp);
-  e = cudaGetLastError();
-  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_resolve launch: ") + cudaGetErrorString(e));
-  return JERK_OK;
+  return run_candidate_search(p, sp, st, "k_search(cand+stats)", [&] { return dispatch_search<MODE_CAND_STATS>(p, sp, st); });
 }
 
 int jerk_snr_filter(jerk_plan* p, const double* d_rowstats, const jerk_cand* d_cands_in, const unsigned long long* d_count_in,
@@ -1602,6 +2133,26 @@ int jerk_sift_candidates(jerk_plan* p, const jerk_cand* d_cands_in, const unsign
   return JERK_OK;
 }
 
+// D2H of the count and of min(count, max_cands) records; the overflow conditions become statuses here, where the call
+// is synchronous anyway
+static int fetch_candidates(jerk_plan* p, jerk_cand* h_cands, int64_t max_cands, unsigned long long* h_count, const jerk_cand* d_cands,
+                            const unsigned long long* d_count, cudaStream_t st) {
+  cudaError_t e = cudaMemcpyAsync(h_count, d_count, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("D2H count: ") + cudaGetErrorString(e));
+  unsigned long long n = *h_count;
+  if (n == ~0ULL) return fail(p, JERK_EOVERFLOW, "seam records overflowed d_work: pass a larger work buffer (16 bytes per extra record) or raise the threshold");
+  const bool over = (int64_t)n > max_cands;
+  if (over) n = (unsigned long long)max_cands;
+  if (n) {
+    e = cudaMemcpyAsync(h_cands, d_cands, (size_t)n * sizeof(jerk_cand), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("D2H candidates: ") + cudaGetErrorString(e));
+  }
+  if (over) return fail(p, JERK_EOVERFLOW, "more candidates than max_cands: the first max_cands records were copied, *h_count holds the total");
+  return JERK_OK;
+}
+
 int jerk_search_candidates_host(jerk_plan* p, const void* h_spec, float threshold, jerk_cand* h_cands, int64_t max_cands,
                                 unsigned long long* h_count, void* d_spec, jerk_cand* d_cands, unsigned long long* d_count,
                                 void* d_work, uint64_t work_bytes, void* stream) {
@@ -1611,17 +2162,7 @@ int jerk_search_candidates_host(jerk_plan* p, const void* h_spec, float threshol
   if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("H2D spectrum: ") + cudaGetErrorString(e));
   int rc = jerk_search_candidates(p, d_spec, threshold, d_cands, max_cands, d_count, d_work, work_bytes, stream);
   if (rc) return rc;
-  e = cudaMemcpyAsync(h_count, d_count, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("D2H count: ") + cudaGetErrorString(e));
-  unsigned long long n = *h_count;
-  if ((int64_t)n > max_cands) n = (unsigned long long)max_cands;
-  if (n) {
-    e = cudaMemcpyAsync(h_cands, d_cands, (size_t)n * sizeof(jerk_cand), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("D2H candidates: ") + cudaGetErrorString(e));
-  }
-  return JERK_OK;
+  return fetch_candidates(p, h_cands, max_cands, h_count, d_cands, d_count, st);
 }
 
 int jerk_search_series_host(jerk_plan* p, const float* h_series, int64_t nsamples, int block, float threshold, jerk_cand* h_cands,
@@ -1637,17 +2178,7 @@ int jerk_search_series_host(jerk_plan* p, const float* h_series, int64_t nsample
   if (rc) return fail(p, rc, "jerk_prepare_spectrum failed (size, alignment or scratch)");
   rc = jerk_search_candidates(p, d_spec, threshold, d_cands, max_cands, d_count, d_work, work_bytes, stream);
   if (rc) return rc;
-  e = cudaMemcpyAsync(h_count, d_count, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("D2H count: ") + cudaGetErrorString(e));
-  unsigned long long n = *h_count;
-  if ((int64_t)n > max_cands) n = (unsigned long long)max_cands;
-  if (n) {
-    e = cudaMemcpyAsync(h_cands, d_cands, (size_t)n * sizeof(jerk_cand), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("D2H candidates: ") + cudaGetErrorString(e));
-  }
-  return JERK_OK;
+  return fetch_candidates(p, h_cands, max_cands, h_count, d_cands, d_count, st);
 }
 
 // ---- harmonic stage (row a-6)
@@ -1659,6 +2190,7 @@ constexpr int64_t kHarmChunkBins = 1 << 16;      // r-chunk of the top-harmonic 
 constexpr int64_t kHarmChunkBinsMax = 1 << 19;   // larger caller buffers are used up to this chunk (fewer segment-edge recomputations)
 constexpr int kHarmJTile = 8192;              // half-bin indices per k_harm block
 constexpr uint64_t kHarmHeader = 256;         // running[4] arg-max records
+constexpr uint64_t kHarmGuard = 65536;        // guard band before the first and after the last stored sub-plane (see ld_gather7): > (4096 + c_max) * 2 * 7/8 floats
 constexpr int kHarmFoldBlocks = 128;          // first level of the arg-max fold
 
 struct HarmBox {
@@ -1676,13 +2208,15 @@ static int host_rnd_eighths(int a, int e) {
   return a < 0 ? -m : m;
 }
 
-// Source boxes of the eight fractions for a top-harmonic box (all index maps are monotone, so boxes map to boxes),
-// their placement in scratch after the header, the per-block arg-max records, and the total bytes needed.
-static uint64_t harm_layout(const jerk_plan* p, const HarmBox& bx, HarmSubBox (&sub)[8], uint64_t* blockbest_off, int* nblocks,
-                            int* ntiles) {
+// Source boxes of the fractions for a top-harmonic box (all index maps are monotone, so boxes map to boxes), their
+// placement in scratch after the header, the arg-max records, and the total bytes needed.  seg_len 4096 (`fused`): the
+// top-harmonic pass itself is the consumer, fraction 8/8 is never stored and the records are one per warp of that launch;
+// other lengths: all eight sub-planes are stored and k_harm sums them (records per k_harm block).
+static uint64_t harm_layout(const jerk_plan* p, const HarmBox& bx, HarmSubBox (&sub)[8], uint64_t* best_off, int* nblocks, int* ntiles) {
+  const bool fused = p->L == 4096;
   const int cz = (p->nz - 1) / 2, cw = (p->nw - 1) / 2;
   const int64_t j_lo = 2 * bx.r_lo, j_hi = 2 * (bx.r_lo + bx.r_cnt) - 1;   // inclusive
-  uint64_t off = kHarmHeader;
+  uint64_t off = kHarmHeader + (fused ? kHarmGuard : 0);
   for (int e = 1; e <= 8; e++) {
     HarmSubBox& sb = sub[e - 1];
     const int64_t js_lo = (j_lo * e + 4) >> 3, js_hi = (j_hi * e + 4) >> 3;
@@ -1693,30 +2227,33 @@ static uint64_t harm_layout(const jerk_plan* p, const HarmBox& bx, HarmSubBox (&
     sb.iw_lo = host_rnd_eighths(bx.iw_lo - cw, e) + cw;
     sb.iw_cnt = host_rnd_eighths(bx.iw_lo + bx.iw_cnt - 1 - cw, e) + cw - sb.iw_lo + 1;
     sb.offset = off;
-    sb.bytes = align_up((uint64_t)sb.iw_cnt * sb.iz_cnt * (uint64_t)(2 * sb.r_cnt) * sizeof(float), 256);
+    sb.bytes = (fused && e == 8) ? 0 : align_up((uint64_t)sb.iw_cnt * sb.iz_cnt * (uint64_t)(2 * sb.r_cnt) * sizeof(float), 256);
     off += sb.bytes;
   }
+  if (fused) off += kHarmGuard;
   *ntiles = (int)((2 * bx.r_cnt + kHarmJTile - 1) / kHarmJTile);
-  *nblocks = bx.iw_cnt * bx.iz_cnt * *ntiles;
-  *blockbest_off = off;
+  *nblocks = fused ? kStashSlots * 2 : bx.iw_cnt * bx.iz_cnt * *ntiles;      // fused: an upper bound on the warps of the launch
+  *best_off = off;
   off += align_up((uint64_t)4 * *nblocks * sizeof(jerk_cand), 256);
   off += align_up((uint64_t)4 * kHarmFoldBlocks * sizeof(jerk_cand), 256);   // partial arg-max records of the two-level fold
   return off;
 }
 
-// Sub-planes of one box (one plane-mode launch with eight jobs), then k_harm in arg-max or store mode.
+// Sub-planes of one box (one plane-mode launch with one job per fraction), then the sums in arg-max or store mode:
+// inside the top-harmonic search pass itself for seg_len 4096 (k_search64<MODE_HARM>), by k_harm otherwise.
 static int harm_box(jerk_plan* p, const void* d_spec, const HarmBox& bx, unsigned char* scratch, uint64_t scratch_bytes,
-                    void* d_work, float* d_out, int out_stage, bool first, cudaStream_t st) {
+                    void* d_work, uint64_t work_bytes, float* d_out, int out_stage, const float* thr4, bool first, cudaStream_t st) {
+  const bool fused = p->L == 4096;
   HarmSubBox sub[8];
   uint64_t bb_off;
   int nblocks, ntiles;
   if (harm_layout(p, bx, sub, &bb_off, &nblocks, &ntiles) > scratch_bytes)
     return fail(p, JERK_ENOMEM, "harmonic scratch buffer too small for this box");
   SearchParams sp;
-  fill_params(p, sp, d_spec, d_work);
+  fill_params(p, sp, d_spec, d_work, work_bytes);
   HarmParams hp;
   memset(&hp, 0, sizeof(hp));
-  for (int e = 1; e <= 8; e++) {
+  for (int e = 1; e <= (fused ? 7 : 8); e++) {
     const HarmSubBox& sb = sub[e - 1];
     float* plane = (float*)(scratch + sb.offset);
     if (!add_job(p, sp, sb.r_lo, sb.r_cnt, sb.iz_lo, sb.iz_cnt, sb.iw_lo, sb.iw_cnt, plane, kChunkTP))
@@ -1728,8 +2265,9 @@ static int harm_box(jerk_plan* p, const void* d_spec, const HarmBox& bx, unsigne
     hp.sub[e - 1].iz_cnt = sb.iz_cnt;
     hp.sub[e - 1].iw_lo = sb.iw_lo;
   }
-  // small boxes: shrink the work items until every resident CTA gets a few
-  while (sp.nitems < 32LL * kMaxCtas && sp.jobs[0].chunk_tp > 32) {
+  // small boxes: shrink the work items until every resident FFT group gets a few
+  const long long want_items = 32LL * 4 * p->sm_count;
+  while (sp.nitems < want_items && sp.jobs[0].chunk_tp > 32) {
     sp.nitems = 0;
     for (int q = 0; q < sp.njobs; q++) {
       SearchJob& jb = sp.jobs[q];
@@ -1738,9 +2276,50 @@ static int harm_box(jerk_plan* p, const void* d_spec, const HarmBox& bx, unsigne
       jb.item_end = sp.nitems;
     }
   }
-  k_reset<<<1, 32, 0, st>>>(sp.work, nullptr);
-  cudaError_t e = dispatch_search<MODE_PLANE>(p, sp, st);
+  k_reset<<<1, 32, 0, st>>>(sp.work, nullptr, 0);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_reset launch: ") + cudaGetErrorString(e));
+  e = dispatch_search<MODE_PLANE>(p, sp, st);
   if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_search(harmonic sub-planes) launch: ") + cudaGetErrorString(e));
+  jerk_cand* best = (jerk_cand*)(scratch + bb_off);
+  jerk_cand* partial = (jerk_cand*)(scratch + bb_off + align_up((uint64_t)4 * nblocks * sizeof(jerk_cand), 256));
+  if (fused) {
+    // the top-harmonic pass: the search of the box itself, summing the seven stored sub-planes into its own powers
+    SearchParams tp;
+    fill_params(p, tp, d_spec, d_work, work_bytes);
+    if (!add_job(p, tp, bx.r_lo, bx.r_cnt, bx.iz_lo, bx.iz_cnt, bx.iw_lo, bx.iw_cnt, nullptr, pick_chunk_tp(p, bx.r_cnt, bx.iz_cnt, bx.iw_cnt)))
+      return fail(p, JERK_EINVAL, "harmonic stage: empty box");
+    HarmGather& hg = tp.hg;
+    for (int f = 0; f < 7; f++) {
+      hg.base[f] = hp.sub[f].base;
+      hg.j0[f] = hp.sub[f].j0;
+      hg.nj[f] = hp.sub[f].nj;
+      hg.iz_lo[f] = hp.sub[f].iz_lo;
+      hg.iz_cnt[f] = hp.sub[f].iz_cnt;
+      hg.iw_lo[f] = hp.sub[f].iw_lo;
+    }
+    hg.cz = (p->nz - 1) / 2;
+    hg.cw = (p->nw - 1) / 2;
+    for (int q = 0; q < 4; q++) hg.thr[q] = thr4 ? thr4[q] : 0.f;
+    hg.warpbest = best;
+    hg.out = d_out;
+    hg.out_stage = out_stage;
+    k_reset<<<1, 32, 0, st>>>(tp.work, nullptr, 0);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_reset launch: ") + cudaGetErrorString(e));
+    if (d_out) {
+      e = launch_search64<MODE_HARM_STORE>(p, tp, st);
+    } else {
+      e = launch_search64<MODE_HARM>(p, tp, st);
+      const int nwarps = (int)search64_grid<MODE_HARM>(p, tp.nitems) * 2 * K64<MODE_HARM>::NG;
+      if (e == cudaSuccess) {
+        k_harm_fold<<<1, 256, 0, st>>>(best, nwarps, nullptr, (jerk_cand*)scratch, first ? 1 : 0);
+        e = cudaGetLastError();
+      }
+    }
+    if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_search64(top-harmonic pass) launch: ") + cudaGetErrorString(e));
+    return JERK_OK;
+  }
   hp.j_lo = 2 * bx.r_lo;
   hp.nj = 2 * bx.r_cnt;
   hp.iz_lo = bx.iz_lo;
@@ -1751,14 +2330,13 @@ static int harm_box(jerk_plan* p, const void* d_spec, const HarmBox& bx, unsigne
   hp.cw = (p->nw - 1) / 2;
   hp.jtile = kHarmJTile;
   hp.ntiles = ntiles;
-  hp.blockbest = (jerk_cand*)(scratch + bb_off);
+  hp.blockbest = best;
   hp.out = d_out;
   hp.out_stage = out_stage;
   if (d_out) {
     k_harm<true><<<nblocks, 256, 0, st>>>(hp);
   } else {
     k_harm<false><<<nblocks, 256, 0, st>>>(hp);
-    jerk_cand* partial = (jerk_cand*)(scratch + bb_off + align_up((uint64_t)4 * nblocks * sizeof(jerk_cand), 256));
     k_harm_fold<<<kHarmFoldBlocks, 256, 0, st>>>(hp.blockbest, nblocks, partial, nullptr, 0);
     k_harm_fold<<<1, 256, 0, st>>>(partial, kHarmFoldBlocks, nullptr, (jerk_cand*)scratch, first ? 1 : 0);
   }
@@ -1810,13 +2388,17 @@ int jerk_harmonic_sum(jerk_plan* p, const void* d_spec, int nstages, const int* 
     he.thr[s] = h_thr[s];
     if (he.stage[s] < 0) return fail(p, JERK_EINVAL, "harmonic stages must be 1, 2, 4 or 8");
   }
+  if (p->numbetween != 2) return fail(p, JERK_EINVAL, "the harmonic stage needs numbetween = 2");
+  if (!bank_covers(p, 0, p->nz, 0, p->nw)) return fail(p, JERK_ESTATE, "the harmonic stage needs the whole bank (jerk_templates)");
+  float thr4[4] = {INFINITY, INFINITY, INFINITY, INFINITY};   // per stage index log2 h: the lowest threshold asked for (unrequested stages are not tracked)
+  for (int s = 0; s < nstages; s++) thr4[he.stage[s]] = fminf(thr4[he.stage[s]], h_thr[s]);
   const int64_t chunk = harm_chunk_for(p, scratch_bytes);
   if (chunk == 0) return fail(p, JERK_ENOMEM, "harmonic scratch buffer too small (see jerk_harmonic_scratch_bytes)");
   cudaStream_t st = (cudaStream_t)stream;
   bool first = true;
   for (int64_t r_lo = 0; r_lo < p->nbins; r_lo += chunk) {
     HarmBox bx{r_lo, std::min<int64_t>(chunk, p->nbins - r_lo), 0, p->nz, 0, p->nw};
-    rc = harm_box(p, d_spec, bx, (unsigned char*)d_scratch, scratch_bytes, d_work, nullptr, 0, first, st);
+    rc = harm_box(p, d_spec, bx, (unsigned char*)d_scratch, scratch_bytes, d_work, work_bytes, nullptr, 0, thr4, first, st);
     if (rc) return rc;
     first = false;
   }
@@ -1832,6 +2414,8 @@ int jerk_harmonic_plane(jerk_plan* p, const void* d_spec, int h, int64_t r_lo, i
   int rc = check_common(p, d_spec, d_work, work_bytes);
   if (rc) return rc;
   if (stage_of(h) < 0) return fail(p, JERK_EINVAL, "h must be 1, 2, 4 or 8");
+  if (p->numbetween != 2) return fail(p, JERK_EINVAL, "the harmonic stage needs numbetween = 2");
+  if (!bank_covers(p, 0, p->nz, 0, p->nw)) return fail(p, JERK_ESTATE, "the harmonic stage needs the whole bank (jerk_templates)");
   if (r_lo < 0 || r_cnt < 0 || r_lo + r_cnt > p->nbins || iz_lo < 0 || iz_cnt < 0 || iz_lo + iz_cnt > p->nz || iw_lo < 0 ||
       iw_cnt < 0 || iw_lo + iw_cnt > p->nw)
     return fail(p, JERK_EINVAL, "harmonic plane sub-range outside the plan's grid");
@@ -1840,7 +2424,7 @@ int jerk_harmonic_plane(jerk_plan* p, const void* d_spec, int h, int64_t r_lo, i
   if (!d_out || !d_scratch) return JERK_EINVAL;
   if ((uintptr_t)d_scratch % 256) return fail(p, JERK_EINVAL, "d_scratch must be 256-byte aligned");
   HarmBox bx{r_lo, r_cnt, iz_lo, iz_cnt, iw_lo, iw_cnt};
-  return harm_box(p, d_spec, bx, (unsigned char*)d_scratch, scratch_bytes, d_work, d_out, stage_of(h), true, (cudaStream_t)stream);
+  return harm_box(p, d_spec, bx, (unsigned char*)d_scratch, scratch_bytes, d_work, work_bytes, d_out, stage_of(h), nullptr, true, (cudaStream_t)stream);
 }
 
 }  // extern "C"

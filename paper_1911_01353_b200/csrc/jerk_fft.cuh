@@ -364,6 +364,15 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&r)[16]) {
       : "memory");
 }
 
+__device__ __forceinline__ void tmem_ld4(uint32_t taddr, float (&r)[4]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];\n\t"
+      "tcgen05.wait::ld.sync.aligned;"
+      : "=f"(r[0]), "=f"(r[1]), "=f"(r[2]), "=f"(r[3])
+      : "r"(taddr)
+      : "memory");
+}
+
 // A thread-private array of P complex values (P = 16 or 32) held in TMEM columns [addr, addr + 2P) of the thread's lane.
 // load16(h, o) / store16(h, o) move entries 16h .. 16h+15; load8(i, o) entries 8i .. 8i+7.
 template <int L>

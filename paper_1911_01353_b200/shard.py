@@ -6,8 +6,9 @@ row (reading S10).  Two partitions are offered:
 
   * by trial  (weak scaling, what bench.py --gpus N times): rank r searches spectra r, r+W, r+2W, ... (other DM
     trials) against its own copy of the bank;
-  * by template (strong scaling of one spectrum): rank r searches a contiguous block of w-rows (a template box for
-    jerk_search_candidates_range); the spectrum is broadcast once, candidate lists are concatenated at the end.
+  * by template (strong scaling of one spectrum): rank r builds, holds and searches a contiguous range of the flat
+    template index ti = iw*nz + iz (jerk_templates_range + jerk_search_candidates_templates); the spectrum is
+    broadcast once, candidate lists are concatenated at the end.
 
 The only collectives are the ones around the search: broadcast of the spectrum, gather of the (small) candidate
 lists, max-over-ranks of device times.  This module holds no arithmetic of the method."""
@@ -93,12 +94,42 @@ def max_over_ranks(value: float, group=None) -> float:
     return float(t.item())
 
 
+def template_range(ntemplates: int, world: int, rank: int) -> tuple[int, int]:
+    """(ti_lo, ti_cnt) of `rank`: a flat split of the template index ti = iw*nz + iz, at most one template of imbalance
+    (w-row blocks would give 8,8,8,8,8,7,7,7 rows of the 61 on 8 ranks: 5 %)."""
+    return block_range(ntemplates, world, rank)
+
+
+def build_bank_shard(plan, group=None):
+    """jerk_templates_range for this rank's share: every rank builds and holds only 1/world of the bank."""
+    import torch.distributed as dist
+    sharded = dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1
+    world = dist.get_world_size(group) if sharded else 1
+    rank = dist.get_rank(group) if sharded else 0
+    ti_lo, ti_cnt = template_range(plan.info.ntemplates, world, rank)
+    plan.templates_range(ti_lo, ti_cnt)
+    return ti_lo, ti_cnt
+
+
+def agree_on_failure(flag: bool, group=None) -> bool:
+    """True on every rank iff `flag` is set on any rank (all_reduce MAX): a rank must never raise before a collective
+    the others are about to enter."""
+    import torch
+    import torch.distributed as dist
+    dev = torch.device("cuda", torch.cuda.current_device()) if dist.get_backend(group) == "nccl" else torch.device("cpu")
+    t = torch.tensor([1 if flag else 0], dtype=torch.int32, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX, group=group)
+    return bool(t.item())
+
+
 def search_candidates_sharded(plan, d_spec, threshold, max_cands: int = 1 << 20, group=None, src: int = 0) -> np.ndarray:
     """Strong-scaling search of ONE spectrum over the ranks of `group` (partition by template):
-    the spectrum is broadcast from `src`, every rank searches its template box with jerk_search_candidates_range
-    against its own bank, and the candidate lists are concatenated on every rank (sorted by (iw, iz, j)).
-    Without an initialised process group it is the whole-grid search on this rank.  No collective touches the search
-    itself: the candidate rule is one-dimensional along r inside a (z,w) row (reading S10)."""
+    the spectrum is broadcast from `src`, every rank searches its flat template range
+    (jerk_search_candidates_templates) against the part of the bank it holds (build_bank_shard, or the whole bank), and
+    the candidate lists are concatenated on every rank (sorted by (iw, iz, j)).  Without an initialised process group
+    it is the whole-grid search on this rank.  No collective touches the search itself: the candidate rule is
+    one-dimensional along r inside a (z,w) row (reading S10).  A candidate- or seam-buffer overflow on any
+    rank raises on EVERY rank (the flag is max-reduced before the gather)."""
     import torch.distributed as dist
     from . import binding
     sharded = dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1
@@ -106,11 +137,13 @@ def search_candidates_sharded(plan, d_spec, threshold, max_cands: int = 1 << 20,
     rank = dist.get_rank(group) if sharded else 0
     if sharded:
         broadcast_spectrum(d_spec, src=src, group=group)
-    iz_lo, iz_cnt, iw_lo, iw_cnt = template_box(plan.info.nz, plan.info.nw, world, rank)
-    d_c, d_n = plan.search_candidates_range(d_spec, threshold, iz_lo, iz_cnt, iw_lo, iw_cnt, max_cands)
-    local, n = binding.candidates_to_numpy(d_c, d_n)
-    if n > max_cands:
-        raise RuntimeError(f"candidate buffer overflow on rank {rank}: {n} > {max_cands}")
+    ti_lo, ti_cnt = template_range(plan.info.ntemplates, world, rank)
+    d_c, d_n = plan.search_candidates_templates(d_spec, threshold, ti_lo, ti_cnt, max_cands)
+    n = int(d_n.item()) & binding.SEAM_OVERFLOW
+    overflow = n > max_cands          # includes the seam-overflow sentinel
+    if (agree_on_failure(overflow, group) if sharded else overflow):
+        raise RuntimeError(f"candidate or seam buffer overflow (rank {rank}: count {n}, max_cands {max_cands})")
+    local, _ = binding.candidates_to_numpy(d_c, d_n)
     if sharded:
         return gather_candidates(local, group=group)
     return np.sort(local, order=["iw", "iz", "j"])

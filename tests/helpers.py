@@ -34,6 +34,34 @@ def oracle_rows(X, zw_list, b_lo, b_cnt, workers=None):
         return list(ex.map(_row_job, jobs))
 
 
+def _point_job(args):
+    z, w, pieces = args
+    tmpl = orc.template(z, w)
+    return [orc.power_row(Xs, z, w, b_rel, cnt, tmpl=tmpl) for (Xs, b_rel, cnt) in pieces]
+
+
+def oracle_point_rows(jobs, cnt=5, workers=None):
+    """jobs: [(X, z, w, [b_lo, ...])] -> per job {b_lo: oracle powers of bins b_lo .. b_lo+cnt-1 (2*cnt half-bin values)}.
+    One template quadrature per job; the workers get only the few hundred bins each piece can reach."""
+    workers = workers or min(8, os.cpu_count() or 1)
+    pad = 700
+    packed = []
+    for X, z, w, b_list in jobs:
+        pieces = []
+        for b_lo in b_list:
+            n = min(cnt, X.size - b_lo)
+            lo, hi = max(0, b_lo - pad), min(X.size, b_lo + n + pad)
+            pieces.append((np.array(X[lo:hi]), b_lo - lo, n))
+        packed.append((float(z), float(w), pieces))
+    if workers <= 1 or len(packed) <= 2:
+        res = [_point_job(j) for j in packed]
+    else:
+        import multiprocessing as mp
+        with ProcessPoolExecutor(max_workers=workers, mp_context=mp.get_context("spawn")) as ex:
+            res = list(ex.map(_point_job, packed, chunksize=4))
+    return [dict(zip(job[3], r)) for job, r in zip(jobs, res)]
+
+
 def assert_power_close(p_gpu, p_ref, what=""):
     p_gpu = np.asarray(p_gpu, dtype=np.float64)
     p_ref = np.asarray(p_ref, dtype=np.float64)

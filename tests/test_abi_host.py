@@ -10,7 +10,8 @@ import numpy as np
 import pytest
 
 from oracle import jerk_oracle as orc
-from paper_1911_01353_b200 import binding, build, synth
+from paper_1911_01353_b200 import binding, build
+import workloads as synth
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
@@ -65,7 +66,8 @@ def test_template_geometry_matches_oracle(lib):
 @pytest.mark.parametrize("args", [
     (0, 20, 2, 60, 20, 2, 1024),        # nbins < 1
     (1000, 20, 3, 60, 20, 2, 1024),     # zmax/dz not an integer
-    (1000, 20, 2, 60, 20, 1, 1024),     # numbetween != 2
+    (1000, 20, 2, 60, 20, 3, 1024),     # numbetween not 1 or 2
+    (1000, 20, 2, 60, 20, 0, 1024),
     (1000, 20, 2, 60, 20, 2, 1000),     # seg_len not a supported power of two
     (1000, 200, 2, 6000, 20, 2, 1024),  # overlap larger than the segment
     (1000, -1, 2, 60, 20, 2, 1024),
@@ -75,6 +77,25 @@ def test_plan_create_rejects(lib, args):
     h = C.c_void_p()
     rc = lib.jerk_plan_create(C.byref(h), *[int(a) if i in (0, 5, 6) else float(a) for i, a in enumerate(args)])
     assert rc == binding.JERK_EINVAL and not h.value
+
+
+def test_numbetween_one_halves_points_and_bank(lib):
+    """numbetween = 1 keeps the integer-bin phase only."""
+    a = binding.Plan(1 << 16, 20, 2, 0, 20, 2, 4096).info
+    b = binding.Plan(1 << 16, 20, 2, 0, 20, 1, 4096).info
+    assert b.numbetween == 1 and b.points * 2 == a.points and b.flops_per_search * 2 == a.flops_per_search
+    assert (b.bank_bytes - 256) * 2 == a.bank_bytes - 256 and (b.step, b.nseg, b.hw_max) == (a.step, a.nseg, a.hw_max)
+
+
+def test_bank_range_bytes(lib):
+    p = binding.Plan(1 << 16, 200, 2, 600, 20, 2, 4096)
+    T = p.info.ntemplates
+    full = lib.jerk_bank_bytes_range(p._h, T)
+    assert full == p.info.bank_bytes
+    part = lib.jerk_bank_bytes_range(p._h, T // 8 + 1)
+    assert part - (full - T * 2 * 4096 * 8) == (T // 8 + 1) * 2 * 4096 * 8       # tables of the whole grid + this rank's filters
+    assert lib.jerk_bank_bytes_range(p._h, T + 1) == 0
+    assert lib.jerk_strerror(binding.JERK_EOVERFLOW).startswith(b"JERK_EOVERFLOW")
 
 
 def test_null_arguments(lib):

@@ -4,7 +4,8 @@ import numpy as np
 import pytest
 
 from oracle import jerk_oracle as orc
-from paper_1911_01353_b200 import binding, build, synth
+from paper_1911_01353_b200 import binding, build
+import workloads as synth
 from tests import helpers as H
 
 pytestmark = pytest.mark.gpu
@@ -38,10 +39,13 @@ def _small_case(nbins=3000, seed=41):
     return X
 
 
-def test_harmonic_plane_and_top_match_oracle_on_full_small_volume():
-    nbins = 3000
+@pytest.mark.parametrize("seg_len", [1024, 4096])
+def test_harmonic_plane_and_top_match_oracle_on_full_small_volume(seg_len):
+    """seg_len 1024: eight stored sub-planes + k_harm; seg_len 4096: the sums are formed inside the top-harmonic search
+    pass (k_search64<MODE_HARM>), seven stored sub-planes."""
+    nbins = 3000 if seg_len == 1024 else 9000
     X = _small_case(nbins)
-    plan = binding.Plan(nbins, 20, 2, 60, 20, 2, 1024)
+    plan = binding.Plan(nbins, 20, 2, 60, 20, 2, seg_len)
     plan.templates()
     d_spec = binding.spectrum_to_device(X)
     P = orc.plane(X, 20, 2, 60, 20)                                    # [7][21][6000] float64
@@ -69,10 +73,11 @@ def test_harmonic_plane_and_top_match_oracle_on_full_small_volume():
     assert np.array_equal(S1, plan.search_plane(d_spec, 0, nbins).cpu().numpy())
 
 
-def test_harmonic_plane_subbox_is_bit_exact_slice():
+@pytest.mark.parametrize("seg_len", [1024, 4096])
+def test_harmonic_plane_subbox_is_bit_exact_slice(seg_len):
     nbins = 3000
     X = _small_case(nbins)
-    plan = binding.Plan(nbins, 20, 2, 60, 20, 2, 1024)
+    plan = binding.Plan(nbins, 20, 2, 60, 20, 2, seg_len)
     plan.templates()
     d_spec = binding.spectrum_to_device(X)
     for h in (2, 8):
@@ -82,11 +87,12 @@ def test_harmonic_plane_subbox_is_bit_exact_slice():
             assert np.array_equal(sub, full[iw_lo:iw_lo + iw_cnt, iz_lo:iz_lo + iz_cnt, 2 * r_lo:2 * (r_lo + r_cnt)])
 
 
-def test_harmonic_chunking_is_invisible_and_thresholds_apply():
+@pytest.mark.parametrize("seg_len", [1024, 4096])
+def test_harmonic_chunking_is_invisible_and_thresholds_apply(seg_len):
     """A scratch buffer that forces many r-chunks gives the same tops; stages under threshold report j = -1."""
     nbins = 3000
     X = _small_case(nbins)
-    plan = binding.Plan(nbins, 20, 2, 60, 20, 2, 1024)
+    plan = binding.Plan(nbins, 20, 2, 60, 20, 2, seg_len)
     plan.templates()
     d_spec = binding.spectrum_to_device(X)
     a = plan.harmonic_sum(d_spec, STAGES, (0.0,) * 4)
@@ -101,6 +107,37 @@ def test_harmonic_chunking_is_invisible_and_thresholds_apply():
     with pytest.raises(binding.JerkError) as e:
         plan.harmonic_sum(d_spec, (1,), (0.0,), scratch_bytes=4096)
     assert e.value.status == binding.JERK_ENOMEM
+
+
+def test_harmonic_prune_kernel_small_volume():
+    """The PRUNE instantiation (hw_max = 258) of the fused top-harmonic pass on a coarse zmax 200 / wmax 600 grid
+    (21 x 13 templates) over a short spectrum with ragged segments: the whole S_h volume and the stage tops vs the oracle."""
+    nbins = 5000
+    rng = np.random.Generator(np.random.PCG64(43))
+    n = 2 * nbins
+    x = rng.standard_normal(n)
+    r0, z0, w0 = 310.5, 20.0, 0.0
+    a = np.sqrt(4.0 * 60.0 / n)
+    for k in range(1, 9):
+        x += synth.chirp_series(n, k * r0, k * z0, k * w0, a / k)
+    X = synth.block_normalise(np.fft.rfft(x)[:nbins]).astype(np.complex64)
+    plan = binding.Plan(nbins, 200, 20, 600, 100, 2, 4096)
+    assert plan.info.hw_max == 258 and plan.info.ntemplates == 21 * 13
+    plan.templates()
+    d_spec = binding.spectrum_to_device(X)
+    P = orc.plane(X, 200, 20, 600, 100)
+    top = plan.harmonic_sum(d_spec, STAGES, (0.0,) * 4)
+    for s, h in enumerate(STAGES):
+        S_ref = orc.harmonic_sum_volume(P, h)
+        g = plan.harmonic_plane(d_spec, h, 0, nbins).cpu().numpy()
+        err = np.abs(g.astype(np.float64) - S_ref) - _harm_tol(h, S_ref)
+        assert err.max() <= 0, f"h={h}: worst excess {err.max()}"
+        rec = top[s]
+        assert np.unravel_index(np.argmax(g), g.shape) == (rec["iw"], rec["iz"], rec["j"]) and g.max() == rec["power"]
+        iw, iz, j = np.unravel_index(np.argmax(S_ref), S_ref.shape)
+        second = np.partition(S_ref.ravel(), -2)[-2]
+        if S_ref[iw, iz, j] - second > 2 * _harm_tol(h, S_ref[iw, iz, j]):
+            assert (rec["iw"], rec["iz"], rec["j"]) == (iw, iz, j)
 
 
 class _OraclePowers:

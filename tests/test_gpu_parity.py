@@ -7,7 +7,8 @@ import numpy as np
 import pytest
 
 from oracle import jerk_oracle as orc
-from paper_1911_01353_b200 import binding, build, synth
+from paper_1911_01353_b200 import binding, build
+import workloads as synth
 from tests import helpers as H
 
 pytestmark = pytest.mark.gpu

@@ -3,7 +3,8 @@ import numpy as np
 import pytest
 
 from oracle import jerk_oracle as orc
-from paper_1911_01353_b200 import binding, build, synth
+from paper_1911_01353_b200 import binding, build
+import workloads as synth
 from tests import helpers as H
 
 pytestmark = pytest.mark.gpu
@@ -74,12 +75,20 @@ def test_snr_filter_matches_the_oracle(setup):
     assert (iw0, iz0, 2 * 12345) in kept_keys
 
 
-def test_stats_mode_needs_seg_len_4096(setup):
+@pytest.mark.parametrize("seg_len", [1024, 2048, 8192])
+def test_row_statistics_on_every_seg_len(setup, seg_len):
+    """The fused statistics in the three-pass kernels k_search<L, MODE_CAND_STATS>: the same sums and candidates as the oracle rows."""
     X, plan, d_spec, zs, ws, rows = setup
-    p2 = binding.Plan(NBINS, ZMAX, DZ, WMAX, DW, 2, 1024)
+    p2 = binding.Plan(NBINS, ZMAX, DZ, WMAX, DW, 2, seg_len)
     p2.templates()
-    with pytest.raises(binding.JerkError):
-        p2.search_candidates_stats(d_spec, THR)
+    d_c, d_n, d_stats = p2.search_candidates_stats(d_spec, THR)
+    stats = d_stats.cpu().numpy()
+    want = np.array([orc.row_stats(P) for P in rows])
+    assert np.abs(stats[:, 0] / want[:, 0] - 1.0).max() < 2e-5
+    assert np.abs(stats[:, 1] / want[:, 1] - 1.0).max() < 1e-4
+    plain, n0 = binding.candidates_to_numpy(*p2.search_candidates(d_spec, THR))
+    fused, n1 = binding.candidates_to_numpy(d_c, d_n)
+    assert n0 == n1 and np.array_equal(np.sort(plain, order=["iw", "iz", "j"]), np.sort(fused, order=["iw", "iz", "j"]))
 
 
 # ------------------------------------------------------------------------------------------------ cross-row sifting

@@ -7,7 +7,8 @@ import numpy as np
 import pytest
 
 from oracle import spectrum_oracle as so
-from paper_1911_01353_b200 import binding, build, synth
+from paper_1911_01353_b200 import binding, build
+import workloads as synth
 
 pytestmark = pytest.mark.gpu
 torch = pytest.importorskip("torch")

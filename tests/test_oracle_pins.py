@@ -14,7 +14,7 @@ import pytest
 from scipy.special import fresnel
 
 from oracle import jerk_oracle as orc
-from paper_1911_01353_b200 import synth
+import workloads as synth
 
 GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
 
@@ -407,3 +407,39 @@ def test_sift_invariants():
                 assert not (abs(a[0] - b[0]) <= 6 and abs(a[1] - b[1]) <= 2 and abs(a[2] - b[2]) <= 1)
         # larger windows never keep more
         assert len(orc.sift(c, 12, 4, 2)) <= len(kept)
+
+
+# --------------------------------------------------------------------------- section I: numbetween = 1
+def test_numbetween1_pins():
+    """power_row_nb1 (phase-0 taps on integer bins) against what fixes it independently:
+    (i) z = w = 0: R_{0,0}(m) = delta_{m0} (the closed-form sinc of pin P1 at integer q), so P[b] = |X[b]|^2 exactly;
+    (ii) library correlation with the phase-0 taps; (iii) P6-style brute force: the de-chirped DFT of a time series at
+    integer r equals the spectral correlation with the discrete full-width response (exact at odd N)."""
+    rng = np.random.default_rng(12)
+    X = (rng.standard_normal(300) + 1j * rng.standard_normal(300)).astype(np.complex128)
+    P = orc.power_row_nb1(X, 0.0, 0.0)
+    assert np.abs(P - np.abs(X) ** 2).max() < 1e-12
+    for (z, w) in [(6.0, -40.0), (-20.0, 60.0)]:
+        c, hw, lat = orc.template(z, w)
+        m, taps = orc.phase_taps(c, hw, lat, 0)
+        full = np.correlate(np.concatenate((np.zeros(600), X, np.zeros(600))), taps, mode="valid")    # sum_k Xp[i+k] conj(taps[k])
+        want = np.abs(full[600 + m[0]: 600 + m[0] + 300]) ** 2
+        got = orc.power_row_nb1(X, z, w)
+        assert np.abs(got - want).max() < 1e-10 * max(1.0, want.max())
+        sub = orc.power_row_nb1(X, z, w, 37, 11)
+        assert np.array_equal(sub, got[37:48])
+    # brute force in the time domain, N odd so that the discrete response has no aliasing ambiguity
+    N, z, w = 255, 3.0, 10.0
+    x = rng.standard_normal(N) + 1j * rng.standard_normal(N)
+    u = np.arange(N) / N
+    Xf = np.array([np.sum(x * np.exp(-2j * np.pi * k * u)) for k in range(N)])
+    r = 100
+    direct = np.sum(x * np.exp(-2j * np.pi * (r * u + z * u * u / 2 + w * u ** 3 / 6)))
+    hw = N // 2
+    q = np.arange(-hw, hw + 1)
+    D = np.array([np.mean(np.exp(2j * np.pi * (z * u * u / 2 + w * u ** 3 / 6 - qq * u))) for qq in q])
+    lattice = np.zeros(4 * hw + 1, dtype=np.complex128)
+    lattice[0::2] = D                                   # phase-0 lattice points q = -hw..hw; the half-bin points are unused
+    Xext = np.concatenate((Xf, Xf, Xf))                 # periodic extension: the routine itself zero-pads
+    got = orc.power_row_nb1(Xext, z, w, N + r, 1, tmpl=(0, hw, lattice))[0]
+    assert abs(got - abs(direct) ** 2) < 1e-9 * abs(direct) ** 2

@@ -1,6 +1,6 @@
 """Host-side multi-rank logic on CPU: world_size-2 (and 3) gloo process groups.  No GPU, no kernels:
-the per-rank "search" is replaced by slicing a fixed synthetic candidate list by template box, which is exactly what
-jerk_search_candidates_range guarantees (tests/test_gpu_parity.py::test_candidates_range_union checks that on the GPU)."""
+the per-rank "search" is replaced by slicing a fixed synthetic candidate list by template range, which is exactly what
+jerk_search_candidates_templates guarantees (tests/test_gpu_parity.py::test_candidates_range_union checks that on the GPU)."""
 import os
 import socket
 
@@ -51,18 +51,35 @@ def _worker(rank, world, port, nz, nw, q):
 
         class _FakePlan:
             info = _Info()
+            overflow_rank = -1
 
-            def search_candidates_range(self, d_spec, thr, iz_lo, iz_cnt, iw_lo, iw_cnt, max_cands):
-                sel = full[(full["iz"] >= iz_lo) & (full["iz"] < iz_lo + iz_cnt) & (full["iw"] >= iw_lo) &
-                           (full["iw"] < iw_lo + iw_cnt) & (full["power"] > thr)]
+            def templates_range(self, ti_lo, ti_cnt):
+                self.bank_range = (ti_lo, ti_cnt)
+
+            def search_candidates_templates(self, d_spec, thr, ti_lo, ti_cnt, max_cands):
+                assert (ti_lo, ti_cnt) == self.bank_range      # a rank searches exactly the part of the bank it built
+                ti = full["iw"].astype(np.int64) * nz + full["iz"]
+                sel = full[(ti >= ti_lo) & (ti < ti_lo + ti_cnt) & (full["power"] > thr)]
                 buf = np.zeros(max_cands * 16, dtype=np.uint8)
                 buf[: sel.size * 16] = np.frombuffer(sel.tobytes(), dtype=np.uint8)
-                return torch.from_numpy(buf), torch.tensor([sel.size], dtype=torch.int64)
+                count = sel.size if rank != self.overflow_rank else max_cands + 1
+                return torch.from_numpy(buf), torch.tensor([count], dtype=torch.int64)
 
-        _FakePlan.info.nz, _FakePlan.info.nw = nz, nw
-        merged2 = shard.search_candidates_sharded(_FakePlan(), X, 40.0, max_cands=4096)
+        _FakePlan.info.nz, _FakePlan.info.nw, _FakePlan.info.ntemplates = nz, nw, nz * nw
+        plan = _FakePlan()
+        lo, cnt = shard.build_bank_shard(plan)
+        assert (lo, cnt) == shard.template_range(nz * nw, world, rank)
+        merged2 = shard.search_candidates_sharded(plan, X, 40.0, max_cands=4096)
         want2 = np.sort(full[full["power"] > 40.0], order=["iw", "iz", "j"])
         ok_merge = ok_merge and np.array_equal(merged2, want2) and bool(torch.view_as_real(X)[-1, 1] == 1999.0)
+        # an overflow on ONE rank raises on EVERY rank (agreed collectively before the gather: nobody hangs)
+        plan.overflow_rank = world - 1
+        try:
+            shard.search_candidates_sharded(plan, X, 40.0, max_cands=4096)
+            ok_merge = False
+        except RuntimeError:
+            pass
+        plan.overflow_rank = -1
         tmax = shard.max_over_ranks(10.0 + rank)
         q.put((rank, ok_merge, ok_bcast, tmax, shard.trial_indices(7, world, rank)))
     finally:

@@ -3,7 +3,7 @@ import numpy as np
 import pytest
 
 from oracle import spectrum_oracle as so
-from paper_1911_01353_b200 import synth
+import workloads as synth
 
 
 def test_rfft_equals_the_written_out_sum():
