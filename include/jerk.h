@@ -287,6 +287,24 @@ int jerk_prepare_spectrum(const float* d_series, int64_t nsamples, int block, vo
                           uint64_t scratch_bytes, void* stream);
 
 /*
+ * jerk_prepare_spectrum_mode — the same with a choice of normalisation (SURVEY.md 8(f) N1 "mean as in config 1;
+ * median-based and red-noise variants"; the spectrum of a real de-dispersed series, whose noise floor is
+ * neither white nor free of strong narrow signals; the paper gives no recipe: readings):
+ *   JERK_NORM_MEAN      every `block`-bin block divided by sqrt(mean |X|^2)             (= jerk_prepare_spectrum)
+ *   JERK_NORM_MEDIAN    every `block`-bin block divided by sqrt(median |X|^2 / ln 2): for exponentially distributed noise
+ *                       powers the median is ln 2 times the mean, and a few strong bins do not move it (even count: mean of
+ *                       the two middle values; zero median: block left as it is)
+ *   JERK_NORM_REDNOISE  the median rule on blocks whose length grows with frequency, to follow a steep low-frequency noise
+ *                       slope: lengths 6, 7, 8, ... each min(block, len + max(1, len / 8)) (integer division), from bin 0
+ * block <= 4096 for the median modes (the block is sorted in shared memory), >= 8 for JERK_NORM_REDNOISE.
+ * jerk_spectrum_scratch_bytes(nsamples) covers every mode (nsamples/2 complex64 + the red-noise block table);
+ * JERK_NORM_MEAN and JERK_NORM_MEDIAN need only the first nsamples/2 * 8 bytes of it.
+ */
+enum { JERK_NORM_MEAN = 0, JERK_NORM_MEDIAN = 1, JERK_NORM_REDNOISE = 2 };
+int jerk_prepare_spectrum_mode(const float* d_series, int64_t nsamples, int block, int mode, void* d_spec, void* d_scratch,
+                               uint64_t scratch_bytes, void* stream);
+
+/*
  * jerk_probe_fma — measurement aid for the roofline denominator: launches a kernel of nothing but
  * independent FP32 fused multiply-add chains (2048 threads per SM, 16 chains per thread, `iters` iterations) on
  * `stream` and returns in *flops (HOST) the number of floating-point operations it executes; the caller times it.

@@ -44,7 +44,7 @@ EXPORTS = [
     "jerk_search_candidates_batch", "jerk_search_candidates_stats", "jerk_snr_filter",
     "jerk_sift_candidates",
     "jerk_search_candidates_host", "jerk_search_series_host", "jerk_harmonic_scratch_bytes", "jerk_harmonic_sum", "jerk_harmonic_plane", "jerk_spectrum_scratch_bytes",
-    "jerk_prepare_spectrum", "jerk_probe_fma", "jerk_strerror",
+    "jerk_prepare_spectrum", "jerk_prepare_spectrum_mode", "jerk_probe_fma", "jerk_strerror",
     "jerk_last_error",
 ]
 
@@ -89,6 +89,7 @@ def load_library() -> C.CDLL:
     lib.jerk_spectrum_scratch_bytes.argtypes = [i64]
     lib.jerk_spectrum_scratch_bytes.restype = u64
     lib.jerk_prepare_spectrum.argtypes = [vp, i64, i32, vp, vp, u64, vp]
+    lib.jerk_prepare_spectrum_mode.argtypes = [vp, i64, i32, i32, vp, vp, u64, vp]
     lib.jerk_probe_fma.argtypes = [vp, i32, C.POINTER(dbl), vp]
     lib.jerk_strerror.argtypes = [i32]
     lib.jerk_strerror.restype = C.c_char_p
@@ -349,9 +350,13 @@ class Plan:
         return self.work[:64].view(dtype=__import__("torch").int64).cpu().numpy().copy()
 
 
-def prepare_spectrum(d_series, block=1000, d_spec=None, d_scratch=None, stream=None):
-    """jerk_prepare_spectrum: float32 device time series (2^11..2^25 samples) -> complex64 device spectrum of N/2 bins,
-    block-normalised; returns the spectrum as a float32 tensor of shape (N/2, 2) (the d_spec layout of the search calls)."""
+NORM_MODES = {"mean": 0, "median": 1, "rednoise": 2}
+
+
+def prepare_spectrum(d_series, block=1000, d_spec=None, d_scratch=None, stream=None, mode="mean"):
+    """jerk_prepare_spectrum_mode: float32 device time series (2^11..2^25 samples) -> complex64 device spectrum of N/2 bins,
+    block-normalised (mode "mean", "median" or "rednoise"); returns the spectrum as a float32 tensor of shape (N/2, 2)
+    (the d_spec layout of the search calls)."""
     import torch
     lib = load_library()
     n = d_series.numel()
@@ -360,8 +365,9 @@ def prepare_spectrum(d_series, block=1000, d_spec=None, d_scratch=None, stream=N
     nbytes = int(lib.jerk_spectrum_scratch_bytes(n))
     if d_scratch is None:
         d_scratch = torch.empty(max(nbytes, 8), dtype=torch.uint8, device=d_series.device)
-    rc = lib.jerk_prepare_spectrum(C.c_void_p(d_series.data_ptr()), int(n), int(block), C.c_void_p(d_spec.data_ptr()),
-                                   C.c_void_p(d_scratch.data_ptr()), d_scratch.numel(), _stream_ptr(stream))
+    rc = lib.jerk_prepare_spectrum_mode(C.c_void_p(d_series.data_ptr()), int(n), int(block), int(NORM_MODES[mode]),
+                                        C.c_void_p(d_spec.data_ptr()), C.c_void_p(d_scratch.data_ptr()), d_scratch.numel(),
+                                        _stream_ptr(stream))
     if rc != 0:
         raise JerkError(rc, lib.jerk_strerror(rc).decode())
     return d_spec

@@ -139,25 +139,27 @@ __global__ void __launch_bounds__(256) k_dft_direct(StridedFft a, int L) {
   a.out[(long long)b * a.out_sb + (long long)k * a.out_se] = r;
 }
 
+// untangled real-input spectrum bin k from the half-length transform Z (M points)
+__device__ __forceinline__ float2 untangle_bin(const float2* __restrict__ Z, int M, int k) {
+  if (k == 0) {
+    const float2 z0 = Z[0];
+    return make_float2(z0.x + z0.y, 0.f);
+  }
+  const float2 zk = Z[k], zm = Z[M - k];
+  const float2 e = make_float2(0.5f * (zk.x + zm.x), 0.5f * (zk.y - zm.y));   // (Z[k] + conj Z[M-k]) / 2
+  const float2 o = make_float2(0.5f * (zk.x - zm.x), 0.5f * (zk.y + zm.y));   // (Z[k] - conj Z[M-k]) / 2
+  float s, c;
+  sincospif((float)k / (float)M, &s, &c);                                     // exp(-i pi k/M) = (c, -s)
+  return make_float2(e.x + (-s * o.x + c * o.y), e.y + (-c * o.x - s * o.y));  // e - i exp(-i pi k/M) o
+}
+
 // One CTA per normalisation block: untangle the half-length transform into the real-input spectrum, reduce the block's
 // power in a fixed order (deterministic), scale.  Every thread re-reads only what it wrote itself.
 __global__ void __launch_bounds__(256) k_untangle_norm(const float2* __restrict__ Z, float2* __restrict__ X, int M, int block) {
   const int k_lo = blockIdx.x * block, k_hi = min(M, k_lo + block);
   double acc = 0.0;
   for (int k = k_lo + threadIdx.x; k < k_hi; k += 256) {
-    float2 x;
-    if (k == 0) {
-      const float2 z0 = Z[0];
-      x = make_float2(z0.x + z0.y, 0.f);
-    } else {
-      const float2 zk = Z[k], zm = Z[M - k];
-      const float2 e = make_float2(0.5f * (zk.x + zm.x), 0.5f * (zk.y - zm.y));   // (Z[k] + conj Z[M-k]) / 2
-      const float2 o = make_float2(0.5f * (zk.x - zm.x), 0.5f * (zk.y + zm.y));   // (Z[k] - conj Z[M-k]) / 2
-      float s, c;
-      sincospif((float)k / (float)M, &s, &c);                                     // exp(-i pi k/M) = (c, -s)
-      // -i * (c - i s) * o = (-s - i c) * o
-      x = make_float2(e.x + (-s * o.x + c * o.y), e.y + (-c * o.x - s * o.y));
-    }
+    const float2 x = untangle_bin(Z, M, k);
     X[k] = x;
     acc += (double)x.x * x.x + (double)x.y * x.y;
   }
@@ -176,6 +178,78 @@ __global__ void __launch_bounds__(256) k_untangle_norm(const float2* __restrict_
   __syncthreads();
   const float sc = s_scale;
   for (int k = k_lo + threadIdx.x; k < k_hi; k += 256) {
+    const float2 x = X[k];
+    X[k] = make_float2(x.x * sc, x.y * sc);
+  }
+}
+
+// Block starts of the red-noise variant (N1 reading): lengths 6, 7, 8, ... growing by len / 8 (at least 1) up
+// to `block`; bounds[0 .. nblk] with bounds[nblk] = M, nblk stored in bounds[-1 + cap] ... by one thread (a few hundred
+// steps at most before the lengths saturate, then M / block more).
+__global__ void k_rednoise_bounds(int* bounds, int cap, int M, int block) {
+  if (blockIdx.x || threadIdx.x) return;
+  int n = 0, k = 0, len = 6;
+  bounds[0] = 0;
+  while (k + len < M && n + 2 < cap) {
+    k += len;
+    bounds[++n] = k;
+    const int g = len / 8;
+    len = min(block, len + (g > 1 ? g : 1));
+  }
+  bounds[++n] = M;
+  bounds[cap] = n;        // number of blocks
+}
+
+// Median variants (SURVEY.md 8(f) N1 "median-based and red-noise variants"): one CTA per normalisation block
+// [lo, hi): untangle, powers into shared memory, bitonic sort, median (mean of the two middle values for an even
+// count), scale by 1 / sqrt(median / ln 2).  bounds == nullptr: uniform blocks of `block` bins.
+__global__ void __launch_bounds__(256) k_untangle_norm_median(const float2* __restrict__ Z, float2* __restrict__ X, int M, int block,
+                                                              const int* __restrict__ bounds, int cap) {
+  extern __shared__ float s_pow[];      // next power of two >= block
+  __shared__ float s_scale;
+  int k_lo, k_hi;
+  if (bounds) {
+    if ((int)blockIdx.x >= bounds[cap]) return;
+    k_lo = bounds[blockIdx.x];
+    k_hi = bounds[blockIdx.x + 1];
+  } else {
+    k_lo = blockIdx.x * block;
+    k_hi = min(M, k_lo + block);
+  }
+  const int n = k_hi - k_lo;
+  int np2 = 1;
+  while (np2 < n) np2 <<= 1;
+  for (int i = threadIdx.x; i < np2; i += 256) {
+    float pw = INFINITY;                 // padding sorts to the end
+    if (i < n) {
+      const float2 x = untangle_bin(Z, M, k_lo + i);
+      X[k_lo + i] = x;
+      pw = fmaf(x.x, x.x, x.y * x.y);
+    }
+    s_pow[i] = pw;
+  }
+  __syncthreads();
+  for (int size = 2; size <= np2; size <<= 1)
+    for (int stride = size >> 1; stride > 0; stride >>= 1) {
+      for (int i = threadIdx.x; i < np2 / 2; i += 256) {
+        const int lo = 2 * i - (i & (stride - 1));          // element whose bit `stride` is 0
+        const int hi = lo + stride;
+        const bool up = (lo & size) == 0;
+        const float a = s_pow[lo], b = s_pow[hi];
+        if ((a > b) == up) {
+          s_pow[lo] = b;
+          s_pow[hi] = a;
+        }
+      }
+      __syncthreads();
+    }
+  if (threadIdx.x == 0) {
+    const float med = (n & 1) ? s_pow[n / 2] : 0.5f * (s_pow[n / 2 - 1] + s_pow[n / 2]);
+    s_scale = med > 0.f ? (float)(1.0 / sqrt((double)med / 0.69314718055994530942)) : 1.0f;
+  }
+  __syncthreads();
+  const float sc = s_scale;
+  for (int k = k_lo + threadIdx.x; k < k_hi; k += 256) {   // every thread re-reads only what it wrote itself
     const float2 x = X[k];
     X[k] = make_float2(x.x * sc, x.y * sc);
   }
@@ -230,16 +304,28 @@ using namespace jerk;
 
 extern "C" {
 
+// blocks of the red-noise schedule are at least 6 bins long: M / 6 + 2 starts at most, + the count
+static uint64_t bounds_cap(int64_t nsamples) { return (uint64_t)(nsamples / 2) / 6 + 4; }
+
 uint64_t jerk_spectrum_scratch_bytes(int64_t nsamples) {
   if (nsamples < 2) return 0;
-  return (uint64_t)(nsamples / 2) * sizeof(float2);
+  return (uint64_t)(nsamples / 2) * sizeof(float2) + (bounds_cap(nsamples) + 1) * sizeof(int);
 }
 
 int jerk_prepare_spectrum(const float* d_series, int64_t nsamples, int block, void* d_spec, void* d_scratch, uint64_t scratch_bytes,
                           void* stream) {
+  return jerk_prepare_spectrum_mode(d_series, nsamples, block, JERK_NORM_MEAN, d_spec, d_scratch, scratch_bytes, stream);
+}
+
+int jerk_prepare_spectrum_mode(const float* d_series, int64_t nsamples, int block, int mode, void* d_spec, void* d_scratch,
+                               uint64_t scratch_bytes, void* stream) {
   if (!d_series || !d_spec || !d_scratch || block < 1) return JERK_EINVAL;
+  if (mode != JERK_NORM_MEAN && mode != JERK_NORM_MEDIAN && mode != JERK_NORM_REDNOISE) return JERK_EINVAL;
+  if (mode != JERK_NORM_MEAN && block > 4096) return JERK_EINVAL;      // the block is sorted in shared memory
+  if (mode == JERK_NORM_REDNOISE && block < 8) return JERK_EINVAL;
   if (nsamples < (1 << 11) || nsamples > (1 << 25) || (nsamples & (nsamples - 1))) return JERK_EINVAL;   // 2^11 .. 2^25 samples
-  if (scratch_bytes < jerk_spectrum_scratch_bytes(nsamples)) return JERK_ENOMEM;
+  // the red-noise block table sits behind the transform scratch; the other modes need the transform scratch only
+  if (scratch_bytes < (mode == JERK_NORM_REDNOISE ? jerk_spectrum_scratch_bytes(nsamples) : (uint64_t)(nsamples / 2) * sizeof(float2))) return JERK_ENOMEM;
   if ((uintptr_t)d_series % 16 || (uintptr_t)d_spec % 16 || (uintptr_t)d_scratch % 16) return JERK_EINVAL;   // 128-bit accesses
   int dev = 0, major = 0;
   if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess ||
@@ -273,7 +359,22 @@ int jerk_prepare_spectrum(const float* d_series, int64_t nsamples, int block, vo
   b.per_cta = M1 >= 4 ? 4 : 1;
   b.tw_den = 0;
   if (run_fft(b, M2, st) != cudaSuccess) return JERK_ECUDA;
-  k_untangle_norm<<<(M + block - 1) / block, 256, 0, st>>>(Z, (float2*)d_spec, M, block);
+  if (mode == JERK_NORM_MEAN) {
+    k_untangle_norm<<<(M + block - 1) / block, 256, 0, st>>>(Z, (float2*)d_spec, M, block);
+  } else {
+    int np2 = 1;
+    while (np2 < block) np2 <<= 1;
+    const size_t smem = (size_t)np2 * sizeof(float);
+    if (mode == JERK_NORM_MEDIAN) {
+      k_untangle_norm_median<<<(M + block - 1) / block, 256, smem, st>>>(Z, (float2*)d_spec, M, block, nullptr, 0);
+    } else {
+      int* bounds = (int*)((unsigned char*)d_scratch + (size_t)M * sizeof(float2));
+      const int cap = (int)bounds_cap(nsamples);
+      k_rednoise_bounds<<<1, 32, 0, st>>>(bounds, cap, M, block);
+      // an upper bound on the number of blocks (the growth phase has fewer than 64): surplus CTAs leave at once
+      k_untangle_norm_median<<<M / block + 66, 256, smem, st>>>(Z, (float2*)d_spec, M, block, bounds, cap);
+    }
+  }
   if (cudaGetLastError() != cudaSuccess) return JERK_ECUDA;
   return JERK_OK;
 }

@@ -22,17 +22,17 @@ def _built():
     binding.load_library()
 
 
-def _run(x, block=1000):
+def _run(x, block=1000, mode="mean"):
     d = torch.from_numpy(np.ascontiguousarray(x, dtype=np.float32)).cuda()
-    out = binding.prepare_spectrum(d, block)
+    out = binding.prepare_spectrum(d, block, mode=mode)
     torch.cuda.synchronize()
     assert torch.equal(d.cpu(), torch.from_numpy(np.ascontiguousarray(x, dtype=np.float32)))   # input untouched
     return out.cpu().numpy().view(np.complex64).reshape(-1)
 
 
-def _check(x, block=1000):
-    got = _run(x, block).astype(np.complex128)
-    ref = so.prepare_spectrum(np.asarray(x, dtype=np.float32).astype(np.float64), block)
+def _check(x, block=1000, mode="mean"):
+    got = _run(x, block, mode).astype(np.complex128)
+    ref = so.prepare_spectrum_mode(np.asarray(x, dtype=np.float32).astype(np.float64), block, mode)
     err = np.abs(got - ref) / np.maximum(1.0, np.abs(ref))
     assert err.max() <= TOL, (err.max(), int(err.argmax()))
     return got, ref
@@ -74,6 +74,24 @@ def test_pure_tone_and_ragged_block():
     assert int(np.argmax(np.abs(got))) == k0
 
 
+@pytest.mark.parametrize("mode", ["median", "rednoise"])
+@pytest.mark.parametrize("log2n,block", [(11, 1000), (12, 64), (16, 777), (21, 1000), (23, 1000), (25, 4096)])
+def test_median_and_rednoise_variants(mode, log2n, block):
+    """SURVEY.md 8(f) N1 "median-based and red-noise variants": red (1/f-like) noise plus a strong tone, every FFT
+    decomposition, ragged last blocks, the largest block the shared-memory sort takes."""
+    rng = np.random.Generator(np.random.PCG64(4242 + log2n))
+    n = 1 << log2n
+    x = rng.standard_normal(n, dtype=np.float32)
+    x += np.cumsum(rng.standard_normal(n, dtype=np.float32)) * np.float32(0.02)          # a random walk: red noise
+    x += (np.sqrt(4.0 * 2e3 / n) * np.cos(2 * np.pi * (n // 8 + 0.0) * np.arange(n) / n)).astype(np.float32)
+    x -= x.mean()
+    got, ref = _check(x, block, mode)
+    if mode == "rednoise" and log2n >= 16:
+        # the low-frequency slope is gone: every 200-bin stretch between bins 200 and 2000 has about unit mean power
+        p = [np.mean(np.abs(got[a:a + 200]) ** 2) for a in range(200, 2000, 200)]
+        assert 0.6 < min(p) and max(p) < 1.5, p
+
+
 def test_errors():
     lib = binding.load_library()
     d = torch.zeros(3000, dtype=torch.float32, device="cuda")
@@ -85,7 +103,12 @@ def test_errors():
     d = torch.zeros(1 << 12, dtype=torch.float32, device="cuda")
     with pytest.raises(binding.JerkError):
         binding.prepare_spectrum(d, d_scratch=torch.empty(16, dtype=torch.uint8, device="cuda"))   # scratch too small
-    assert lib.jerk_spectrum_scratch_bytes(1 << 12) == (1 << 11) * 8
+    assert lib.jerk_spectrum_scratch_bytes(1 << 12) >= (1 << 11) * 8
+    d = torch.zeros(1 << 12, dtype=torch.float32, device="cuda")
+    with pytest.raises(binding.JerkError):
+        binding.prepare_spectrum(d, 8192, mode="median")  # block larger than the shared-memory sort
+    with pytest.raises(binding.JerkError):
+        binding.prepare_spectrum(d, 4, mode="rednoise")   # block below the first block of the schedule
 
 
 def test_pipeline_from_host_series_equals_the_separate_calls():
