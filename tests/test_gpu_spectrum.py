@@ -81,8 +81,11 @@ def test_median_and_rednoise_variants(mode, log2n, block):
     decomposition, ragged last blocks, the largest block the shared-memory sort takes."""
     rng = np.random.Generator(np.random.PCG64(4242 + log2n))
     n = 1 << log2n
+    from scipy.signal import lfilter
     x = rng.standard_normal(n, dtype=np.float32)
-    x += np.cumsum(rng.standard_normal(n, dtype=np.float32)) * np.float32(0.02)          # a random walk: red noise
+    # red noise: an AR(1) process with a 30-sample memory (a Lorentzian spectrum, ~900 x the white level in power at the
+    # lowest bins: fp32 carries that dynamic range within the tolerance, a pure random walk does not)
+    x += lfilter([1.0], [1.0, -(1.0 - 1.0 / 30.0)], rng.standard_normal(n)).astype(np.float32)
     x += (np.sqrt(4.0 * 2e3 / n) * np.cos(2 * np.pi * (n // 8 + 0.0) * np.arange(n) / n)).astype(np.float32)
     x -= x.mean()
     got, ref = _check(x, block, mode)
