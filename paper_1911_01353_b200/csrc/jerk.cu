@@ -624,6 +624,16 @@ k_search(const __grid_constant__ SearchParams sp) {
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
+// one probe of the barrier (the answer takes ~90 cycles: start it early, use it late): 1 iff phase `parity` is complete
+__device__ __forceinline__ uint32_t mbar_probe(uint32_t bar, uint32_t parity) {
+  uint32_t done;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(done)
+      : "r"(bar), "r"(parity)
+      : "memory");
+  return done;
+}
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   uint32_t done = 0;
   while (!done) {
@@ -969,7 +979,7 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
 #pragma unroll
       for (int k1 = 0; k1 < 64; k1++) v[k1] = ex[64 * k1 + t];
       bar_sync_named(barid, NT);                         // ex is about to be reused as the exchange buffer
-      fft64_passes<-1>(v, tmT, ex, t, barid, nohook, nohook);
+      fft64_passes<-1>(v, tmT, ex, t, barid, nohook, nohook, nohook);
       bar_sync_named(barid, NT);                         // all pass-2 loads of ex done
 #pragma unroll
       for (int r = 0; r < 64; r++) ex[t + 64 * dft64_out_index(r)] = v[r];
@@ -1000,6 +1010,7 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
     }
     if (t == 0)   // G of the first template-phase of the item (ex is free: the barrier above; chunks start at phase 0)
       bulk_copy_g2s(smem_u32(ex), sp.G + (size_t)ti_n * sp.nb * L, (uint32_t)(L * 8), mbG);
+    uint32_t g_ready = 0;   // answer of the probe of mbG started before the epilogue of the previous template-phase
     for (int tp = tp_lo; tp < tp_hi; tp++) {
       const int ph = two ? (tp & 1) : 0;
       const int ti = ti_n;
@@ -1015,7 +1026,7 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
       if ((MODE == MODE_HARM || MODE == MODE_HARM_STORE) && ph == 0 && t == 0) harm_prefetch(sp, jb, s0, c, ti);
       // ---- a-3: Y = F .* G (G from the exchange buffer, F from TMEM), inverse FFT
       float2 v[P];
-      mbar_wait(mbG, tphase);
+      if (!g_ready) mbar_wait(mbG, tphase);
       __syncwarp();   // tcgen05.ld is .sync.aligned: the warp must be converged
       {
         const float4* g4 = reinterpret_cast<const float4*>(ex) + t;
@@ -1036,7 +1047,11 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
         }
       }
       mbar_arrive(mbR);
-      const auto pre = [&] { mbar_wait(mbR, tphase); };
+      uint32_t r_ready = 0;
+      const auto mid = [&] { r_ready = mbar_probe(mbR, tphase); };
+      const auto pre = [&] {
+        if (!r_ready) mbar_wait(mbR, tphase);
+      };
       const auto post = [&] {
         mbar_arrive(mbW);
         if (t == 0 && tp + 1 < tp_hi) {
@@ -1045,8 +1060,9 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
         }
         __syncwarp();
       };
-      fft64_passes<1>(v, tmT, ex, t, barid, pre, post);
+      fft64_passes<1>(v, tmT, ex, t, barid, mid, pre, post);
       tphase ^= 1u;
+      g_ready = tp + 1 < tp_hi ? mbar_probe(mbG, tphase) : 0u;   // has the next G landed?  (asked now, needed after the epilogue)
       // ---- a-4: overlap discard + power.  n = t + 64*n1 ; b = s0 + n - c ; j = 2b + ph.
       // valid outputs: n in [n_lo, n_hi) = window [hw_max, hw_max + step) clipped to the bins this call covers (32-bit: all
       // bin indices are below 2^30)

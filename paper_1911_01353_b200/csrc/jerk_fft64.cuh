@@ -221,27 +221,45 @@ __device__ __forceinline__ void bar_sync_named(int id, int nthreads) {
 
 // Both passes on the 64 points of thread t (0..63) of one FFT group.  On entry v[k1] = x[64 k1 + t]; on exit register r
 // holds X[t + 64 * dft64_out_index(r)].  ex: the group's exchange buffer (kEx64 float2); barid: its named barrier.
-// before_store() runs before the first write to ex (the caller's write-after-read protection of ex), after_load() right
+// mid() runs between the two layers of pass 1 (a cheap place to start a barrier probe whose answer before_store() needs),
+// before_store() before the first write to ex (the caller's write-after-read protection of ex), after_load() right
 // after the last read of ex.
-template <int SIGN, class TW, class PRE, class POST>
-__device__ __forceinline__ void fft64_passes(float2 (&v)[64], const TW& tw, float2* ex, int t, int barid, PRE before_store,
+// The exchange is spread over the arithmetic: each of the four second-layer columns of pass 1 is stored as soon as it is
+// done (the stores of column A issue under the butterflies of column A + 1), and the pass-2 loads are issued in the order
+// the first radix-4 layer consumes them (registers b, 16 + b, 32 + b, 48 + b), so that layer starts after four loads
+// instead of thirty-two.
+template <int SIGN, class TW, class MID, class PRE, class POST>
+__device__ __forceinline__ void fft64_passes(float2 (&v)[64], const TW& tw, float2* ex, int t, int barid, MID mid, PRE before_store,
                                              POST after_load) {
-  dft64<SIGN>(v);
-  before_store();
-  {
-    float2* w = ex + t;
 #pragma unroll
-    for (int r = 0; r < 64; r++) w[kS64 * dft64_out_index(r)] = v[r];   // element (k0 = t, n0)
+  for (int b = 0; b < 16; b++) {
+    float2 q[4] = {v[b], v[16 + b], v[32 + b], v[48 + b]};
+    Dft<4, SIGN>::run(q);
+    v[b] = q[0]; v[16 + b] = q[1]; v[32 + b] = q[2]; v[48 + b] = q[3];
   }
+  mid();
+  float2* w = ex + t;
+#define JERK_FFT64_COL(A)                                                                  \
+  dft64_stage2_col<SIGN, A>(v);                                                            \
+  if (A == 0) before_store();                                                              \
+  _Pragma("unroll") for (int k2 = 0; k2 < 16; k2++) w[kS64 * (A + 4 * k2)] = v[16 * A + k2];   /* element (k0 = t, n0 = A + 4 k2) */
+  JERK_FFT64_COL(0)
+  JERK_FFT64_COL(1)
+  JERK_FFT64_COL(2)
+  JERK_FFT64_COL(3)
+#undef JERK_FFT64_COL
   bar_sync_named(barid, 64);
   {
     const float4* rd = reinterpret_cast<const float4*>(ex + kS64 * t);
 #pragma unroll
-    for (int q = 0; q < 32; q++) {
-      const float4 x = rd[q];
-      v[2 * q] = make_float2(x.x, x.y);
-      v[2 * q + 1] = make_float2(x.z, x.w);
-    }
+    for (int p = 0; p < 8; p++)
+#pragma unroll
+      for (int a = 0; a < 4; a++) {
+        const int q = 8 * a + p;
+        const float4 x = rd[q];
+        v[2 * q] = make_float2(x.x, x.y);
+        v[2 * q + 1] = make_float2(x.z, x.w);
+      }
   }
   after_load();
   dft64_tw<SIGN>(v, tw);
