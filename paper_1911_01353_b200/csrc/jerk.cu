@@ -221,9 +221,18 @@ struct SearchJob {
   int ntp;                       // template-phases selected = 2*iz_cnt*iw_cnt
   int chunk_tp;                  // template-phases per work item (even)
   float* plane;                  // plane mode: P[iw_rel][iz_rel][j - 2*r_lo]
+  float* bmax;                   // plane mode, optional: block maxima of every (row, segment) unit, [row][seg - seg_first][kBmaxBlocks][2] (harmonic stage)
   long long item_end;            // work items of jobs 0..this one (exclusive prefix sum of nchunks*seg_count)
 };
 constexpr int kMaxJobs = 8;
+// Block maxima of a plane-mode unit (the bounds of the harmonic stage): outputs n of a unit fall into six blocks by
+// n >> 9 -> {0,1 | 2 | 3 | 4 | 5 | 6,7} (the first and last merged: the valid window [hw_max, hw_max + step) cuts them
+// short) and two halves by bit 5 of n (which warp of the FFT group owns the output).
+constexpr int kBmaxBlocks = 6;
+__host__ __device__ __forceinline__ int bmax_block(int n) {
+  const int g = (n >> 9) - 1;
+  return g < 0 ? 0 : (g > kBmaxBlocks - 1 ? kBmaxBlocks - 1 : g);
+}
 
 // Harmonic stage fused into the top-harmonic search (row a-6): sub-plane of fraction e/8, e = 1..7, as written by the
 // plane-mode kernel: P_e[iw_rel][iz_rel][j - j0], row length nj.
@@ -232,6 +241,8 @@ struct HarmGather {
   long long j0[7], nj[7];
   int iz_lo[7], iz_cnt[7], iw_lo[7];
   int cz, cw;                // centre indices (nz-1)/2, (nw-1)/2
+  const float* bmax[7];      // arg-max mode: block maxima of sub-plane e (SearchJob::bmax of the launch that stored it)
+  int seg_first[7], seg_count[7];
   float thr[4];              // arg-max mode: only sums above thr[log2 h] can be reported
   jerk_cand* warpbest;       // arg-max mode: [4][gridDim.x * warps per CTA] best record of every warp, h = 1,2,4,8
   float* out;                // store mode: S_h of the job's box, out[iw_rel][iz_rel][j - 2 r_lo]
@@ -697,115 +708,145 @@ __device__ __forceinline__ void ld_gather7(float (&g)[7], const float* const (&q
         "n"(KOFF * 4), "n"(KOFF * 5), "n"(KOFF * 6), "n"(KOFF * 7));
 }
 
-// the valid half-bin range of one (segment, template) unit -> the seven contiguous sub-plane ranges it will gather;
-// one thread asks for them to be brought into L2 (bulk prefetch) two transforms before the gathers
-__device__ __forceinline__ void harm_prefetch(const SearchParams& sp, const SearchJob& jb, int s0, int c, int ti) {
+// row pointers of the seven sub-planes for template ti, positioned at the source of point j = jt + 128 n1 + ph for
+// n1 = n1_first (see harm_unit)
+__device__ __forceinline__ void harm_pointers(const SearchParams& sp, int ti, long long jt, int n1_first, const float* (&q0)[7],
+                                              const float* (&q1)[7]) {
   const HarmGather& hg = sp.hg;
-  const long long b_lo = max((long long)jb.r_lo, (long long)s0 + sp.hw_max - c);
-  const long long b_hi = min((long long)(jb.r_lo + jb.r_cnt), (long long)s0 + sp.hw_max + sp.step - c);   // exclusive
-  if (b_hi <= b_lo) return;
   const int az = ti % sp.nz - hg.cz, aw = ti / sp.nz - hg.cw;
 #pragma unroll
   for (int e = 1; e <= 7; e++) {
     const int ize = rnd_eighths(az, e) + hg.cz, iwe = rnd_eighths(aw, e) + hg.cw;
-    const float* row = hg.base[e - 1] + ((long long)(iwe - hg.iw_lo[e - 1]) * hg.iz_cnt[e - 1] + (ize - hg.iz_lo[e - 1])) * hg.nj[e - 1] - hg.j0[e - 1];
-    const uintptr_t lo = (uintptr_t)(row + ((2 * b_lo * e + 4) >> 3)) & ~(uintptr_t)15;
-    const uintptr_t hi = ((uintptr_t)(row + (((2 * b_hi - 1) * e + 4) >> 3) + 1) + 15) & ~(uintptr_t)15;
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(lo), "r"((uint32_t)(hi - lo)) : "memory");
+    const float* row = hg.base[e - 1] + ((long long)(iwe - hg.iw_lo[e - 1]) * hg.iz_cnt[e - 1] + (ize - hg.iz_lo[e - 1])) * hg.nj[e - 1] -
+                       hg.j0[e - 1] + 16 * n1_first * e;
+    q0[e - 1] = row + ((jt * e + 4) >> 3);
+    q1[e - 1] = row + (((jt + 1) * e + 4) >> 3);
   }
 }
 
-// One batch of the gathers of harm_unit: registers k = K0 .. K0+3 (< KHI) of register group a, both phases: 14 loads per
-// register, all issued before the first sum.
-constexpr int kHarmBatch = 4;   // registers per batch: 56 loads in flight per thread (about what one warp can have outstanding)
-template <bool STORE, int K0, int KHI>
-__device__ __forceinline__ void harm_batch(const HarmGather& hg, const float* const (&q0)[7], const float* const (&q1)[7],
-                                           uint32_t tmP, const float* p1s, int a, int t, int n_lo, int n_hi,
-                                           bool inner_valid, float2* dst, float (&mx)[4]) {
-  constexpr int kB = kHarmBatch;
-  float g0[kB][7], g1[kB][7];
-  bool ok[kB];
+// One batch of the gathers of harm_unit: the four registers 16 a + k (a = 0..3) of one k, i.e. n1 = 4 k + a: 256 contiguous
+// bins, both phases: 56 loads, all issued before the first sum.  q0 / q1 point at n1 = 4 k.
+template <bool STORE>
+__device__ __forceinline__ void harm_batch(const HarmGather& hg, const float* const (&q0)[7], const float* const (&q1)[7], uint32_t tmP,
+                                           const float* p1s, int k, int t, int n_lo, int n_hi, bool inner_valid, float2* dst,
+                                           float (&mx)[4]) {
+  float g0[4][7], g1[4][7];
+  bool ok[4];
 #pragma unroll
-  for (int b = 0; b < kB; b++) {
-    if (K0 + b >= KHI) continue;
-    const int n1 = a + 4 * (K0 + b);
+  for (int a = 0; a < 4; a++) {
+    const int n1 = 4 * k + a;
     const int n = t + 64 * n1;
-    ok[b] = (inner_valid && n1 >= 8 && n1 < 56) || (n >= n_lo && n < n_hi);
+    ok[a] = (inner_valid && n1 >= 8 && n1 < 56) || (n >= n_lo && n < n_hi);
   }
-  if (K0 + 0 < KHI) { ld_gather7<256 * (K0 + 0)>(g0[0], q0); ld_gather7<256 * (K0 + 0)>(g1[0], q1); }
-  if (K0 + 1 < KHI) { ld_gather7<256 * (K0 + 1)>(g0[1], q0); ld_gather7<256 * (K0 + 1)>(g1[1], q1); }
-  if (K0 + 2 < KHI) { ld_gather7<256 * (K0 + 2)>(g0[2], q0); ld_gather7<256 * (K0 + 2)>(g1[2], q1); }
-  if (kB > 3 && K0 + 3 < KHI) { ld_gather7<256 * (K0 + 3)>(g0[kB - 1], q0); ld_gather7<256 * (K0 + 3)>(g1[kB - 1], q1); }
+  ld_gather7<64 * 0>(g0[0], q0); ld_gather7<64 * 0>(g1[0], q1);
+  ld_gather7<64 * 1>(g0[1], q0); ld_gather7<64 * 1>(g1[1], q1);
+  ld_gather7<64 * 2>(g0[2], q0); ld_gather7<64 * 2>(g1[2], q1);
+  ld_gather7<64 * 3>(g0[3], q0); ld_gather7<64 * 3>(g1[3], q1);
   // Scheduling fence: the sums sit behind a branch the compiler cannot resolve (cz >= 0 always), i.e. in another basic
   // block, so that every load of the batch is issued before the first sum waits for one (ptxas otherwise pulls each
   // sum up next to its own loads, which serialises the round trips).
-  if (hg.cz < -1 - K0) return;       // (a different condition per batch: equal ones would be merged and the batches with them)
-  constexpr int KB = K0 > 12 ? 12 : K0;   // four columns that hold the batch and stay inside the 16 of this register group
+  if (hg.cz < 0) return;
   float p0c[4];
-  tmem_ld4(tmP + 16 * a + KB, p0c);   // the powers of this unit: phase 0 from tensor memory, phase 1 from shared memory
+  tmem_ld1x4(tmP + k, p0c);   // the powers of this batch: phase 0 from tensor memory (columns 16 a + k), phase 1 from shared memory
 #pragma unroll
-  for (int b = 0; b < kB; b++) {
-    const int k = K0 + b;
-    if (k >= KHI) continue;
-    const int n1 = a + 4 * k;
+  for (int a = 0; a < 4; a++) {
     float sa[4], sb[4];
-    harm_stage_sums(p0c[k - KB], g0[b], sa);
-    harm_stage_sums(p1s[(16 * a + k) * 64 + t], g1[b], sb);
+    harm_stage_sums(p0c[a], g0[a], sa);
+    harm_stage_sums(p1s[(16 * a + k) * 64 + t], g1[a], sb);
     if (STORE) {
-      if (ok[b]) dst[64 * n1] = make_float2(sa[hg.out_stage], sb[hg.out_stage]);
-    } else if (ok[b]) {
+      if (ok[a]) dst[64 * (4 * k + a)] = make_float2(sa[hg.out_stage], sb[hg.out_stage]);
+    } else if (ok[a]) {
 #pragma unroll
       for (int q = 0; q < 4; q++) mx[q] = fmaxf(mx[q], fmaxf(sa[q], sb[q]));
     }
   }
 }
 
-// One (segment, template) unit of the top-harmonic pass, called when phase 1 is done.  Phase-0 powers are in tensor
-// memory at tmP, phase-1 powers in shared memory p1s (register r of thread t at r*64 + t; both written and read by the
-// same thread); register r = 16 a + k holds n = t + 64 n1, n1 = a + 4 k.  Point j = 2 (s0 + n - c) + ph reads sub-plane e
-// at (j e + 4) >> 3 = ((jt e + 4) >> 3) + 16 n1 e with jt = 2 (s0 - c + t) + ph: one pointer per (fraction, phase), moved
-// on by 16 e per a, and compile-time offsets 64 k e.  The loop over a is rolled: the unrolled version (5000
-// instructions on top of the transforms) thrashed the instruction cache (no_instruction stalls 1.2 per issue).
-template <bool STORE, bool PRUNE>
-__device__ __forceinline__ void harm_unit(const SearchParams& sp, const SearchJob& jb, const float* p1s, uint32_t tmP, int t, int lane,
-                                          int s0, int c, int ti, int box_row, int n_lo, int n_hi, HarmRecord* rec, float* stash) {
+// Can any sum of this warp over the top bins n in [256 kp, 256 kp + 512) reach the warp's record?  Upper bound of S_h:
+// the thread's own largest power there (pm) plus, per fraction e, the largest stored power its sources can come from.
+// The <= 449 + 1 source bins of a fraction lie in at most two blocks of the producer's block maxima (each block is at
+// least 512 outputs long, SearchJob::bmax), those of the first and of the last source bin, times two halves: four
+// values per fraction, fetched by 28 lanes in parallel.  Exact pruning: a pair of batches is skipped only if every
+// stage's bound stays below the record (initially the stage threshold), so no arg-max or tie can be lost.
+__device__ __forceinline__ bool harm_bounds_need(const SearchParams& sp, int s0, int c, int ti, int kp, int n_lo, int n_hi, int lane,
+                                                 float pm, const HarmRecord* rec) {
   const HarmGather& hg = sp.hg;
+  const int n_first = max(256 * kp, n_lo), n_last = min(256 * kp + 511, n_hi - 1);
+  if (n_last < n_first) return false;                     // no valid point in this pair of batches
+  float val = 0.f;
+  if (lane < 28) {
+    const int e = (lane >> 2) + 1, slot = lane & 3;
+    const long long j = (slot & 2) ? 2LL * (s0 - c + n_last) + 1 : 2LL * (s0 - c + n_first);
+    const int x = (int)(((j * e + 4) >> 3) >> 1);           // source bin of the first / last point
+    const int az = ti % sp.nz - hg.cz, aw = ti / sp.nz - hg.cw;
+    const int ize = rnd_eighths(az, e) + hg.cz, iwe = rnd_eighths(aw, e) + hg.cw;
+    const int cs = sp.geom[iwe * sp.nz + ize].c;
+    const int row = (iwe - hg.iw_lo[e - 1]) * hg.iz_cnt[e - 1] + (ize - hg.iz_lo[e - 1]);
+    const int u = x + cs - (int)sp.seg_base - sp.hw_max;     // the unit that owns bin x of this template: segment u / step, output n
+    const int seg = u / sp.step;
+    const int n = u - seg * sp.step + sp.hw_max;
+    val = __ldg(hg.bmax[e - 1] + ((((size_t)row * hg.seg_count[e - 1] + (seg - hg.seg_first[e - 1])) * kBmaxBlocks + bmax_block(n)) << 1) + (slot & 1));
+  }
+  val = fmaxf(val, __shfl_xor_sync(0xffffffffu, val, 1));
+  val = fmaxf(val, __shfl_xor_sync(0xffffffffu, val, 2));   // lanes 4 (e - 1) .. 4 (e - 1) + 3 hold the bound of fraction e
+  float be[7];
+#pragma unroll
+  for (int e = 1; e <= 7; e++) be[e - 1] = __shfl_sync(0xffffffffu, val, 4 * (e - 1));
+  float ub[4];
+  harm_stage_sums(pm, be, ub);
+  bool need = false;
+#pragma unroll
+  for (int q = 0; q < 4; q++) need |= ub[q] >= rec[q].s;
+  return __any_sync(0xffffffffu, need);
+}
+
+// One (segment, template) unit of the top-harmonic pass, called when phase 1 is done.  Phase-0 powers are in tensor
+// memory at tmP, phase-1 powers in shared memory p1s (register r of thread t at r*64 + t), the per-thread maxima of both
+// phases over the four registers of every k in pms[k*64 + t] (all written and read by the same thread); register
+// r = 16 a + k holds n = t + 64 n1, n1 = 4 k + a... see harm_batch.  Point j = 2 (s0 - c + n) + ph reads sub-plane e at
+// (j e + 4) >> 3 = ((jt e + 4) >> 3) + 16 n1 e with jt = 2 (s0 - c + t) + ph: one pointer per (fraction, phase), moved
+// on by 64 e per k.  The loop over k is rolled (an unrolled gather body of 5000 instructions on top of the transforms
+// thrashed the instruction cache: no_instruction stalls 1.2 per issue).
+template <bool STORE, bool PRUNE>
+__device__ __forceinline__ void harm_unit(const SearchParams& sp, const SearchJob& jb, const float* p1s, const float* pms, uint32_t tmP, int t,
+                                          int lane, int s0, int c, int ti, int box_row, int n_lo, int n_hi, HarmRecord* rec, float* stash) {
+  const HarmGather& hg = sp.hg;
+  constexpr int KLO = PRUNE ? 1 : 0, KHI = PRUNE ? 15 : 16;   // PRUNE: k = 0 and 15 (n1 < 4, n1 >= 60) are never valid
+  const long long jt = 2LL * (s0 - c + t);
   const float* q0[7];
   const float* q1[7];
-  {
-    const int az = ti % sp.nz - hg.cz, aw = ti / sp.nz - hg.cw;
-    const long long jt = 2LL * (s0 - c + t);
-#pragma unroll
-    for (int e = 1; e <= 7; e++) {
-      const int ize = rnd_eighths(az, e) + hg.cz, iwe = rnd_eighths(aw, e) + hg.cw;
-      const float* row = hg.base[e - 1] + ((long long)(iwe - hg.iw_lo[e - 1]) * hg.iz_cnt[e - 1] + (ize - hg.iz_lo[e - 1])) * hg.nj[e - 1] -
-                         hg.j0[e - 1];
-      q0[e - 1] = row + ((jt * e + 4) >> 3);
-      q1[e - 1] = row + (((jt + 1) * e + 4) >> 3);
-    }
-  }
+  bool have = false;
+  int kq = 0;
   // registers with n1 = n / 64 in [8, 56) are valid for every thread of a segment inside the box (hw_max <= 512)
   const bool inner_valid = __all_sync(0xffffffffu, n_lo <= t + 64 * 8 && n_hi >= t + 64 * 56);
   float2* dst = nullptr;
   if (STORE) dst = reinterpret_cast<float2*>(hg.out + (size_t)box_row * (size_t)(2 * jb.r_cnt) + 2 * (ptrdiff_t)(s0 - c - (int)jb.r_lo + t));
   float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
-  // The gathers are latency-bound (two warps per scheduler, every register busy during the transforms): they are issued
-  // in batches of kB registers = 14 kB independent loads (about the number of loads one warp can have outstanding),
-  // all of a batch before the first sum.
-  constexpr int KLO = PRUNE ? 1 : 0, KHI = PRUNE ? 15 : 16;   // PRUNE: k = 0 and 15 (n1 < 4, n1 >= 60) are never valid
+  // The gathers cost far more than the transforms (896 four-byte loads per thread and template through one L1 pipe per SM:
+  // ~15 us per template and SM against 6.4 us of arithmetic), so in arg-max mode they are done only for the pairs of
+  // batches whose bound (harm_bounds_need) can reach the record.  In batches of 56 independent loads per thread (about
+  // what one warp can have outstanding), all issued before the first sum.
 #pragma unroll 1
-  for (int a = 0; a < 4; a++) {
-    harm_batch<STORE, KLO, KHI>(hg, q0, q1, tmP, p1s, a, t, n_lo, n_hi, inner_valid, dst, mx);
-    harm_batch<STORE, KLO + kHarmBatch, KHI>(hg, q0, q1, tmP, p1s, a, t, n_lo, n_hi, inner_valid, dst, mx);
-    harm_batch<STORE, KLO + 2 * kHarmBatch, KHI>(hg, q0, q1, tmP, p1s, a, t, n_lo, n_hi, inner_valid, dst, mx);
-    harm_batch<STORE, KLO + 3 * kHarmBatch, KHI>(hg, q0, q1, tmP, p1s, a, t, n_lo, n_hi, inner_valid, dst, mx);
-    if (KLO + 4 * kHarmBatch < KHI) harm_batch<STORE, KLO + 4 * kHarmBatch, KHI>(hg, q0, q1, tmP, p1s, a, t, n_lo, n_hi, inner_valid, dst, mx);
-    if (KLO + 5 * kHarmBatch < KHI) harm_batch<STORE, KLO + 5 * kHarmBatch, KHI>(hg, q0, q1, tmP, p1s, a, t, n_lo, n_hi, inner_valid, dst, mx);
+  for (int kp = KLO; kp < KHI; kp += 2) {
+    if (!STORE && !harm_bounds_need(sp, s0, c, ti, kp, n_lo, n_hi, lane, fmaxf(pms[kp * 64 + t], pms[(kp + 1) * 64 + t]), rec)) continue;
+    if (!have) {
+      harm_pointers(sp, ti, jt, 4 * kp, q0, q1);
+      have = true;
+    } else {
+#pragma unroll
+      for (int e = 1; e <= 7; e++) {
+        q0[e - 1] += 64 * e * (kp - kq);
+        q1[e - 1] += 64 * e * (kp - kq);
+      }
+    }
+    harm_batch<STORE>(hg, q0, q1, tmP, p1s, kp, t, n_lo, n_hi, inner_valid, dst, mx);
 #pragma unroll
     for (int e = 1; e <= 7; e++) {
-      q0[e - 1] += 16 * e;
-      q1[e - 1] += 16 * e;
+      q0[e - 1] += 64 * e;
+      q1[e - 1] += 64 * e;
     }
+    harm_batch<STORE>(hg, q0, q1, tmP, p1s, kp + 1, t, n_lo, n_hi, inner_valid, dst, mx);
+    kq = kp + 1;     // where the pointers stand
   }
   if (STORE) return;
   // Arg-max.  Hot path: four running maxima per thread and one vote per unit.  Only when some sum of this warp reaches
@@ -814,11 +855,7 @@ __device__ __forceinline__ void harm_unit(const SearchParams& sp, const SearchJo
 #pragma unroll
   for (int q = 0; q < 4; q++) trig |= mx[q] >= rec[q].s;
   if (!__any_sync(0xffffffffu, trig)) return;
-#pragma unroll
-  for (int e = 1; e <= 7; e++) {
-    q0[e - 1] -= 64 * e;
-    q1[e - 1] -= 64 * e;
-  }
+  harm_pointers(sp, ti, jt, 0, q0, q1);
   float* st0 = stash;          // [64][64] phase-0 powers, register r of thread t at r*64 + t (written and read by the same thread)
 #pragma unroll 1
   for (int a = 0; a < 4; a++) {
@@ -832,7 +869,6 @@ __device__ __forceinline__ void harm_unit(const SearchParams& sp, const SearchJo
   int bj[4] = {-1, -1, -1, -1};
 #pragma unroll
   for (int q = 0; q < 4; q++) bs[q] = hg.thr[q];
-  const int jt = 2 * (s0 - c + t);
 #pragma unroll 1
   for (int r = 0; r < 64; r++) {
     const int n1 = dft64_out_index(r);
@@ -846,7 +882,7 @@ __device__ __forceinline__ void harm_unit(const SearchParams& sp, const SearchJo
       for (int e = 1; e <= 7; e++) g[e - 1] = __ldg((ph ? q1[e - 1] : q0[e - 1]) + 16 * n1 * e);
       float sv[4];
       harm_stage_sums(p8, g, sv);
-      const int j = jt + 128 * n1 + ph;
+      const int j = (int)jt + 128 * n1 + ph;
 #pragma unroll
       for (int q = 0; q < 4; q++)
         if (sv[q] > bs[q] || (sv[q] == bs[q] && bj[q] >= 0 && j < bj[q])) {   // only sums above the threshold; ties -> smallest j
@@ -902,6 +938,7 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, grp = warp >> 1, t = threadIdx.x & 63;
   float2* ex = ex_all + grp * kEx64;
   float* p1s = reinterpret_cast<float*>(mbar_all + 4 * NG) + grp * (P * NT);   // harmonic modes: [P][NT] phase-1 powers of the group
+  float* pms = reinterpret_cast<float*>(mbar_all + 4 * NG) + NG * (P * NT) + grp * (16 * NT);   // and [16][NT] per-thread maxima of every k
   const uint32_t mbS = smem_u32(mbar_all + 4 * grp);   // segment copy landed (tx)
   const uint32_t mbG = mbS + 8;                        // G copy landed (tx)
   const uint32_t mbR = mbS + 16;                       // all 64 threads have read G out of ex
@@ -1023,7 +1060,6 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
           ti_n += sp.nz - iz_cnt;
         }
       }
-      if ((MODE == MODE_HARM || MODE == MODE_HARM_STORE) && ph == 0 && t == 0) harm_prefetch(sp, jb, s0, c, ti);
       // ---- a-3: Y = F .* G (G from the exchange buffer, F from TMEM), inverse FFT
       float2 v[P];
       if (!g_ready) mbar_wait(mbG, tphase);
@@ -1084,6 +1120,10 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
           for (int i = 0; i < 32; i++) q32[i] = pw[32 * h + i];
           tmem_st32(tmP + 32 * h, q32);
         }
+        if (MODE == MODE_HARM) {   // the largest phase-0 power of the four registers 16 a + k of every k (bounds of harm_unit)
+#pragma unroll
+          for (int k = 0; k < 16; k++) pms[k * NT + t] = fmaxf(fmaxf(pw[k], pw[16 + k]), fmaxf(pw[32 + k], pw[48 + k]));
+        }
       } else if (MODE == MODE_PLANE && !two) {
         // numbetween = 1: one float per bin, row index = template
         float* dst = jb.plane + (size_t)tp * (size_t)jb.r_cnt + (ptrdiff_t)(s0 - c - (int)jb.r_lo + t);
@@ -1103,6 +1143,9 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
         // registers with n1 = n / 64 in [8, 56) are valid for every thread of a segment inside the box (hw_max <= 512):
         // no predicate; registers known to be outside every window (PRUNE) are skipped
         const bool inner_valid = __all_sync(0xffffffffu, n_lo <= t + 64 * 8 && n_hi >= t + 64 * 56);
+        float bm[kBmaxBlocks];   // block maxima of this thread's valid outputs (both phases); powers are >= 0
+#pragma unroll
+        for (int g = 0; g < kBmaxBlocks; g++) bm[g] = 0.f;
 #pragma unroll
         for (int h = 0; h < 2; h++) {
           float p0c[32];
@@ -1114,13 +1157,34 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
             const int n1 = dft64_out_index(r);
             const int n = t + 64 * n1;
             const bool ok = (inner_valid && n1 >= 8 && n1 < 56) || (n >= n_lo && n < n_hi);
-            if (ok) dst[64 * n1] = make_float2(p0c[i], pw[r]);
+            if (ok) {
+              dst[64 * n1] = make_float2(p0c[i], pw[r]);
+              bm[bmax_block(64 * n1)] = fmaxf(bm[bmax_block(64 * n1)], fmaxf(p0c[i], pw[r]));
+            }
+          }
+        }
+        if (jb.bmax) {   // one value per (row, segment, block, warp of the group): plain stores, every entry has one owner
+#pragma unroll
+          for (int g = 0; g < kBmaxBlocks; g++) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) bm[g] = fmaxf(bm[g], __shfl_xor_sync(0xffffffffu, bm[g], o));
+          }
+          if (lane < kBmaxBlocks) {
+            float mine = bm[0];
+#pragma unroll
+            for (int g = 1; g < kBmaxBlocks; g++) mine = lane == g ? bm[g] : mine;
+            jb.bmax[((((size_t)(tp >> 1) * jb.seg_count + (wi.seg - jb.seg_first)) * kBmaxBlocks + lane) << 1) + (warp & 1)] = mine;
           }
         }
       } else if (MODE == MODE_HARM || MODE == MODE_HARM_STORE) {
 #pragma unroll
         for (int r = 0; r < P; r++) p1s[r * NT + t] = pw[r];
-        harm_unit<MODE == MODE_HARM_STORE, PRUNE>(sp, jb, p1s, tmP, t, lane, s0, c, ti, tp >> 1, n_lo, n_hi, s_rec[warp],
+        if (MODE == MODE_HARM) {
+#pragma unroll
+          for (int k = 0; k < 16; k++)
+            pms[k * NT + t] = fmaxf(pms[k * NT + t], fmaxf(fmaxf(pw[k], pw[16 + k]), fmaxf(pw[32 + k], pw[48 + k])));
+        }
+        harm_unit<MODE == MODE_HARM_STORE, PRUNE>(sp, jb, p1s, pms, tmP, t, lane, s0, c, ti, tp >> 1, n_lo, n_hi, s_rec[warp],
                                                    sp.stash + ((size_t)blockIdx.x * NG + grp) * (2 * L));
       } else {
         if (MODE == MODE_CAND_STATS) {
@@ -1636,7 +1700,7 @@ struct K64 {
   static constexpr int NG = (MODE == MODE_CAND || MODE == MODE_CAND_STATS) ? 2 : 4;
   static constexpr int CTAS_PER_SM = NG == 2 ? 2 : 1;
   static constexpr size_t SMEM = (size_t)NG * kEx64 * sizeof(float2) + 4 * NG * sizeof(unsigned long long) +
-                                 ((MODE == MODE_HARM || MODE == MODE_HARM_STORE) ? (size_t)NG * 64 * 64 * sizeof(float) : 0);   // + phase-1 powers
+                                 ((MODE == MODE_HARM || MODE == MODE_HARM_STORE) ? (size_t)NG * (64 + 16) * 64 * sizeof(float) : 0);   // + phase-1 powers, per-k maxima
 };
 
 // CTAs of a k_search64 launch: every SM full, never more FFT groups than stash slots or work items
@@ -1736,20 +1800,28 @@ static bool bank_covers(const jerk_plan* p, int iz_lo, int iz_cnt, int iw_lo, in
   return first >= p->bank_ti_lo && last < p->bank_ti_lo + p->bank_ti_cnt;
 }
 
-// Appends the box (r, iz, iw) as a job of `sp` (sp.nb and sp.nspec must be set).  Returns false when the box is empty (nothing appended).
-// Segments whose outputs b = s0 + n - c (n in [hw_max, hw_max+step), |c| <= c_max) can touch [r_lo, r_lo+r_cnt) are selected.
-static bool add_job(const jerk_plan* p, SearchParams& sp, int64_t r_lo, int64_t r_cnt, int iz_lo, int iz_cnt, int iw_lo,
-                    int iw_cnt, float* plane, int chunk_tp) {
-  if (r_cnt <= 0 || iz_cnt <= 0 || iw_cnt <= 0 || sp.njobs >= kMaxJobs) return false;
+// segments whose outputs b = s0 + n - c (n in [hw_max, hw_max+step), |c| <= c_max) can touch bins [r_lo, r_lo+r_cnt)
+static void job_segments(const jerk_plan* p, int64_t r_lo, int64_t r_cnt, int64_t* first, int64_t* count) {
   int64_t lo = r_lo - p->c_max - p->seg_base - p->hw_max - p->step + 1;  // s*step >= lo
   int64_t hi = r_lo + r_cnt - 1 + p->c_max - p->seg_base - p->hw_max;    // s*step <= hi
   int64_t s_first = lo <= 0 ? 0 : (lo + p->step - 1) / p->step;
   int64_t s_last = hi < 0 ? -1 : hi / p->step;
   if (s_last > p->nseg - 1) s_last = p->nseg - 1;
-  if (s_last < s_first) return false;
+  *first = s_first;
+  *count = s_last < s_first ? 0 : s_last - s_first + 1;
+}
+
+// Appends the box (r, iz, iw) as a job of `sp` (sp.nb and sp.nspec must be set).  Returns false when the box is empty (nothing appended).
+// Segments whose outputs b = s0 + n - c (n in [hw_max, hw_max+step), |c| <= c_max) can touch [r_lo, r_lo+r_cnt) are selected.
+static bool add_job(const jerk_plan* p, SearchParams& sp, int64_t r_lo, int64_t r_cnt, int iz_lo, int iz_cnt, int iw_lo,
+                    int iw_cnt, float* plane, int chunk_tp) {
+  if (r_cnt <= 0 || iz_cnt <= 0 || iw_cnt <= 0 || sp.njobs >= kMaxJobs) return false;
+  int64_t s_first, s_count;
+  job_segments(p, r_lo, r_cnt, &s_first, &s_count);
+  if (s_count == 0) return false;
   SearchJob& jb = sp.jobs[sp.njobs];
   jb.seg_first = s_first;
-  jb.seg_count = s_last - s_first + 1;
+  jb.seg_count = s_count;
   jb.r_lo = r_lo;
   jb.r_cnt = r_cnt;
   jb.iz_lo = iz_lo;
@@ -1759,6 +1831,7 @@ static bool add_job(const jerk_plan* p, SearchParams& sp, int64_t r_lo, int64_t 
   jb.ntp = sp.nb * iz_cnt * iw_cnt;
   jb.chunk_tp = chunk_tp;
   jb.plane = plane;
+  jb.bmax = nullptr;
   long long nchunks = (jb.ntp + chunk_tp - 1) / chunk_tp;
   sp.nitems += nchunks * jb.seg_count * sp.nspec;
   jb.item_end = sp.nitems;
@@ -2217,6 +2290,8 @@ struct HarmSubBox {       // source box of fraction e/8
   int64_t r_lo, r_cnt;
   int iz_lo, iz_cnt, iw_lo, iw_cnt;
   uint64_t offset, bytes;  // inside the scratch buffer
+  int64_t seg_first, seg_count;     // segments of the launch that stores it
+  uint64_t bmax_offset;             // block maxima [row][seg][kBmaxBlocks][2] (fused path)
 };
 
 static int host_rnd_eighths(int a, int e) {
@@ -2246,7 +2321,15 @@ static uint64_t harm_layout(const jerk_plan* p, const HarmBox& bx, HarmSubBox (&
     sb.bytes = (fused && e == 8) ? 0 : align_up((uint64_t)sb.iw_cnt * sb.iz_cnt * (uint64_t)(2 * sb.r_cnt) * sizeof(float), 256);
     off += sb.bytes;
   }
-  if (fused) off += kHarmGuard;
+  if (fused) {
+    off += kHarmGuard;
+    for (int e = 1; e <= 7; e++) {      // block maxima of the stored sub-planes: the bounds of the top-harmonic pass
+      HarmSubBox& sb = sub[e - 1];
+      job_segments(p, sb.r_lo, sb.r_cnt, &sb.seg_first, &sb.seg_count);
+      sb.bmax_offset = off;
+      off += align_up((uint64_t)sb.iw_cnt * sb.iz_cnt * (uint64_t)sb.seg_count * kBmaxBlocks * 2 * sizeof(float), 256);
+    }
+  }
   *ntiles = (int)((2 * bx.r_cnt + kHarmJTile - 1) / kHarmJTile);
   *nblocks = fused ? kStashSlots * 2 : bx.iw_cnt * bx.iz_cnt * *ntiles;      // fused: an upper bound on the warps of the launch
   *best_off = off;
@@ -2274,6 +2357,7 @@ static int harm_box(jerk_plan* p, const void* d_spec, const HarmBox& bx, unsigne
     float* plane = (float*)(scratch + sb.offset);
     if (!add_job(p, sp, sb.r_lo, sb.r_cnt, sb.iz_lo, sb.iz_cnt, sb.iw_lo, sb.iw_cnt, plane, kChunkTP))
       return fail(p, JERK_EINVAL, "harmonic stage: empty sub-box");
+    if (fused && !d_out) sp.jobs[sp.njobs - 1].bmax = (float*)(scratch + sb.bmax_offset);
     hp.sub[e - 1].base = plane;
     hp.sub[e - 1].j0 = 2 * sb.r_lo;
     hp.sub[e - 1].nj = 2 * sb.r_cnt;
@@ -2313,6 +2397,11 @@ static int harm_box(jerk_plan* p, const void* d_spec, const HarmBox& bx, unsigne
       hg.iz_lo[f] = hp.sub[f].iz_lo;
       hg.iz_cnt[f] = hp.sub[f].iz_cnt;
       hg.iw_lo[f] = hp.sub[f].iw_lo;
+    }
+    for (int f = 0; f < 7; f++) {
+      hg.bmax[f] = (const float*)(scratch + sub[f].bmax_offset);
+      hg.seg_first[f] = (int)sub[f].seg_first;
+      hg.seg_count[f] = (int)sub[f].seg_count;
     }
     hg.cz = (p->nz - 1) / 2;
     hg.cw = (p->nw - 1) / 2;

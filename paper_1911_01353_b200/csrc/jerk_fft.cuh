@@ -373,6 +373,19 @@ __device__ __forceinline__ void tmem_ld4(uint32_t taddr, float (&r)[4]) {
       : "memory");
 }
 
+// four single columns taddr, taddr + 16, taddr + 32, taddr + 48 of the thread's lane
+__device__ __forceinline__ void tmem_ld1x4(uint32_t taddr, float (&r)[4]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%4];\n\t"
+      "tcgen05.ld.sync.aligned.32x32b.x1.b32 {%1}, [%5];\n\t"
+      "tcgen05.ld.sync.aligned.32x32b.x1.b32 {%2}, [%6];\n\t"
+      "tcgen05.ld.sync.aligned.32x32b.x1.b32 {%3}, [%7];\n\t"
+      "tcgen05.wait::ld.sync.aligned;"
+      : "=f"(r[0]), "=f"(r[1]), "=f"(r[2]), "=f"(r[3])
+      : "r"(taddr), "r"(taddr + 16), "r"(taddr + 32), "r"(taddr + 48)
+      : "memory");
+}
+
 // A thread-private array of P complex values (P = 16 or 32) held in TMEM columns [addr, addr + 2P) of the thread's lane.
 // load16(h, o) / store16(h, o) move entries 16h .. 16h+15; load8(i, o) entries 8i .. 8i+7.
 template <int L>
