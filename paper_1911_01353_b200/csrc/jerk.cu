@@ -762,42 +762,67 @@ __device__ __forceinline__ void harm_batch(const HarmGather& hg, const float* co
   }
 }
 
-// Can any sum of this warp over the top bins n in [256 kp, 256 kp + 512) reach the warp's record?  Upper bound of S_h:
-// the thread's own largest power there (pm) plus, per fraction e, the largest stored power its sources can come from.
-// The <= 449 + 1 source bins of a fraction lie in at most two blocks of the producer's block maxima (each block is at
-// least 512 outputs long, SearchJob::bmax), those of the first and of the last source bin, times two halves: four
-// values per fraction, fetched by 28 lanes in parallel.  Exact pruning: a pair of batches is skipped only if every
-// stage's bound stays below the record (initially the stage threshold), so no arg-max or tie can be lost.
-__device__ __forceinline__ bool harm_bounds_need(const SearchParams& sp, int s0, int c, int ti, int kp, int n_lo, int n_hi, int lane,
-                                                 float pm, const HarmRecord* rec) {
+// Which pairs of batches (top bins n in [256 kp, 256 kp + 512), kp = KLO, KLO + 2, ...) can hold a sum that reaches the
+// warp's record?  Upper bound of S_h over a pair: the thread's own largest power there (pms) plus, per fraction e, the
+// largest stored power its sources can come from.  The <= 449 + 1 source bins of a fraction lie in at most two blocks of
+// the producer's block maxima (each block is at least 512 outputs long, SearchJob::bmax), those of the first and of the
+// last source bin, times two halves: four values per fraction, fetched by 28 lanes in parallel, for all pairs at once
+// (one round trip per template instead of one per pair).  Exact pruning: a pair is skipped only if every stage's bound
+// stays below the record (initially the stage threshold), so no arg-max or tie can be lost.  Bit i of the result: pair i.
+template <int KLO, int KHI>
+__device__ __forceinline__ uint32_t harm_bounds_mask(const SearchParams& sp, int s0, int c, int ti, int n_lo, int n_hi, int lane, int t,
+                                                     const float* pms, float* scr, const HarmRecord* rec) {
+  constexpr int NP = (KHI - KLO) / 2;
   const HarmGather& hg = sp.hg;
-  const int n_first = max(256 * kp, n_lo), n_last = min(256 * kp + 511, n_hi - 1);
-  if (n_last < n_first) return false;                     // no valid point in this pair of batches
-  float val = 0.f;
-  if (lane < 28) {
-    const int e = (lane >> 2) + 1, slot = lane & 3;
-    const long long j = (slot & 2) ? 2LL * (s0 - c + n_last) + 1 : 2LL * (s0 - c + n_first);
-    const int x = (int)(((j * e + 4) >> 3) >> 1);           // source bin of the first / last point
+  float val[NP];
+  {
+    const int e = min((lane >> 2) + 1, 7), slot = lane & 3;
     const int az = ti % sp.nz - hg.cz, aw = ti / sp.nz - hg.cw;
     const int ize = rnd_eighths(az, e) + hg.cz, iwe = rnd_eighths(aw, e) + hg.cw;
     const int cs = sp.geom[iwe * sp.nz + ize].c;
-    const int row = (iwe - hg.iw_lo[e - 1]) * hg.iz_cnt[e - 1] + (ize - hg.iz_lo[e - 1]);
-    const int u = x + cs - (int)sp.seg_base - sp.hw_max;     // the unit that owns bin x of this template: segment u / step, output n
-    const int seg = u / sp.step;
-    const int n = u - seg * sp.step + sp.hw_max;
-    val = __ldg(hg.bmax[e - 1] + ((((size_t)row * hg.seg_count[e - 1] + (seg - hg.seg_first[e - 1])) * kBmaxBlocks + bmax_block(n)) << 1) + (slot & 1));
+    const float* bm = hg.bmax[e - 1] + (size_t)((iwe - hg.iw_lo[e - 1]) * hg.iz_cnt[e - 1] + (ize - hg.iz_lo[e - 1])) * hg.seg_count[e - 1] * (kBmaxBlocks * 2) +
+                      (slot & 1);
+    const int segf = hg.seg_first[e - 1];
+#pragma unroll
+    for (int i = 0; i < NP; i++) {
+      const int kp = KLO + 2 * i;
+      const int n_first = max(256 * kp, n_lo), n_last = min(256 * kp + 511, n_hi - 1);
+      val[i] = 0.f;
+      if (n_last >= n_first && lane < 28) {
+        const long long j = (slot & 2) ? 2LL * (s0 - c + n_last) + 1 : 2LL * (s0 - c + n_first);
+        const int x = (int)(((j * e + 4) >> 3) >> 1);           // source bin of the first / last point of the pair
+        const int u = x + cs - (int)sp.seg_base - sp.hw_max;     // the unit that owns bin x of this template: segment u / step, output n
+        const int seg = u / sp.step;
+        const int n = u - seg * sp.step + sp.hw_max;
+        val[i] = __ldg(bm + ((seg - segf) * kBmaxBlocks + bmax_block(n)) * 2);
+      }
+    }
   }
-  val = fmaxf(val, __shfl_xor_sync(0xffffffffu, val, 1));
-  val = fmaxf(val, __shfl_xor_sync(0xffffffffu, val, 2));   // lanes 4 (e - 1) .. 4 (e - 1) + 3 hold the bound of fraction e
-  float be[7];
+  // evaluation, rolled over the pairs (the values go through shared memory: scr[i*64 + t] is this thread's own slot)
 #pragma unroll
-  for (int e = 1; e <= 7; e++) be[e - 1] = __shfl_sync(0xffffffffu, val, 4 * (e - 1));
-  float ub[4];
-  harm_stage_sums(pm, be, ub);
-  bool need = false;
+  for (int i = 0; i < NP; i++) scr[i * 64 + t] = val[i];
+  float recs[4];
 #pragma unroll
-  for (int q = 0; q < 4; q++) need |= ub[q] >= rec[q].s;
-  return __any_sync(0xffffffffu, need);
+  for (int q = 0; q < 4; q++) recs[q] = rec[q].s;
+  uint32_t mask = 0;
+#pragma unroll 1
+  for (int i = 0; i < NP; i++) {
+    const int kp = KLO + 2 * i;
+    float v = scr[i * 64 + t];
+    v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 1));
+    v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 2));   // lanes 4 (e - 1) .. 4 (e - 1) + 3 hold the bound of fraction e
+    float be[7];
+#pragma unroll
+    for (int e = 1; e <= 7; e++) be[e - 1] = __shfl_sync(0xffffffffu, v, 4 * (e - 1));
+    float ub[4];
+    harm_stage_sums(fmaxf(pms[kp * 64 + t], pms[(kp + 1) * 64 + t]), be, ub);
+    bool need = false;
+#pragma unroll
+    for (int q = 0; q < 4; q++) need |= ub[q] >= recs[q];
+    const bool any_valid = min(256 * kp + 511, n_hi - 1) >= max(256 * kp, n_lo);
+    if (any_valid && __any_sync(0xffffffffu, need)) mask |= 1u << i;
+  }
+  return mask;
 }
 
 // One (segment, template) unit of the top-harmonic pass, called when phase 1 is done.  Phase-0 powers are in tensor
@@ -808,8 +833,9 @@ __device__ __forceinline__ bool harm_bounds_need(const SearchParams& sp, int s0,
 // on by 64 e per k.  The loop over k is rolled (an unrolled gather body of 5000 instructions on top of the transforms
 // thrashed the instruction cache: no_instruction stalls 1.2 per issue).
 template <bool STORE, bool PRUNE>
-__device__ __forceinline__ void harm_unit(const SearchParams& sp, const SearchJob& jb, const float* p1s, const float* pms, uint32_t tmP, int t,
-                                          int lane, int s0, int c, int ti, int box_row, int n_lo, int n_hi, HarmRecord* rec, float* stash) {
+__device__ __forceinline__ void harm_unit(const SearchParams& sp, const SearchJob& jb, const float (&pw)[64], float* p1s, const float* pms,
+                                          uint32_t tmP, int t, int lane, int s0, int c, int ti, int box_row, int n_lo, int n_hi,
+                                          HarmRecord* rec, float* stash) {
   const HarmGather& hg = sp.hg;
   constexpr int KLO = PRUNE ? 1 : 0, KHI = PRUNE ? 15 : 16;   // PRUNE: k = 0 and 15 (n1 < 4, n1 >= 60) are never valid
   const long long jt = 2LL * (s0 - c + t);
@@ -826,9 +852,13 @@ __device__ __forceinline__ void harm_unit(const SearchParams& sp, const SearchJo
   // ~15 us per template and SM against 6.4 us of arithmetic), so in arg-max mode they are done only for the pairs of
   // batches whose bound (harm_bounds_need) can reach the record.  In batches of 56 independent loads per thread (about
   // what one warp can have outstanding), all issued before the first sum.
+  const uint32_t need = STORE ? 0xffffffffu : harm_bounds_mask<KLO, KHI>(sp, s0, c, ti, n_lo, n_hi, lane, t, pms, p1s, rec);
+  if (need == 0) return;
+#pragma unroll
+  for (int r = 0; r < 64; r++) p1s[r * 64 + t] = pw[r];   // phase-1 powers: only for the units that gather
 #pragma unroll 1
   for (int kp = KLO; kp < KHI; kp += 2) {
-    if (!STORE && !harm_bounds_need(sp, s0, c, ti, kp, n_lo, n_hi, lane, fmaxf(pms[kp * 64 + t], pms[(kp + 1) * 64 + t]), rec)) continue;
+    if (!((need >> ((kp - KLO) >> 1)) & 1u)) continue;
     if (!have) {
       harm_pointers(sp, ti, jt, 4 * kp, q0, q1);
       have = true;
@@ -1177,14 +1207,12 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
           }
         }
       } else if (MODE == MODE_HARM || MODE == MODE_HARM_STORE) {
-#pragma unroll
-        for (int r = 0; r < P; r++) p1s[r * NT + t] = pw[r];
         if (MODE == MODE_HARM) {
 #pragma unroll
           for (int k = 0; k < 16; k++)
             pms[k * NT + t] = fmaxf(pms[k * NT + t], fmaxf(fmaxf(pw[k], pw[16 + k]), fmaxf(pw[32 + k], pw[48 + k])));
         }
-        harm_unit<MODE == MODE_HARM_STORE, PRUNE>(sp, jb, p1s, pms, tmP, t, lane, s0, c, ti, tp >> 1, n_lo, n_hi, s_rec[warp],
+        harm_unit<MODE == MODE_HARM_STORE, PRUNE>(sp, jb, pw, p1s, pms, tmP, t, lane, s0, c, ti, tp >> 1, n_lo, n_hi, s_rec[warp],
                                                    sp.stash + ((size_t)blockIdx.x * NG + grp) * (2 * L));
       } else {
         if (MODE == MODE_CAND_STATS) {
