@@ -14,6 +14,7 @@
 
 #include <algorithm>
 #include <string>
+#include <type_traits>
 #include <vector>
 
 #include "../../include/jerk.h"
@@ -254,8 +255,9 @@ struct HarmGather {
   int seg_first[7], seg_count[7];
   float thr[4];              // arg-max mode: only sums above thr[log2 h] can be reported
   jerk_cand* warpbest;       // arg-max mode: [4][gridDim.x * warps per CTA] best record of every warp, h = 1,2,4,8
-  float* out;                // store mode: S_h of the job's box, out[iw_rel][iz_rel][j - 2 r_lo]
+  float* out;                // store mode: S_h of the box, out[iw - out_iw_lo][iz - out_iz_lo][j - 2 r_lo]
   int out_stage;             // store mode: log2 h
+  int out_iz_lo, out_iz_cnt, out_iw_lo;
 };
 
 constexpr int kMaxBatch = 32;   // spectra per launch of the batched candidate search
@@ -778,13 +780,20 @@ __device__ __forceinline__ void harm_batch(const HarmGather& hg, const float* co
 // largest stored power its sources can come from.  The <= 449 + 1 source bins of a fraction lie in at most two blocks of
 // the producer's block maxima (each block is at least 512 outputs long, SearchJob::bmax), those of the first and of the
 // last source bin, times two halves: four values per fraction, fetched by 28 lanes in parallel, for all pairs at once
-// (one round trip per template instead of one per pair).  Exact pruning: a pair is skipped only if every stage's bound
-// stays below the record (initially the stage threshold), so no arg-max or tie can be lost.  Bit i of the result: pair i.
+// (one round trip per template instead of one per pair); the four are folded with two shuffles, and lane i then
+// evaluates pair i (its seven bounds come through shared memory, the warp's own maxima from a warp reduction), so the
+// whole test has no loop over the pairs.  Exact pruning: a pair is skipped only if every stage's bound stays below the
+// record (initially the stage threshold), so no arg-max or tie can be lost.  Bit i of the result: pair i.
 template <int KLO, int KHI>
 __device__ __forceinline__ uint32_t harm_bounds_mask(const SearchParams& sp, int s0, int c, int ti, int n_lo, int n_hi, int lane, int t,
                                                      const float* pms, float* scr, const HarmRecord* rec) {
   constexpr int NP = (KHI - KLO) / 2;
   const HarmGather& hg = sp.hg;
+  // scratch: be[pair][8] in this warp's own slots of the group's buffer (scr[r * 64 + t] belongs to thread t): pairs
+  // 0..3 in its 32 floats of row 0, pairs 4..7 in those of row 1
+  float* ws = scr + (t & 32);
+  const auto ws_at = [&](int i) { return ws + 64 * (i >> 2) + 8 * (i & 3); };
+  // lane = 4 (e - 1) + slot, 28 lanes: the block maximum at the first (slot < 2) / last source bin of every pair, two halves
   float val[NP];
   {
     const int e = min((lane >> 2) + 1, 7), slot = lane & 3;
@@ -794,6 +803,8 @@ __device__ __forceinline__ uint32_t harm_bounds_mask(const SearchParams& sp, int
     const float* bm = hg.bmax[e - 1] + (size_t)((iwe - hg.iw_lo[e - 1]) * hg.iz_cnt[e - 1] + (ize - hg.iz_lo[e - 1])) * hg.seg_count[e - 1] * (kBmaxBlocks * 2) +
                       (slot & 1);
     const int segf = hg.seg_first[e - 1];
+    const int uoff = cs - (int)sp.seg_base - sp.hw_max;
+    const float inv_step = 1.0f / (float)sp.step;
 #pragma unroll
     for (int i = 0; i < NP; i++) {
       const int kp = KLO + 2 * i;
@@ -802,37 +813,51 @@ __device__ __forceinline__ uint32_t harm_bounds_mask(const SearchParams& sp, int
       if (n_last >= n_first && lane < 28) {
         const long long j = (slot & 2) ? 2LL * (s0 - c + n_last) + 1 : 2LL * (s0 - c + n_first);
         const int x = (int)(((j * e + 4) >> 3) >> 1);           // source bin of the first / last point of the pair
-        const int u = x + cs - (int)sp.seg_base - sp.hw_max;     // the unit that owns bin x of this template: segment u / step, output n
-        const int seg = u / sp.step;
-        const int n = u - seg * sp.step + sp.hw_max;
-        val[i] = __ldg(bm + ((seg - segf) * kBmaxBlocks + bmax_block(n)) * 2);
+        const int u = x + uoff;                                  // the unit that owns bin x of this template: segment u / step, output n
+        int seg = (int)((float)u * inv_step);                    // u / step: float estimate, corrected by at most one
+        int r = u - seg * sp.step;
+        if (r < 0) {
+          r += sp.step;
+          seg--;
+        } else if (r >= sp.step) {
+          r -= sp.step;
+          seg++;
+        }
+        val[i] = __ldg(bm + ((seg - segf) * kBmaxBlocks + bmax_block(r + sp.hw_max)) * 2);
       }
     }
   }
-  // evaluation, rolled over the pairs (the values go through shared memory: scr[i*64 + t] is this thread's own slot)
+  // the bound of fraction e for pair i = the largest of its four values (lanes 4 (e - 1) .. 4 (e - 1) + 3), left at ws_at(i)[e - 1]
 #pragma unroll
-  for (int i = 0; i < NP; i++) scr[i * 64 + t] = val[i];
-  float recs[4];
+  for (int i = 0; i < NP; i++) val[i] = fmaxf(val[i], __shfl_xor_sync(0xffffffffu, val[i], 1));
 #pragma unroll
-  for (int q = 0; q < 4; q++) recs[q] = rec[q].s;
-  uint32_t mask = 0;
-#pragma unroll 1
+  for (int i = 0; i < NP; i++) val[i] = fmaxf(val[i], __shfl_xor_sync(0xffffffffu, val[i], 2));
+  if ((lane & 3) == 0 && lane < 28) {
+#pragma unroll
+    for (int i = 0; i < NP; i++) ws_at(i)[lane >> 2] = val[i];
+  }
+  // the warp's own largest power of every pair (powers are >= 0: their bit patterns order like unsigned integers); lane i keeps pair i's
+  float own = 0.f;
+#pragma unroll
   for (int i = 0; i < NP; i++) {
     const int kp = KLO + 2 * i;
-    float v = scr[i * 64 + t];
-    v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 1));
-    v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 2));   // lanes 4 (e - 1) .. 4 (e - 1) + 3 hold the bound of fraction e
-    float be[7];
-#pragma unroll
-    for (int e = 1; e <= 7; e++) be[e - 1] = __shfl_sync(0xffffffffu, v, 4 * (e - 1));
-    float ub[4];
-    harm_stage_sums(fmaxf(pms[kp * 64 + t], pms[(kp + 1) * 64 + t]), be, ub);
-    bool need = false;
-#pragma unroll
-    for (int q = 0; q < 4; q++) need |= ub[q] >= recs[q];
-    const bool any_valid = min(256 * kp + 511, n_hi - 1) >= max(256 * kp, n_lo);
-    if (any_valid && __any_sync(0xffffffffu, need)) mask |= 1u << i;
+    const float m = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(fmaxf(pms[kp * 64 + t], pms[(kp + 1) * 64 + t]))));
+    own = lane == i ? m : own;
   }
+  __syncwarp();
+  bool need = false;
+  if (lane < NP) {
+    const float4 b03 = *reinterpret_cast<const float4*>(ws_at(lane)), b46 = *reinterpret_cast<const float4*>(ws_at(lane) + 4);
+    const float be[7] = {b03.x, b03.y, b03.z, b03.w, b46.x, b46.y, b46.z};
+    float ub[4];
+    harm_stage_sums(own, be, ub);
+#pragma unroll
+    for (int q = 0; q < 4; q++) need |= ub[q] >= rec[q].s;
+    const int kp = KLO + 2 * lane;
+    need = need && (min(256 * kp + 511, n_hi - 1) >= max(256 * kp, n_lo));
+  }
+  const uint32_t mask = __ballot_sync(0xffffffffu, need);
+  __syncwarp();                                // ws is reused for the phase-1 powers of the units that gather
   return mask;
 }
 
@@ -845,7 +870,7 @@ __device__ __forceinline__ uint32_t harm_bounds_mask(const SearchParams& sp, int
 // thrashed the instruction cache: no_instruction stalls 1.2 per issue).
 template <bool STORE, bool PRUNE>
 __device__ __forceinline__ void harm_unit(const SearchParams& sp, const SearchJob& jb, const float (&pw)[64], float* p1s, const float* pms,
-                                          uint32_t tmP, int t, int lane, int s0, int c, int ti, int box_row, int n_lo, int n_hi,
+                                          uint32_t tmP, int t, int lane, int s0, int c, int ti, int n_lo, int n_hi,
                                           HarmRecord* rec, float* stash) {
   const HarmGather& hg = sp.hg;
   constexpr int KLO = PRUNE ? 1 : 0, KHI = PRUNE ? 15 : 16;   // PRUNE: k = 0 and 15 (n1 < 4, n1 >= 60) are never valid
@@ -857,7 +882,10 @@ __device__ __forceinline__ void harm_unit(const SearchParams& sp, const SearchJo
   // registers with n1 = n / 64 in [8, 56) are valid for every thread of a segment inside the box (hw_max <= 512)
   const bool inner_valid = __all_sync(0xffffffffu, n_lo <= t + 64 * 8 && n_hi >= t + 64 * 56);
   float2* dst = nullptr;
-  if (STORE) dst = reinterpret_cast<float2*>(hg.out + (size_t)box_row * (size_t)(2 * jb.r_cnt) + 2 * (ptrdiff_t)(s0 - c - (int)jb.r_lo + t));
+  if (STORE) {
+    const int row = (ti / sp.nz - hg.out_iw_lo) * hg.out_iz_cnt + (ti % sp.nz - hg.out_iz_lo);
+    dst = reinterpret_cast<float2*>(hg.out + (size_t)row * (size_t)(2 * jb.r_cnt) + 2 * (ptrdiff_t)(s0 - c - (int)jb.r_lo + t));
+  }
   float mx[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
   // The gathers cost far more than the transforms (896 four-byte loads per thread and template through one L1 pipe per SM:
   // ~15 us per template and SM against 6.4 us of arithmetic), so in arg-max mode they are done only for the pairs of
@@ -1195,29 +1223,33 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
         float bm[kBmaxBlocks];   // block maxima of this thread's valid outputs (both phases); powers are >= 0
 #pragma unroll
         for (int g = 0; g < kBmaxBlocks; g++) bm[g] = 0.f;
+        // two copies of the store loop, chosen by a warp-uniform branch: with inner_valid the 48 inner registers need no predicate at all
+        const auto emit = [&](auto inner_c) {
+          constexpr bool INNER = decltype(inner_c)::value;
 #pragma unroll
-        for (int h = 0; h < 2; h++) {
-          float p0c[32];
-          tmem_ld32(tmP + 32 * h, p0c);
+          for (int h = 0; h < 2; h++) {
+            float p0c[32];
+            tmem_ld32(tmP + 32 * h, p0c);
 #pragma unroll
-          for (int i = 0; i < 32; i++) {
-            const int r = 32 * h + i;
-            if (PRUNE && ((r & 15) == 0 || (r & 15) == 15)) continue;
-            const int n1 = dft64_out_index(r);
-            const int n = t + 64 * n1;
-            const bool ok = (inner_valid && n1 >= 8 && n1 < 56) || (n >= n_lo && n < n_hi);
-            if (ok) {
-              dst[64 * n1] = make_float2(p0c[i], pw[r]);
-              bm[bmax_block(64 * n1)] = fmaxf(bm[bmax_block(64 * n1)], fmaxf(p0c[i], pw[r]));
+            for (int i = 0; i < 32; i++) {
+              const int r = 32 * h + i;
+              if (PRUNE && ((r & 15) == 0 || (r & 15) == 15)) continue;
+              const int n1 = dft64_out_index(r);
+              const int n = t + 64 * n1;
+              const bool ok = (INNER && n1 >= 8 && n1 < 56) ? true : (n >= n_lo && n < n_hi);
+              if (ok) {
+                dst[64 * n1] = make_float2(p0c[i], pw[r]);
+                bm[bmax_block(64 * n1)] = fmaxf(bm[bmax_block(64 * n1)], fmaxf(p0c[i], pw[r]));
+              }
             }
           }
-        }
+        };
+        if (inner_valid) emit(std::true_type{});
+        else emit(std::false_type{});
         if (jb.bmax) {   // one value per (row, segment, block, warp of the group): plain stores, every entry has one owner
+          // (powers are >= 0, so their bit patterns order like unsigned integers: one warp reduction per block)
 #pragma unroll
-          for (int g = 0; g < kBmaxBlocks; g++) {
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) bm[g] = fmaxf(bm[g], __shfl_xor_sync(0xffffffffu, bm[g], o));
-          }
+          for (int g = 0; g < kBmaxBlocks; g++) bm[g] = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(bm[g])));
           if (lane < kBmaxBlocks) {
             float mine = bm[0];
 #pragma unroll
@@ -1231,7 +1263,7 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
           for (int k = 0; k < 16; k++)
             pms[k * NT + t] = fmaxf(pms[k * NT + t], fmaxf(fmaxf(pw[k], pw[16 + k]), fmaxf(pw[32 + k], pw[48 + k])));
         }
-        harm_unit<MODE == MODE_HARM_STORE, PRUNE>(sp, jb, pw, p1s, pms, tmP, t, lane, s0, c, ti, tp >> 1, n_lo, n_hi, s_rec[warp],
+        harm_unit<MODE == MODE_HARM_STORE, PRUNE>(sp, jb, pw, p1s, pms, tmP, t, lane, s0, c, ti, n_lo, n_hi, s_rec[warp],
                                                    sp.stash + ((size_t)blockIdx.x * NG + grp) * (2 * L));
       } else {
         if (MODE == MODE_CAND_STATS) {
@@ -1971,11 +2003,14 @@ struct TemplateBox {
 // class -- the same one in every call, whatever the box -- so results do not depend on how the grid is cut into boxes.
 // Small grids (fewer than 1024 templates) form one class and keep the plain box job.  Returns the k_order parameters in
 // `op` (op.total = 0: no list needed).
-static void add_class_jobs(const jerk_plan* p, SearchParams& sp, const TemplateBox* boxes, int nboxes, void* d_work, OrderParams& op) {
+static void add_class_jobs(const jerk_plan* p, SearchParams& sp, const TemplateBox* boxes, int nboxes, void* d_work, OrderParams& op,
+                           int64_t r_lo = 0, int64_t r_cnt = -1) {      // bins [r_lo, r_lo + r_cnt) (default: the whole spectrum)
   memset(&op, 0, sizeof(op));
+  if (r_cnt < 0) r_cnt = p->nbins;
   if (p->ncls < 2) {
     for (int b = 0; b < nboxes; b++)
-      add_job(p, sp, 0, p->nbins, boxes[b].iz_lo, boxes[b].iz_cnt, boxes[b].iw_lo, boxes[b].iw_cnt, nullptr, kChunkTP);
+      add_job(p, sp, r_lo, r_cnt, boxes[b].iz_lo, boxes[b].iz_cnt, boxes[b].iw_lo, boxes[b].iw_cnt, nullptr,
+              r_cnt == p->nbins ? kChunkTP : pick_chunk_tp(p, r_cnt, boxes[b].iz_cnt, boxes[b].iw_cnt));
     return;
   }
   long long total = 0;
@@ -2013,10 +2048,17 @@ static void add_class_jobs(const jerk_plan* p, SearchParams& sp, const TemplateB
     int64_t base = -((int64_t)p->c_max + hw);      // as in jerk_plan_create, with the class's half-width
     if (base & 1) base -= 1;
     jb.seg_base = base;
-    jb.seg_first = 0;
-    jb.seg_count = (p->nbins + p->c_max - hw - base + jb.step - 1) / jb.step;
-    jb.r_lo = 0;
-    jb.r_cnt = p->nbins;
+    {   // segments whose outputs b = s0 + n - c (n in [hw, hw + step), |c| <= c_max) can touch the bins of the call
+      const int64_t nseg = (p->nbins + p->c_max - hw - base + jb.step - 1) / jb.step;
+      const int64_t lo = r_lo - p->c_max - base - hw - jb.step + 1, hi = r_lo + r_cnt - 1 + p->c_max - base - hw;
+      const int64_t s_first = lo <= 0 ? 0 : (lo + jb.step - 1) / jb.step;
+      const int64_t s_last = std::min<int64_t>(hi < 0 ? -1 : hi / jb.step, nseg - 1);
+      if (s_last < s_first) continue;
+      jb.seg_first = s_first;
+      jb.seg_count = s_last - s_first + 1;
+    }
+    jb.r_lo = r_lo;
+    jb.r_cnt = r_cnt;
     jb.iz_cnt = n;                                 // (a one-row box of n templates: the kernels' box arithmetic stays defined)
     jb.iw_cnt = 1;
     jb.ntp = sp.nb * n;
@@ -2026,6 +2068,17 @@ static void add_class_jobs(const jerk_plan* p, SearchParams& sp, const TemplateB
     jb.item_end = sp.nitems;
     sp.njobs++;
     off += n;
+  }
+  // a short r-range: shrink the work items until every resident FFT group gets a few
+  const long long want_items = 32LL * 4 * (p->sm_count > 0 ? p->sm_count : 148);
+  while (sp.nitems < want_items && sp.njobs && sp.jobs[0].chunk_tp > 32) {
+    sp.nitems = 0;
+    for (int q = 0; q < sp.njobs; q++) {
+      SearchJob& jb = sp.jobs[q];
+      jb.chunk_tp >>= 1;
+      sp.nitems += (long long)((jb.ntp + jb.chunk_tp - 1) / jb.chunk_tp) * jb.seg_count * sp.nspec;
+      jb.item_end = sp.nitems;
+    }
   }
 }
 
@@ -2598,8 +2651,13 @@ static int harm_box(jerk_plan* p, const void* d_spec, const HarmBox& bx, unsigne
     // the top-harmonic pass: the search of the box itself, summing the seven stored sub-planes into its own powers
     SearchParams tp;
     fill_params(p, tp, d_spec, d_work, work_bytes);
-    if (!add_job(p, tp, bx.r_lo, bx.r_cnt, bx.iz_lo, bx.iz_cnt, bx.iw_lo, bx.iw_cnt, nullptr, pick_chunk_tp(p, bx.r_cnt, bx.iz_cnt, bx.iw_cnt)))
-      return fail(p, JERK_EINVAL, "harmonic stage: empty box");
+    OrderParams op;
+    memset(&op, 0, sizeof(op));
+    {   // on the overlap classes of the candidate searches (add_class_jobs): a template has one segmentation in every call
+      const TemplateBox tb{bx.iz_lo, bx.iz_cnt, bx.iw_lo, bx.iw_cnt};
+      add_class_jobs(p, tp, &tb, 1, d_work, op, bx.r_lo, bx.r_cnt);
+      if (tp.njobs == 0) return fail(p, JERK_EINVAL, "harmonic stage: empty box");
+    }
     HarmGather& hg = tp.hg;
     for (int f = 0; f < 7; f++) {
       hg.base[f] = hp.sub[f].base;
@@ -2620,9 +2678,17 @@ static int harm_box(jerk_plan* p, const void* d_spec, const HarmBox& bx, unsigne
     hg.warpbest = best;
     hg.out = d_out;
     hg.out_stage = out_stage;
+    hg.out_iz_lo = bx.iz_lo;
+    hg.out_iz_cnt = bx.iz_cnt;
+    hg.out_iw_lo = bx.iw_lo;
     k_reset<<<1, 32, 0, st>>>(tp.work, nullptr, 0);
     e = cudaGetLastError();
     if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_reset launch: ") + cudaGetErrorString(e));
+    if (op.total) {
+      k_order<<<1, 1024, 0, st>>>(op);
+      e = cudaGetLastError();
+      if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_order launch: ") + cudaGetErrorString(e));
+    }
     if (d_out) {
       e = launch_search64<MODE_HARM_STORE>(p, tp, st);
     } else {
