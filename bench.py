@@ -328,10 +328,13 @@ def run_cufft_comparator(args, cfg, out):
 
 
 def harmonic_scratch_bytes(plan, free_bytes):
-    """Scratch for the harmonic row: 4x the default (a 262144-bin r-chunk: fewer segment-edge recomputations) when the
-    device has room, else the default."""
+    """Scratch for the harmonic row: 8x the library's default (a 524288-bin r-chunk, the longest the library uses: fewest
+    segment-edge recomputations; 80 GB of the 180 GB of a B200) when the device has room, else 4x, else the default."""
     base = plan.harmonic_scratch_bytes()
-    return 4 * base if free_bytes > 4 * base + (8 << 30) else base
+    for mult in (8, 4):
+        if free_bytes > mult * base + (8 << 30):
+            return mult * base
+    return base
 
 
 def run_row(args):
@@ -517,7 +520,7 @@ def main():
     ap.add_argument("--row", default="search", choices=["search", "harmonic", "spectrum", "stats", "plane", "batch", "cufft"],
                     help="search (default) = the headline bench line; the others time another row of the path and print their own line")
     ap.add_argument("--batch", type=int, default=4, help="--row batch: spectra per call")
-    ap.add_argument("--scratch-gb", type=int, default=0, help="--row harmonic: scratch buffer size in GiB (default: 4x the library's default chunk)")
+    ap.add_argument("--scratch-gb", type=int, default=0, help="--row harmonic: scratch buffer size in GiB (default: 8x the library's default chunk when the device has room)")
     ap.add_argument("--log2n", type=int, default=0,
                     help="profiling aid: shorten the time series to 2^LOG2N samples (same grid, same kernel); not the headline")
     args = ap.parse_args()
@@ -660,12 +663,23 @@ def main():
             measured_fp32 = binding.probe_fp32_tflops()
         except Exception:
             measured_fp32 = None
+        try:
+            issue = binding.probe_issue_slots()
+        except Exception:
+            issue = None
         traffic, traffic_unit = (None, None) if args.log2n else _ncu_traffic(args.config)
         roofline = {
             "bound": "alu", "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
             "traffic": traffic, "traffic_unit": traffic_unit,
             "kernel": "k_search64<cand>" if cfg.seg_len == 4096 else f"k_search<{cfg.seg_len},cand>", "kernel_ms": kernel_ms,
             "algorithmic_flops_per_launch": info.flops_per_search,
+            # what the launch executes: the overlap classes give narrow templates longer steps, i.e. fewer (segment,
+            # template-phase) units than the nominal ceil(nbins/step) * 2T of SURVEY.md 8(d) for the same points
+            "executed_units_per_launch": int(info.units_per_search), "executed_flops_per_launch": info.flops_per_search_executed,
+            "frac_executed": info.flops_per_search_executed / (kernel_ms * 1e-3) / 1e12 / FP32_PEAK_TFLOPS,
+            "note": "achieved/frac use the nominal algorithmic flops of the workload (SURVEY.md 8(d): 5L log2 L + 6L + 3 step per unit, "
+                    "ceil(nbins/step) * 2T units, step = L - 2 hw_max); frac_executed counts only the units the kernel runs (DESIGN.md 6.2)",
+            "issue_probe": issue,      # jerk_probe_issue: what a non-FMA instruction costs next to packed FP32
             "peak_measured_ffma": measured_fp32, "frac_of_measured_ffma": (achieved / measured_fp32) if measured_fp32 else None,
             "peak_source": "FP32 FMA nominal: 148 SMs x 128 lanes x 2 x 1.965 GHz (DESIGN.md); MEASURED_PEAKS.json has no fp32 entry"
                            + (f"; hbm_gbs={peaks.get('hbm_gbs')} (not the bound here)" if peaks else ""),
@@ -677,7 +691,7 @@ def main():
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(cfg.nbins * 8),
                     "d2h_bytes_per_step": int(8 + min(n_e2e, max_cands) * 16), "ms_per_step": e2e_ms / args.steps},
-            "gpu_launches": 5 * args.steps,      # k_reset, k_search64, k_seam_clear, k_seam_insert, k_seam_resolve per search
+            "gpu_launches": (6 if int(info.nclasses) > 1 else 5) * args.steps,   # k_reset, (k_order,) k_search64, k_seam_clear, k_seam_insert, k_seam_resolve per search
             "roofline": roofline,
             "bank_build_ms": bank_ms, "spectrum_prep_ms": prep_ms, "e2e_from_series_ms": series_ms, "candidates_found": n_found, "step_ms": step_ms,
         }

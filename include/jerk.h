@@ -72,8 +72,15 @@ typedef struct jerk_plan_info_t {
   int64_t nseg;          /* segments covering [0, nbins) for every template               */
   int64_t points;        /* numbetween*nbins*nz*nw (r,z,w) points of one full search       */
   uint64_t bank_bytes;   /* size of the template bank buffer jerk_templates fills          */
-  uint64_t work_bytes;   /* size of the scratch buffer the search calls need               */
+  uint64_t work_bytes;   /* size of the scratch buffer the search calls need (counters, the   */
+                         /* template list of the overlap classes, power stash, 2^20 seam records) */
   double flops_per_search; /* algorithmic FP32 flops: nseg_nominal*2T*(5L log2 L + 6L + 3 step) */
+  /* Overlap classes of the candidate searches: templates of similar half-width share a segmentation with
+   * step = L - 2*hw_class instead of L - 2*hw_max (fewer segments for narrow templates; same results).             */
+  int32_t nclasses;      /* 1: one segmentation (small grids)                                                      */
+  int32_t reserved;
+  int64_t units_per_search;          /* (segment, template-phase) units a whole-grid candidate search executes     */
+  double flops_per_search_executed;  /* the same per-unit formula summed over those units (step of each class)     */
 } jerk_plan_info_t;
 
 /*
@@ -250,10 +257,15 @@ int jerk_search_series_host(jerk_plan* plan, const float* h_series, int64_t nsam
  * For each of nstages (1..4) stages (h_harm[s] in {1,2,4,8}, thresholds h_thr[s]; HOST arrays) d_top[s]
  * (DEVICE, nstages records) receives the arg-max of S_h over the whole (j,iz,iw) grid — the position of the
  * top harmonic, power = S_h; ties go to the smallest (iw,iz,j) — if it exceeds the threshold, else
- * {j=-1, iz=0, iw=0, power=0}.  The volume is processed in r-chunks sized to d_scratch: for each chunk the
- * eight sub-planes of fractions k/8 are recomputed by the fused plane-mode kernel into d_scratch and summed.
+ * {j=-1, iz=0, iw=0, power=0}.  The volume is processed in r-chunks sized to d_scratch.  seg_len 4096: per chunk one
+ * plane-mode launch stores the seven sub-planes of fractions 1/8..7/8 (and the block maxima of every unit) in
+ * d_scratch, and the search of the chunk itself (fraction 8/8, never stored) adds the gathered sub-harmonic powers to
+ * its own powers on chip and keeps the arg-max; the gathers are skipped wherever an exact upper bound built from the
+ * block maxima cannot reach the running record.  Other seg_len: all eight sub-planes are stored and summed by a
+ * separate kernel.
  * d_scratch: DEVICE, 256-byte aligned, >= 1/256 of jerk_harmonic_scratch_bytes(plan) (that size gives the
- * default 65536-bin chunk; smaller buffers give smaller chunks); d_work as for the search calls.
+ * default 65536-bin chunk; smaller buffers give smaller chunks, larger ones longer chunks up to 524288 bins with
+ * fewer segment-edge recomputations); d_work as for the search calls.
  * Asynchronous on `stream`.  Errors: JERK_EINVAL, JERK_ENOMEM, JERK_ESTATE, JERK_ECUDA.
  */
 uint64_t jerk_harmonic_scratch_bytes(const jerk_plan* plan);
@@ -311,6 +323,18 @@ int jerk_prepare_spectrum_mode(const float* d_series, int64_t nsamples, int bloc
  * d_out: DEVICE, >= 4 bytes (never written in practice).  Errors: JERK_EINVAL, JERK_ENODEV, JERK_ECUDA.
  */
 int jerk_probe_fma(void* d_out, int iters, double* flops, void* stream);
+
+/*
+ * jerk_probe_issue — measurement aid for the issue-slot model of the search kernel.  Runs six short
+ * kernels at the occupancy of k_search64 (8 warps per SM, two per scheduler); every round of a warp is 8 independent
+ * packed FP32 fused multiply-adds followed by 4 companion instructions of one kind: [0] none, [1] integer
+ * byte-permute, [2] 128-bit shared-memory load, [3] three-input FP32 maximum with |.| operands, [4] scalar FP32
+ * fused multiply-add, [5] warp shuffle.  h_cycles_per_round (HOST, 6 doubles) receives the scheduler cycles one
+ * round takes; ([k] - [0]) / 4 is what one companion instruction costs next to packed arithmetic (0 would mean it
+ * issues in the shadow of the two-cycle packed instructions).  Synchronises `stream`.
+ * d_scratch: DEVICE, >= 256 bytes, 8-byte aligned.  Errors: JERK_EINVAL, JERK_ENODEV, JERK_ECUDA.
+ */
+int jerk_probe_issue(void* d_scratch, int iters, double* h_cycles_per_round, void* stream);
 
 const char* jerk_strerror(int status);
 const char* jerk_last_error(const jerk_plan* plan);

@@ -34,6 +34,8 @@ class PlanInfo(C.Structure):
         ("ntemplates", C.c_int32), ("hw_max", C.c_int32), ("c_max", C.c_int32), ("step", C.c_int32),
         ("seg_base", C.c_int64), ("nseg", C.c_int64), ("points", C.c_int64),
         ("bank_bytes", C.c_uint64), ("work_bytes", C.c_uint64), ("flops_per_search", C.c_double),
+        ("nclasses", C.c_int32), ("reserved", C.c_int32), ("units_per_search", C.c_int64),
+        ("flops_per_search_executed", C.c_double),
     ]
 
 
@@ -42,7 +44,7 @@ EXPORTS = [
     "jerk_templates", "jerk_templates_range", "jerk_bank_bytes_range", "jerk_templates_taps", "jerk_search_plane",
     "jerk_search_candidates", "jerk_search_candidates_range", "jerk_search_candidates_templates",
     "jerk_search_candidates_batch", "jerk_search_candidates_stats", "jerk_snr_filter",
-    "jerk_sift_candidates",
+    "jerk_sift_candidates", "jerk_probe_issue",
     "jerk_search_candidates_host", "jerk_search_series_host", "jerk_harmonic_scratch_bytes", "jerk_harmonic_sum", "jerk_harmonic_plane", "jerk_spectrum_scratch_bytes",
     "jerk_prepare_spectrum", "jerk_prepare_spectrum_mode", "jerk_probe_fma", "jerk_strerror",
     "jerk_last_error",
@@ -91,6 +93,7 @@ def load_library() -> C.CDLL:
     lib.jerk_prepare_spectrum.argtypes = [vp, i64, i32, vp, vp, u64, vp]
     lib.jerk_prepare_spectrum_mode.argtypes = [vp, i64, i32, i32, vp, vp, u64, vp]
     lib.jerk_probe_fma.argtypes = [vp, i32, C.POINTER(dbl), vp]
+    lib.jerk_probe_issue.argtypes = [vp, i32, C.POINTER(dbl), vp]
     lib.jerk_strerror.argtypes = [i32]
     lib.jerk_strerror.restype = C.c_char_p
     lib.jerk_last_error.argtypes = [vp]
@@ -392,6 +395,22 @@ def probe_fp32_tflops(iters=1 << 15, reps=5):
         if i > 0:
             best = ms if best is None else min(best, ms)
     return fl.value / (best * 1e-3) / 1e12
+
+
+def probe_issue_slots(iters=2000):
+    """jerk_probe_issue: scheduler cycles per round of 8 packed FMAs + 4 companion instructions, by companion kind."""
+    import torch
+    lib = load_library()
+    d = torch.zeros(64, dtype=torch.int64, device="cuda")
+    out = (C.c_double * 6)()
+    rc = lib.jerk_probe_issue(C.c_void_p(d.data_ptr()), int(iters), out, _stream_ptr(None))
+    if rc != 0:
+        raise JerkError(rc, lib.jerk_strerror(rc).decode())
+    kinds = ("none", "int_prmt", "lds128", "fmnmx3_abs", "ffma_scalar", "shfl")
+    base = out[0]
+    return {"cycles_per_round": {k: out[i] for i, k in enumerate(kinds)},
+            "packed_fma_cycles": base / 8.0,
+            "companion_cost_cycles": {k: (out[i] - base) / 4.0 for i, k in enumerate(kinds) if i}}
 
 
 def candidates_to_numpy(d_cands, d_count):

@@ -2217,6 +2217,25 @@ int jerk_plan_info(const jerk_plan* p, jerk_plan_info_t* info) {
   double nseg_nom = ceil((double)p->nbins / (double)p->step);
   double l2 = log2((double)p->L);
   info->flops_per_search = nseg_nom * (double)p->numbetween * p->T * (5.0 * p->L * l2 + 6.0 * p->L + 3.0 * p->step);
+  // what a whole-grid candidate search executes: every overlap class on its own segmentation
+  info->nclasses = p->ncls;
+  if (p->ncls < 2) {
+    info->units_per_search = p->nseg * (int64_t)p->numbetween * p->T;
+    info->flops_per_search_executed = (double)info->units_per_search * (5.0 * p->L * l2 + 6.0 * p->L + 3.0 * p->step);
+  } else {
+    std::vector<int64_t> cnt(p->ncls, 0);
+    for (const TemplateGeom& g : p->geom) cnt[(g.hw - p->cls_lo) / p->cls_width]++;
+    for (int k = 0; k < p->ncls; k++) {
+      if (!cnt[k]) continue;
+      const int hw = p->cls_hw[k], step = p->L - 2 * hw;
+      int64_t base = -((int64_t)p->c_max + hw);
+      if (base & 1) base -= 1;
+      const int64_t nseg = (p->nbins + p->c_max - hw - base + step - 1) / step;
+      const int64_t units = nseg * p->numbetween * cnt[k];
+      info->units_per_search += units;
+      info->flops_per_search_executed += (double)units * (5.0 * p->L * l2 + 6.0 * p->L + 3.0 * step);
+    }
+  }
   return JERK_OK;
 }
 
