@@ -502,7 +502,8 @@ def run_strong(args, torch, dist, rank, local_rank, world):
             "metric": METRIC, "value": cfg.points / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
             "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": cd, "clocks": clocks, "gathered_equals_whole_grid_search": check, "templates_per_rank": int(ti_cnt),
-            "bank_bytes_per_rank": int(plan.bank.numel()), "candidates": int(merged.size), "gpu_launches": 5 * args.steps,
+            "bank_bytes_per_rank": int(plan.bank.numel()), "candidates": int(merged.size),
+            "gpu_launches": (6 if int(plan.info.nclasses) > 1 else 5) * args.steps,
         }))
     return 0
 

@@ -333,3 +333,26 @@ def test_numbetween_one(seg_len, zmax, wmax):
         assert (zs[best["iz"]], ws[best["iw"]], int(best["j"])) == (z0, w0, r0)
     with pytest.raises(binding.JerkError):
         plan.harmonic_sum(d_spec)
+
+
+# ------------------------------------------------------------------------------------------------ strong scaling under NCCL
+def test_strong_scaling_two_ranks_nccl():
+    """the template-sharded search on TWO GPUs under NCCL (bench.py --scaling strong through torchrun):
+    every rank builds and searches half of the bank, the gathered list must equal rank 0's whole-grid search.  Skipped
+    when fewer than two GPUs are visible (nothing in this build run has more than one)."""
+    import json
+    import os
+    import subprocess
+    import sys
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", "29517", os.path.join(root, "bench.py"), "--gpus", "2", "--scaling", "strong", "--config", "2",
+           "--steps", "1", "--warmup", "3"]
+    res = subprocess.run(cmd, capture_output=True, text=True, timeout=900, cwd=root)
+    assert res.returncode == 0, res.stderr[-2000:]
+    line = json.loads([l for l in res.stdout.splitlines() if l.startswith("{")][-1])
+    assert line["n_gpus"] == 2 and line["scaling"] == "strong"
+    assert line["gathered_equals_whole_grid_search"] is True
