@@ -1984,7 +1984,7 @@ static bool add_job(const jerk_plan* p, SearchParams& sp, int64_t r_lo, int64_t 
 static int pick_chunk_tp(const jerk_plan* p, int64_t r_cnt, int iz_cnt, int iw_cnt) {
   long long ntp = 2LL * iz_cnt * iw_cnt;
   long long segs = r_cnt / p->step + 2;
-  long long want_items = 32LL * 4 * 148;    // >= 32 rounds of work items per resident FFT group of a B200: tail < 3 %
+  long long want_items = 32LL * 4 * (p->sm_count > 0 ? p->sm_count : 148);   // >= 32 rounds of work items per resident FFT group: tail < 3 %
   int c = kChunkTP;
   while (c > 32 && ((ntp + c - 1) / c) * segs < want_items) c >>= 1;
   return c;
