@@ -802,29 +802,30 @@ __device__ __forceinline__ uint32_t harm_bounds_mask(const SearchParams& sp, int
     const int cs = sp.geom[iwe * sp.nz + ize].c;
     const float* bm = hg.bmax[e - 1] + (size_t)((iwe - hg.iw_lo[e - 1]) * hg.iz_cnt[e - 1] + (ize - hg.iz_lo[e - 1])) * hg.seg_count[e - 1] * (kBmaxBlocks * 2) +
                       (slot & 1);
-    const int segf = hg.seg_first[e - 1];
+    const int segf = hg.seg_first[e - 1], seg_last = hg.seg_count[e - 1] - 1;
     const int uoff = cs - (int)sp.seg_base - sp.hw_max;
-    const float inv_step = 1.0f / (float)sp.step;
+    const int step = sp.step, hwm = sp.hw_max;
+    const float inv_step = 1.0f / (float)step;
+    const bool last = (slot & 2) != 0;
+    const int ph = last ? 1 : 0;
+    const int boff = s0 - c;
+    // Branch-free, 32-bit: point j = 2 b + ph (b = s0 - c + n < 2^30) reads source half-bin (j e + 4) >> 3, i.e. source
+    // bin x = (j e + 4) >> 4 = (b >> 3) e + (((2 (b & 7) + ph) e + 4) >> 4).  Invalid pairs load a clamped (legal) entry
+    // and are zeroed afterwards.
 #pragma unroll
     for (int i = 0; i < NP; i++) {
       const int kp = KLO + 2 * i;
       const int n_first = max(256 * kp, n_lo), n_last = min(256 * kp + 511, n_hi - 1);
-      val[i] = 0.f;
-      if (n_last >= n_first && lane < 28) {
-        const long long j = (slot & 2) ? 2LL * (s0 - c + n_last) + 1 : 2LL * (s0 - c + n_first);
-        const int x = (int)(((j * e + 4) >> 3) >> 1);           // source bin of the first / last point of the pair
-        const int u = x + uoff;                                  // the unit that owns bin x of this template: segment u / step, output n
-        int seg = (int)((float)u * inv_step);                    // u / step: float estimate, corrected by at most one
-        int r = u - seg * sp.step;
-        if (r < 0) {
-          r += sp.step;
-          seg--;
-        } else if (r >= sp.step) {
-          r -= sp.step;
-          seg++;
-        }
-        val[i] = __ldg(bm + ((seg - segf) * kBmaxBlocks + bmax_block(r + sp.hw_max)) * 2);
-      }
+      const int bb = boff + (last ? n_last : n_first);
+      const int x = (bb >> 3) * e + (((2 * (bb & 7) + ph) * e + 4) >> 4);
+      const int u = x + uoff;                                  // the unit that owns bin x of this template: segment u / step, output r + hw_max
+      int seg = (int)((float)u * inv_step);                    // u / step: float estimate, corrected by at most one
+      int r = u - seg * step;
+      seg += (r >= step) - (r < 0);
+      r += (r < 0 ? step : 0) - (r >= step ? step : 0);
+      const int sidx = min(max(seg - segf, 0), seg_last);
+      const float v = __ldg(bm + (sidx * kBmaxBlocks + bmax_block(r + hwm)) * 2);
+      val[i] = (n_last >= n_first && lane < 28) ? v : 0.f;
     }
   }
   // the bound of fraction e for pair i = the largest of its four values (lanes 4 (e - 1) .. 4 (e - 1) + 3), left at ws_at(i)[e - 1]
