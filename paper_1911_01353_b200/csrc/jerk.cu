@@ -1272,29 +1272,36 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
           // over the valid points of this unit, one fp64 atomic pair per warp
           // four independent accumulator pairs (no 64-long dependent chains); registers whose n1 = n / 64 lies in [8, 56)
           // are valid for every thread of an interior segment (hw_max <= 512) and are summed without a predicate
-          float a1[4] = {0.f, 0.f, 0.f, 0.f}, a2[4] = {0.f, 0.f, 0.f, 0.f};
+          // (packed: two powers per FADD2 / FFMA2, two accumulator pairs per sum)
+          float2 b1[2] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f)}, b2[2] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
           const bool inner_valid = __all_sync(0xffffffffu, n_lo <= t + 64 * 8 && n_hi >= t + 64 * 56);
           if (inner_valid) {
 #pragma unroll
-            for (int r = 0; r < P; r++) {
-              const int n1 = dft64_out_index(r);
-              float p = pw[r];
-              if (n1 < 8 || n1 >= 56) {
-                const int n = t + 64 * n1;
-                p = (n >= n_lo && n < n_hi) ? p : 0.f;
+            for (int r = 0; r < P; r += 2) {
+              float pa = pw[r], pb = pw[r + 1];
+              const int n1a = dft64_out_index(r), n1b = dft64_out_index(r + 1);
+              if (n1a < 8 || n1a >= 56) {
+                const int n = t + 64 * n1a;
+                pa = (n >= n_lo && n < n_hi) ? pa : 0.f;
               }
-              a1[r & 3] += p;
-              a2[r & 3] = fmaf(p, p, a2[r & 3]);
+              if (n1b < 8 || n1b >= 56) {
+                const int n = t + 64 * n1b;
+                pb = (n >= n_lo && n < n_hi) ? pb : 0.f;
+              }
+              const float2 pp = make_float2(pa, pb);
+              b1[(r >> 1) & 1] = __fadd2_rn(b1[(r >> 1) & 1], pp);
+              b2[(r >> 1) & 1] = __ffma2_rn(pp, pp, b2[(r >> 1) & 1]);
             }
           } else {
 #pragma unroll
-            for (int r = 0; r < P; r++) {
-              const int n = t + 64 * dft64_out_index(r);
-              const float p = (n >= n_lo && n < n_hi) ? pw[r] : 0.f;
-              a1[r & 3] += p;
-              a2[r & 3] = fmaf(p, p, a2[r & 3]);
+            for (int r = 0; r < P; r += 2) {
+              const int na = t + 64 * dft64_out_index(r), nb2 = t + 64 * dft64_out_index(r + 1);
+              const float2 pp = make_float2((na >= n_lo && na < n_hi) ? pw[r] : 0.f, (nb2 >= n_lo && nb2 < n_hi) ? pw[r + 1] : 0.f);
+              b1[(r >> 1) & 1] = __fadd2_rn(b1[(r >> 1) & 1], pp);
+              b2[(r >> 1) & 1] = __ffma2_rn(pp, pp, b2[(r >> 1) & 1]);
             }
           }
+          const float a1[4] = {b1[0].x, b1[0].y, b1[1].x, b1[1].y}, a2[4] = {b2[0].x, b2[0].y, b2[1].x, b2[1].y};
           float s1 = (a1[0] + a1[1]) + (a1[2] + a1[3]), s2 = (a2[0] + a2[1]) + (a2[2] + a2[3]);
 #pragma unroll
           for (int o = 16; o > 0; o >>= 1) {

@@ -129,3 +129,34 @@ def test_seg_len_zero_is_the_library_choice(lib):
     assert p.info.seg_len == 4096 and p.info.step == 4096 - 2 * 258
     with pytest.raises(binding.JerkError):
         binding.Plan(1 << 20, 200.0, 2.0, 600.0, 20.0, 2, 512)
+
+
+def test_overlap_classes_of_the_plan(lib):
+    """Host logic of the overlap classes: the zmax 200 / wmax 600 grid splits into 16 classes whose own
+    segmentations add up to fewer (segment, template-phase) units than the nominal ceil(nbins/step) * 2T of SURVEY.md
+    8(d) -- recomputed here from the oracle's half-widths -- and small grids keep one class with the nominal count."""
+    import math
+    nbins = 1 << 22
+    p = binding.Plan(nbins, 200, 2, 600, 20, 2, 4096)
+    i = p.info
+    assert i.nclasses == 16 and i.hw_max == 258 and i.step == 3580
+    zs, ws = orc.grid_values(200, 2), orc.grid_values(600, 20)
+    hws = sorted(orc.halfwidth(float(z), float(w)) for w in ws for z in zs)
+    lo, hi = hws[0], hws[-1]
+    width = (hi - lo + 16) // 16
+    units = 0
+    for k in range(16):
+        members = [h for h in hws if (h - lo) // width == k]
+        if not members:
+            continue
+        hw, step = max(members), 4096 - 2 * max(members)
+        base = -(i.c_max + hw)
+        base -= base & 1
+        nseg = -((nbins + i.c_max - hw - base) // -step)
+        units += nseg * 2 * len(members)
+    assert units == i.units_per_search
+    nominal = math.ceil(nbins / i.step) * 2 * i.ntemplates
+    assert 0.93 < units / nominal < 0.95
+    assert 0.93 < i.flops_per_search_executed / i.flops_per_search < 0.95
+    small = binding.Plan(32768, 20, 2, 60, 20, 2, 4096).info
+    assert small.nclasses == 1 and small.units_per_search == small.nseg * 2 * small.ntemplates
