@@ -289,14 +289,21 @@ def run_cufft_comparator(args, cfg, out):
     info = plan.info
     d_spec = binding.spectrum_to_device(X)
     spec = torch.view_as_complex(d_spec)
-    # bank in natural order: element k = 64*k1 + t of a (template, phase) sits at float2 slot 2*((k1>>1)*64 + t) + (k1&1)
+    # bank -> natural order.  Element k = 64*k1 + t of a (template, phase), k1 = 16 a + b, sits at float2 slot
+    # 2*((2 b + a/2)*64 + t) + (a & 1), in the mixed form of the fused first radix-4 layer (csrc/jerk.cu bank_slot<4096>):
+    # a = 0 plain (re, im); a = 1, 2: (c, t) with g = c (1 + i t); a = 3: (c3 / c1, t3)
     k = torch.arange(L, device="cuda")
     k1, t = k >> 6, k & 63
-    slot = 2 * ((k1 >> 1) * 64 + t) + (k1 & 1)
+    a, b = k1 >> 4, k1 & 15
+    slot = 2 * ((2 * b + (a >> 1)) * 64 + t) + (a & 1)
+    slot_c1 = 2 * ((2 * b) * 64 + t) + 1                      # the a = 1 entry of the same butterfly
     geom_bytes = (info.ntemplates * 8 + 255) // 256 * 256
     bank = plan.bank[geom_bytes:geom_bytes + info.ntemplates * 2 * L * 8].view(torch.float32).view(-1, L, 2)
     ntp_blk, nseg_blk = 512, 64                      # 512 template-phases x 64 segments per block: 1 GB of complex64
-    G = torch.view_as_complex(bank[:ntp_blk][:, slot, :].contiguous())           # [ntp, L] natural order
+    raw = bank[:ntp_blk][:, slot, :]                                             # [ntp, L, 2] in natural element order
+    c1 = bank[:ntp_blk][:, slot_c1, 0]
+    c = torch.where(a[None, :] == 3, raw[..., 0] * c1, raw[..., 0])
+    G = torch.where(a[None, :] == 0, torch.complex(raw[..., 0], raw[..., 1]), torch.complex(c, c * raw[..., 1]))   # [ntp, L]
     seg0 = info.nseg // 2
     starts = info.seg_base + (seg0 + torch.arange(nseg_blk, device="cuda")) * info.step
     idx = starts[:, None] + torch.arange(L, device="cuda")[None, :]

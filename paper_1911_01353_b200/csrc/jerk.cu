@@ -150,12 +150,22 @@ __device__ __forceinline__ int bank_slot(int k) {
   return (((u * (Gm::R1 / 2) + (k2 >> 1)) * Gm::NT + t) << 1) + (k2 & 1);
 }
 
-// seg_len 4096 is searched by k_search64 (64 threads x 64 points per FFT): thread t reads float4 #(e*64 + t), which holds
-// elements k = 64*k1 + t for k1 = 2e, 2e+1
+// seg_len 4096 is searched by k_search64 (64 threads x 64 points per FFT), which fuses the multiplication by G with the
+// first radix-4 layer of the inverse transform (butterfly b of thread t combines elements k = 64 (16 a + b) + t, a = 0..3).
+// Thread t reads float4 #((2 b + a / 2) * 64 + t): float2 slot of element (a, b, t); the values are stored in the mixed
+// form of dft16_layerA_tw (bank_mixed_store below).
 template <>
 __device__ __forceinline__ int bank_slot<4096>(int k) {
   const int k1 = k >> 6, t = k & 63;
-  return ((((k1 >> 1) << 6) + t) << 1) + (k1 & 1);
+  const int a = k1 >> 4, b = k1 & 15;
+  return ((((2 * b + (a >> 1)) << 6) + t) << 1) + (a & 1);
+}
+// g = c (1 + i t) with a real part kept away from zero (relative 1e-12: far below fp32 rounding of the product)
+__device__ __forceinline__ float2 bank_mixed(float2 g) {
+  float c = g.x;
+  const float lim = fmaxf(1e-12f * fabsf(g.y), 1e-30f);
+  if (fabsf(c) < lim) c = copysignf(lim, c);
+  return make_float2(c, g.y / c);
 }
 
 template <int L>
@@ -203,9 +213,23 @@ __global__ void __launch_bounds__(FftGeom<L>::NT) k_bank(BankParams bp) {
       for (int n2 = 0; n2 < 16; n2++) {
         int k = Gm::b3_of(t, u) + 16 * Gm::R1 * n2;
         float2 x = v[u * 16 + n2];
-        out[bank_slot<L>(k)] = make_float2(x.x * sc, -x.y * sc);  // conj(FFT)/L
+        const float2 gk = make_float2(x.x * sc, -x.y * sc);       // conj(FFT)/L
+        if (L == 4096) exA[k] = gk;                                // staged in natural order, converted below
+        else out[bank_slot<L>(k)] = gk;
       }
     __syncthreads();
+    if (L == 4096) {
+      // mixed form per radix-4 butterfly (a = 0..3 at k = 64 (16 a + b) + t64): plain, (c1, t1), (c2, t2), (c3 / c1, t3)
+      for (int q = t; q < 1024; q += Gm::NT) {
+        const int b = q >> 6, t64 = q & 63;
+        const float2 g0 = exA[64 * b + t64], m1 = bank_mixed(exA[64 * (16 + b) + t64]), m2 = bank_mixed(exA[64 * (32 + b) + t64]),
+                     m3 = bank_mixed(exA[64 * (48 + b) + t64]);
+        float4* o4 = reinterpret_cast<float4*>(out) + (2 * b) * 64 + t64;
+        o4[0] = make_float4(g0.x, g0.y, m1.x, m1.y);
+        o4[64] = make_float4(m2.x, m2.y, m3.x / m1.x, m3.y);
+      }
+      __syncthreads();
+    }
   }
 }
 
@@ -1092,11 +1116,12 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
 #pragma unroll
       for (int r = 0; r < 64; r++) ex[t + 64 * dft64_out_index(r)] = v[r];
       bar_sync_named(barid, NT);
+      // chunk h of the tensor-memory copy serves the radix-4 butterflies b = 4h .. 4h+3 of pass 1: entry 4 m + a = F[64 (16 a + 4 h + m) + t]
 #pragma unroll
       for (int h = 0; h < 4; h++) {
         float2 fq[16];
 #pragma unroll
-        for (int i = 0; i < 16; i++) fq[i] = ex[64 * (16 * h + i) + t];
+        for (int i = 0; i < 16; i++) fq[i] = ex[64 * (16 * (i & 3) + 4 * h + (i >> 2)) + t];
         tmF.store16(h, fq);
       }
       bar_sync_named(barid, NT);
@@ -1152,11 +1177,21 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
           float(&nxt)[32] = (h & 1) ? fa : fb;
           tmem_ld32_wait(cur);
           if (h < 3) tmF.issue16(h + 1, nxt);
+          // Y = F .* G fused with the first radix-4 layer of the inverse transform: the bank holds G in the mixed form
+          // of dft16_layerA_tw, (g0.re, g0.im), (c1, t1), (c2, t2), (c3 / c1, t3) with g = c (1 + i t), so a butterfly of
+          // four products costs 13 packed instructions instead of 8 + 8
 #pragma unroll
-          for (int i = 0; i < 8; i++) {
-            const float4 g = g4[(8 * h + i) * NT];
-            v[16 * h + 2 * i] = cmul(make_float2(cur[4 * i], cur[4 * i + 1]), make_float2(g.x, g.y));
-            v[16 * h + 2 * i + 1] = cmul(make_float2(cur[4 * i + 2], cur[4 * i + 3]), make_float2(g.z, g.w));
+          for (int m = 0; m < 4; m++) {
+            const int b = 4 * h + m;
+            const float4 ga = g4[(8 * h + 2 * m) * NT], gb = g4[(8 * h + 2 * m + 1) * NT];
+            const float2 w[4] = {make_float2(ga.x, ga.y), make_float2(ga.z, ga.w), make_float2(gb.x, gb.y), make_float2(gb.z, gb.w)};
+            float2 x0 = make_float2(cur[8 * m], cur[8 * m + 1]), x1 = make_float2(cur[8 * m + 2], cur[8 * m + 3]);
+            float2 x2 = make_float2(cur[8 * m + 4], cur[8 * m + 5]), x3 = make_float2(cur[8 * m + 6], cur[8 * m + 7]);
+            dft16_layerA_tw<1, false>(x0, x1, x2, x3, w);
+            v[b] = x0;
+            v[16 + b] = x1;
+            v[32 + b] = x2;
+            v[48 + b] = x3;
           }
         }
       }
@@ -1174,7 +1209,7 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
         }
         __syncwarp();
       };
-      fft64_passes<1>(v, tmT, ex, t, barid, mid, pre, post);
+      fft64_passes<1, true>(v, tmT, ex, t, barid, mid, pre, post);
       tphase ^= 1u;
       g_ready = tp + 1 < tp_hi ? mbar_probe(mbG, tphase) : 0u;   // has the next G landed?  (asked now, needed after the epilogue)
       // ---- a-4: overlap discard + power.  n = t + 64*n1 ; b = s0 + n - c ; j = 2b + ph.

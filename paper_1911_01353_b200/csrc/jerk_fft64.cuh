@@ -228,14 +228,18 @@ __device__ __forceinline__ void bar_sync_named(int id, int nthreads) {
 // done (the stores of column A issue under the butterflies of column A + 1), and the pass-2 loads are issued in the order
 // the first radix-4 layer consumes them (registers b, 16 + b, 32 + b, 48 + b), so that layer starts after four loads
 // instead of thirty-two.
-template <int SIGN, class TW, class MID, class PRE, class POST>
+// FIRST_DONE: the caller has already run the first radix-4 layer of pass 1 (the search kernel fuses it with the
+// multiplication by G: dft16_layerA_tw on F and the mixed-form filter).
+template <int SIGN, bool FIRST_DONE = false, class TW, class MID, class PRE, class POST>
 __device__ __forceinline__ void fft64_passes(float2 (&v)[64], const TW& tw, float2* ex, int t, int barid, MID mid, PRE before_store,
                                              POST after_load) {
+  if (!FIRST_DONE) {
 #pragma unroll
-  for (int b = 0; b < 16; b++) {
-    float2 q[4] = {v[b], v[16 + b], v[32 + b], v[48 + b]};
-    Dft<4, SIGN>::run(q);
-    v[b] = q[0]; v[16 + b] = q[1]; v[32 + b] = q[2]; v[48 + b] = q[3];
+    for (int b = 0; b < 16; b++) {
+      float2 q[4] = {v[b], v[16 + b], v[32 + b], v[48 + b]};
+      Dft<4, SIGN>::run(q);
+      v[b] = q[0]; v[16 + b] = q[1]; v[32 + b] = q[2]; v[48 + b] = q[3];
+    }
   }
   mid();
   float2* w = ex + t;
