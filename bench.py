@@ -415,7 +415,7 @@ def other_rows(steps=3):
             n_steps = 2 if idx == 4 else steps
             ts = _time_steps(lambda: plan.search_candidates(d_spec, cfg.threshold), 3, n_steps)
             n = int(plan.search_candidates(d_spec, cfg.threshold)[1].item())
-            rows[f"config{idx}_candidates_seg{L if L else '0(4096)'}"] = _row_entry(
+            rows[f"config{idx}_candidates_seg{L if L else '0(%d)' % int(plan.info.seg_len)}"] = _row_entry(
                 ts, cfg.points, plan.info.flops_per_search, {"seg_len": int(plan.info.seg_len), "candidates": n})
             if idx == 2 and L == cfg.seg_len:
                 plane = torch.empty((cfg.nw, cfg.nz, 2 * cfg.nbins), dtype=torch.float32, device="cuda")

@@ -89,7 +89,8 @@ typedef struct jerk_plan_info_t {
  * Requirements: nbins >= 1; zmax, wmax >= 0; dz, dw > 0 with zmax/dz and wmax/dw integers;
  * numbetween 2 (the half-bin phases p = 0, 1) or 1 (integer bins only, p = 0: half the work; the FDAS-style option of
  * SURVEY.md 8(f) N4; planes then hold one float per bin and the harmonic stage is not offered); seg_len in {1024, 2048, 4096, 8192} and seg_len - 2*hw_max >= 2, or seg_len == 0 for the library's
- * choice (4096, the fastest kernel, whenever it leaves a positive step; the result does not depend on seg_len); nz, nw < 32768.
+ * choice (4096, the fastest kernel, whenever it leaves a positive step; 1024 for searches too small to fill that kernel's
+ * resident FFT groups; the result does not depend on seg_len); nz, nw < 32768.
  * *out receives a plan that jerk_plan_destroy frees.  Errors: JERK_EINVAL.
  */
 int jerk_plan_create(jerk_plan** out, int64_t nbins, double zmax, double dz, double wmax, double dw,

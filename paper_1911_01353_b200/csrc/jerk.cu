@@ -2203,7 +2203,13 @@ int jerk_plan_create(jerk_plan** out, int64_t nbins, double zmax, double dz, dou
     }
   // seg_len 0: the library's choice.  The result does not depend on the segment length (SURVEY.md 8(c) pin P9); 4096 is
   // the length of the two-pass kernel (k_search64) and is taken whenever the templates leave a positive step.
-  if (seg_len == 0) seg_len = 4096 - 2 * p->hw_max >= 2 ? 4096 : 8192;
+  if (seg_len == 0) {
+    seg_len = 4096 - 2 * p->hw_max >= 2 ? 4096 : 8192;
+    // a tiny search (config 1: 147 templates x 10 segments) cannot fill the 592 resident FFT groups of the two-pass
+    // kernel even with the smallest work items (32 template-phases); the 1024-point kernel has four times the segments
+    const int64_t items4096 = ((int64_t)numbetween * p->T + 31) / 32 * (nbins / (4096 - 2 * p->hw_max) + 2);
+    if (seg_len == 4096 && items4096 < 2 * 592 && 1024 - 2 * p->hw_max >= 512) seg_len = 1024;
+  }
   p->L = seg_len;
   p->step = seg_len - 2 * p->hw_max;
   if (p->step < 2) {

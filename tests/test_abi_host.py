@@ -127,6 +127,8 @@ def test_synth_configs_are_deterministic():
 def test_seg_len_zero_is_the_library_choice(lib):
     p = binding.Plan(1 << 20, 200.0, 2.0, 600.0, 20.0, 2, 0)
     assert p.info.seg_len == 4096 and p.info.step == 4096 - 2 * 258
+    assert binding.Plan(32768, 20.0, 2.0, 60.0, 20.0, 2, 0).info.seg_len == 1024      # config 1: too few work items for the two-pass kernel
+    assert binding.Plan(1 << 20, 100.0, 2.0, 300.0, 20.0, 2, 0).info.seg_len == 4096  # config 2
     with pytest.raises(binding.JerkError):
         binding.Plan(1 << 20, 200.0, 2.0, 600.0, 20.0, 2, 512)
 
