@@ -362,3 +362,52 @@ def test_strong_scaling_two_ranks_nccl():
     line = json.loads([l for l in res.stdout.splitlines() if l.startswith("{")][-1])
     assert line["n_gpus"] == 2 and line["scaling"] == "strong"
     assert line["gathered_equals_whole_grid_search"] is True
+
+
+# ------------------------------------------------------------------------------------------------ out-of-bounds canaries
+def _padded(nbytes, device="cuda", pad=1 << 16):
+    """A uint8 view of `nbytes` bytes (256-byte aligned) inside a buffer with 64 KB canary bands on both sides."""
+    full = torch.full((nbytes + 2 * pad + 256,), 0xA5, dtype=torch.uint8, device=device)
+    off = pad + (-(full.data_ptr() + pad)) % 256
+    return full, full[off:off + nbytes], off
+
+
+def _canaries_intact(full, off, nbytes):
+    return bool((full[:off] == 0xA5).all().item()) and bool((full[off + nbytes:] == 0xA5).all().item())
+
+
+@pytest.mark.parametrize("seg_len,zmax,wmax", [(4096, 60.0, 180.0), (1024, 20.0, 60.0)])
+def test_no_write_outside_caller_buffers(seg_len, zmax, wmax):
+    """compute-sanitizer is closed on this pool, so the memcheck substitute is explicit: every caller-owned buffer the
+    library writes (bank, d_work, candidates, count, plane, harmonic scratch, stage tops) sits between 64 KB canary bands
+    that must be untouched after bank build, candidate search (low threshold: seams, overlap classes for the first grid),
+    a plane box that starts and ends inside segments, and a harmonic-summed search with chunking."""
+    nbins = 23456
+    X = synth.random_spectrum(nbins, 909)
+    plan = binding.Plan(nbins, zmax, 2, wmax, 20, 2, seg_len)
+    lib = binding.load_library()
+    bank_full, plan.bank, bank_off = _padded(int(plan.info.bank_bytes))
+    assert lib.jerk_templates(plan._h, C.c_void_p(plan.bank.data_ptr()), int(plan.info.bank_bytes), None) == 0
+    work_full, plan.work, work_off = _padded(int(plan.info.work_bytes))
+    d_spec = binding.spectrum_to_device(X)
+    max_cands = 5000                                        # smaller than the number of candidates: the excess must be dropped, not written
+    cand_full, d_cands, cand_off = _padded(max_cands * 16)
+    cnt_full, d_cnt8, cnt_off = _padded(8)
+    d_count = d_cnt8.view(torch.int64)
+    plan.search_candidates(d_spec, 4.0, max_cands=max_cands, d_cands=d_cands, d_count=d_count)
+    assert int(d_count.item()) > max_cands
+    r_lo, r_cnt, iz_lo, iz_cnt, iw_lo, iw_cnt = 777, 9001, 3, 5, 1, 2
+    plane_full, plane8, plane_off = _padded(iw_cnt * iz_cnt * 2 * r_cnt * 4)
+    out = plane8.view(torch.float32).view(iw_cnt, iz_cnt, 2 * r_cnt)
+    plan.search_plane(d_spec, r_lo, r_cnt, iz_lo, iz_cnt, iw_lo, iw_cnt, out=out)
+    nscr = int(plan.harmonic_scratch_bytes()) // 3          # a third of the default: several r-chunks
+    nscr -= nscr % 256
+    scr_full, plan.scratch, scr_off = _padded(nscr)
+    top = plan.harmonic_sum(d_spec, (1, 2, 4, 8), (8.0, 12.0, 18.0, 28.0), scratch_bytes=nscr)
+    torch.cuda.synchronize()
+    assert (top["j"] >= 0).all()
+    for name, full, off, n in (("bank", bank_full, bank_off, int(plan.info.bank_bytes)), ("work", work_full, work_off, int(plan.info.work_bytes)),
+                               ("cands", cand_full, cand_off, max_cands * 16), ("count", cnt_full, cnt_off, 8),
+                               ("plane", plane_full, plane_off, plane8.numel()), ("scratch", scr_full, scr_off, nscr)):
+        assert _canaries_intact(full, off, n), f"write outside the {name} buffer"
+    assert np.isfinite(out.cpu().numpy()).all()
