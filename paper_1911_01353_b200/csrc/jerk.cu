@@ -810,7 +810,7 @@ __device__ __forceinline__ void harm_batch(const HarmGather& hg, const float* co
 // record (initially the stage threshold), so no arg-max or tie can be lost.  Bit i of the result: pair i.
 template <int KLO, int KHI>
 __device__ __forceinline__ uint32_t harm_bounds_mask(const SearchParams& sp, int s0, int c, int ti, int n_lo, int n_hi, int lane, int t,
-                                                     const float* pms, float* scr, const HarmRecord* rec) {
+                                                     const float* pms, const float (&pw)[64], float* scr, const HarmRecord* rec) {
   constexpr int NP = (KHI - KLO) / 2;
   const HarmGather& hg = sp.hg;
   // scratch: be[pair][8] in this warp's own slots of the group's buffer (scr[r * 64 + t] belongs to thread t): pairs
@@ -863,11 +863,17 @@ __device__ __forceinline__ uint32_t harm_bounds_mask(const SearchParams& sp, int
   }
   // the warp's own largest power of every pair (powers are >= 0: their bit patterns order like unsigned integers); lane i keeps pair i's
   float own = 0.f;
+  {
+    const float4 pa = reinterpret_cast<const float4*>(pms)[t], pb = reinterpret_cast<const float4*>(pms)[64 + t];   // phase 0, per pair
+    const float p0m[8] = {pa.x, pa.y, pa.z, pa.w, pb.x, pb.y, pb.z, pb.w};
 #pragma unroll
-  for (int i = 0; i < NP; i++) {
-    const int kp = KLO + 2 * i;
-    const float m = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(fmaxf(pms[kp * 64 + t], pms[(kp + 1) * 64 + t]))));
-    own = lane == i ? m : own;
+    for (int i = 0; i < NP; i++) {
+      const int k0 = KLO + 2 * i, k1 = k0 + 1;
+      const float p1m = fmaxf(fmaxf(fmaxf(pw[k0], pw[16 + k0]), fmaxf(pw[32 + k0], pw[48 + k0])),
+                              fmaxf(fmaxf(pw[k1], pw[16 + k1]), fmaxf(pw[32 + k1], pw[48 + k1])));
+      const float m = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(fmaxf(p0m[i], p1m))));
+      own = lane == i ? m : own;
+    }
   }
   __syncwarp();
   bool need = false;
@@ -887,8 +893,8 @@ __device__ __forceinline__ uint32_t harm_bounds_mask(const SearchParams& sp, int
 }
 
 // One (segment, template) unit of the top-harmonic pass, called when phase 1 is done.  Phase-0 powers are in tensor
-// memory at tmP, phase-1 powers in shared memory p1s (register r of thread t at r*64 + t), the per-thread maxima of both
-// phases over the four registers of every k in pms[k*64 + t] (all written and read by the same thread); register
+// memory at tmP, phase-1 powers in shared memory p1s (register r of thread t at r*64 + t), the per-thread phase-0
+// maxima of every pair of batches in pms ([2][64] float4, written and read by the same thread); register
 // r = 16 a + k holds n = t + 64 n1, n1 = 4 k + a... see harm_batch.  Point j = 2 (s0 - c + n) + ph reads sub-plane e at
 // (j e + 4) >> 3 = ((jt e + 4) >> 3) + 16 n1 e with jt = 2 (s0 - c + t) + ph: one pointer per (fraction, phase), moved
 // on by 64 e per k.  The loop over k is rolled (an unrolled gather body of 5000 instructions on top of the transforms
@@ -916,7 +922,7 @@ __device__ __forceinline__ void harm_unit(const SearchParams& sp, const SearchJo
   // ~15 us per template and SM against 6.4 us of arithmetic), so in arg-max mode they are done only for the pairs of
   // batches whose bound (harm_bounds_need) can reach the record.  In batches of 56 independent loads per thread (about
   // what one warp can have outstanding), all issued before the first sum.
-  const uint32_t need = STORE ? 0xffffffffu : harm_bounds_mask<KLO, KHI>(sp, s0, c, ti, n_lo, n_hi, lane, t, pms, p1s, rec);
+  const uint32_t need = STORE ? 0xffffffffu : harm_bounds_mask<KLO, KHI>(sp, s0, c, ti, n_lo, n_hi, lane, t, pms, pw, p1s, rec);
   if (need == 0) return;
 #pragma unroll
   for (int r = 0; r < 64; r++) p1s[r * 64 + t] = pw[r];   // phase-1 powers: only for the units that gather
@@ -1235,7 +1241,17 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
         }
         if (MODE == MODE_HARM) {   // the largest phase-0 power of the four registers 16 a + k of every k (bounds of harm_unit)
 #pragma unroll
-          for (int k = 0; k < 16; k++) pms[k * NT + t] = fmaxf(fmaxf(pw[k], pw[16 + k]), fmaxf(pw[32 + k], pw[48 + k]));
+          for (int q4 = 0; q4 < 2; q4++) {   // per pair of batches (k = KLO + 2 i, KLO + 2 i + 1): [2][NT] float4, pairs 4 q4 .. 4 q4 + 3
+            float pm[4];
+#pragma unroll
+            for (int u = 0; u < 4; u++) {
+              const int k0 = (PRUNE ? 1 : 0) + 2 * (4 * q4 + u), k1 = k0 + 1;
+              pm[u] = k1 < 16 ? fmaxf(fmaxf(fmaxf(pw[k0], pw[16 + k0]), fmaxf(pw[32 + k0], pw[48 + k0])),
+                                      fmaxf(fmaxf(pw[k1], pw[16 + k1]), fmaxf(pw[32 + k1], pw[48 + k1])))
+                              : 0.f;
+            }
+            reinterpret_cast<float4*>(pms)[q4 * NT + t] = make_float4(pm[0], pm[1], pm[2], pm[3]);
+          }
         }
       } else if (MODE == MODE_PLANE && !two) {
         // numbetween = 1: one float per bin, row index = template
@@ -1294,11 +1310,6 @@ __global__ void __launch_bounds__(64 * NG, NG == 2 ? 2 : 1) k_search64(const __g
           }
         }
       } else if (MODE == MODE_HARM || MODE == MODE_HARM_STORE) {
-        if (MODE == MODE_HARM) {
-#pragma unroll
-          for (int k = 0; k < 16; k++)
-            pms[k * NT + t] = fmaxf(pms[k * NT + t], fmaxf(fmaxf(pw[k], pw[16 + k]), fmaxf(pw[32 + k], pw[48 + k])));
-        }
         harm_unit<MODE == MODE_HARM_STORE, PRUNE>(sp, jb, pw, p1s, pms, tmP, t, lane, s0, c, ti, n_lo, n_hi, s_rec[warp],
                                                    sp.stash + ((size_t)blockIdx.x * NG + grp) * (2 * L));
       } else {
