@@ -411,3 +411,14 @@ def test_no_write_outside_caller_buffers(seg_len, zmax, wmax):
                                ("plane", plane_full, plane_off, plane8.numel()), ("scratch", scr_full, scr_off, nscr)):
         assert _canaries_intact(full, off, n), f"write outside the {name} buffer"
     assert np.isfinite(out.cpu().numpy()).all()
+
+
+# ------------------------------------------------------------------------------------------------ measurement aids
+def test_probes_report_sane_numbers():
+    """jerk_probe_fma / jerk_probe_issue (the denominators and the issue-slot model of DESIGN.md 6.2): a packed FP32
+    instruction takes about two scheduler cycles, no companion instruction is free, the FFMA probe is near the nominal peak."""
+    p = binding.probe_issue_slots(iters=500)
+    assert 1.9 < p["packed_fma_cycles"] < 2.3
+    assert all(c > 0.5 for c in p["companion_cost_cycles"].values())
+    tf = binding.probe_fp32_tflops(iters=1 << 13, reps=3)
+    assert 50.0 < tf < 80.0
