@@ -417,10 +417,10 @@ def other_rows(steps=3):
             n = int(plan.search_candidates(d_spec, cfg.threshold)[1].item())
             rows[f"config{idx}_candidates_seg{L if L else '0(%d)' % int(plan.info.seg_len)}"] = _row_entry(
                 ts, cfg.points, plan.info.flops_per_search, {"seg_len": int(plan.info.seg_len), "candidates": n})
-            if idx == 2 and L == cfg.seg_len:
+            if idx == 2:
                 plane = torch.empty((cfg.nw, cfg.nz, 2 * cfg.nbins), dtype=torch.float32, device="cuda")
                 ts = _time_steps(lambda: plan.search_plane(d_spec, 0, cfg.nbins, out=plane), 3, steps)
-                rows["config2_plane_mode_seg2048"] = _row_entry(ts, cfg.points, plan.info.flops_per_search,
+                rows[f"config2_plane_mode_seg{L if L else '0(%d)' % int(plan.info.seg_len)}"] = _row_entry(ts, cfg.points, plan.info.flops_per_search,
                                                                 {"plane_bytes": plane.numel() * 4, "plane_GBps": plane.numel() * 4 / np.median(ts) / 1e6})
                 del plane
             del plan
