@@ -160,10 +160,11 @@ __device__ __forceinline__ int bank_slot<4096>(int k) {
   const int a = k1 >> 4, b = k1 & 15;
   return ((((2 * b + (a >> 1)) << 6) + t) << 1) + (a & 1);
 }
-// g = c (1 + i t) with a real part kept away from zero (relative 1e-12: far below fp32 rounding of the product)
+// g = c (1 + i t) with a real part kept away from zero (relative 1e-8: below fp32 rounding of the product; |t| <= 1e8
+// keeps t * F far from overflow for any sensible spectrum)
 __device__ __forceinline__ float2 bank_mixed(float2 g) {
   float c = g.x;
-  const float lim = fmaxf(1e-12f * fabsf(g.y), 1e-30f);
+  const float lim = fmaxf(1e-8f * fabsf(g.y), 1e-30f);
   if (fabsf(c) < lim) c = copysignf(lim, c);
   return make_float2(c, g.y / c);
 }
