@@ -44,7 +44,8 @@ typedef enum jerk_status {
   JERK_ECUDA = -3,    /* a CUDA runtime call or launch failed                              */
   JERK_ESTATE = -4,   /* jerk_templates has not been called for this plan                  */
   JERK_ENODEV = -5,   /* no sm_100 device is current                                       */
-  JERK_EOVERFLOW = -6 /* (host entry points) more candidates than max_cands, or more seam records than d_work holds */
+  JERK_EOVERFLOW = -6, /* (host entry points) more candidates than max_cands, or more seam records than d_work holds */
+  JERK_ELIMIT = -7    /* the request is larger than a fixed, built-in capacity (jerk_prepare_spectrum_static)          */
 } jerk_status;
 
 typedef struct jerk_plan jerk_plan;
@@ -316,6 +317,37 @@ int jerk_prepare_spectrum(const float* d_series, int64_t nsamples, int block, vo
 enum { JERK_NORM_MEAN = 0, JERK_NORM_MEDIAN = 1, JERK_NORM_REDNOISE = 2 };
 int jerk_prepare_spectrum_mode(const float* d_series, int64_t nsamples, int block, int mode, void* d_spec, void* d_scratch,
                                uint64_t scratch_bytes, void* stream);
+
+/*
+ * jerk_prepare_spectrum_static — jerk_prepare_spectrum (mean normalisation) without a scratch argument, for callers
+ * that have no device memory to give and no way to get any: code that runs where cudaMalloc is off limits (inside a
+ * host framework whose memory pool owns the whole GPU and forbids side allocations, a real-time acquisition loop that
+ * must not take the allocator's lock or its implicit device synchronisation, a plug-in that is handed exactly two
+ * buffers — input and output — by its host application).  The transform's intermediate array, which the other entry
+ * points take as d_scratch, is here an 8 MiB array built into the library image; the call itself allocates nothing
+ * (no cudaMalloc, cudaFree or allocating library routine) and computes exactly what jerk_prepare_spectrum computes.
+ *
+ * Limit: nsamples <= JERK_STATIC_SPECTRUM_MAX_SAMPLES (2^21, i.e. 2^20 bins); longer series get JERK_ELIMIT and must
+ * use jerk_prepare_spectrum with their own scratch.  The price of the built-in array: every GPU on which this library
+ * is loaded keeps those 8 MiB until the process exits, whether or not this call is ever made.
+ *
+ * Sharing: there is ONE array per GPU, used by every call on that GPU from any thread or stream.  Two calls whose GPU
+ * work can overlap (different streams, or the same series prepared twice at once) race on it and both results are
+ * then undefined: issue them on one stream, or order the streams with events.  The array still holds the previous
+ * call's intermediate data when the next call starts; that is harmless, because every call overwrites the part it
+ * later reads, so nothing is (or needs to be) cleared.
+ *
+ * First call on a device: the library looks up, once per device and with that device current, the device address of
+ * its array (a symbol-address query that allocates nothing but is a set-up step rather than stream work).  Make the
+ * first call on each device during initialisation, before any stream capture is begun.
+ *
+ * d_series, d_spec, stream, alignment and the lower size limit (2^11) as jerk_prepare_spectrum; both buffers remain
+ * caller-owned, d_series is not modified.  Asynchronous on `stream`.
+ * Errors: JERK_ELIMIT (nsamples above the limit), JERK_EINVAL (null, size not a power of two or < 2^11, alignment,
+ * block < 1), JERK_ENODEV (no sm_100 device current), JERK_ECUDA (address query or launch failed).
+ */
+#define JERK_STATIC_SPECTRUM_MAX_SAMPLES (1 << 21)
+int jerk_prepare_spectrum_static(const float* d_series, int64_t nsamples, int block, void* d_spec, void* stream);
 
 /*
  * jerk_probe_fma — measurement aid for the roofline denominator: launches a kernel of nothing but

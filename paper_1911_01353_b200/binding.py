@@ -14,7 +14,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libjerk_b200.so")
 
-JERK_OK, JERK_EINVAL, JERK_ENOMEM, JERK_ECUDA, JERK_ESTATE, JERK_ENODEV, JERK_EOVERFLOW = 0, -1, -2, -3, -4, -5, -6
+JERK_OK, JERK_EINVAL, JERK_ENOMEM, JERK_ECUDA, JERK_ESTATE, JERK_ENODEV, JERK_EOVERFLOW, JERK_ELIMIT = 0, -1, -2, -3, -4, -5, -6, -7
+STATIC_SPECTRUM_MAX_SAMPLES = 1 << 21   # JERK_STATIC_SPECTRUM_MAX_SAMPLES (include/jerk.h)
 SEAM_OVERFLOW = (1 << 64) - 1      # *d_count after a search whose seam records did not fit in d_work (include/jerk.h)
 
 CAND_DTYPE = np.dtype([("j", "<i4"), ("iz", "<i2"), ("iw", "<i2"), ("power", "<f4"), ("flags", "<u4")])
@@ -46,7 +47,7 @@ EXPORTS = [
     "jerk_search_candidates_batch", "jerk_search_candidates_stats", "jerk_snr_filter",
     "jerk_sift_candidates", "jerk_probe_issue",
     "jerk_search_candidates_host", "jerk_search_series_host", "jerk_harmonic_scratch_bytes", "jerk_harmonic_sum", "jerk_harmonic_plane", "jerk_spectrum_scratch_bytes",
-    "jerk_prepare_spectrum", "jerk_prepare_spectrum_mode", "jerk_probe_fma", "jerk_strerror",
+    "jerk_prepare_spectrum", "jerk_prepare_spectrum_mode", "jerk_prepare_spectrum_static", "jerk_probe_fma", "jerk_strerror",
     "jerk_last_error",
 ]
 
@@ -92,6 +93,7 @@ def load_library() -> C.CDLL:
     lib.jerk_spectrum_scratch_bytes.restype = u64
     lib.jerk_prepare_spectrum.argtypes = [vp, i64, i32, vp, vp, u64, vp]
     lib.jerk_prepare_spectrum_mode.argtypes = [vp, i64, i32, i32, vp, vp, u64, vp]
+    lib.jerk_prepare_spectrum_static.argtypes = [vp, i64, i32, vp, vp]
     lib.jerk_probe_fma.argtypes = [vp, i32, C.POINTER(dbl), vp]
     lib.jerk_probe_issue.argtypes = [vp, i32, C.POINTER(dbl), vp]
     lib.jerk_strerror.argtypes = [i32]
@@ -371,6 +373,28 @@ def prepare_spectrum(d_series, block=1000, d_spec=None, d_scratch=None, stream=N
     rc = lib.jerk_prepare_spectrum_mode(C.c_void_p(d_series.data_ptr()), int(n), int(block), int(NORM_MODES[mode]),
                                         C.c_void_p(d_spec.data_ptr()), C.c_void_p(d_scratch.data_ptr()), d_scratch.numel(),
                                         _stream_ptr(stream))
+    if rc != 0:
+        raise JerkError(rc, lib.jerk_strerror(rc).decode())
+    return d_spec
+
+
+def prepare_spectrum_static(d_series, block=1000, d_spec=None, stream=None):
+    """jerk_prepare_spectrum_static: prepare_spectrum(mode="mean") for callers that must not allocate device memory (a
+    host framework that owns the GPU's memory pool, a latency-critical loop, a plug-in given only its input and output).
+    The library keeps the transform's intermediate data in an 8 MiB array of its own, so there is no d_scratch argument
+    and the C call allocates nothing; pass d_spec (float32 (N/2, 2) on the series' device) to keep this wrapper from
+    allocating the output either.  At most STATIC_SPECTRUM_MAX_SAMPLES (2^21) samples: longer series raise JerkError
+    (JERK_ELIMIT).  All calls on a GPU share that one array: keep them on one stream (overlapping calls race), and make
+    the first call on each device before any stream capture (it does a one-time address look-up)."""
+    import torch
+    lib = load_library()
+    n = d_series.numel()
+    if n > STATIC_SPECTRUM_MAX_SAMPLES:     # refused by the library as well; checked first so that no output is allocated for nothing
+        raise JerkError(JERK_ELIMIT, lib.jerk_strerror(JERK_ELIMIT).decode())
+    if d_spec is None:
+        d_spec = torch.empty((n // 2, 2), dtype=torch.float32, device=d_series.device)
+    rc = lib.jerk_prepare_spectrum_static(C.c_void_p(d_series.data_ptr()), int(n), int(block), C.c_void_p(d_spec.data_ptr()),
+                                          _stream_ptr(stream))
     if rc != 0:
         raise JerkError(rc, lib.jerk_strerror(rc).decode())
     return d_spec

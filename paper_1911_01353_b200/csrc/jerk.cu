@@ -2173,6 +2173,7 @@ const char* jerk_strerror(int status) {
     case JERK_ESTATE: return "JERK_ESTATE: template bank not built";
     case JERK_ENODEV: return "JERK_ENODEV: no sm_100 device";
     case JERK_EOVERFLOW: return "JERK_EOVERFLOW: more candidates or seam records than the caller's buffers hold";
+    case JERK_ELIMIT: return "JERK_ELIMIT: request exceeds a fixed built-in capacity (jerk_prepare_spectrum_static: at most 2^21 samples; use jerk_prepare_spectrum with caller scratch)";
   }
   return "unknown jerk status";
 }

@@ -14,6 +14,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <mutex>
+
 #include "../../include/jerk.h"
 #include "jerk_fft.cuh"
 
@@ -376,6 +378,41 @@ static cudaError_t launch_issue_probe(float* out, int iters, long long* cycles, 
 
 using namespace jerk;
 
+// ---------------------------------------------------------------------------------------------------------------------
+// jerk_prepare_spectrum_static: spectrum preparation for callers that cannot hand the library a scratch buffer
+// (include/jerk.h has the user-facing text).  The intermediate array Z of the four-step transform lives in the
+// file-scope device array below instead of in caller memory.  8 MiB per GPU that loads the library, held until the
+// process exits, which is why the limit is 2^21 samples and not the 2^25 of the caller-scratch entry points.
+//
+// g_static_scratch is a device symbol: in host code its name is only a handle (a host-side shadow variable), never
+// a device address, so nothing in this file passes `g_static_scratch` or `&g_static_scratch[0]` to a kernel.  The
+// address a kernel can use comes from cudaGetSymbolAddress, asked once per device with that device current; every
+// device has its own copy of the array at its own address, hence the table indexed by device ordinal.
+constexpr int64_t kStaticMaxSamples = JERK_STATIC_SPECTRUM_MAX_SAMPLES;
+constexpr uint64_t kStaticScratchBytes = (uint64_t)(kStaticMaxSamples / 2) * sizeof(float2);
+constexpr int kStaticMaxDevices = 64;
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+static void* g_static_scratch_addr[kStaticMaxDevices];   // [device ordinal] -> device address of that device's copy (null: not asked yet)
+static std::mutex g_static_scratch_mutex;
+
+// Device address of the current device's copy of g_static_scratch (looked up on the first call per device).
+static int static_scratch_for_current_device(void** out) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) return JERK_ENODEV;
+  if (dev < 0 || dev >= kStaticMaxDevices) return JERK_ENODEV;
+  std::lock_guard<std::mutex> lock(g_static_scratch_mutex);
+  if (!g_static_scratch_addr[dev]) {
+    void* ptr = nullptr;
+    if (cudaGetSymbolAddress((void**)&ptr, g_static_scratch) != cudaSuccess || !ptr) {
+      (void)cudaGetLastError();   // leave no sticky "last error" behind for the caller's next launch check
+      return JERK_ECUDA;
+    }
+    g_static_scratch_addr[dev] = ptr;
+  }
+  *out = g_static_scratch_addr[dev];
+  return JERK_OK;
+}
+
 extern "C" {
 
 // blocks of the red-noise schedule are at least 6 bins long: M / 6 + 2 starts at most, + the count
@@ -451,6 +488,18 @@ int jerk_prepare_spectrum_mode(const float* d_series, int64_t nsamples, int bloc
   }
   if (cudaGetLastError() != cudaSuccess) return JERK_ECUDA;
   return JERK_OK;
+}
+
+int jerk_prepare_spectrum_static(const float* d_series, int64_t nsamples, int block, void* d_spec, void* stream) {
+  if (!d_series || !d_spec || block < 1) return JERK_EINVAL;
+  if (nsamples > kStaticMaxSamples) return JERK_ELIMIT;   // before anything else looks at the size: the array cannot grow
+  void* scratch = nullptr;
+  const int rc = static_scratch_for_current_device(&scratch);
+  if (rc != JERK_OK) return rc;
+  // Same three launches as jerk_prepare_spectrum, with Z in the static array.  Launch B writes all nsamples/2 elements
+  // of Z before the third launch reads them, so whatever an earlier call left in the array is never read and nothing
+  // has to be cleared.  No cudaMalloc / cudaFree / allocating library call on this path.
+  return jerk_prepare_spectrum_mode(d_series, nsamples, block, JERK_NORM_MEAN, d_spec, scratch, kStaticScratchBytes, stream);
 }
 
 int jerk_probe_issue(void* d_scratch, int iters, double* h_cycles_per_round, void* stream) {
