@@ -124,6 +124,8 @@ int jerk_templates(jerk_plan* plan, void* d_bank, uint64_t bank_bytes, void* str
  * (>= jerk_bank_bytes_range(plan, ti_cnt) bytes: the c/hw tables of the whole grid + ti_cnt filters).  This is what one
  * rank of a template-sharded multi-GPU search holds ("each GPU holds 1/G of the bank"); afterwards the
  * plan searches only boxes / ranges inside it (JERK_ESTATE otherwise).  jerk_templates is the range [0, ntemplates).
+ * ti_cnt == 0 is allowed (a rank left without templates when there are more ranks than templates): only the tables are
+ * written, and the plan then accepts empty search ranges only.
  */
 uint64_t jerk_bank_bytes_range(const jerk_plan* plan, int ti_cnt);
 int jerk_templates_range(jerk_plan* plan, int ti_lo, int ti_cnt, void* d_bank, uint64_t bank_bytes, void* stream);
@@ -263,7 +265,8 @@ int jerk_search_series_host(jerk_plan* plan, const float* h_series, int64_t nsam
  * plane-mode launch stores the seven sub-planes of fractions 1/8..7/8 (and the block maxima of every unit) in
  * d_scratch, and the search of the chunk itself (fraction 8/8, never stored) adds the gathered sub-harmonic powers to
  * its own powers on chip and keeps the arg-max; the gathers are skipped wherever an exact upper bound built from the
- * block maxima cannot reach the running record.  Other seg_len: all eight sub-planes are stored and summed by a
+ * block maxima cannot reach the running record.  Other seg_len, and seg_len 4096 with templates wider than
+ * hw_max = 512 (the bound needs blocks of at least 449 valid outputs): all eight sub-planes are stored and summed by a
  * separate kernel.
  * d_scratch: DEVICE, 256-byte aligned, >= 1/256 of jerk_harmonic_scratch_bytes(plan) (that size gives the
  * default 65536-bin chunk; smaller buffers give smaller chunks, larger ones longer chunks up to 524288 bins with

@@ -2332,7 +2332,9 @@ uint64_t jerk_bank_bytes_range(const jerk_plan* p, int ti_cnt) {
 
 int jerk_templates_range(jerk_plan* p, int ti_lo, int ti_cnt, void* d_bank, uint64_t bank_bytes, void* stream) {
   if (!p || !d_bank) return JERK_EINVAL;
-  if (ti_lo < 0 || ti_cnt < 1 || ti_lo + ti_cnt > p->T) return fail(p, JERK_EINVAL, "template range outside [0, ntemplates)");
+  // ti_cnt == 0 (a rank of a sharded search that is left without templates: more ranks than templates) is legal: the
+  // geometry tables are copied, no filter is built, and only empty ranges can be searched afterwards
+  if (ti_lo < 0 || ti_cnt < 0 || ti_lo > p->T - ti_cnt) return fail(p, JERK_EINVAL, "template range outside [0, ntemplates)");
   if (bank_bytes < jerk_bank_bytes_range(p, ti_cnt)) return fail(p, JERK_ENOMEM, "bank buffer smaller than jerk_bank_bytes_range");
   if ((uintptr_t)d_bank % kBankAlign) return fail(p, JERK_EINVAL, "d_bank must be 256-byte aligned");
   int rc = ensure_device(p);
@@ -2351,7 +2353,8 @@ int jerk_templates_range(jerk_plan* p, int ti_lo, int ti_cnt, void* d_bank, uint
   bp.ti_lo = ti_lo;
   bp.geom = (const TemplateGeom*)d_bank;
   bp.G = (float2*)((unsigned char*)d_bank + p->geom_bytes);
-  switch (p->L) {
+  switch (ti_cnt ? p->L : 0) {
+    case 0: break;
     case 1024: e = launch_bank<1024>(p, bp, ti_cnt, st); break;
     case 2048: e = launch_bank<2048>(p, bp, ti_cnt, st); break;
     case 4096: e = launch_bank<4096>(p, bp, ti_cnt, st); break;
@@ -2543,7 +2546,7 @@ int jerk_snr_filter(jerk_plan* p, const double* d_rowstats, const jerk_cand* d_c
   cudaStream_t st = (cudaStream_t)stream;
   cudaError_t e = cudaMemsetAsync(d_count_out, 0, sizeof(unsigned long long), st);
   if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("count memset: ") + cudaGetErrorString(e));
-  k_snr_filter<<<p->sm_count, 256, 0, st>>>(d_rowstats, p->nz, 2.0 * (double)p->nbins, d_cands_in, d_count_in, max_in, snr_threshold,
+  k_snr_filter<<<p->sm_count, 256, 0, st>>>(d_rowstats, p->nz, (double)p->numbetween * (double)p->nbins, d_cands_in, d_count_in, max_in, snr_threshold,
                                             d_cands_out, max_out, d_count_out);
   e = cudaGetLastError();
   if (e != cudaSuccess) return fail(p, JERK_ECUDA, std::string("k_snr_filter launch: ") + cudaGetErrorString(e));
@@ -2648,8 +2651,14 @@ static int host_rnd_eighths(int a, int e) {
 // placement in scratch after the header, the arg-max records, and the total bytes needed.  seg_len 4096 (`fused`): the
 // top-harmonic pass itself is the consumer, fraction 8/8 is never stored and the records are one per warp of that launch;
 // other lengths: all eight sub-planes are stored and k_harm sums them (records per k_harm block).
+// The fused path's pruning bounds a pair of batches (512 outputs, at most 449 source bins of a fraction) by the block maxima
+// at its first and last source bin only (harm_bounds_mask), which is exact as long as no block of a unit is shorter
+// than 449 outputs.  The edge blocks are cut to 1024 - hw_max outputs by the valid window: hw_max <= 575 would do, 512 is
+// the documented gate.  Wider templates take the stored-sub-plane path (k_harm), which has no bounds.
+static bool harm_fused(const jerk_plan* p) { return p->L == 4096 && p->hw_max <= 512; }
+
 static uint64_t harm_layout(const jerk_plan* p, const HarmBox& bx, HarmSubBox (&sub)[8], uint64_t* best_off, int* nblocks, int* ntiles) {
-  const bool fused = p->L == 4096;
+  const bool fused = harm_fused(p);
   const int cz = (p->nz - 1) / 2, cw = (p->nw - 1) / 2;
   const int64_t j_lo = 2 * bx.r_lo, j_hi = 2 * (bx.r_lo + bx.r_cnt) - 1;   // inclusive
   uint64_t off = kHarmHeader + (fused ? kHarmGuard : 0);
@@ -2687,7 +2696,7 @@ static uint64_t harm_layout(const jerk_plan* p, const HarmBox& bx, HarmSubBox (&
 // inside the top-harmonic search pass itself for seg_len 4096 (k_search64<MODE_HARM>), by k_harm otherwise.
 static int harm_box(jerk_plan* p, const void* d_spec, const HarmBox& bx, unsigned char* scratch, uint64_t scratch_bytes,
                     void* d_work, uint64_t work_bytes, float* d_out, int out_stage, const float* thr4, bool first, cudaStream_t st) {
-  const bool fused = p->L == 4096;
+  const bool fused = harm_fused(p);
   HarmSubBox sub[8];
   uint64_t bb_off;
   int nblocks, ntiles;

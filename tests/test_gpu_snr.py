@@ -91,6 +91,45 @@ def test_row_statistics_on_every_seg_len(setup, seg_len):
     assert n0 == n1 and np.array_equal(np.sort(plain, order=["iw", "iz", "j"]), np.sort(fused, order=["iw", "iz", "j"]))
 
 
+@pytest.mark.parametrize("seg_len", [4096, 2048])
+def test_row_statistics_and_snr_with_numbetween_one(setup, seg_len):
+    """numbetween = 1 (SURVEY.md 8(f) N4 with N2): a row holds nbins points, not 2 nbins -- the sums, and the mean and
+    sigma the S/N filter derives from them, are those of the oracle's phase-0 points (oracle section I = even j of section C)."""
+    X, plan, d_spec, zs, ws, rows = setup
+    p1 = binding.Plan(NBINS, ZMAX, DZ, WMAX, DW, 1, seg_len)
+    p1.templates()
+    rows1 = [P[0::2] for P in rows]
+    assert np.abs(orc.power_row_nb1(X, float(zs[3]), float(ws[2]), 12000, 64) - rows1[2 * zs.size + 3][12000:12064]).max() < 1e-9
+    d_c, d_n, d_stats = p1.search_candidates_stats(d_spec, THR)
+    stats = d_stats.cpu().numpy()
+    want = np.array([orc.row_stats(P) for P in rows1])
+    assert np.abs(stats[:, 0] / want[:, 0] - 1.0).max() < 2e-5
+    assert np.abs(stats[:, 1] / want[:, 1] - 1.0).max() < 1e-4
+    d_o, d_no = p1.snr_filter(d_stats, d_c, d_n, SNR_THR)
+    kept, nk = binding.candidates_to_numpy(d_o, d_no)
+    cands, n = binding.candidates_to_numpy(d_c, d_n)
+    assert 0 < nk < n
+    kept_keys = {(int(c["iw"]), int(c["iz"]), int(c["j"])): c for c in kept}
+    nz = zs.size
+    strong = 0
+    for c in cands:
+        P = rows1[int(c["iw"]) * nz + int(c["iz"])]
+        mean, std = orc.row_mean_std(P)
+        s_ref = float(orc.snr(P[int(c["j"])], mean, std))
+        key = (int(c["iw"]), int(c["iz"]), int(c["j"]))
+        if s_ref > 1.02 * SNR_THR:
+            strong += 1
+            assert key in kept_keys, (key, s_ref)
+        if s_ref < 0.98 * SNR_THR:
+            assert key not in kept_keys, (key, s_ref)
+        if key in kept_keys:
+            s_gpu = float(np.array(kept_keys[key]["flags"], dtype=np.uint32).view(np.float32))
+            assert abs(s_gpu - s_ref) <= 2e-3 * max(1.0, abs(s_ref))
+    assert strong > 0
+    iz0, iw0 = int(np.argmin(np.abs(zs - 10.0))), int(np.argmin(np.abs(ws - 40.0)))
+    assert (iw0, iz0, 12345) in kept_keys
+
+
 # ------------------------------------------------------------------------------------------------ cross-row sifting
 def _to_tuples(a):
     return [(int(c["j"]), int(c["iz"]), int(c["iw"]), float(c["power"])) for c in a]
