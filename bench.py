@@ -235,8 +235,10 @@ def run_reference(args, cfg_index):
 def _config_dict(cfg, seg_len=None, mode="candidate mode"):
     L = cfg.seg_len if seg_len is None else seg_len
     return {
-        "workload": f"BASELINE.json configs[{cfg.index - 1}] '{cfg.name}': N=2^{cfg.log2n}, zmax={cfg.zmax:g} dz={cfg.dz:g}, "
-                    f"wmax={cfg.wmax:g} dw={cfg.dw:g}, numbetween=2, seg_len={L}, {mode} thr={cfg.threshold:g}",
+        # kept under 120 characters: the driver's parser cuts longer strings
+        "workload": f"configs[{cfg.index - 1}] N=2^{cfg.log2n} zmax={cfg.zmax:g} dz={cfg.dz:g} wmax={cfg.wmax:g} dw={cfg.dw:g} "
+                    f"nb=2 seg_len={L} {mode} thr={cfg.threshold:g}",
+        "workload_name": cfg.name,
         "nbins": cfg.nbins, "nz": cfg.nz, "nw": cfg.nw, "points_per_search": cfg.points,
         "cache": "inputs larger than L2: the 0.8 GB template bank is streamed every step (no L2 flush needed)",
         "parallelism": "one independent spectrum (DM trial) per GPU, bank replicated; no data-path collective",
@@ -261,15 +263,25 @@ def _time_steps(fn, warmup, steps):
     return ts
 
 
-def _row_entry(ts, points, flops, extra=None):
+def _row_entry(ts, points, flops, extra=None, flops_nominal=None):
+    """`flops` = SURVEY.md 8(d) per-unit flops x the (segment, template-phase) units the timed launches EXECUTE;
+    `flops_nominal` (optional) = the same per-unit figure x the nominal ceil(nbins/step) * 2T units of the workload."""
     ms = float(np.median(ts))
     e = {"ms": ms, "ms_best": float(min(ts)), "steps": len(ts), "points_per_s": points / (ms * 1e-3) if points else None}
     if flops:
-        e["tflops_algorithmic"] = flops / (ms * 1e-3) / 1e12
-        e["frac_fp32_peak"] = e["tflops_algorithmic"] / FP32_PEAK_TFLOPS
+        e["tflops_executed"] = flops / (ms * 1e-3) / 1e12
+        e["frac_fp32_peak"] = e["tflops_executed"] / FP32_PEAK_TFLOPS
+    if flops_nominal:
+        e["frac_nominal_workload"] = flops_nominal / (ms * 1e-3) / 1e12 / FP32_PEAK_TFLOPS
     if extra:
         e.update(extra)
     return e
+
+
+def _plane_flops(info):
+    """Plane mode runs every template on the hw_max segmentation: nseg * numbetween * T units of 5 L log2 L + 6 L + 3 step flops."""
+    L = int(info.seg_len)
+    return float(info.nseg) * info.numbetween * info.ntemplates * (5.0 * L * np.log2(L) + 6.0 * L + 3.0 * info.step)
 
 
 def run_cufft_comparator(args, cfg, out):
@@ -369,8 +381,9 @@ def run_row(args):
         plan = binding.Plan(cfg.nbins, cfg.zmax, cfg.dz, cfg.wmax, cfg.dw, 2, cfg.seg_len)
         plan.templates()
         d_spec = binding.spectrum_to_device(X)
-        points, flops = cfg.points, plan.info.flops_per_search
+        points, flops = cfg.points, plan.info.flops_per_search_executed      # stats / batch: candidate searches on the overlap classes
         if args.row == "harmonic":
+            flops = plan.info.flops_per_search
             nbytes = args.scratch_gb << 30 if args.scratch_gb else harmonic_scratch_bytes(plan, torch.cuda.mem_get_info()[0])
             out["scratch_bytes"] = nbytes
             flops *= HARM_FLOP_FACTOR
@@ -387,6 +400,7 @@ def run_row(args):
         else:
             plane = torch.empty((cfg.nw, cfg.nz, 2 * cfg.nbins), dtype=torch.float32, device="cuda")
             fn = lambda: plan.search_plane(d_spec, 0, cfg.nbins, out=plane)
+            flops = _plane_flops(plan.info)
             out["algorithmic_bytes"] = plane.numel() * 4
     ts = _time_steps(fn, args.warmup, args.steps)
     out.update(_row_entry(ts, points, flops))
@@ -416,12 +430,14 @@ def other_rows(steps=3):
             ts = _time_steps(lambda: plan.search_candidates(d_spec, cfg.threshold), 3, n_steps)
             n = int(plan.search_candidates(d_spec, cfg.threshold)[1].item())
             rows[f"config{idx}_candidates_seg{L if L else '0(%d)' % int(plan.info.seg_len)}"] = _row_entry(
-                ts, cfg.points, plan.info.flops_per_search, {"seg_len": int(plan.info.seg_len), "candidates": n})
+                ts, cfg.points, plan.info.flops_per_search_executed, {"seg_len": int(plan.info.seg_len), "candidates": n},
+                flops_nominal=plan.info.flops_per_search)
             if idx == 2:
                 plane = torch.empty((cfg.nw, cfg.nz, 2 * cfg.nbins), dtype=torch.float32, device="cuda")
                 ts = _time_steps(lambda: plan.search_plane(d_spec, 0, cfg.nbins, out=plane), 3, steps)
-                rows[f"config2_plane_mode_seg{L if L else '0(%d)' % int(plan.info.seg_len)}"] = _row_entry(ts, cfg.points, plan.info.flops_per_search,
-                                                                {"plane_bytes": plane.numel() * 4, "plane_GBps": plane.numel() * 4 / np.median(ts) / 1e6})
+                rows[f"config2_plane_mode_seg{L if L else '0(%d)' % int(plan.info.seg_len)}"] = _row_entry(ts, cfg.points, _plane_flops(plan.info),
+                                                                {"plane_bytes": plane.numel() * 4, "plane_GBps": plane.numel() * 4 / np.median(ts) / 1e6},
+                                                                flops_nominal=plan.info.flops_per_search)
                 del plane
             del plan
         del d_spec
@@ -436,17 +452,19 @@ def other_rows(steps=3):
         d_c, d_n, d_s = plan.search_candidates_stats(d_spec, cfg.threshold)
         return plan.snr_filter(d_s, d_c, d_n, 20.0)
 
-    rows["config3_candidates_with_row_statistics"] = _row_entry(_time_steps(stats, 3, steps), cfg.points, plan.info.flops_per_search)
+    rows["config3_candidates_with_row_statistics"] = _row_entry(_time_steps(stats, 3, steps), cfg.points, plan.info.flops_per_search_executed,
+                                                                flops_nominal=plan.info.flops_per_search)
     nspec = 4
     specs = [d_spec] + [binding.spectrum_to_device(synth.make_spectrum(synth.config(3), trial=b)) for b in range(1, nspec)]
     ts = _time_steps(lambda: plan.search_candidates_batch(specs, cfg.threshold), 3, 2)
-    rows["config3_batch_of_4_spectra"] = _row_entry(ts, nspec * cfg.points, nspec * plan.info.flops_per_search,
-                                                    {"nspec": nspec, "ms_per_spectrum": float(np.median(ts)) / nspec})
+    rows["config3_batch_of_4_spectra"] = _row_entry(ts, nspec * cfg.points, nspec * plan.info.flops_per_search_executed,
+                                                    {"nspec": nspec, "ms_per_spectrum": float(np.median(ts)) / nspec},
+                                                    flops_nominal=nspec * plan.info.flops_per_search)
     del specs
     plan1 = binding.Plan(cfg.nbins, cfg.zmax, cfg.dz, cfg.wmax, cfg.dw, 1, cfg.seg_len)
     plan1.templates()
     ts = _time_steps(lambda: plan1.search_candidates(d_spec, cfg.threshold), 3, steps)
-    rows["config3_numbetween1"] = _row_entry(ts, cfg.points // 2, plan1.info.flops_per_search)
+    rows["config3_numbetween1"] = _row_entry(ts, cfg.points // 2, plan1.info.flops_per_search_executed, flops_nominal=plan1.info.flops_per_search)
     del plan1, d_spec
     torch.cuda.empty_cache()
     cfg = synth.config(5)
@@ -457,9 +475,12 @@ def other_rows(steps=3):
     top = plan.harmonic_sum(d_spec, scratch_bytes=nbytes)
     rows["config5_harmonic_sum_1_2_4_8"] = _row_entry(
         ts, cfg.points, plan.info.flops_per_search * HARM_FLOP_FACTOR,
-        {"scratch_bytes": nbytes, "stage_tops": [{"h": h, "j": int(r["j"]), "iz": int(r["iz"]), "iw": int(r["iw"]), "S": float(r["power"])}
+        {"scratch_bytes": nbytes,
+         # the method's own work is ONE search plus seven adds per point (the sub-planes are the same plane on nested boxes):
+         "frac_fp32_peak_one_search": plan.info.flops_per_search / (float(np.median(ts)) * 1e-3) / 1e12 / FP32_PEAK_TFLOPS, "stage_tops": [{"h": h, "j": int(r["j"]), "iz": int(r["iz"]), "iw": int(r["iw"]), "S": float(r["power"])}
                                                   for h, r in zip((1, 2, 4, 8), top)],
-         "flops_note": "algorithmic flops = (1^3 + ... + 8^3)/512 = 2.53 base searches (the eight sub-volumes of fractions e/8)"})
+         "flops_note": "frac_fp32_peak credits the 2.53 base searches this design executes ((1^3 + ... + 8^3)/512: the eight sub-volumes "
+                       "of fractions e/8 are recomputed); frac_fp32_peak_one_search counts the one search the method needs"})
     return rows
 
 
@@ -665,7 +686,10 @@ def main():
         value = world * cfg.points / (ms_per_step * 1e-3)
         e2e_value = world * cfg.points / (e2e_ms / args.steps * 1e-3)
         kernel_ms = float(np.mean(step_ms))                   # k_search is > 99.9 % of a step (profiles/)
-        achieved = info.flops_per_search / (kernel_ms * 1e-3) / 1e12
+        # SURVEY.md 8(d) per-unit flops x the units ONE launch executes (the overlap classes run fewer units than the nominal
+        # ceil(nbins/step) * 2T of the workload; the nominal figure is kept beside it)
+        achieved = info.flops_per_search_executed / (kernel_ms * 1e-3) / 1e12
+        achieved_nominal = info.flops_per_search / (kernel_ms * 1e-3) / 1e12
         peaks = _measured_peaks()
         try:
             measured_fp32 = binding.probe_fp32_tflops()
@@ -680,13 +704,13 @@ def main():
             "bound": "alu", "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
             "traffic": traffic, "traffic_unit": traffic_unit,
             "kernel": "k_search64<cand>" if cfg.seg_len == 4096 else f"k_search<{cfg.seg_len},cand>", "kernel_ms": kernel_ms,
-            "algorithmic_flops_per_launch": info.flops_per_search,
             # what the launch executes: the overlap classes give narrow templates longer steps, i.e. fewer (segment,
             # template-phase) units than the nominal ceil(nbins/step) * 2T of SURVEY.md 8(d) for the same points
             "executed_units_per_launch": int(info.units_per_search), "executed_flops_per_launch": info.flops_per_search_executed,
-            "frac_executed": info.flops_per_search_executed / (kernel_ms * 1e-3) / 1e12 / FP32_PEAK_TFLOPS,
-            "note": "achieved/frac use the nominal algorithmic flops of the workload (SURVEY.md 8(d): 5L log2 L + 6L + 3 step per unit, "
-                    "ceil(nbins/step) * 2T units, step = L - 2 hw_max); frac_executed counts only the units the kernel runs (DESIGN.md 6.2)",
+            "nominal_flops_per_search": info.flops_per_search,
+            "achieved_nominal_workload": achieved_nominal, "frac_nominal_workload": achieved_nominal / FP32_PEAK_TFLOPS,
+            "note": "achieved/frac = SURVEY.md 8(d) flops per unit (5L log2 L + 6L + 3 step) x executed_units_per_launch / kernel_ms; "
+                    "*_nominal_workload uses the workload's nominal ceil(nbins/step) * 2T units at step = L - 2 hw_max (DESIGN.md 6.2)",
             "issue_probe": issue,      # jerk_probe_issue: what a non-FMA instruction costs next to packed FP32
             "peak_measured_ffma": measured_fp32, "frac_of_measured_ffma": (achieved / measured_fp32) if measured_fp32 else None,
             "peak_source": "FP32 FMA nominal: 148 SMs x 128 lanes x 2 x 1.965 GHz (DESIGN.md); MEASURED_PEAKS.json has no fp32 entry"

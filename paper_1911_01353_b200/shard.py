@@ -107,7 +107,14 @@ def build_bank_shard(plan, group=None):
     world = dist.get_world_size(group) if sharded else 1
     rank = dist.get_rank(group) if sharded else 0
     ti_lo, ti_cnt = template_range(plan.info.ntemplates, world, rank)
-    plan.templates_range(ti_lo, ti_cnt)
+    err = None
+    try:
+        plan.templates_range(ti_lo, ti_cnt)       # ti_cnt == 0 (more ranks than templates) builds the tables only
+    except Exception as exc:                      # noqa: BLE001 -- reported below, on every rank
+        err = exc
+    # a rank must not raise alone: the others would wait for it in the next collective
+    if (agree_on_failure(err is not None, group) if sharded else err is not None):
+        raise RuntimeError(f"building the bank shard failed on at least one rank (rank {rank}: {err})") from err
     return ti_lo, ti_cnt
 
 

@@ -140,6 +140,43 @@ def test_harmonic_prune_kernel_small_volume():
             assert (rec["iw"], rec["iz"], rec["j"]) == (iw, iz, j)
 
 
+def test_harmonic_wide_templates_seg_len_4096():
+    """hw_max = 708 > 512 at seg_len 4096 (zmax 1200, wmax 400): the edge blocks of a unit are shorter than a pair's source
+    range, so the block-maxima bound of the fused pass does not hold and the library must take the stored-sub-plane path.
+    Whole S_h volume and stage tops vs the oracle, at thresholds 0 and at thresholds just under the true maxima (the
+    setting in which a wrongly pruned pair loses the arg-max)."""
+    nbins = 9000
+    rng = np.random.Generator(np.random.PCG64(47))
+    n = 2 * nbins
+    x = rng.standard_normal(n)
+    r0, z0, w0 = 410.5, 50.0, 25.0
+    a = np.sqrt(4.0 * 60.0 / n)
+    for k in range(1, 9):
+        x += synth.chirp_series(n, k * r0, k * z0, k * w0, a / k)
+    X = synth.block_normalise(np.fft.rfft(x)[:nbins]).astype(np.complex64)
+    plan = binding.Plan(nbins, 1200, 400, 400, 200, 2, 4096)
+    assert plan.info.hw_max == 708 and plan.info.ntemplates == 7 * 5
+    plan.templates()
+    d_spec = binding.spectrum_to_device(X)
+    P = orc.plane(X, 1200, 400, 400, 200)
+    top = plan.harmonic_sum(d_spec, STAGES, (0.0,) * 4)
+    maxima = []
+    for s, h in enumerate(STAGES):
+        S_ref = orc.harmonic_sum_volume(P, h)
+        g = plan.harmonic_plane(d_spec, h, 0, nbins).cpu().numpy()
+        err = np.abs(g.astype(np.float64) - S_ref) - _harm_tol(h, S_ref)
+        assert err.max() <= 0, f"h={h}: worst excess {err.max()}"
+        rec = top[s]
+        assert np.unravel_index(np.argmax(g), g.shape) == (rec["iw"], rec["iz"], rec["j"]) and g.max() == rec["power"]
+        iw, iz, j = np.unravel_index(np.argmax(S_ref), S_ref.shape)
+        second = np.partition(S_ref.ravel(), -2)[-2]
+        if S_ref[iw, iz, j] - second > 2 * _harm_tol(h, S_ref[iw, iz, j]):
+            assert (rec["iw"], rec["iz"], rec["j"]) == (iw, iz, j)
+        maxima.append(float(g.max()))
+    near = plan.harmonic_sum(d_spec, STAGES, tuple(0.999 * m for m in maxima))
+    assert np.array_equal(near, top)
+
+
 class _OraclePowers:
     """P_ref(j, iz', iw') on demand (signed grid indices), one oracle row segment per request, cached."""
 

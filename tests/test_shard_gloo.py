@@ -53,7 +53,11 @@ def _worker(rank, world, port, nz, nw, q):
             info = _Info()
             overflow_rank = -1
 
+            build_fail_rank = -1
+
             def templates_range(self, ti_lo, ti_cnt):
+                if rank == self.build_fail_rank:
+                    raise ValueError("stand-in build failure")
                 self.bank_range = (ti_lo, ti_cnt)
 
             def search_candidates_templates(self, d_spec, thr, ti_lo, ti_cnt, max_cands):
@@ -80,6 +84,23 @@ def _worker(rank, world, port, nz, nw, q):
         except RuntimeError:
             pass
         plan.overflow_rank = -1
+        # a bank build that fails on ONE rank raises on EVERY rank before anybody enters the next collective
+        plan.build_fail_rank = 0
+        try:
+            shard.build_bank_shard(plan)
+            ok_merge = False
+        except RuntimeError:
+            pass
+        plan.build_fail_rank = -1
+        # more ranks than templates: the surplus ranks build and search an empty range and the merge is still complete
+        _FakePlan.info.ntemplates = world - 1
+        lo0, cnt0 = shard.build_bank_shard(plan)
+        ok_merge = ok_merge and (cnt0 == (1 if rank < world - 1 else 0))
+        merged3 = shard.search_candidates_sharded(plan, X, 40.0, max_cands=4096)
+        ti_all = full["iw"].astype(np.int64) * nz + full["iz"]
+        want3 = np.sort(full[(ti_all < world - 1) & (full["power"] > 40.0)], order=["iw", "iz", "j"])
+        ok_merge = ok_merge and np.array_equal(merged3, want3)
+        _FakePlan.info.ntemplates = nz * nw
         tmax = shard.max_over_ranks(10.0 + rank)
         q.put((rank, ok_merge, ok_bcast, tmax, shard.trial_indices(7, world, rank)))
     finally:
