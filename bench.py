@@ -245,6 +245,85 @@ def _config_dict(cfg, seg_len=None, mode="candidate mode"):
     }
 
 
+# ------------------------------------------------------------------------------------------------ measurement probes
+# bench_probes.cu (beside this file) holds two measurement kernels that are not part of the library: built here into
+# bench_probes.so (nvcc, sm_100a) and called through ctypes.
+_PROBE_SRC = os.path.join(ROOT, "bench_probes.cu")
+_PROBE_LIB = os.path.join(ROOT, "bench_probes.so")
+_probes = None
+
+
+def build_probes(force=False):
+    """nvcc bench_probes.cu -> bench_probes.so (skipped when the library is newer than the source)."""
+    import subprocess
+    from paper_1911_01353_b200 import build as _build
+    if not force and os.path.exists(_PROBE_LIB) and os.path.getmtime(_PROBE_LIB) >= os.path.getmtime(_PROBE_SRC):
+        return _PROBE_LIB
+    cmd = [_build.nvcc_path(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
+           "-shared", "-o", _PROBE_LIB, _PROBE_SRC]
+    res = subprocess.run(cmd, capture_output=True, text=True)
+    if res.returncode != 0:
+        sys.stderr.write(res.stdout + res.stderr)
+        raise RuntimeError("nvcc failed building bench_probes.so")
+    return _PROBE_LIB
+
+
+def _load_probes():
+    global _probes
+    if _probes is None:
+        import ctypes as C
+        lib = C.CDLL(build_probes())
+        lib.bench_probe_fma.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double), C.c_void_p]
+        lib.bench_probe_issue.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double), C.c_void_p]
+        _probes = lib
+    return _probes
+
+
+def _cur_stream():
+    import ctypes as C
+    import torch
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def probe_fp32_tflops(iters=1 << 15, reps=5):
+    """Measured FP32 FMA throughput of the current device in TFLOP/s (bench_probe_fma timed with CUDA events, best of reps)."""
+    import torch
+    import ctypes as C
+    lib = _load_probes()
+    d = torch.zeros(4, dtype=torch.float32, device="cuda")
+    fl = C.c_double(0.0)
+    best = None
+    for i in range(reps + 1):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        rc = lib.bench_probe_fma(C.c_void_p(d.data_ptr()), int(iters), C.byref(fl), _cur_stream())
+        b.record()
+        torch.cuda.synchronize()
+        if rc != 0:
+            raise RuntimeError(f"bench probe failed with status {rc}")
+        ms = a.elapsed_time(b)
+        if i > 0:
+            best = ms if best is None else min(best, ms)
+    return fl.value / (best * 1e-3) / 1e12
+
+
+def probe_issue_slots(iters=2000):
+    """bench_probe_issue: scheduler cycles per round of 8 packed FMAs + 4 companion instructions, by companion kind."""
+    import torch
+    import ctypes as C
+    lib = _load_probes()
+    d = torch.zeros(64, dtype=torch.int64, device="cuda")
+    out = (C.c_double * 6)()
+    rc = lib.bench_probe_issue(C.c_void_p(d.data_ptr()), int(iters), out, _cur_stream())
+    if rc != 0:
+        raise RuntimeError(f"bench probe failed with status {rc}")
+    kinds = ("none", "int_prmt", "lds128", "fmnmx3_abs", "ffma_scalar", "shfl")
+    base = out[0]
+    return {"cycles_per_round": {k: out[i] for i, k in enumerate(kinds)},
+            "packed_fma_cycles": base / 8.0,
+            "companion_cost_cycles": {k: (out[i] - base) / 4.0 for i, k in enumerate(kinds) if i}}
+
+
 # ------------------------------------------------------------------------------------------------ timing helpers
 def _time_steps(fn, warmup, steps):
     """Per-step CUDA-event times (ms) of fn on the current stream after `warmup` (>= 3) untimed calls."""
@@ -284,17 +363,17 @@ def _plane_flops(info):
     return float(info.nseg) * info.numbetween * info.ntemplates * (5.0 * L * np.log2(L) + 6.0 * L + 3.0 * info.step)
 
 
-def run_cufft_comparator(args, cfg, out):
-    """--row cufft (PAPER.md:45 compares its shared-memory FFT with a cuFFT-based convolution): the
-    UNFUSED pipeline on the same GPU, built from library calls only (torch.fft = cuFFT, torch elementwise kernels): for a
-    block of segments x template-phases  Y = F * G  ->  batched inverse FFT  ->  |y|^2 over the valid window  ->  row max.
-    It is a comparator, not a product path: it uses this library's bank (re-ordered to natural order), is checked
-    against jerk_search_plane on one block, is timed on a bounded sample of the config-3 workload and extrapolated."""
+def cufft_unfused_block(cfg, warmup=3, steps=3, check_templates=(0, 100, 255)):
+    """SURVEY.md 8(f) N4; PAPER.md:45 compares its shared-memory FFT with a cuFFT-based convolution: the UNFUSED pipeline on
+    the same GPU, built from library calls only (torch.fft = cuFFT, torch elementwise kernels): for a block of segments x
+    template-phases  Y = F * G  ->  batched inverse FFT  ->  |y|^2 over the valid window  ->  row max.
+    It is a comparator, not a product path: it uses this library's bank (re-ordered to natural order), is checked against
+    jerk_search_plane on the rows of `check_templates` (flat template indices < 256, both phases), is timed on a bounded
+    sample of the workload and extrapolated.  Returns the row's dict."""
     import torch
     from paper_1911_01353_b200 import binding
     import workloads as synth
-    L = cfg.seg_len
-    assert L == 4096, "the comparator re-orders the seg_len-4096 bank layout"
+    L = 4096                                         # the comparator re-orders the seg_len-4096 bank layout
     X = synth.make_spectrum(cfg)
     plan = binding.Plan(cfg.nbins, cfg.zmax, cfg.dz, cfg.wmax, cfg.dw, 2, L)
     plan.templates()
@@ -311,37 +390,53 @@ def run_cufft_comparator(args, cfg, out):
     slot_c1 = 2 * ((2 * b) * 64 + t) + 1                      # the a = 1 entry of the same butterfly
     geom_bytes = (info.ntemplates * 8 + 255) // 256 * 256
     bank = plan.bank[geom_bytes:geom_bytes + info.ntemplates * 2 * L * 8].view(torch.float32).view(-1, L, 2)
-    ntp_blk, nseg_blk = 512, 64                      # 512 template-phases x 64 segments per block: 1 GB of complex64
+    ntp_blk = min(512, 2 * int(info.ntemplates))     # 512 template-phases x 64 segments per block: 1 GB of complex64
+    nseg_blk = min(64, int(info.nseg))
     raw = bank[:ntp_blk][:, slot, :]                                             # [ntp, L, 2] in natural element order
     c1 = bank[:ntp_blk][:, slot_c1, 0]
     c = torch.where(a[None, :] == 3, raw[..., 0] * c1, raw[..., 0])
     G = torch.where(a[None, :] == 0, torch.complex(raw[..., 0], raw[..., 1]), torch.complex(c, c * raw[..., 1]))   # [ntp, L]
-    seg0 = info.nseg // 2
+    seg0 = (int(info.nseg) - nseg_blk) // 2
     starts = info.seg_base + (seg0 + torch.arange(nseg_blk, device="cuda")) * info.step
     idx = starts[:, None] + torch.arange(L, device="cuda")[None, :]
+    inside = (idx >= 0) & (idx < cfg.nbins)                                     # X[k] = 0 outside the spectrum
+    idx_c = idx.clamp(0, cfg.nbins - 1)
     lo, hi = info.hw_max, info.hw_max + info.step
 
     def block():
-        F = torch.fft.fft(spec[idx], dim=1)                                    # [nseg, L]   (a-2)
+        F = torch.fft.fft(torch.where(inside, spec[idx_c], torch.zeros((), dtype=spec.dtype, device="cuda")), dim=1)   # [nseg, L]   (a-2)
         Y = F[:, None, :] * G[None, :, :]                                      # [nseg, ntp, L]   (a-3, written to HBM)
         y = torch.fft.ifft(Y, dim=2, norm="forward")                           # unnormalised inverse FFT (cuFFT, batched)
         P = (y.real * y.real + y.imag * y.imag)[:, :, lo:hi]                   # (a-4)
         return P, P.amax(dim=2)                                                # (a-5, reduced to a row maximum)
 
     P, mx = block()
-    # check one template-phase row of the block against the fused kernel's plane output
-    geom_c = int(plan.template_geometry(0, 0)[0])
-    b_first = int(starts[0].item()) + lo - geom_c
-    ours = plan.search_plane(d_spec, b_first, info.step, 0, 1, 0, 1)[0, 0]     # P[j], j = 2*(b - b_first) + p
-    theirs = torch.stack([P[0, 0], P[0, 1]], dim=1).reshape(-1)
-    err = float(((ours - theirs).abs() / torch.clamp(ours, min=1.0)).max())
-    assert err < 1e-3, err
-    ts = _time_steps(block, args.warmup, args.steps)
+    # check template rows of the block (all its segments, both phases) against the fused kernel's plane output
+    err = 0.0
+    for ti in check_templates:
+        if 2 * ti + 1 >= ntp_blk:
+            continue
+        iz, iw = ti % int(info.nz), ti // int(info.nz)
+        geom_c = int(plan.template_geometry(iz, iw)[0])
+        b_first = int(starts[0].item()) + lo - geom_c
+        b_lo, b_hi = max(b_first, 0), min(b_first + nseg_blk * int(info.step), cfg.nbins)
+        ours = plan.search_plane(d_spec, b_lo, b_hi - b_lo, iz, 1, iw, 1)[0, 0]     # P[j], j = 2*(b - b_lo) + p
+        theirs = torch.stack([P[:, 2 * ti].reshape(-1), P[:, 2 * ti + 1].reshape(-1)], dim=1)     # [bins of the block, phase]
+        theirs = theirs[b_lo - b_first:b_hi - b_first].reshape(-1)
+        err = max(err, float(((ours - theirs).abs() / torch.clamp(ours, min=1.0)).max()))
+    ts = _time_steps(block, warmup, steps)
     units = ntp_blk * nseg_blk
     total_units = 2 * info.ntemplates * info.nseg
-    out.update({"ms_block": ts, "units_per_block": units, "max_rel_diff_vs_fused_plane": err,
-                "extrapolated_ms_per_search": min(ts) * total_units / units,
-                "note": "library-only unfused pipeline (cuFFT through torch.fft + elementwise kernels); comparator, not a product path"})
+    ms = float(np.median(ts))
+    return {"ms": ms, "ms_block": ts, "units_per_block": units, "max_rel_diff_vs_fused_plane": err, "checked_templates": list(check_templates),
+            "extrapolated_ms_per_search": float(min(ts)) * total_units / units,
+            "note": "library-only unfused pipeline (cuFFT through torch.fft + elementwise kernels); comparator, not a product path"}
+
+
+def run_cufft_comparator(args, cfg, out):
+    """--row cufft: cufft_unfused_block on the chosen config, one JSON line."""
+    out.update(cufft_unfused_block(cfg, args.warmup, args.steps))
+    assert out["max_rel_diff_vs_fused_plane"] < 1e-3, out["max_rel_diff_vs_fused_plane"]
     print(json.dumps(out))
     return 0
 
@@ -454,6 +549,26 @@ def other_rows(steps=3):
 
     rows["config3_candidates_with_row_statistics"] = _row_entry(_time_steps(stats, 3, steps), cfg.points, plan.info.flops_per_search_executed,
                                                                 flops_nominal=plan.info.flops_per_search)
+    # threshold sensitivity of the rare candidate path (a warp with a power above the threshold stashes its powers and
+    # runs the local-max test): the S/N front end of 8(f) N2 works at powers of 8-12, not 25
+    for thr in (12.0, 9.0):
+        pt = binding.Plan(cfg.nbins, cfg.zmax, cfg.dz, cfg.wmax, cfg.dw, 2, cfg.seg_len, extra_seams=1 << 24)
+        try:
+            pt.templates()
+            max_c = 1 << 26
+            d_c = torch.empty(max_c * 16, dtype=torch.uint8, device="cuda")
+            d_n = torch.zeros(1, dtype=torch.int64, device="cuda")
+            ts = _time_steps(lambda: pt.search_candidates(d_spec, thr, max_c, d_c, d_n), 3, steps)
+            n = int(d_n.item())
+            rows[f"config3_candidates_thr{thr:g}"] = _row_entry(
+                ts, cfg.points, pt.info.flops_per_search_executed,
+                {"threshold": thr, "candidates": n if n >= 0 else "seam records overflowed d_work", "max_cands": max_c},
+                flops_nominal=pt.info.flops_per_search)
+            del d_c, d_n
+        except Exception as exc:      # noqa: BLE001 -- a row, not the headline: report and go on
+            rows[f"config3_candidates_thr{thr:g}"] = {"error": repr(exc)}
+        del pt
+        torch.cuda.empty_cache()
     nspec = 4
     specs = [d_spec] + [binding.spectrum_to_device(synth.make_spectrum(synth.config(3), trial=b)) for b in range(1, nspec)]
     ts = _time_steps(lambda: plan.search_candidates_batch(specs, cfg.threshold), 3, 2)
@@ -466,6 +581,11 @@ def other_rows(steps=3):
     ts = _time_steps(lambda: plan1.search_candidates(d_spec, cfg.threshold), 3, steps)
     rows["config3_numbetween1"] = _row_entry(ts, cfg.points // 2, plan1.info.flops_per_search_executed, flops_nominal=plan1.info.flops_per_search)
     del plan1, d_spec
+    torch.cuda.empty_cache()
+    try:
+        rows["cufft_unfused_block"] = cufft_unfused_block(cfg, 3, steps)
+    except Exception as exc:          # noqa: BLE001
+        rows["cufft_unfused_block"] = {"error": repr(exc)}
     torch.cuda.empty_cache()
     cfg = synth.config(5)
     X = synth.make_spectrum(cfg)
@@ -492,6 +612,10 @@ def run_strong(args, torch, dist, rank, local_rank, world):
     X = synth.make_spectrum(cfg)                         # every rank can make it; only rank 0's copy is used (broadcast)
     plan = binding.Plan(cfg.nbins, cfg.zmax, cfg.dz, cfg.wmax, cfg.dw, 2, cfg.seg_len)
     ti_lo, ti_cnt = shard.build_bank_shard(plan)
+    # the split is cut at equal executed units (jerk_template_units), not equal template counts: host-only, same on every rank
+    units = plan.template_units()
+    ranges = [shard.template_range(int(plan.info.ntemplates), world, r, units) for r in range(world)]
+    units_per_rank = [int(units[lo:lo + cnt].sum()) for lo, cnt in ranges]
     d_spec = binding.spectrum_to_device(X if rank == 0 else np.zeros_like(X))
     step = lambda: shard.search_candidates_sharded(plan, d_spec, cfg.threshold)
     merged = step()
@@ -524,12 +648,14 @@ def run_strong(args, torch, dist, rank, local_rank, world):
     if rank == 0:
         ms = total_ms / args.steps
         cd = _config_dict(cfg)
-        cd["parallelism"] = (f"tp{world} over the template bank: rank r builds and searches templates [r T/{world}, (r+1) T/{world}); spectrum "
+        cd["parallelism"] = (f"tp{world} over the template bank: rank r builds and searches a contiguous template range cut at equal executed units; spectrum "
                              "broadcast + candidate all-gather inside the timed step; no collective inside the search")
         print(json.dumps({
             "metric": METRIC, "value": cfg.points / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
             "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": cd, "clocks": clocks, "gathered_equals_whole_grid_search": check, "templates_per_rank": int(ti_cnt),
+            "config": cd, "clocks": clocks, "gathered_equals_whole_grid_search": check, "templates_per_rank": [int(c) for _, c in ranges],
+            # imbalance is visible apart from overhead: the slowest rank sets the step time
+            "units_per_rank": units_per_rank, "units_imbalance_max_over_mean": max(units_per_rank) / (sum(units_per_rank) / world),
             "bank_bytes_per_rank": int(plan.bank.numel()), "candidates": int(merged.size),
             "gpu_launches": (6 if int(plan.info.nclasses) > 1 else 5) * args.steps,
         }))
@@ -692,11 +818,11 @@ def main():
         achieved_nominal = info.flops_per_search / (kernel_ms * 1e-3) / 1e12
         peaks = _measured_peaks()
         try:
-            measured_fp32 = binding.probe_fp32_tflops()
+            measured_fp32 = probe_fp32_tflops()
         except Exception:
             measured_fp32 = None
         try:
-            issue = binding.probe_issue_slots()
+            issue = probe_issue_slots()
         except Exception:
             issue = None
         traffic, traffic_unit = (None, None) if args.log2n else _ncu_traffic(args.config)
@@ -711,7 +837,7 @@ def main():
             "achieved_nominal_workload": achieved_nominal, "frac_nominal_workload": achieved_nominal / FP32_PEAK_TFLOPS,
             "note": "achieved/frac = SURVEY.md 8(d) flops per unit (5L log2 L + 6L + 3 step) x executed_units_per_launch / kernel_ms; "
                     "*_nominal_workload uses the workload's nominal ceil(nbins/step) * 2T units at step = L - 2 hw_max (DESIGN.md 6.2)",
-            "issue_probe": issue,      # jerk_probe_issue: what a non-FMA instruction costs next to packed FP32
+            "issue_probe": issue,      # bench_probe_issue: what a non-FMA instruction costs next to packed FP32
             "peak_measured_ffma": measured_fp32, "frac_of_measured_ffma": (achieved / measured_fp32) if measured_fp32 else None,
             "peak_source": "FP32 FMA nominal: 148 SMs x 128 lanes x 2 x 1.965 GHz (DESIGN.md); MEASURED_PEAKS.json has no fp32 entry"
                            + (f"; hbm_gbs={peaks.get('hbm_gbs')} (not the bound here)" if peaks else ""),

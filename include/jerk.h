@@ -104,6 +104,15 @@ int jerk_plan_info(const jerk_plan* plan, jerk_plan_info_t* info);
 /* Centre c and half-width hw (bins) of template (iz, iw) as the plan computed them (host only). */
 int jerk_template_geometry(const jerk_plan* plan, int iz, int iw, int* c, int* hw);
 
+/*
+ * jerk_template_units — work per template, for balancing a template-sharded search: h_units[ti]
+ * (HOST, n = ntemplates entries, flat index ti = iw*nz + iz) receives the number of (segment, template-phase) units a
+ * whole-spectrum candidate search executes for template ti.  Templates are searched on the segmentation of their overlap
+ * class (step = seg_len - 2 hw_class), so wide templates cost more units than narrow ones; the sum over ti is
+ * jerk_plan_info's units_per_search.  Host-only.  Errors: JERK_EINVAL (null, n != ntemplates).
+ */
+int jerk_template_units(const jerk_plan* plan, int64_t* h_units, int n);
+
 /* Bytes of a plane-mode output for a sub-range: iw_cnt*iz_cnt*(2*r_cnt)*sizeof(float). */
 uint64_t jerk_plane_bytes(int64_t r_cnt, int iz_cnt, int iw_cnt);
 
@@ -351,26 +360,6 @@ int jerk_prepare_spectrum_mode(const float* d_series, int64_t nsamples, int bloc
  */
 #define JERK_STATIC_SPECTRUM_MAX_SAMPLES (1 << 21)
 int jerk_prepare_spectrum_static(const float* d_series, int64_t nsamples, int block, void* d_spec, void* stream);
-
-/*
- * jerk_probe_fma — measurement aid for the roofline denominator: launches a kernel of nothing but
- * independent FP32 fused multiply-add chains (2048 threads per SM, 16 chains per thread, `iters` iterations) on
- * `stream` and returns in *flops (HOST) the number of floating-point operations it executes; the caller times it.
- * d_out: DEVICE, >= 4 bytes (never written in practice).  Errors: JERK_EINVAL, JERK_ENODEV, JERK_ECUDA.
- */
-int jerk_probe_fma(void* d_out, int iters, double* flops, void* stream);
-
-/*
- * jerk_probe_issue — measurement aid for the issue-slot model of the search kernel.  Runs six short
- * kernels at the occupancy of k_search64 (8 warps per SM, two per scheduler); every round of a warp is 8 independent
- * packed FP32 fused multiply-adds followed by 4 companion instructions of one kind: [0] none, [1] integer
- * byte-permute, [2] 128-bit shared-memory load, [3] three-input FP32 maximum with |.| operands, [4] scalar FP32
- * fused multiply-add, [5] warp shuffle.  h_cycles_per_round (HOST, 6 doubles) receives the scheduler cycles one
- * round takes; ([k] - [0]) / 4 is what one companion instruction costs next to packed arithmetic (0 would mean it
- * issues in the shadow of the two-cycle packed instructions).  Synchronises `stream`.
- * d_scratch: DEVICE, >= 256 bytes, 8-byte aligned.  Errors: JERK_EINVAL, JERK_ENODEV, JERK_ECUDA.
- */
-int jerk_probe_issue(void* d_scratch, int iters, double* h_cycles_per_round, void* stream);
 
 const char* jerk_strerror(int status);
 const char* jerk_last_error(const jerk_plan* plan);

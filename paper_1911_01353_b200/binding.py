@@ -41,13 +41,13 @@ class PlanInfo(C.Structure):
 
 
 EXPORTS = [
-    "jerk_plan_create", "jerk_plan_destroy", "jerk_plan_info", "jerk_template_geometry", "jerk_plane_bytes",
+    "jerk_plan_create", "jerk_plan_destroy", "jerk_plan_info", "jerk_template_geometry", "jerk_template_units", "jerk_plane_bytes",
     "jerk_templates", "jerk_templates_range", "jerk_bank_bytes_range", "jerk_templates_taps", "jerk_search_plane",
     "jerk_search_candidates", "jerk_search_candidates_range", "jerk_search_candidates_templates",
     "jerk_search_candidates_batch", "jerk_search_candidates_stats", "jerk_snr_filter",
-    "jerk_sift_candidates", "jerk_probe_issue",
+    "jerk_sift_candidates",
     "jerk_search_candidates_host", "jerk_search_series_host", "jerk_harmonic_scratch_bytes", "jerk_harmonic_sum", "jerk_harmonic_plane", "jerk_spectrum_scratch_bytes",
-    "jerk_prepare_spectrum", "jerk_prepare_spectrum_mode", "jerk_prepare_spectrum_static", "jerk_probe_fma", "jerk_strerror",
+    "jerk_prepare_spectrum", "jerk_prepare_spectrum_mode", "jerk_prepare_spectrum_static", "jerk_strerror",
     "jerk_last_error",
 ]
 
@@ -68,6 +68,7 @@ def load_library() -> C.CDLL:
     lib.jerk_plan_destroy.argtypes = [vp]
     lib.jerk_plan_info.argtypes = [vp, C.POINTER(PlanInfo)]
     lib.jerk_template_geometry.argtypes = [vp, i32, i32, C.POINTER(i32), C.POINTER(i32)]
+    lib.jerk_template_units.argtypes = [vp, C.POINTER(i64), i32]
     lib.jerk_plane_bytes.argtypes = [i64, i32, i32]
     lib.jerk_plane_bytes.restype = u64
     lib.jerk_templates.argtypes = [vp, vp, u64, vp]
@@ -94,8 +95,6 @@ def load_library() -> C.CDLL:
     lib.jerk_prepare_spectrum.argtypes = [vp, i64, i32, vp, vp, u64, vp]
     lib.jerk_prepare_spectrum_mode.argtypes = [vp, i64, i32, i32, vp, vp, u64, vp]
     lib.jerk_prepare_spectrum_static.argtypes = [vp, i64, i32, vp, vp]
-    lib.jerk_probe_fma.argtypes = [vp, i32, C.POINTER(dbl), vp]
-    lib.jerk_probe_issue.argtypes = [vp, i32, C.POINTER(dbl), vp]
     lib.jerk_strerror.argtypes = [i32]
     lib.jerk_strerror.restype = C.c_char_p
     lib.jerk_last_error.argtypes = [vp]
@@ -144,6 +143,13 @@ class Plan:
         c, hw = C.c_int(), C.c_int()
         self._check(self._lib.jerk_template_geometry(self._h, int(iz), int(iw), C.byref(c), C.byref(hw)))
         return c.value, hw.value
+
+    def template_units(self):
+        """jerk_template_units: int64[ntemplates], the (segment, template-phase) units a candidate search runs per template."""
+        n = int(self.info.ntemplates)
+        buf = (C.c_int64 * n)()
+        self._check(self._lib.jerk_template_units(self._h, buf, n))
+        return np.frombuffer(buf, dtype=np.int64).copy()
 
     def plane_bytes(self, r_cnt, iz_cnt, iw_cnt):
         return int(self._lib.jerk_plane_bytes(int(r_cnt), int(iz_cnt), int(iw_cnt)))
@@ -398,43 +404,6 @@ def prepare_spectrum_static(d_series, block=1000, d_spec=None, stream=None):
     if rc != 0:
         raise JerkError(rc, lib.jerk_strerror(rc).decode())
     return d_spec
-
-
-def probe_fp32_tflops(iters=1 << 15, reps=5):
-    """Measured FP32 FMA throughput of the current device in TFLOP/s (jerk_probe_fma timed with CUDA events, best of reps)."""
-    import torch
-    lib = load_library()
-    d = torch.zeros(4, dtype=torch.float32, device="cuda")
-    fl = C.c_double(0.0)
-    best = None
-    for i in range(reps + 1):
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record()
-        rc = lib.jerk_probe_fma(C.c_void_p(d.data_ptr()), int(iters), C.byref(fl), _stream_ptr(None))
-        b.record()
-        torch.cuda.synchronize()
-        if rc != 0:
-            raise JerkError(rc, lib.jerk_strerror(rc).decode())
-        ms = a.elapsed_time(b)
-        if i > 0:
-            best = ms if best is None else min(best, ms)
-    return fl.value / (best * 1e-3) / 1e12
-
-
-def probe_issue_slots(iters=2000):
-    """jerk_probe_issue: scheduler cycles per round of 8 packed FMAs + 4 companion instructions, by companion kind."""
-    import torch
-    lib = load_library()
-    d = torch.zeros(64, dtype=torch.int64, device="cuda")
-    out = (C.c_double * 6)()
-    rc = lib.jerk_probe_issue(C.c_void_p(d.data_ptr()), int(iters), out, _stream_ptr(None))
-    if rc != 0:
-        raise JerkError(rc, lib.jerk_strerror(rc).decode())
-    kinds = ("none", "int_prmt", "lds128", "fmnmx3_abs", "ffma_scalar", "shfl")
-    base = out[0]
-    return {"cycles_per_round": {k: out[i] for i, k in enumerate(kinds)},
-            "packed_fma_cycles": base / 8.0,
-            "companion_cost_cycles": {k: (out[i] - base) / 4.0 for i, k in enumerate(kinds) if i}}
 
 
 def candidates_to_numpy(d_cands, d_count):

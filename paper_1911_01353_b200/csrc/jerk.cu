@@ -2037,7 +2037,7 @@ static bool add_job(const jerk_plan* p, SearchParams& sp, int64_t r_lo, int64_t 
 // template-phases per work item: kChunkTP when the box is large; smaller (even, >= 16) when the box alone could not
 // give every resident CTA a few items
 static int pick_chunk_tp(const jerk_plan* p, int64_t r_cnt, int iz_cnt, int iw_cnt) {
-  long long ntp = 2LL * iz_cnt * iw_cnt;
+  long long ntp = (long long)p->numbetween * iz_cnt * iw_cnt;   // template-phases
   long long segs = r_cnt / p->step + 2;
   long long want_items = 32LL * 4 * (p->sm_count > 0 ? p->sm_count : 148);   // >= 32 rounds of work items per resident FFT group: tail < 3 %
   int c = kChunkTP;
@@ -2298,6 +2298,23 @@ int jerk_plan_info(const jerk_plan* p, jerk_plan_info_t* info) {
       info->flops_per_search_executed += (double)units * (5.0 * p->L * l2 + 6.0 * p->L + 3.0 * step);
     }
   }
+  return JERK_OK;
+}
+
+int jerk_template_units(const jerk_plan* p, int64_t* h_units, int n) {
+  if (!p || !h_units || n != p->T) return JERK_EINVAL;
+  if (p->ncls < 2) {
+    for (int ti = 0; ti < p->T; ti++) h_units[ti] = p->nseg * (int64_t)p->numbetween;
+    return JERK_OK;
+  }
+  std::vector<int64_t> nseg_cls(p->ncls, 0);
+  for (int k = 0; k < p->ncls; k++) {      // the segmentation of class k, as in jerk_plan_info / add_class_jobs
+    const int hw = p->cls_hw[k], step = p->L - 2 * hw;
+    int64_t base = -((int64_t)p->c_max + hw);
+    if (base & 1) base -= 1;
+    nseg_cls[k] = (p->nbins + p->c_max - hw - base + step - 1) / step;
+  }
+  for (int ti = 0; ti < p->T; ti++) h_units[ti] = nseg_cls[(p->geom[ti].hw - p->cls_lo) / p->cls_width] * (int64_t)p->numbetween;
   return JERK_OK;
 }
 

@@ -94,10 +94,39 @@ def max_over_ranks(value: float, group=None) -> float:
     return float(t.item())
 
 
-def template_range(ntemplates: int, world: int, rank: int) -> tuple[int, int]:
-    """(ti_lo, ti_cnt) of `rank`: a flat split of the template index ti = iw*nz + iz, at most one template of imbalance
-    (w-row blocks would give 8,8,8,8,8,7,7,7 rows of the 61 on 8 ranks: 5 %)."""
-    return block_range(ntemplates, world, rank)
+def template_range(ntemplates: int, world: int, rank: int, units=None) -> tuple[int, int]:
+    """(ti_lo, ti_cnt) of `rank`: a contiguous split of the flat template index ti = iw*nz + iz.
+    Without `units`: equal template COUNTS (at most one template of imbalance).  With `units` (int64[ntemplates] from
+    Plan.template_units(): the (segment, template-phase) units a search executes per template -- wide templates run on
+    shorter steps and cost more) the cuts are placed at equal WORK: rank r starts at the first template whose cumulative
+    units reach r/world of the total, so every rank's share is within one template's units of the mean.  The slowest
+    rank sets the step time; on the zmax 200 / wmax 600 grid an equal-count split leaves 6 % between ranks on 8 GPUs."""
+    if units is None:
+        return block_range(ntemplates, world, rank)
+    units = np.asarray(units, dtype=np.int64)
+    if units.shape != (ntemplates,) or world < 1 or not 0 <= rank < world:
+        raise ValueError("template_range: bad arguments")
+    cum = np.concatenate(([0], np.cumsum(units)))                 # cum[t] = units of templates [0, t)
+    total = int(cum[-1])
+    # cut r = the t whose cum[t] is nearest to r * total / world (integer arithmetic; ties to the smaller t)
+    def cut(r):
+        if r <= 0:
+            return 0
+        if r >= world:
+            return ntemplates
+        target = r * total
+        t = int(np.searchsorted(cum * world, target, side="left"))    # first t with cum[t] * world >= target
+        if t > 0 and target - int(cum[t - 1]) * world <= int(cum[min(t, ntemplates)]) * world - target:
+            t -= 1
+        return min(max(t, 0), ntemplates)
+    lo, hi = cut(rank), cut(rank + 1)
+    return lo, max(hi - lo, 0)
+
+
+def _units_of(plan):
+    """Per-template work of `plan` (Plan.template_units), or None for a plan object that does not report it."""
+    f = getattr(plan, "template_units", None)
+    return f() if callable(f) else None
 
 
 def build_bank_shard(plan, group=None):
@@ -106,7 +135,7 @@ def build_bank_shard(plan, group=None):
     sharded = dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1
     world = dist.get_world_size(group) if sharded else 1
     rank = dist.get_rank(group) if sharded else 0
-    ti_lo, ti_cnt = template_range(plan.info.ntemplates, world, rank)
+    ti_lo, ti_cnt = template_range(plan.info.ntemplates, world, rank, _units_of(plan))
     err = None
     try:
         plan.templates_range(ti_lo, ti_cnt)       # ti_cnt == 0 (more ranks than templates) builds the tables only
@@ -144,7 +173,7 @@ def search_candidates_sharded(plan, d_spec, threshold, max_cands: int = 1 << 20,
     rank = dist.get_rank(group) if sharded else 0
     if sharded:
         broadcast_spectrum(d_spec, src=src, group=group)
-    ti_lo, ti_cnt = template_range(plan.info.ntemplates, world, rank)
+    ti_lo, ti_cnt = template_range(plan.info.ntemplates, world, rank, _units_of(plan))
     d_c, d_n = plan.search_candidates_templates(d_spec, threshold, ti_lo, ti_cnt, max_cands)
     n = int(d_n.item()) & binding.SEAM_OVERFLOW
     overflow = n > max_cands          # includes the seam-overflow sentinel

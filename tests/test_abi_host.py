@@ -162,3 +162,43 @@ def test_overlap_classes_of_the_plan(lib):
     assert 0.93 < i.flops_per_search_executed / i.flops_per_search < 0.95
     small = binding.Plan(32768, 20, 2, 60, 20, 2, 4096).info
     assert small.nclasses == 1 and small.units_per_search == small.nseg * 2 * small.ntemplates
+
+
+def test_template_units_balance_the_strong_scaling_split(lib):
+    """jerk_template_units (SURVEY.md 8(e), strong scaling): per-template units sum to units_per_search, follow the overlap
+    classes (wider templates, more units), and shard.template_range cut at equal units leaves <= 1 % between 8 ranks on
+    the config-3 grid where the equal-count split leaves 6 %."""
+    from paper_1911_01353_b200 import shard
+    cfg = synth.config(3)
+    plan = binding.Plan(cfg.nbins, cfg.zmax, cfg.dz, cfg.wmax, cfg.dw, 2, 4096)
+    u = plan.template_units()
+    T = int(plan.info.ntemplates)
+    assert u.shape == (T,) and int(u.sum()) == int(plan.info.units_per_search)
+    # recomputed from the oracle's half-widths: a template of a wider class never has fewer units
+    zs, ws = orc.grid_values(cfg.zmax, cfg.dz), orc.grid_values(cfg.wmax, cfg.dw)
+    hw = np.array([orc.halfwidth(float(z), float(w)) for w in ws for z in zs])
+    order = np.argsort(hw, kind="stable")
+    assert np.all(np.diff(u[order]) >= 0)
+    for world in (2, 3, 4, 8):
+        parts = [shard.template_range(T, world, r, u) for r in range(world)]
+        assert parts[0][0] == 0 and parts[-1][0] + parts[-1][1] == T
+        assert all(parts[i][0] + parts[i][1] == parts[i + 1][0] for i in range(world - 1))
+        work = [int(u[lo:lo + cnt].sum()) for lo, cnt in parts]
+        assert max(work) / min(work) <= 1.01, (world, work)
+    flat = [int(u[lo:lo + cnt].sum()) for lo, cnt in (shard.template_range(T, 8, r) for r in range(8))]
+    assert max(flat) / min(flat) > 1.04
+    # a small grid is one class: equal units per template, the balanced split equals the equal-count split up to a template
+    c1 = synth.config(1)
+    p1 = binding.Plan(c1.nbins, c1.zmax, c1.dz, c1.wmax, c1.dw, 2, 1024)
+    u1 = p1.template_units()
+    assert len(set(u1.tolist())) == 1
+    for r in range(4):
+        a, b = shard.template_range(u1.size, 4, r, u1), shard.template_range(u1.size, 4, r)
+        assert abs(a[0] - b[0]) <= 1 and abs(a[1] - b[1]) <= 1
+    # more ranks than templates: every template is assigned exactly once, surplus ranks get empty ranges
+    uu = np.array([5, 5, 5], dtype=np.int64)
+    parts = [shard.template_range(3, 7, r, uu) for r in range(7)]
+    seen = np.zeros(3, dtype=int)
+    for lo, cnt in parts:
+        seen[lo:lo + cnt] += 1
+    assert (seen == 1).all()

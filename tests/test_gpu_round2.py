@@ -417,10 +417,22 @@ def test_no_write_outside_caller_buffers(seg_len, zmax, wmax):
 
 # ------------------------------------------------------------------------------------------------ measurement aids
 def test_probes_report_sane_numbers():
-    """jerk_probe_fma / jerk_probe_issue (the denominators and the issue-slot model of DESIGN.md 6.2): a packed FP32
+    """bench.py's bench_probe_fma / bench_probe_issue (bench_probes.cu, outside the library; the denominators and the issue-slot model of DESIGN.md 6.2): a packed FP32
     instruction takes about two scheduler cycles, no companion instruction is free, the FFMA probe is near the nominal peak."""
-    p = binding.probe_issue_slots(iters=500)
+    import bench
+    p = bench.probe_issue_slots(iters=500)
     assert 1.9 < p["packed_fma_cycles"] < 2.3
     assert all(c > 0.5 for c in p["companion_cost_cycles"].values())
-    tf = binding.probe_fp32_tflops(iters=1 << 13, reps=3)
+    tf = bench.probe_fp32_tflops(iters=1 << 13, reps=3)
     assert 50.0 < tf < 80.0
+
+
+def test_cufft_comparator_agrees_with_the_fused_plane():
+    """SURVEY.md 8(f) N4 / PAPER.md:45: the unfused cuFFT pipeline of bench.py (library calls only: torch.fft + elementwise
+    kernels on this library's bank) gives the powers of jerk_search_plane to 1e-3 * max(1, P) -- on config 2 (the whole
+    1 GB block path: 512 template-phases x 64 segments) for three templates, all segments of the block, both phases."""
+    import bench
+    row = bench.cufft_unfused_block(synth.config(2), warmup=1, steps=1, check_templates=(0, 100, 255))
+    assert row["units_per_block"] == 512 * 64
+    assert row["max_rel_diff_vs_fused_plane"] < 1e-3, row
+    assert row["extrapolated_ms_per_search"] > 0
