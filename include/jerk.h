@@ -288,6 +288,19 @@ int jerk_harmonic_sum(jerk_plan* plan, const void* d_spec, int nstages, const in
                       uint64_t work_bytes, void* stream);
 
 /*
+ * jerk_harmonic_sum_range — the same restricted to top-harmonic positions r_lo <= b < r_lo + r_cnt (half-bin indices
+ * 2 r_lo <= j < 2 (r_lo + r_cnt)): d_top[s] is the arg-max of S_h over that part of the volume.  This is one rank's share of
+ * a harmonic stage sharded by r-range ("the r-range partition ... needed for the harmonic stage"): the
+ * sub-harmonic powers a range needs lie at r e/8 <= r, so every rank reads the whole spectrum and holds the whole bank, and
+ * the ranks' records are folded by (largest power, then smallest (iw, iz, j)).  The values do not depend on how the r axis
+ * is cut: the union over disjoint ranges equals jerk_harmonic_sum bit for bit.  r_cnt == 0: every stage reports j = -1.
+ * jerk_harmonic_sum is the range [0, nbins).  Errors: as jerk_harmonic_sum, JERK_EINVAL for a range outside [0, nbins).
+ */
+int jerk_harmonic_sum_range(jerk_plan* plan, const void* d_spec, int nstages, const int* h_harm, const float* h_thr,
+                            int64_t r_lo, int64_t r_cnt, jerk_cand* d_top, void* d_scratch, uint64_t scratch_bytes,
+                            void* d_work, uint64_t work_bytes, void* stream);
+
+/*
  * jerk_harmonic_plane — plane-output mode of the same stage: writes S_h (h in {1,2,4,8}) for the box
  * r_lo <= b < r_lo+r_cnt, iz_lo <= iz < iz_lo+iz_cnt, iw_lo <= iw < iw_lo+iw_cnt as
  * d_out[iw_rel][iz_rel][j - 2*r_lo] (float32, >= jerk_plane_bytes(r_cnt, iz_cnt, iw_cnt)).  The box is handled

@@ -46,7 +46,7 @@ EXPORTS = [
     "jerk_search_candidates", "jerk_search_candidates_range", "jerk_search_candidates_templates",
     "jerk_search_candidates_batch", "jerk_search_candidates_stats", "jerk_snr_filter",
     "jerk_sift_candidates",
-    "jerk_search_candidates_host", "jerk_search_series_host", "jerk_harmonic_scratch_bytes", "jerk_harmonic_sum", "jerk_harmonic_plane", "jerk_spectrum_scratch_bytes",
+    "jerk_search_candidates_host", "jerk_search_series_host", "jerk_harmonic_scratch_bytes", "jerk_harmonic_sum", "jerk_harmonic_sum_range", "jerk_harmonic_plane", "jerk_spectrum_scratch_bytes",
     "jerk_prepare_spectrum", "jerk_prepare_spectrum_mode", "jerk_prepare_spectrum_static", "jerk_strerror",
     "jerk_last_error",
 ]
@@ -89,6 +89,7 @@ def load_library() -> C.CDLL:
     lib.jerk_harmonic_scratch_bytes.argtypes = [vp]
     lib.jerk_harmonic_scratch_bytes.restype = u64
     lib.jerk_harmonic_sum.argtypes = [vp, vp, i32, C.POINTER(i32), C.POINTER(C.c_float), vp, vp, u64, vp, u64, vp]
+    lib.jerk_harmonic_sum_range.argtypes = [vp, vp, i32, C.POINTER(i32), C.POINTER(C.c_float), i64, i64, vp, vp, u64, vp, u64, vp]
     lib.jerk_harmonic_plane.argtypes = [vp, vp, i32, i64, i64, i32, i32, i32, i32, vp, u64, vp, u64, vp, u64, vp]
     lib.jerk_spectrum_scratch_bytes.argtypes = [i64]
     lib.jerk_spectrum_scratch_bytes.restype = u64
@@ -328,17 +329,20 @@ class Plan:
             self.scratch = torch.empty(nbytes, dtype=torch.uint8, device=device)
         return self.scratch
 
-    def harmonic_sum(self, d_spec, harms=(1, 2, 4, 8), thresholds=(25.0, 35.0, 50.0, 75.0), scratch_bytes=None, stream=None):
-        """jerk_harmonic_sum: returns a structured numpy array (CAND_DTYPE) with one record per stage (synchronises)."""
+    def harmonic_sum(self, d_spec, harms=(1, 2, 4, 8), thresholds=(25.0, 35.0, 50.0, 75.0), scratch_bytes=None, stream=None,
+                     r_lo=0, r_cnt=None):
+        """jerk_harmonic_sum (or jerk_harmonic_sum_range when r_lo / r_cnt restrict the top-harmonic positions): returns a
+        structured numpy array (CAND_DTYPE) with one record per stage (synchronises)."""
         import torch
         n = len(harms)
+        r_cnt = int(self.info.nbins) - int(r_lo) if r_cnt is None else int(r_cnt)
         d_top = torch.zeros(n * 16, dtype=torch.uint8, device=d_spec.device)
         work = self._ensure_work(d_spec.device)
         scratch = self._ensure_scratch(d_spec.device, scratch_bytes)
         nbytes = scratch.numel() if scratch_bytes is None else int(scratch_bytes)
-        self._check(self._lib.jerk_harmonic_sum(
+        self._check(self._lib.jerk_harmonic_sum_range(
             self._h, C.c_void_p(d_spec.data_ptr()), n, (C.c_int * n)(*[int(h) for h in harms]),
-            (C.c_float * n)(*[float(t) for t in thresholds]), C.c_void_p(d_top.data_ptr()), C.c_void_p(scratch.data_ptr()),
+            (C.c_float * n)(*[float(t) for t in thresholds]), int(r_lo), r_cnt, C.c_void_p(d_top.data_ptr()), C.c_void_p(scratch.data_ptr()),
             nbytes, C.c_void_p(work.data_ptr()), work.numel(), _stream_ptr(stream)))
         return d_top.cpu().numpy().view(CAND_DTYPE).copy()
 

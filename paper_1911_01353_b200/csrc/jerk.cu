@@ -2866,6 +2866,13 @@ uint64_t jerk_harmonic_scratch_bytes(const jerk_plan* p) {
 
 int jerk_harmonic_sum(jerk_plan* p, const void* d_spec, int nstages, const int* h_harm, const float* h_thr, jerk_cand* d_top,
                       void* d_scratch, uint64_t scratch_bytes, void* d_work, uint64_t work_bytes, void* stream) {
+  if (!p) return JERK_EINVAL;
+  return jerk_harmonic_sum_range(p, d_spec, nstages, h_harm, h_thr, 0, p->nbins, d_top, d_scratch, scratch_bytes, d_work, work_bytes, stream);
+}
+
+int jerk_harmonic_sum_range(jerk_plan* p, const void* d_spec, int nstages, const int* h_harm, const float* h_thr, int64_t r_lo,
+                            int64_t r_cnt, jerk_cand* d_top, void* d_scratch, uint64_t scratch_bytes, void* d_work, uint64_t work_bytes,
+                            void* stream) {
   int rc = check_common(p, d_spec, d_work, work_bytes);
   if (rc) return rc;
   if (nstages < 1 || nstages > 4 || !h_harm || !h_thr || !d_top || !d_scratch) return JERK_EINVAL;
@@ -2881,12 +2888,17 @@ int jerk_harmonic_sum(jerk_plan* p, const void* d_spec, int nstages, const int* 
   if (!bank_covers(p, 0, p->nz, 0, p->nw)) return fail(p, JERK_ESTATE, "the harmonic stage needs the whole bank (jerk_templates)");
   float thr4[4] = {INFINITY, INFINITY, INFINITY, INFINITY};   // per stage index log2 h: the lowest threshold asked for (unrequested stages are not tracked)
   for (int s = 0; s < nstages; s++) thr4[he.stage[s]] = fminf(thr4[he.stage[s]], h_thr[s]);
+  if (r_lo < 0 || r_cnt < 0 || r_lo > p->nbins - r_cnt) return fail(p, JERK_EINVAL, "harmonic r-range outside [0, nbins)");
   const int64_t chunk = harm_chunk_for(p, scratch_bytes);
   if (chunk == 0) return fail(p, JERK_ENOMEM, "harmonic scratch buffer too small (see jerk_harmonic_scratch_bytes)");
   cudaStream_t st = (cudaStream_t)stream;
   bool first = true;
-  for (int64_t r_lo = 0; r_lo < p->nbins; r_lo += chunk) {
-    HarmBox bx{r_lo, std::min<int64_t>(chunk, p->nbins - r_lo), 0, p->nz, 0, p->nw};
+  if (r_cnt == 0) {   // an empty range (a surplus rank of a sharded stage): no running record, every stage reports j = -1
+    cudaError_t e0 = cudaMemsetAsync(d_scratch, 0xFF, kHarmHeader, st);
+    if (e0 != cudaSuccess) return fail(p, JERK_ECUDA, std::string("harmonic header memset: ") + cudaGetErrorString(e0));
+  }
+  for (int64_t r0 = r_lo; r0 < r_lo + r_cnt; r0 += chunk) {
+    HarmBox bx{r0, std::min<int64_t>(chunk, r_lo + r_cnt - r0), 0, p->nz, 0, p->nw};
     rc = harm_box(p, d_spec, bx, (unsigned char*)d_scratch, scratch_bytes, d_work, work_bytes, nullptr, 0, thr4, first, st);
     if (rc) return rc;
     first = false;

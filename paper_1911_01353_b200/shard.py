@@ -11,7 +11,9 @@ row (reading S10).  Two partitions are offered:
     broadcast once, candidate lists are concatenated at the end.
 
 The only collectives are the ones around the search: broadcast of the spectrum, gather of the (small) candidate
-lists, max-over-ranks of device times.  This module holds no arithmetic of the method."""
+lists, max-over-ranks of device times.  The harmonic stage shards by r-range of the top harmonic (harmonic_sum_sharded):
+whole bank and whole spectrum on every rank, the four stage records gathered and folded at the end.  This module holds no
+arithmetic of the method."""
 from __future__ import annotations
 
 import numpy as np
@@ -183,3 +185,59 @@ def search_candidates_sharded(plan, d_spec, threshold, max_cands: int = 1 << 20,
     if sharded:
         return gather_candidates(local, group=group)
     return np.sort(local, order=["iw", "iz", "j"])
+
+
+def fold_stage_records(records: np.ndarray) -> np.ndarray:
+    """records: structured array [nranks][nstages] of jerk_cand stage tops (j = -1: nothing above the threshold in that
+    rank's range).  Per stage the record with the largest power wins; equal powers go to the smallest (iw, iz, j) -- the
+    tie rule of jerk_harmonic_sum (include/jerk.h), so the fold of disjoint ranges equals the single call."""
+    records = np.asarray(records)
+    out = records[0].copy()
+    for s in range(records.shape[1]):
+        best = None
+        for r in range(records.shape[0]):
+            c = records[r, s]
+            if int(c["j"]) < 0:
+                continue
+            key = (-float(c["power"]), int(c["iw"]), int(c["iz"]), int(c["j"]))
+            if best is None or key < best[0]:
+                best = (key, c)
+        if best is None:
+            out[s] = records[0, s]
+            out[s]["j"], out[s]["iz"], out[s]["iw"], out[s]["power"], out[s]["flags"] = -1, 0, 0, 0.0, 0
+        else:
+            out[s] = best[1]
+    return out
+
+
+def harmonic_sum_sharded(plan, d_spec, harms=(1, 2, 4, 8), thresholds=(25.0, 35.0, 50.0, 75.0), group=None, src: int = 0,
+                         scratch_bytes=None) -> np.ndarray:
+    """The harmonic-sum stage of ONE spectrum over the ranks of `group` (r-range partition): the spectrum is
+    broadcast from `src`, rank r runs jerk_harmonic_sum_range on the contiguous block r of the top-harmonic bins (the
+    sub-harmonic sources of a range lie below it, so every rank needs the whole spectrum and the whole bank; work per
+    top-harmonic bin is uniform, so equal blocks are balanced), the per-rank stage records (4 x 16 bytes) are all-gathered and
+    folded with the tie rule.  Returns the same array on every rank, equal to plan.harmonic_sum on one GPU.  A failure
+    on any rank raises on every rank."""
+    import torch
+    import torch.distributed as dist
+    sharded = dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1
+    world = dist.get_world_size(group) if sharded else 1
+    rank = dist.get_rank(group) if sharded else 0
+    if sharded:
+        broadcast_spectrum(d_spec, src=src, group=group)
+    r_lo, r_cnt = block_range(int(plan.info.nbins), world, rank)
+    err, mine = None, None
+    try:
+        mine = plan.harmonic_sum(d_spec, harms, thresholds, scratch_bytes=scratch_bytes, r_lo=r_lo, r_cnt=r_cnt)
+    except Exception as exc:                      # noqa: BLE001 -- agreed below
+        err = exc
+    if (agree_on_failure(err is not None, group) if sharded else err is not None):
+        raise RuntimeError(f"harmonic stage failed on at least one rank (rank {rank}: {err})") from err
+    if not sharded:
+        return fold_stage_records(mine[None, :])
+    dev = torch.device("cuda", torch.cuda.current_device()) if dist.get_backend(group) == "nccl" else torch.device("cpu")
+    buf = torch.from_numpy(np.frombuffer(mine.tobytes(), dtype=np.uint8).copy()).to(dev)
+    bufs = [torch.empty_like(buf) for _ in range(world)]
+    dist.all_gather(bufs, buf, group=group)
+    recs = np.stack([np.frombuffer(b.cpu().numpy().tobytes(), dtype=mine.dtype) for b in bufs])
+    return fold_stage_records(recs)

@@ -88,6 +88,38 @@ def oracle_candidates_for_row(X, z, w, thr, b_lo, b_cnt, nbins):
     return j[keep], pw[keep], margin[keep], P, 2 * lo
 
 
+def _cand_job(args):
+    Xs, off, z, w, thr, b_lo, b_cnt, nbins = args
+    lo = max(0, b_lo - 1)
+    hi = min(nbins, b_lo + b_cnt + 1)
+    P = orc.power_row(Xs, z, w, lo - off, hi - lo)       # Xs = X[off : ...] reaches every tap of the range (or the true spectrum edge)
+    j, pw, margin = orc.row_candidates(P, thr, j_offset=2 * lo)
+    keep = (j >= 2 * b_lo) & (j < 2 * (b_lo + b_cnt))
+    if lo > 0:
+        keep &= j > 2 * lo
+    if hi < nbins:
+        keep &= j < 2 * hi - 1
+    return j[keep], pw[keep], margin[keep], P, 2 * lo
+
+
+def oracle_candidates_for_rows(X, jobs, thr, workers=None):
+    """oracle_candidates_for_row for many (z, w, b_lo, b_cnt) jobs in parallel processes; each worker gets only the bins
+    its taps can reach (a slice that starts at 0 / ends at nbins keeps the true zero-padded spectrum edge)."""
+    workers = workers or min(8, os.cpu_count() or 1)
+    X = np.asarray(X)
+    pad = 700
+    packed = []
+    for z, w, b_lo, b_cnt in jobs:
+        off = max(0, int(b_lo) - 1 - pad)
+        end = min(X.size, int(b_lo) + int(b_cnt) + 1 + pad)
+        packed.append((X[off:end], off, float(z), float(w), float(thr), int(b_lo), int(b_cnt), int(X.size)))
+    if workers <= 1 or len(packed) <= 2:
+        return [_cand_job(a) for a in packed]
+    import multiprocessing as mp
+    with ProcessPoolExecutor(max_workers=workers, mp_context=mp.get_context("spawn")) as ex:
+        return list(ex.map(_cand_job, packed))
+
+
 def compare_row_candidates(gpu_j, gpu_p, ref_j, ref_p, ref_margin, P_ref, j0, thr):
     """Candidate parity for one (z,w) row (BASELINE.json north_star + reading S11).
 

@@ -177,6 +177,37 @@ def test_harmonic_wide_templates_seg_len_4096():
     assert np.array_equal(near, top)
 
 
+@pytest.mark.parametrize("seg_len,world", [(4096, 3), (1024, 2), (4096, 7)])
+def test_harmonic_r_ranges_fold_to_the_single_call(seg_len, world):
+    """jerk_harmonic_sum_range (the harmonic stage shards by r-range): the stage tops of `world` disjoint
+    blocks of the top-harmonic axis, folded with the tie rule (shard.fold_stage_records), equal the single call bit for bit;
+    every block's record lies inside its block; an empty block reports nothing; one rank is the whole call."""
+    from paper_1911_01353_b200 import shard
+    nbins = 9000
+    X = _small_case(nbins)
+    plan = binding.Plan(nbins, 20, 2, 60, 20, 2, seg_len)
+    plan.templates()
+    d_spec = binding.spectrum_to_device(X)
+    thr = (0.0, 0.0, 30.0, 1e9)
+    whole = plan.harmonic_sum(d_spec, STAGES, thr)
+    recs = []
+    for r in range(world):
+        lo, cnt = shard.block_range(nbins, world, r)
+        part = plan.harmonic_sum(d_spec, STAGES, thr, r_lo=lo, r_cnt=cnt)
+        for c in part:
+            assert c["j"] == -1 or 2 * lo <= c["j"] < 2 * (lo + cnt)
+        recs.append(part)
+    folded = shard.fold_stage_records(np.stack(recs))
+    assert folded.tobytes() == whole.tobytes()
+    assert whole[3]["j"] == -1 and whole[0]["j"] >= 0
+    empty = plan.harmonic_sum(d_spec, STAGES, thr, r_lo=100, r_cnt=0)
+    assert (empty["j"] == -1).all() and (empty["power"] == 0).all()
+    assert shard.harmonic_sum_sharded(plan, d_spec, STAGES, thr).tobytes() == whole.tobytes()      # no process group: this rank does it all
+    with pytest.raises(binding.JerkError) as e:
+        plan.harmonic_sum(d_spec, STAGES, thr, r_lo=nbins - 10, r_cnt=11)
+    assert e.value.status == binding.JERK_EINVAL
+
+
 class _OraclePowers:
     """P_ref(j, iz', iw') on demand (signed grid indices), one oracle row segment per request, cached."""
 

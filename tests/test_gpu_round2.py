@@ -436,3 +436,55 @@ def test_cufft_comparator_agrees_with_the_fused_plane():
     assert row["units_per_block"] == 512 * 64
     assert row["max_rel_diff_vs_fused_plane"] < 1e-3, row
     assert row["extrapolated_ms_per_search"] > 0
+
+
+def test_config3_candidate_list_is_complete_on_random_windows():
+    """Completeness at full size (reading S11): the tests above check every RETURNED record; here the
+    oracle decides what must be there.  Config 3 at threshold 9 (1.1e7 candidates: the rare path, the seam records and the
+    hash table of the full-size launch are all busy; threshold 12 would leave ~0.2 candidates per window), 64 random (z,w)
+    rows x a 20 000-bin window -- one window at bin 0, one ending at nbins - 1, the rest
+    at random places (each spans five or more segments of its overlap class): the GPU's records of that row and window
+    and orc.row_candidates agree as sets, up to the near-threshold / near-tie allowances of compare_row_candidates."""
+    cfg, X, plan0, d_spec = _setup(3)
+    thr = 9.0
+    plan = binding.Plan(cfg.nbins, cfg.zmax, cfg.dz, cfg.wmax, cfg.dw, 2, cfg.seg_len, extra_seams=1 << 24)
+    plan.bank = plan0.bank                 # the same caller-owned bank (rebuilt in place with identical contents)
+    plan.templates()
+    max_c = 1 << 24
+    d_c, d_n = plan.search_candidates(d_spec, thr, max_cands=max_c)
+    n = int(d_n.item())
+    assert 5e6 < n <= max_c, n               # neither the candidate buffer nor the seam records overflowed (-1)
+    cands = d_c[: n * 16].cpu().numpy().view(binding.CAND_DTYPE)
+    zs, ws = orc.grid_values(cfg.zmax, cfg.dz), orc.grid_values(cfg.wmax, cfg.dw)
+    rng = np.random.default_rng(1911)
+    wlen = 20000
+    jobs, keys = [], []
+    for k in range(64):
+        iz, iw = int(rng.integers(0, cfg.nz)), int(rng.integers(0, cfg.nw))
+        if k == 0:
+            iz, iw = 0, 0                                   # widest templates (first class boundary), window at the start
+        if k == 1:
+            iz, iw = cfg.nz - 1, cfg.nw - 1
+        b_lo = 0 if k % 8 == 0 else (cfg.nbins - wlen if k % 8 == 1 else int(rng.integers(0, cfg.nbins - wlen)))
+        jobs.append((zs[iz], ws[iw], b_lo, wlen))
+        keys.append((iz, iw, b_lo))
+    refs = H.oracle_candidates_for_rows(X, jobs, thr)
+    ti_all = cands["iw"].astype(np.int64) * cfg.nz + cands["iz"]
+    cands = cands[np.isin(ti_all, [iw * cfg.nz + iz for iz, iw, _ in keys])]      # the 64 rows only, before sorting
+    order = np.lexsort((cands["j"], cands["iz"], cands["iw"]))
+    cs = cands[order]
+    ti_sorted = cs["iw"].astype(np.int64) * cfg.nz + cs["iz"]
+    total_ref = total_strong = 0
+    for (iz, iw, b_lo), (rj, rp, rm, P_ref, j0) in zip(keys, refs):
+        a, b = np.searchsorted(ti_sorted, [iw * cfg.nz + iz, iw * cfg.nz + iz + 1])
+        row = cs[a:b]
+        sel = (row["j"] >= 2 * b_lo) & (row["j"] < 2 * (b_lo + wlen))
+        if b_lo > 0:
+            sel &= row["j"] > j0                            # the window's artificial edges, as in oracle_candidates_for_row
+        if b_lo + wlen < cfg.nbins:
+            sel &= row["j"] < j0 + P_ref.size - 1
+        matched, strong = H.compare_row_candidates(row["j"][sel], row["power"][sel], rj, rp, rm, P_ref, j0, thr)
+        assert matched == strong
+        total_ref += rj.size
+        total_strong += strong
+    assert total_ref > 100 and total_strong > 40, (total_ref, total_strong)

@@ -101,6 +101,37 @@ def _worker(rank, world, port, nz, nw, q):
         want3 = np.sort(full[(ti_all < world - 1) & (full["power"] > 40.0)], order=["iw", "iz", "j"])
         ok_merge = ok_merge and np.array_equal(merged3, want3)
         _FakePlan.info.ntemplates = nz * nw
+        # harmonic stage by r-range: every rank reports the top of its block, the fold is the global top with the tie rule
+        class _HarmPlan:
+            info = _Info()
+            fail_rank = -1
+
+            def harmonic_sum(self, d_spec, harms, thresholds, scratch_bytes=None, r_lo=0, r_cnt=None):
+                if rank == self.fail_rank:
+                    raise ValueError("stand-in harmonic failure")
+                out = np.zeros(len(harms), dtype=shard.CAND_FIELDS)
+                for s_i, h in enumerate(harms):
+                    # stand-in volume: power(j) of stage h peaks at j = 1000 h (value 90) and at j = 5000 (value 90 too: a tie
+                    # that must go to the smaller j), plus a 50 everywhere; stage 8 has nothing above its threshold
+                    peaks = [(1000 * h, 90.0), (5000, 90.0), (2 * r_lo, 50.0)] if h != 8 else []
+                    inside = [(j, p) for j, p in peaks if 2 * r_lo <= j < 2 * (r_lo + r_cnt) and p > thresholds[s_i]]
+                    if inside:
+                        j, pw = min(inside, key=lambda t: (-t[1], t[0]))
+                        out[s_i] = (j, 3, 1, pw, 0)
+                    else:
+                        out[s_i] = (-1, 0, 0, 0.0, 0)
+                return out
+
+        _HarmPlan.info.nbins = 6000
+        hp = _HarmPlan()
+        tops = shard.harmonic_sum_sharded(hp, X, (1, 2, 4, 8), (25.0, 25.0, 25.0, 25.0))
+        ok_merge = ok_merge and [int(t["j"]) for t in tops] == [1000, 2000, 4000, -1] and float(tops[0]["power"]) == 90.0
+        hp.fail_rank = world - 1
+        try:
+            shard.harmonic_sum_sharded(hp, X, (1, 2), (25.0, 25.0))
+            ok_merge = False
+        except RuntimeError:
+            pass
         tmax = shard.max_over_ranks(10.0 + rank)
         q.put((rank, ok_merge, ok_bcast, tmax, shard.trial_indices(7, world, rank)))
     finally:
@@ -144,3 +175,16 @@ def test_block_range_balanced():
             assert sum(c for _, c in parts) == n
             assert max(c for _, c in parts) - min(c for _, c in parts) <= 1
             assert all(parts[i][0] + parts[i][1] == parts[i + 1][0] for i in range(w - 1))
+
+
+def test_fold_stage_records_tie_rule():
+    rec = np.zeros((3, 2), dtype=shard.CAND_FIELDS)
+    rec[0] = [(-1, 0, 0, 0.0, 0), (10, 5, 2, 40.0, 0)]
+    rec[1] = [(7, 1, 1, 30.0, 0), (4, 5, 1, 40.0, 0)]            # stage 1: same power, smaller iw wins
+    rec[2] = [(9, 0, 0, 30.0, 0), (-1, 0, 0, 0.0, 0)]            # stage 0: same power, smaller (iw, iz) wins
+    out = shard.fold_stage_records(rec)
+    assert (int(out[0]["j"]), int(out[0]["iz"]), int(out[0]["iw"])) == (9, 0, 0)
+    assert (int(out[1]["j"]), int(out[1]["iz"]), int(out[1]["iw"])) == (4, 5, 1)
+    none = np.zeros((2, 1), dtype=shard.CAND_FIELDS)
+    none["j"] = -1
+    assert int(shard.fold_stage_records(none)[0]["j"]) == -1
