@@ -601,6 +601,19 @@ def other_rows(steps=3):
                                                   for h, r in zip((1, 2, 4, 8), top)],
          "flops_note": "frac_fp32_peak credits the 2.53 base searches this design executes ((1^3 + ... + 8^3)/512: the eight sub-volumes "
                        "of fractions e/8 are recomputed); frac_fp32_peak_one_search counts the one search the method needs"})
+    # the same stage with the scratch size the library itself asks for (jerk_harmonic_scratch_bytes: 65536-bin r-chunks)
+    try:
+        base = int(plan.harmonic_scratch_bytes())
+        plan.scratch = None
+        torch.cuda.empty_cache()
+        ts = _time_steps(lambda: plan.harmonic_sum(d_spec, scratch_bytes=base), 3, 2)
+        top_d = plan.harmonic_sum(d_spec, scratch_bytes=base)
+        rows["config5_harmonic_sum_default_scratch"] = _row_entry(
+            ts, cfg.points, plan.info.flops_per_search * HARM_FLOP_FACTOR,
+            {"scratch_bytes": base, "same_stage_tops_as_large_scratch": bool(top_d.tobytes() == top.tobytes()),
+             "frac_fp32_peak_one_search": plan.info.flops_per_search / (float(np.median(ts)) * 1e-3) / 1e12 / FP32_PEAK_TFLOPS})
+    except Exception as exc:          # noqa: BLE001
+        rows["config5_harmonic_sum_default_scratch"] = {"error": repr(exc)}
     return rows
 
 
